@@ -1,0 +1,380 @@
+"""TEST INFRASTRUCTURE ONLY - CPU oracle, never imported by the product path.
+
+O-1 / O-2 of SURVEY.md 8(c): the per-account program Eq. (1) is lifted to a smooth
+QP in buys p >= 0 and per-lot sells r_l >= 0 (trade vector dw = w - w0 = p - sum_l r_l, PAPER.md:107;
+"continuous public benchmark rows") and solved by a textbook primal-dual interior
+point method (Mehrotra predictor-corrector; KKT/duality reference [6] of the paper):
+
+    min  1/2 v'Hv + c'v   s.t.  A v = b,  G v <= h
+    v = (p ; r_1 ; ... ; r_L) over the assets whose box is not degenerate (lo_i < hi_i);
+    assets with lo_i = hi_i (exclusions) are substituted out as constants.
+
+    H = gamma J' Sigma J,   J = [I, -I, ..., -I]
+    c_p = gamma (Sigma x0)_i - mu_i + kappa dt_i + c_buy ,  c_r,l = -(gamma (Sigma x0)_i - mu_i) + kappa dt_i + slope_il
+    rows of G:  -v <= 0;  r_il <= width_il (lots only);  lo <= w <= hi;  band_lo <= E w <= band_hi;
+                sum dt_i (p_i + sum_l r_il) <= tau
+
+Two linear-algebra modes share ONE iteration (`solve`):
+  dense       - H, G materialised, reduced KKT matrix solved by numpy.linalg.solve (the plain definition)
+  structured  - same reduced matrix applied through its structure (per-asset diagonal + rank one,
+                plus low rank from B, groups and the turnover row) by Sherman-Morrison / Woodbury;
+                admitted only because tests pin it to the dense mode.
+
+Accuracy target: residuals <= 1e-10 relative; the GPU path is compared at 1e-4 / 1e-6.
+Pins: tests/test_oracle_pins.py (closed form, brute-force enumeration, separable knapsack, capped simplex,
+cap/penalty duality, invariances, KKT certificates).
+"""
+from __future__ import annotations
+
+import numpy as np
+
+from .problem import Account, sigma_apply
+
+
+class LiftedQP:
+    def __init__(self, acc: Account):
+        self.acc = acc
+        N = acc.N
+        free = acc.hi > acc.lo
+        self.free = np.nonzero(free)[0]
+        nf = len(self.free)
+        self.nf = nf
+        w_base = acc.w0.copy()
+        w_base[~free] = acc.lo[~free]
+        self.w_base = w_base
+        fi = self.free
+        # variables: block 0 = buys p, blocks 1..L = per-lot sells
+        if acc.lot_slope is not None:
+            L = acc.lot_slope.shape[1]
+            alive = np.arange(L)[None, :] < acc.lot_count[fi][:, None]          # (nf, L)
+            nolot = acc.lot_count[fi] == 0
+        else:
+            L = 1
+            alive = np.ones((nf, 1), dtype=bool)
+            nolot = np.ones(nf, dtype=bool)
+        va = [np.arange(nf)]            # asset (index into free list) of each variable
+        vs = [np.ones(nf)]              # sign in w = w_base + J v
+        vub = [np.full(nf, np.inf)]     # upper bound on the variable
+        vcost = [np.full(nf, acc.c_buy)]
+        # no trade cost and no cap at all: buys and sells need not be split (and must not be: (p, r) would be
+        # non-unique and the barrier system singular) -> one signed trade variable per asset, no sign rows
+        self.signed = (not np.isfinite(acc.tau)) and acc.kappa == 0.0 and acc.c_buy == 0.0 and acc.lot_slope is None
+        for l in range(0 if self.signed else L):
+            if acc.lot_slope is not None:
+                idx = np.nonzero(alive[:, l] | (nolot & (l == 0)))[0]
+                ub = np.where(nolot[idx], np.inf, acc.lot_width[fi[idx], l])
+                cost = np.where(nolot[idx], 0.0, acc.lot_slope[fi[idx], l])
+            else:
+                idx = np.arange(nf); ub = np.full(nf, np.inf); cost = np.zeros(nf)
+            va.append(idx); vs.append(-np.ones(len(idx))); vub.append(ub); vcost.append(cost)
+        self.va = np.concatenate(va); self.vs = np.concatenate(vs)
+        self.vub = np.concatenate(vub); vcost = np.concatenate(vcost)
+        self.n = len(self.va)
+        self.vj = np.concatenate([np.zeros(nf, dtype=np.int64)] + [np.full(len(va[1 + l]), 1 + l, dtype=np.int64) for l in range(len(va) - 1)])
+        self.nv = 1 + L
+        self.sg = np.zeros((nf, 1 + L)); self.sg[self.va, self.vj] = self.vs
+        x0 = w_base if acc.w_b is None else w_base - acc.w_b
+        g0 = acc.gamma * sigma_apply(acc, x0) - acc.mu                              # gradient of smooth part at w_base
+        self.c = self.vs * g0[fi][self.va] + acc.kappa * acc.dt[fi][self.va] + vcost
+        self.Bf = acc.B[fi]; self.df = acc.d[fi]; self.dtf = acc.dt[fi]
+        # equality: budget
+        self.a_row = self.vs.copy()
+        self.b_eq = acc.budget - float(w_base.sum())
+        # inequality rows
+        self.ub_idx = np.nonzero(np.isfinite(self.vub))[0]
+        self.has_lo = np.isfinite(acc.lo[fi]); self.has_hi = np.isfinite(acc.hi[fi])
+        self.lo_idx = np.nonzero(self.has_lo)[0]; self.hi_idx = np.nonzero(self.has_hi)[0]
+        self.G = acc.G
+        if acc.G > 0:
+            self.gid = acc.group_id[fi]
+            gbase = np.bincount(acc.group_id, weights=w_base, minlength=acc.G)
+            self.band_hi_rhs = acc.band_hi - gbase
+            self.band_lo_rhs = -(acc.band_lo - gbase)
+        self.has_tau = np.isfinite(acc.tau)
+        if self.has_tau:
+            t_fix = float(np.sum(acc.dt[~free] * np.abs(w_base[~free] - acc.w0[~free])))
+            self.tau_rhs = acc.tau - t_fix
+            self.t_row = self.dtf[self.va]
+        self.nn = 0 if self.signed else self.n          # number of sign rows -v <= 0
+        hs = [np.zeros(self.nn), self.vub[self.ub_idx],
+              -(acc.lo[fi][self.lo_idx] - acc.w0[fi][self.lo_idx]),
+              acc.hi[fi][self.hi_idx] - acc.w0[fi][self.hi_idx]]
+        if acc.G > 0:
+            hs += [self.band_hi_rhs, self.band_lo_rhs]
+        if self.has_tau:
+            hs += [np.array([self.tau_rhs])]
+        self.h = np.concatenate(hs)
+        self.m = len(self.h)
+        sizes = [self.nn, len(self.ub_idx), len(self.lo_idx), len(self.hi_idx)] + ([acc.G, acc.G] if acc.G > 0 else []) + ([1] if self.has_tau else [])
+        self.off = np.concatenate([[0], np.cumsum(sizes)])
+
+    # ---- operators -------------------------------------------------------------------------
+    def J(self, v):
+        return np.bincount(self.va, weights=self.vs * v, minlength=self.nf)
+
+    def JT(self, x):
+        return self.vs * x[self.va]
+
+    def H_mul(self, v):
+        x = self.J(v)
+        y = self.Bf @ (self.acc.f * (self.Bf.T @ x)) + self.df * x
+        return self.acc.gamma * self.JT(y)
+
+    def G_mul(self, v):
+        x = self.J(v)
+        out = [-v[:self.nn], v[self.ub_idx], -x[self.lo_idx], x[self.hi_idx]]
+        if self.G > 0:
+            gs = np.bincount(self.gid, weights=x, minlength=self.G)
+            out += [gs, -gs]
+        if self.has_tau:
+            out += [np.array([self.t_row @ v])]
+        return np.concatenate(out)
+
+    def _split(self, z):
+        return [z[self.off[i]:self.off[i + 1]] for i in range(len(self.off) - 1)]
+
+    def GT_mul(self, z):
+        parts = self._split(z)
+        out = -parts[0].copy() if self.nn else np.zeros(self.n)
+        np.add.at(out, self.ub_idx, parts[1])
+        xa = np.zeros(self.nf)
+        xa[self.lo_idx] -= parts[2]
+        xa[self.hi_idx] += parts[3]
+        j = 4
+        if self.G > 0:
+            xa += (parts[j] - parts[j + 1])[self.gid]
+            j += 2
+        out += self.JT(xa)
+        if self.has_tau:
+            out += self.t_row * parts[j][0]
+        return out
+
+    def recover(self, v):
+        w = self.w_base.copy()
+        w[self.free] += self.J(v)
+        return w
+
+    # ---- reduced KKT solves: [H + G' Th G, a; a', 0] [dv; dy] = [r1; r2] ----------------------
+    def _theta_parts(self, th):
+        parts = self._split(th)
+        Delta = parts[0].copy() if self.nn else np.zeros(self.n)
+        np.add.at(Delta, self.ub_idx, parts[1])
+        a = self.acc.gamma * self.df
+        a = a.copy()
+        a[self.lo_idx] += parts[2]
+        a[self.hi_idx] += parts[3]
+        j = 4
+        cg = None
+        if self.G > 0:
+            cg = parts[j] + parts[j + 1]; j += 2
+        ct = parts[j][0] if self.has_tau else None
+        return Delta, a, cg, ct
+
+    def dense_matrices(self):
+        """Materialise H, G (for the dense mode and for tests)."""
+        n = self.n
+        Jm = np.zeros((self.nf, n)); Jm[self.va, np.arange(n)] = self.vs
+        Sig = (self.Bf * self.acc.f) @ self.Bf.T + np.diag(self.df)
+        H = self.acc.gamma * Jm.T @ Sig @ Jm
+        rows = [-np.eye(n)[:self.nn], np.eye(n)[self.ub_idx], -Jm[self.lo_idx], Jm[self.hi_idx]]
+        if self.G > 0:
+            E = np.zeros((self.G, self.nf)); E[self.gid, np.arange(self.nf)] = 1.0
+            rows += [E @ Jm, -E @ Jm]
+        if self.has_tau:
+            rows += [self.t_row[None, :]]
+        return H, np.vstack(rows)
+
+    def solver_dense(self):
+        H, Gm = self.dense_matrices()
+        a = self.a_row
+
+        def solve(th, r1, r2):
+            K = H + Gm.T @ (th[:, None] * Gm)
+            n = self.n
+            M = np.zeros((n + 1, n + 1)); M[:n, :n] = K; M[:n, n] = a; M[n, :n] = a
+            sol = np.linalg.solve(M, np.concatenate([r1, [r2]]))
+            return sol[:n], sol[n]
+        return solve
+
+    def solver_structured(self):
+        acc = self.acc
+        a_row = self.a_row
+
+        def solve(th, r1, r2):
+            Delta, a, cg, ct = self._theta_parts(th)
+            # per-asset blocks diag(Delta_vars) + a_i s s' (s = +-1), at most (1+L) x (1+L): solved densely
+            # with pivoting (a Sherman-Morrison form cancels catastrophically when an interior variable has
+            # Delta -> 0 next to an active one with Delta -> inf, which is the normal end state of the IPM)
+            nv = self.nv
+            Dg = np.ones((self.nf, nv)); Dg[self.va, self.vj] = Delta
+            blocks = a[:, None, None] * (self.sg[:, :, None] * self.sg[:, None, :])
+            blocks[:, np.arange(nv), np.arange(nv)] += Dg
+
+            def K0inv(X):
+                Xg = np.zeros((self.nf, nv, X.shape[1])); Xg[self.va, self.vj] = X
+                return np.linalg.solve(blocks, Xg)[self.va, self.vj]
+
+            # factor part gamma (J'B) F (J'B)' by Woodbury (weights gamma f are moderate)
+            YB = self.vs[:, None] * self.Bf[self.va]
+            KYB = K0inv(YB)
+            capB = np.diag(1.0 / (acc.gamma * acc.f)) + YB.T @ KYB
+            capB = 0.5 * (capB + capB.T)
+
+            def K1inv(X):
+                Z = K0inv(X)
+                return Z - KYB @ np.linalg.solve(capB, YB.T @ Z)
+
+            # global rows (budget equality, band rows, turnover row) stay in a bordered system
+            #   [K1 R'; R -W^-1] [dv; dl] = [r1; (r2, 0, .., 0)],  W = theta of the row (budget: W^-1 = 0)
+            # so rows whose theta -> inf turn into equalities without cancellation.
+            rows = [a_row]; winv = [0.0]
+            if self.G > 0:
+                for g in range(self.G):
+                    rows.append(np.where(self.gid[self.va] == g, self.vs, 0.0)); winv.append(1.0 / cg[g])
+            if self.has_tau:
+                rows.append(self.t_row); winv.append(1.0 / ct)
+            R = np.stack(rows, axis=1)                                         # (n, nr)
+            Z = K1inv(np.concatenate([r1[:, None], R], axis=1))
+            z1, ZR = Z[:, 0], Z[:, 1:]
+            Sc = R.T @ ZR + np.diag(winv)
+            rhs = R.T @ z1
+            rhs[0] -= r2
+            dl = np.linalg.solve(0.5 * (Sc + Sc.T), rhs)
+            dv = z1 - ZR @ dl
+            return dv, dl[0]
+        return solve
+
+    def initial_point(self, witness=None):
+        acc = self.acc
+        fi = self.free
+        scale = 1.0 / max(acc.N, 1)
+        if self.signed:
+            return np.zeros(self.n) if witness is None else (witness - self.w_base)[fi].copy()
+        v = np.full(self.n, 0.01 * scale)
+        if witness is not None:
+            delta = (witness - self.w_base)[fi]
+            buy = np.maximum(delta, 0.0)
+            v[: self.nf] += buy
+            sell = np.maximum(-delta, 0.0)
+            # distribute sells over the sell variables of each asset proportionally to their caps
+            sv = np.arange(self.nf, self.n)
+            capv = np.where(np.isfinite(self.vub[sv]), self.vub[sv], 1.0)
+            tot = np.bincount(self.va[sv], weights=capv, minlength=self.nf)
+            v[sv] += sell[self.va[sv]] * capv / np.maximum(tot[self.va[sv]], 1e-300)
+        fin = np.isfinite(self.vub)
+        v[fin] = np.minimum(v[fin], 0.9 * self.vub[fin])
+        return v
+
+
+def solve(acc: Account, mode: str = "auto", witness=None, tol: float = None, max_iter: int = 200,
+          verbose: bool = False):
+    """Mehrotra predictor-corrector on the lifted QP. Returns dict(w, status, iters, mult, v, qp).
+
+    mult: multipliers in the paper's convention: nu (budget), theta (turnover >= 0),
+    lam_hi / lam_lo (bands >= 0), box_lo / box_hi (>= 0, full length N with zeros on substituted assets).
+    """
+    qp = LiftedQP(acc)
+    if mode == "auto":
+        mode = "dense" if qp.n <= 1500 else "structured"
+    kkt = qp.solver_dense() if mode == "dense" else qp.solver_structured()
+    refine = 1 if mode == "dense" else 6
+    if tol is None:
+        tol = 1e-12 if mode == "dense" else 1e-11
+    best = None            # (merit, v, y, s, z, it): fallback when the linear algebra gives out before tol
+    n, m = qp.n, qp.m
+    v = qp.initial_point(witness)
+    cscale = max(1.0, float(np.max(np.abs(qp.c))))
+    hscale = max(1.0 / max(acc.N, 1), 1e-12)
+    s = np.maximum(qp.h - qp.G_mul(v), 1e-2 * hscale)
+    z = np.full(m, cscale)
+    y = 0.0
+    status = "max_iter"
+    it = 0
+    for it in range(1, max_iter + 1):
+        Hv = qp.H_mul(v)
+        r_d = Hv + qp.c + qp.GT_mul(z) + qp.a_row * y
+        r_g = qp.G_mul(v) + s - qp.h
+        r_a = float(qp.a_row @ v) - qp.b_eq
+        mu_c = float(s @ z) / m
+        fval = 0.5 * float(v @ Hv) + float(qp.c @ v)
+        nd = float(np.max(np.abs(r_d))) / cscale
+        ng = float(np.max(np.abs(r_g)))
+        if verbose:
+            print(f"  it {it:3d} rd {nd:.2e} rg {ng:.2e} ra {abs(r_a):.2e} mu {mu_c:.2e} f {fval:.12e}")
+        if nd <= 10 * tol and ng <= tol and abs(r_a) <= tol and mu_c * m <= tol * max(1.0, abs(fval)):
+            status = "optimal"
+            break
+        merit = max(nd / 10, ng, abs(r_a), mu_c * m / max(1.0, abs(fval)))
+        if not np.isfinite(merit):
+            break
+        if best is None or merit < best[0]:
+            best = (merit, v.copy(), y, s.copy(), z.copy(), it)
+        elif it > best[5] + 12:
+            break
+        th = z / s
+
+        def newton(r_c):
+            rhs1 = -r_d - qp.GT_mul((z * r_g - r_c) / s)
+            dv, dy = kkt(th, rhs1, -r_a)
+            # iterative refinement on the reduced system (residual evaluated through the operators)
+            nr = max(float(np.max(np.abs(rhs1))), 1e-300)
+            for _ in range(refine):
+                res1 = rhs1 - (qp.H_mul(dv) + qp.GT_mul(th * qp.G_mul(dv)) + qp.a_row * dy)
+                res2 = -r_a - float(qp.a_row @ dv)
+                if float(np.max(np.abs(res1))) <= 1e-14 * nr:
+                    break
+                ddv, ddy = kkt(th, res1, res2)
+                dv = dv + ddv; dy = dy + ddy
+            ds = -r_g - qp.G_mul(dv)
+            dz = (-r_c - z * ds) / s
+            return dv, dy, ds, dz
+
+        def max_step(x, dx):
+            neg = dx < 0
+            if not np.any(neg):
+                return 1.0
+            return min(1.0, float(np.min(-x[neg] / dx[neg])))
+
+        try:
+            dv_a, dy_a, ds_a, dz_a = newton(s * z)
+        except np.linalg.LinAlgError:
+            break
+        al = min(max_step(s, ds_a), max_step(z, dz_a))
+        mu_aff = float((s + al * ds_a) @ (z + al * dz_a)) / m
+        sigma = max((mu_aff / mu_c) ** 3, 0.03 if mu_c * m < 1e-6 else 0.0)   # do not outrun the linear algebra near the end
+        try:
+            dv, dy, ds, dz = newton(s * z + ds_a * dz_a - sigma * mu_c)
+        except np.linalg.LinAlgError:
+            break
+        al = min(1.0, 0.995 * min(max_step(s, ds) if np.any(ds < 0) else 1e30, max_step(z, dz) if np.any(dz < 0) else 1e30))
+        v = v + al * dv; y = y + al * dy; s = s + al * ds; z = z + al * dz
+    if status != "optimal" and best is not None:
+        # never silent: only an iterate with merit <= max(100 tol, 1e-9) is accepted, else the status says failed
+        merit, v, y, s, z, it_best = best
+        status = "optimal" if merit <= max(100 * tol, 1e-9) else f"failed(merit={merit:.1e})"
+    w = qp.recover(v)
+    # multipliers, paper convention g_i(w) <= 0 with lambda_i >= 0
+    parts = qp._split(z)
+    box_lo = np.zeros(acc.N); box_hi = np.zeros(acc.N)
+    box_lo[qp.free[qp.lo_idx]] = parts[2]; box_hi[qp.free[qp.hi_idx]] = parts[3]
+    j = 4
+    lam_hi = lam_lo = np.zeros(0)
+    if acc.G > 0:
+        lam_hi, lam_lo = parts[j], parts[j + 1]; j += 2
+    theta = float(parts[j][0]) if qp.has_tau else 0.0
+    mult = dict(nu=float(y), theta=theta, lam_hi=lam_hi, lam_lo=lam_lo, box_lo=box_lo, box_hi=box_hi)
+    return dict(w=w, status=status, iters=it, mult=mult, v=v, qp=qp, mode=mode)
+
+
+def solve_instance(inst, accounts=None, mode="auto", **kw):
+    """Solve the listed accounts of an `instances.gen.Instance`; returns (W (len, N), list of result dicts)."""
+    from .problem import account_from_instance
+    accounts = range(inst.A) if accounts is None else accounts
+    W = []; res = []
+    for a in accounts:
+        acc = account_from_instance(inst, a)
+        r = solve(acc, mode=mode, witness=inst.witness[a] if inst.witness is not None else None, **kw)
+        if r["status"] != "optimal":
+            raise RuntimeError(f"oracle IPM did not converge on account {a}: {r['status']} after {r['iters']} iterations")
+        W.append(r["w"]); res.append(r)
+    return np.array(W), res
