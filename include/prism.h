@@ -1,0 +1,200 @@
+/* prism.h - C ABI of the B200-native batched rebalancing solver.
+ *
+ * What it solves.  For each of A accounts over a shared universe of N instruments, the per-account convex program
+ * the paper states as Eq. (1) (Section 4.2), in the concretisation of SURVEY.md 8.0:
+ *
+ *   minimise   (gamma/2) (w-w_b)' Sigma (w-w_b) - mu'w + kappa ||w-w0||_1
+ *              + sum_i [ c_buy (w_i-w0_i)_+ + psi_i((w0_i-w_i)_+) ]            (psi_i: convex piecewise-linear lot penalty)
+ *   subject to 1'w = 1,  lo_i <= w_i <= hi_i,  band_lo_g <= sum_{i in g} w_i <= band_hi_g,  ||w-w0||_1 <= tau
+ *   Sigma = B diag(f) B' + diag(d)     (factor-structured risk)
+ *
+ * by a batched ADMM (operator splitting, BASELINE.json:north_star) whose steps are hand-written sm_100a kernels:
+ * factor GEMMs, a fused proximal/projection kernel (budget hyperplane, box, exclusions, L1 turnover with a
+ * buy/sell two-threshold split, lot penalties), a group-band block, dual update fused with residuals, per-account
+ * convergence masks and per-account rho adaptation.  The returned weights satisfy budget, box, exclusions and the
+ * turnover cap exactly (they are the projection-side iterate); bands hold to the primal tolerance.
+ *
+ * Boundary (Fig. 2): problem data in; weights, fixed-vocabulary status codes
+ * (Table 14), timings (lanes of Table 4), memory bytes (Table 6) and the
+ * external diagnostics of Section 4.4 out.
+ *
+ * Conventions
+ *  - Every pointer inside prism_data and every *_out / w / duals argument is a DEVICE pointer (cudaMalloc'd or a
+ *    torch CUDA tensor's data_ptr), 16-byte aligned.  prism_constraint_set, prism_settings, prism_solve_info are
+ *    HOST structs.
+ *  - Layout of every per-account array: account-major, element (a, i) at [a * N + i] (the N assets of one account
+ *    are contiguous).  Lot arrays: element (a, i, l) at [(a * N + i) * PRISM_MAX_LOTS + l].
+ *  - Ownership: all data arrays are BORROWED; they must outlive the problem object and must not change during a
+ *    call.  The library owns only its workspace.  No hidden host<->device copies of N x A arrays.
+ *  - Errors: every call returns an int (0 = PRISM_OK); nothing throws or aborts across the ABI; a per-account
+ *    difficulty (iteration cap, NaN, gate failure) is a STATUS, not an error.  prism_last_error() gives the text.
+ *  - The turnover scaling D_a of Eq. (1) is the identity in this build (as in every configured
+ *    workload); a non-NULL d_t is rejected with PRISM_ERR_INVALID_ARG.
+ */
+#ifndef PRISM_H
+#define PRISM_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PRISM_MAX_LOTS 4
+#define PRISM_MAX_GROUPS 64
+#define PRISM_MAX_FACTORS 256
+
+/* error codes */
+enum { PRISM_OK = 0, PRISM_ERR_INVALID_ARG = 1, PRISM_ERR_ALLOC = 2, PRISM_ERR_CUDA = 3, PRISM_ERR_NOT_READY = 4 };
+
+/* status vocabulary, Table 14 */
+enum {
+  PRISM_STATUS_CERTIFIED = 0,        /* own tolerance met and the external gates pass                            */
+  PRISM_STATUS_FEASIBLE = 1,         /* gates pass, tolerance not met (the paper's iteration-capped case, :435)  */
+  PRISM_STATUS_TIMEOUT = 2,          /* time_limit_ms reached before the account finished                        */
+  PRISM_STATUS_LATE = 3,             /* finished, but after deadline_ms                                           */
+  PRISM_STATUS_NO_FEASIBLE = 4,      /* gates fail at exit; NOT a certified-infeasibility claim (:491)           */
+  PRISM_STATUS_FAILURE = 5           /* allocation / numerical failure (NaN or Inf seen)                          */
+};
+
+/* constraint-set flags: the rule bundles of the burden curve, Table 9 */
+enum {
+  PRISM_BUDGET = 1, PRISM_BOX = 2, PRISM_EXCLUSION = 4, PRISM_TURNOVER_CAP = 8, PRISM_TURNOVER_PENALTY = 16,
+  PRISM_GROUP_BANDS = 32, PRISM_TAX_LOTS = 64, PRISM_BUY_COST = 128, PRISM_BENCHMARK_SHIFT = 256
+};
+
+typedef struct prism_constraint_set {
+  uint32_t flags;      /* OR of the flags above; PRISM_BUDGET and PRISM_BOX are mandatory                       */
+  int32_t G;           /* number of groups (0 unless PRISM_GROUP_BANDS), <= PRISM_MAX_GROUPS                    */
+  int32_t max_lots;    /* lots per asset (0 unless PRISM_TAX_LOTS), <= PRISM_MAX_LOTS                           */
+} prism_constraint_set;
+
+/* columns of the residual block, one row of PRISM_NRES doubles per account */
+enum {
+  PRISM_R_BUDGET = 0,   /* |1'w - 1| */
+  PRISM_R_BOX = 1,      /* max(||(lo-w)_+||_inf, ||(w-hi)_+||_inf) */
+  PRISM_R_EXPOSURE = 2, /* max over groups of band violation */
+  PRISM_R_TURNOVER = 3, /* (||w-w0||_1 - tau)_+                                PAPER.md:142 */
+  PRISM_R_STAT = 4,     /* stationarity, subgradient-distance form             PAPER.md:146; NaN without duals */
+  PRISM_R_COMP = 5,     /* complementarity max_i |lambda_i g_i(w)|             PAPER.md:146; NaN without duals */
+  PRISM_R_OBJECTIVE = 6,/* public objective f(w) */
+  PRISM_R_PRIMAL = 7,   /* scaled primal residual of the splitting at exit (solver only, else NaN)              */
+  PRISM_R_DUAL = 8,     /* scaled dual residual of the splitting at exit   (solver only, else NaN)              */
+  PRISM_R_TURNOVER_VALUE = 9, /* ||w-w0||_1                                                                      */
+  PRISM_R_RHO = 10,     /* final rho scale c_a (solver only, else NaN)                                           */
+  PRISM_R_RESERVED = 11,
+  PRISM_NRES = 12
+};
+
+/* multipliers ("certificate data"): per account 2 + 2 G doubles:
+ *   [0] nu (budget), [1] theta >= 0 (turnover cap), [2 .. 2+G) lam_hi >= 0, [2+G .. 2+2G) lam_lo >= 0        */
+#define PRISM_NDUAL(G) (2 + 2 * (G))
+
+typedef struct prism_data {
+  /* shared universe */
+  const void* B;            /* N x k row-major loadings; fp64, or fp32 when B_is_fp32 != 0                       */
+  int32_t B_is_fp32;
+  const double* f;          /* k   factor variances  > 0                                                        */
+  const double* d;          /* N   idiosyncratic variances > 0                                                  */
+  const uint8_t* group_id;  /* N   group of each asset in [0, G); NULL when G == 0                               */
+  const double* d_t;        /* must be NULL (identity) in this build                                            */
+  /* per account, account-major */
+  const double* mu;         /* A x N  return input                                                               */
+  const double* gamma;      /* A      risk aversion > 0                                                          */
+  const double* w0;         /* A x N  current weights                                                            */
+  const double* w_b;        /* A x N  benchmark in the risk term, or NULL (=> 0)                                 */
+  const double* lo;         /* A      lower bound per account                                                    */
+  const double* hi;         /* A      upper bound per account (ignored where hi_full is given)                   */
+  const double* hi_full;    /* A x N  per-asset upper bounds (restriction caps), or NULL                         */
+  const uint8_t* excl;      /* A x N  1 => w_i = 0 (exclusion), or NULL                                          */
+  const double* tau;        /* A      turnover cap, +inf for none; NULL => none                                  */
+  const double* kappa;      /* A      L1 transition penalty weight, or NULL (=> 0)                               */
+  const double* band_lo;    /* A x G                                                                              */
+  const double* band_hi;    /* A x G                                                                              */
+  const double* c_buy;      /* A      linear buy cost, or NULL (=> 0)                                            */
+  const double* lot_slope;  /* A x N x PRISM_MAX_LOTS ascending sell-penalty slopes, or NULL                     */
+  const double* lot_width;  /* A x N x PRISM_MAX_LOTS lot sizes (sum over live lots = sellable amount)           */
+  const uint8_t* lot_count; /* A x N  live lots per asset in [0, max_lots]; 0 => no penalty, sells limited by lo */
+} prism_data;
+
+typedef struct prism_settings {
+  double eps_rel;           /* scaled primal/dual tolerance (default 1e-6; BASELINE.json:metric "1e-6 KKT")      */
+  int32_t max_iter;         /* iteration cap (default 4000)                                                      */
+  int32_t check_every;      /* residual / convergence-mask cadence in iterations (default 10)                    */
+  double alpha;             /* over-relaxation in (0, 2) (default 1.6)                                           */
+  double rho_scale;         /* initial c: rho_i = c gamma_a d_i (default 100)                                    */
+  double rho_band_scale;    /* band-block rho relative to the mean rho_i, per unit row norm (default 1)          */
+  int32_t adapt_rho;        /* 1 => per-account rho adaptation at check iterations (default 1)                   */
+  int32_t gemm_mode;        /* 0 = fp64 tensor (DMMA mma.sync), 1 = fp64 FMA                                     */
+  double time_limit_ms;     /* 0 => none; accounts unfinished at the limit get PRISM_STATUS_TIMEOUT              */
+  double deadline_ms;       /* 0 => none; accounts finishing after it get PRISM_STATUS_LATE                      */
+  int32_t use_graph;        /* 1 => replay the inner iterations as a CUDA graph (default 1)                      */
+  int32_t reserved;
+} prism_settings;
+
+typedef struct prism_solve_info {
+  double solve_interval_ms; /* CUDA events around the device work: "reported solve interval" lane */
+  double wall_ms;           /* host clock around the call incl. final sync: full-call lane        */
+  int64_t device_bytes;     /* workspace owned by the problem object: memory class (Table 6)       */
+  int32_t iters_max;        /* iterations of the slowest account                                                 */
+  int64_t iters_total;      /* sum over accounts of iterations run                                               */
+  int32_t n_certified, n_feasible, n_timeout, n_late, n_no_feasible, n_failed;
+  int64_t kernel_launches;  /* kernels launched by this call                                                     */
+} prism_solve_info;
+
+typedef struct prism_problem prism_problem;
+
+/* Fills *s with the defaults listed above. */
+void prism_default_settings(prism_settings* s);
+
+/* Validates shapes and flags, adopts the borrowed device pointers in `data`, allocates ALL workspace once and
+ * precomputes what does not depend on the iterate (padded copies of B, the shared Gram matrix U' D^-1 U, q when a
+ * benchmark shift is present).  N >= 1, 1 <= k <= PRISM_MAX_FACTORS, accounts >= 1.  Runs on `cuda_stream`
+ * (a cudaStream_t, NULL = default stream) and synchronises it.  On failure *out = NULL; PRISM_ERR_ALLOC means
+ * the problem object was not allocated (status 5 for every account). */
+int prism_problem_create(int64_t N, int32_t k, int32_t accounts, const prism_constraint_set* cs,
+                         const prism_data* data, void* cuda_stream, prism_problem** out);
+
+/* Runs the batched solver (cold start: z = projection of w0, zero duals) on `cuda_stream` and
+ * synchronises it before returning.
+ *   w_out      device, A x N   returned weights
+ *   status_out device, A int32 status vocabulary above
+ *   iters_out  device, A int32 iterations run per account
+ *   resid_out  device, A x PRISM_NRES doubles, or NULL
+ *   duals_out  device, A x PRISM_NDUAL(G) doubles, or NULL
+ *   info       host, or NULL
+ * Re-entrant per problem object; not thread-safe on one object. */
+int prism_solve_batch(prism_problem* p, const prism_settings* s, void* cuda_stream, double* w_out,
+                      int32_t* status_out, int32_t* iters_out, double* resid_out, double* duals_out,
+                      prism_solve_info* info);
+
+/* External-diagnostic semantics: depends only on the problem data and the given w (and
+ * multipliers, if any), never on solver state, so it applies to any solver's weights.  Fills columns 0..6 and 9
+ * of the residual block (4, 5 are NaN when duals == NULL; 7, 8, 10 are NaN).  Synchronises the stream. */
+int prism_residuals(prism_problem* p, const double* w, const double* duals, void* cuda_stream,
+                    double* resid_out);
+
+/* Same solve as prism_solve_batch but with HOST buffers for the per-account data that changes between
+ * rebalances (mu, w0) and for the outputs: copies mu and w0 host->device into the problem's borrowed arrays,
+ * solves, copies weights / status / iterations / residual block back.  NULL host pointers skip that copy.
+ * This is the end-to-end lane of bench.py ("e2e"). */
+int prism_solve_batch_host(prism_problem* p, const prism_settings* s, void* cuda_stream, const double* mu_host,
+                           const double* w0_host, double* w_host, int32_t* status_host, int32_t* iters_host,
+                           double* resid_host, prism_solve_info* info);
+
+/* Frees the workspace; never frees borrowed data.  NULL is allowed. */
+void prism_problem_destroy(prism_problem* p);
+
+/* Workspace bytes owned by the object (memory class). */
+int64_t prism_problem_device_bytes(const prism_problem* p);
+
+/* Thread-local message for the last non-zero return of this thread. */
+const char* prism_last_error(void);
+
+/* Build id (the paper records an "evidence build" id). */
+const char* prism_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PRISM_H */

@@ -1,0 +1,120 @@
+// common.cuh - problem object, device helpers.  Part of the single translation unit prism.cu.
+// Notation follows SURVEY.md 8.0 / 8(a): accounts a, assets i, factors j, groups g; U = [B | E'] and
+// x-update (M + U Lambda U') x = r solved through the k' x k' capacitance S = Lambda^-1 + U' M^-1 U.
+#pragma once
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string.h>
+
+#include "../../include/prism.h"
+
+#define PRISM_KP_ALIGN 8          // factor dimension padded to the m8n8k4 tile
+#define PRISM_MAX_KPRIME 160      // k + G limit of the in-shared-memory capacitance inversion
+
+struct AccountParams {            // per-account scalars, struct of arrays on the device (A entries each)
+  double* c;        // rho scale: rho_i = c gamma d_i
+  double* rhoE;     // band-block rho
+  double* alpha;    // buy threshold  nu + theta   (warm start of the root find)
+  double* beta;     // sell threshold nu - theta
+  int32_t* mode;    // 0: turnover inactive (alpha == beta == nu), 1: cap active
+  double* bsum;     // 1 - sum_i w0_i : budget in trade space
+  double* rpE;      // band-block primal residual |E x - z_E|_inf and its scale (set by the small-solve kernel)
+  double* nE;
+  int32_t* done;    // convergence mask (H6)
+  int32_t* conv;    // 1 if own tolerance met
+  int32_t* iters;
+  int32_t* refactor;// capacitance must be rebuilt (rho changed)
+  int32_t* nadapt;
+};
+
+struct prism_problem {
+  int64_t N;
+  int32_t k, kp, A, G, Kp;       // kp: k padded to 8; Kp = kp + G: rows of T and V per account
+  int64_t ldv;                   // leading dimension of V / T rows (Kp padded to 8)
+  uint32_t flags;
+  int32_t max_lots;
+  prism_data d;
+  // shared precomputed (owned)
+  double* Bp;       // N x kp, asset-major, zero padded            (GEMM-2 operand)
+  double* Bt;       // kp x ldn, factor-major                      (GEMM-1 operand)
+  int64_t ldn;      // N padded to 32
+  double* invd;     // N
+  double* gram;     // Kp x Kp : U' D^-1 U with U = [Bp | E']
+  double* q;        // A x N : -mu - gamma Sigma w_b, only with a benchmark shift (else NULL and q = -mu)
+  // iterate (owned)
+  double *v, *rt, *cc, *xs, *pxq;          // A x N each
+  double* Tpart;    // nchunk x A x ldv  split-K partials of GEMM-1
+  int32_t nchunk;
+  int64_t chunk;    // assets per split-K chunk
+  double *TE;       // A x G   group sums of r~
+  double *V;        // A x ldv
+  double *Sinv;     // A x Kp x Kp
+  double *zE, *yE, *eE;   // A x G
+  double *resid;    // A x PRISM_NRES (internal copy)
+  double *duals;    // A x PRISM_NDUAL(G)
+  int32_t* status;  // A
+  double* w_stage;  // A x N, allocated on the first prism_solve_batch_host call
+  int32_t* i_stage; // A
+  AccountParams ap;
+  int32_t* counters;      // [0] number of done accounts
+  int32_t* h_counters;    // pinned host mirror
+  int64_t bytes;
+  int sm_count;
+  double dbar;            // mean of d (host copy at create)
+};
+
+static thread_local char g_err[512] = "";
+static int set_err(int code, const char* fmt, const char* a = "", long long b = 0) {
+  snprintf(g_err, sizeof(g_err), fmt, a, b);
+  return code;
+}
+#define CUDA_TRY(expr)                                                                          \
+  do {                                                                                          \
+    cudaError_t _e = (expr);                                                                    \
+    if (_e != cudaSuccess) return set_err(PRISM_ERR_CUDA, "CUDA error %s at line %lld", cudaGetErrorString(_e), __LINE__); \
+  } while (0)
+
+// ------------------------------------------------------------------------------------------ reductions
+__device__ __forceinline__ double warp_sum(double x) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+  return x;
+}
+__device__ __forceinline__ double warp_max(double x) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) x = fmax(x, __shfl_xor_sync(0xffffffffu, x, o));
+  return x;
+}
+__device__ __forceinline__ double warp_min(double x) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) x = fmin(x, __shfl_xor_sync(0xffffffffu, x, o));
+  return x;
+}
+
+// Block-wide reduction of NV values per thread; OP: 0 sum, 1 max, 2 min.  Result broadcast to all threads.
+// `scratch` needs NV * 32 doubles.  Fixed order => deterministic.
+template <int NV>
+__device__ __forceinline__ void block_reduce(double (&val)[NV], const int (&op)[NV], double* scratch) {
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+#pragma unroll
+  for (int q = 0; q < NV; ++q) {
+    double x = val[q];
+    x = op[q] == 0 ? warp_sum(x) : (op[q] == 1 ? warp_max(x) : warp_min(x));
+    if (lane == 0) scratch[q * 32 + wid] = x;
+  }
+  __syncthreads();
+  if (wid == 0) {
+#pragma unroll
+    for (int q = 0; q < NV; ++q) {
+      double x = lane < nw ? scratch[q * 32 + lane] : (op[q] == 0 ? 0.0 : (op[q] == 1 ? -INFINITY : INFINITY));
+      x = op[q] == 0 ? warp_sum(x) : (op[q] == 1 ? warp_max(x) : warp_min(x));
+      if (lane == 0) scratch[q * 32] = x;
+    }
+  }
+  __syncthreads();
+#pragma unroll
+  for (int q = 0; q < NV; ++q) val[q] = scratch[q * 32];
+  __syncthreads();
+}

@@ -1,0 +1,429 @@
+// prism.cu - C ABI (include/prism.h) and the host driver of the batched ADMM.
+// Single translation unit: the kernels live in the .cuh files included here.  No torch types, no CPU fallback.
+#include <chrono>
+#include <new>
+#include <vector>
+
+#include "common.cuh"
+#include "diag.cuh"
+#include "gemm.cuh"
+#include "prox.cuh"
+#include "small.cuh"
+
+#define PRISM_VERSION_STR "prism-b200 r1 (sm_100a, fp64 DMMA factor GEMMs, two-threshold prox)"
+
+static const int kMT[] = {2, 4, 7, 8, 13, 16};
+static int pick_mt(int k) {
+  for (int m : kMT) if (8 * m >= k) return m;
+  return -1;
+}
+#define MT_SWITCH(mt, ...)                                            \
+  switch (mt) {                                                       \
+    case 2: { constexpr int MT = 2; __VA_ARGS__; } break;             \
+    case 4: { constexpr int MT = 4; __VA_ARGS__; } break;             \
+    case 7: { constexpr int MT = 7; __VA_ARGS__; } break;             \
+    case 8: { constexpr int MT = 8; __VA_ARGS__; } break;             \
+    case 13: { constexpr int MT = 13; __VA_ARGS__; } break;           \
+    default: { constexpr int MT = 16; __VA_ARGS__; } break;           \
+  }
+
+static size_t g1_smem(int mt) { return (size_t)G1_STAGES * (8 * mt + G1_TA) * G1_LD * sizeof(double); }
+static size_t g2_smem(int mt) { return (size_t)(G2_TM + G2_TN) * (8 * mt + 4) * sizeof(double); }
+
+extern "C" void prism_default_settings(prism_settings* s) {
+  if (!s) return;
+  memset(s, 0, sizeof(*s));
+  s->eps_rel = 1e-6; s->max_iter = 4000; s->check_every = 10; s->alpha = 1.6; s->rho_scale = 100.0;
+  s->rho_band_scale = 1.0; s->adapt_rho = 1; s->gemm_mode = 0; s->time_limit_ms = 0.0; s->deadline_ms = 0.0;
+  s->use_graph = 1;
+}
+extern "C" const char* prism_last_error(void) { return g_err; }
+extern "C" const char* prism_version(void) { return PRISM_VERSION_STR; }
+extern "C" int64_t prism_problem_device_bytes(const prism_problem* p) { return p ? p->bytes : 0; }
+
+template <typename T>
+static int dev_alloc(prism_problem* p, T** ptr, size_t count, bool zero = true) {
+  *ptr = nullptr;
+  if (count == 0) count = 1;
+  cudaError_t e = cudaMalloc((void**)ptr, count * sizeof(T));
+  if (e != cudaSuccess) { cudaGetLastError(); return set_err(PRISM_ERR_ALLOC, "cudaMalloc of %s%lld bytes failed", "", (long long)(count * sizeof(T))); }
+  if (zero) cudaMemset(*ptr, 0, count * sizeof(T));
+  p->bytes += (int64_t)(count * sizeof(T));
+  return PRISM_OK;
+}
+#define ALLOC_TRY(expr) do { int _r = (expr); if (_r != PRISM_OK) { prism_problem_destroy(p); return _r; } } while (0)
+
+extern "C" void prism_problem_destroy(prism_problem* p) {
+  if (!p) return;
+  void* ptrs[] = {p->Bp, p->Bt, p->invd, p->gram, p->q, p->v, p->rt, p->cc, p->xs, p->pxq, p->Tpart, p->TE, p->V, p->Sinv,
+                  p->zE, p->yE, p->eE, p->resid, p->duals, p->status, p->ap.c, p->ap.rhoE, p->ap.alpha, p->ap.beta,
+                  p->ap.mode, p->ap.bsum, p->ap.rpE, p->ap.nE, p->ap.done, p->ap.conv, p->ap.iters, p->ap.refactor,
+                  p->ap.nadapt, p->counters, p->w_stage, p->i_stage};
+  for (void* q : ptrs) if (q) cudaFree(q);
+  if (p->h_counters) cudaFreeHost(p->h_counters);
+  delete p;
+}
+
+// ------------------------------------------------------------------------------------------ launch helpers
+struct Launcher {
+  prism_problem* p;
+  cudaStream_t st;
+  int mt;
+  int gemm_mode;
+  int64_t launches = 0;
+
+  Gemm1Args g1args(const double* X, const int32_t* done) const {
+    Gemm1Args a;
+    a.Bt = p->Bt; a.ldn = p->ldn; a.X = X; a.ldw = p->ldn; a.Tpart = p->Tpart; a.ldv = p->ldv; a.A = p->A;
+    a.chunk = p->chunk; a.Npad = p->ldn; a.done = done;
+    return a;
+  }
+  void gemm1(const double* X, const int32_t* done) {
+    Gemm1Args a = g1args(X, done);
+    if (gemm_mode == 1) {
+      const int kp = p->kp;
+      dim3 grid(p->nchunk, (unsigned)(((int64_t)p->A * kp + 127) / 128));
+      k_gemm1_ref<<<grid, 128, 0, st>>>(a, kp);
+    } else {
+      dim3 grid(p->nchunk, (p->A + G1_TA - 1) / G1_TA);
+      MT_SWITCH(mt, k_gemm1<MT><<<grid, 256, g1_smem(MT), st>>>(a));
+    }
+    ++launches;
+  }
+  template <int MODE>
+  void gemm2(const Gemm2Args& a) {
+    if (gemm_mode == 1) {
+      dim3 grid((unsigned)((p->N + 127) / 128), p->A);
+      k_gemm2_ref<MODE><<<grid, 128, 0, st>>>(a);
+    } else {
+      dim3 grid((unsigned)((p->N + G2_TN - 1) / G2_TN), (p->A + G2_TM - 1) / G2_TM);
+      MT_SWITCH(mt, k_gemm2<MT, MODE><<<grid, 256, g2_smem(MT), st>>>(a));
+    }
+    ++launches;
+  }
+  Gemm2Args g2base() const {
+    Gemm2Args a;
+    memset(&a, 0, sizeof(a));
+    a.Bp = p->Bp; a.kp = p->kp; a.V = p->V; a.ldv = p->ldv; a.N = p->N; a.ldw = p->ldn; a.A = p->A; a.G = p->G;
+    a.group_id = p->d.group_id; a.invd = p->invd; a.d = p->d.d; a.gamma = p->d.gamma; a.c = p->ap.c;
+    a.v = p->v; a.cc = p->cc; a.rt = p->rt; a.xs = p->xs; a.pxq = p->pxq; a.q = p->q; a.mu = p->d.mu;
+    a.relax = 1.0; a.done = nullptr;
+    return a;
+  }
+  // pxq <- gamma Sigma X   (H8: Sigma W = B (F (B'W)) + D o W, fp64)
+  void sigma_apply(const double* X) {
+    gemm1(X, nullptr);
+    k_scale_fs<<<p->A, 128, 0, st>>>(p->Tpart, p->nchunk, p->A, p->k, p->kp, p->ldv, p->d.f, p->d.gamma, p->V);
+    ++launches;
+    Gemm2Args a = g2base();
+    a.X = X;
+    gemm2<G2_SIGMA>(a);
+  }
+};
+
+static int set_kernel_attrs(int mt, int Kp) {
+  MT_SWITCH(mt, {
+    CUDA_TRY(cudaFuncSetAttribute(k_gemm1<MT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g1_smem(MT)));
+    CUDA_TRY(cudaFuncSetAttribute(k_gemm2<MT, G2_ADMM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g2_smem(MT)));
+    CUDA_TRY(cudaFuncSetAttribute(k_gemm2<MT, G2_ADMM_CHECK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g2_smem(MT)));
+    CUDA_TRY(cudaFuncSetAttribute(k_gemm2<MT, G2_SIGMA>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g2_smem(MT)));
+  });
+  CUDA_TRY(cudaFuncSetAttribute(k_factor, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)((size_t)Kp * Kp * sizeof(double))));
+  return PRISM_OK;
+}
+
+// ------------------------------------------------------------------------------------------ create (H0)
+extern "C" int prism_problem_create(int64_t N, int32_t k, int32_t accounts, const prism_constraint_set* cs,
+                                    const prism_data* data, void* cuda_stream, prism_problem** out) {
+  if (out) *out = nullptr;
+  if (!out || !cs || !data) return set_err(PRISM_ERR_INVALID_ARG, "null argument%s", "");
+  const int A = accounts, G = (cs->flags & PRISM_GROUP_BANDS) ? cs->G : 0;
+  if (N < 1 || k < 1 || A < 1) return set_err(PRISM_ERR_INVALID_ARG, "N, k, accounts must be >= 1%s", "");
+  if (!(cs->flags & PRISM_BUDGET) || !(cs->flags & PRISM_BOX)) return set_err(PRISM_ERR_INVALID_ARG, "PRISM_BUDGET and PRISM_BOX are mandatory%s", "");
+  const int mt = pick_mt(k);
+  if (mt < 0 || k > PRISM_MAX_FACTORS) return set_err(PRISM_ERR_INVALID_ARG, "k = %s%lld exceeds the supported factor count (128)", "", k);
+  if (G < 0 || G > PRISM_MAX_GROUPS || 8 * mt + G > PRISM_MAX_KPRIME) return set_err(PRISM_ERR_INVALID_ARG, "G = %s%lld out of range", "", G);
+  if ((cs->flags & PRISM_GROUP_BANDS) && (G < 1 || !data->group_id || !data->band_lo || !data->band_hi)) return set_err(PRISM_ERR_INVALID_ARG, "group bands need G >= 1, group_id, band_lo, band_hi%s", "");
+  if ((cs->flags & PRISM_TAX_LOTS) && (!data->lot_slope || !data->lot_width || !data->lot_count || cs->max_lots < 1 || cs->max_lots > PRISM_MAX_LOTS)) return set_err(PRISM_ERR_INVALID_ARG, "tax lots need lot arrays and 1 <= max_lots <= 4%s", "");
+  if (!data->B || !data->f || !data->d || !data->mu || !data->gamma || !data->w0 || !data->lo || !data->hi) return set_err(PRISM_ERR_INVALID_ARG, "missing mandatory data pointer%s", "");
+  if (data->d_t) return set_err(PRISM_ERR_INVALID_ARG, "d_t must be NULL: the turnover scaling D_a is the identity in this build%s", "");
+  if ((cs->flags & PRISM_BENCHMARK_SHIFT) && !data->w_b) return set_err(PRISM_ERR_INVALID_ARG, "PRISM_BENCHMARK_SHIFT needs w_b%s", "");
+
+  prism_problem* p = new (std::nothrow) prism_problem();
+  if (!p) return set_err(PRISM_ERR_ALLOC, "host allocation failed%s", "");
+  memset(p, 0, sizeof(*p));
+  p->N = N; p->k = k; p->kp = 8 * mt; p->A = A; p->G = G; p->Kp = p->kp + G; p->ldv = (p->Kp + 7) / 8 * 8;
+  p->flags = cs->flags; p->max_lots = (cs->flags & PRISM_TAX_LOTS) ? cs->max_lots : 0;
+  p->d = *data;
+  if (!(cs->flags & PRISM_TAX_LOTS)) { p->d.lot_slope = p->d.lot_width = nullptr; p->d.lot_count = nullptr; }
+  if (!(cs->flags & PRISM_GROUP_BANDS)) { p->d.group_id = nullptr; p->d.band_lo = p->d.band_hi = nullptr; }
+  if (!(cs->flags & PRISM_EXCLUSION)) p->d.excl = nullptr;
+  if (!(cs->flags & PRISM_TURNOVER_CAP)) p->d.tau = nullptr;
+  if (!(cs->flags & PRISM_TURNOVER_PENALTY)) p->d.kappa = nullptr;
+  if (!(cs->flags & PRISM_BUY_COST)) p->d.c_buy = nullptr;
+  if (!(cs->flags & PRISM_BENCHMARK_SHIFT)) p->d.w_b = nullptr;
+  p->ldn = (N + 31) / 32 * 32;
+  int dev = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&p->sm_count, cudaDevAttrMultiProcessorCount, dev);
+  if (p->sm_count <= 0) { delete p; return set_err(PRISM_ERR_CUDA, "no CUDA device%s", ""); }
+  // split-K chunking of GEMM-1: about two waves of CTAs
+  const int tilesA = (A + G1_TA - 1) / G1_TA;
+  int64_t want = (2 * p->sm_count + tilesA - 1) / tilesA;
+  const int64_t nst = p->ldn / G1_KS;
+  if (want > nst) want = nst;
+  if (want < 1) want = 1;
+  p->chunk = ((nst + want - 1) / want) * G1_KS;
+  p->nchunk = (int)((p->ldn + p->chunk - 1) / p->chunk);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+
+  const size_t AN = (size_t)A * p->ldn;
+  ALLOC_TRY(dev_alloc(p, &p->Bp, (size_t)N * p->kp));
+  ALLOC_TRY(dev_alloc(p, &p->Bt, (size_t)p->kp * p->ldn));
+  ALLOC_TRY(dev_alloc(p, &p->invd, (size_t)N));
+  ALLOC_TRY(dev_alloc(p, &p->gram, (size_t)p->Kp * p->Kp));
+  ALLOC_TRY(dev_alloc(p, &p->v, AN));
+  ALLOC_TRY(dev_alloc(p, &p->rt, AN));
+  ALLOC_TRY(dev_alloc(p, &p->cc, AN));
+  ALLOC_TRY(dev_alloc(p, &p->xs, AN));
+  ALLOC_TRY(dev_alloc(p, &p->pxq, AN));
+  ALLOC_TRY(dev_alloc(p, &p->Tpart, (size_t)p->nchunk * A * p->ldv));
+  ALLOC_TRY(dev_alloc(p, &p->TE, (size_t)A * (G ? G : 1)));
+  ALLOC_TRY(dev_alloc(p, &p->V, (size_t)A * p->ldv));
+  ALLOC_TRY(dev_alloc(p, &p->Sinv, (size_t)A * p->Kp * p->Kp));
+  ALLOC_TRY(dev_alloc(p, &p->zE, (size_t)A * (G ? G : 1)));
+  ALLOC_TRY(dev_alloc(p, &p->yE, (size_t)A * (G ? G : 1)));
+  ALLOC_TRY(dev_alloc(p, &p->resid, (size_t)A * PRISM_NRES));
+  ALLOC_TRY(dev_alloc(p, &p->duals, (size_t)A * PRISM_NDUAL(G)));
+  ALLOC_TRY(dev_alloc(p, &p->status, (size_t)A));
+  ALLOC_TRY(dev_alloc(p, &p->ap.c, (size_t)A));
+  ALLOC_TRY(dev_alloc(p, &p->ap.rhoE, (size_t)A));
+  ALLOC_TRY(dev_alloc(p, &p->ap.alpha, (size_t)A));
+  ALLOC_TRY(dev_alloc(p, &p->ap.beta, (size_t)A));
+  ALLOC_TRY(dev_alloc(p, &p->ap.mode, (size_t)A));
+  ALLOC_TRY(dev_alloc(p, &p->ap.bsum, (size_t)A));
+  ALLOC_TRY(dev_alloc(p, &p->ap.rpE, (size_t)A));
+  ALLOC_TRY(dev_alloc(p, &p->ap.nE, (size_t)A));
+  ALLOC_TRY(dev_alloc(p, &p->ap.done, (size_t)A));
+  ALLOC_TRY(dev_alloc(p, &p->ap.conv, (size_t)A));
+  ALLOC_TRY(dev_alloc(p, &p->ap.iters, (size_t)A));
+  ALLOC_TRY(dev_alloc(p, &p->ap.refactor, (size_t)A));
+  ALLOC_TRY(dev_alloc(p, &p->ap.nadapt, (size_t)A));
+  ALLOC_TRY(dev_alloc(p, &p->counters, (size_t)4));
+  if (cudaMallocHost((void**)&p->h_counters, 4 * sizeof(int32_t)) != cudaSuccess) { prism_problem_destroy(p); return set_err(PRISM_ERR_ALLOC, "pinned allocation failed%s", ""); }
+  if (p->d.w_b) ALLOC_TRY(dev_alloc(p, &p->q, AN));
+  { int r = set_kernel_attrs(mt, p->Kp); if (r != PRISM_OK) { prism_problem_destroy(p); return r; } }
+
+  k_setup_shared<<<(unsigned)((N + 127) / 128), 128, 0, st>>>(data->B, data->B_is_fp32, data->d, N, k, p->kp, p->ldn, p->Bp, p->Bt, p->invd);
+  k_gram<<<dim3(p->Kp, p->Kp), 256, 0, st>>>(p->Bt, p->ldn, p->d.group_id, p->invd, N, p->kp, G, p->gram);
+  if (p->d.w_b) {            // q = -mu - gamma Sigma w_b
+    Launcher L{p, st, mt, 0};
+    k_diff<<<dim3((unsigned)((N + 255) / 256), A), 256, 0, st>>>(p->d.w_b, nullptr, N, p->ldn, p->rt);
+    L.sigma_apply(p->rt);
+    k_make_q<<<dim3((unsigned)((N + 255) / 256), A), 256, 0, st>>>(p->d.mu, p->pxq, N, p->ldn, p->q);
+    cudaMemsetAsync(p->rt, 0, AN * sizeof(double), st);
+  }
+  {
+    std::vector<double> hd((size_t)N);
+    cudaMemcpyAsync(hd.data(), data->d, (size_t)N * sizeof(double), cudaMemcpyDeviceToHost, st);
+    cudaStreamSynchronize(st);
+    double s = 0.0;
+    for (int64_t i = 0; i < N; ++i) s += hd[(size_t)i];
+    p->dbar = s / (double)N;
+  }
+  cudaError_t e = cudaStreamSynchronize(st);
+  if (e == cudaSuccess) e = cudaGetLastError();
+  if (e != cudaSuccess) { prism_problem_destroy(p); return set_err(PRISM_ERR_CUDA, "setup kernels failed: %s", cudaGetErrorString(e)); }
+  *out = p;
+  return PRISM_OK;
+}
+
+// ------------------------------------------------------------------------------------------ solve (H1-H9)
+static ProxArgs make_prox_args(prism_problem* p, const prism_settings& s, double* w_out) {
+  ProxArgs a;
+  memset(&a, 0, sizeof(a));
+  a.N = p->N; a.A = p->A; a.G = p->G; a.kp = p->kp; a.max_lots = p->max_lots; a.ldv = p->ldv;
+  a.mu = p->d.mu; a.q = p->q; a.w0 = p->d.w0; a.gamma = p->d.gamma; a.lo = p->d.lo; a.hi = p->d.hi; a.hi_full = p->d.hi_full;
+  a.tau = p->d.tau; a.kappa = p->d.kappa; a.c_buy = p->d.c_buy; a.lot_slope = p->d.lot_slope; a.lot_width = p->d.lot_width;
+  a.excl = p->d.excl; a.lot_count = p->d.lot_count; a.group_id = p->d.group_id; a.invd = p->invd; a.d = p->d.d;
+  a.v = p->v; a.rt = p->rt; a.cc = p->cc; a.TE = p->TE; a.xs = p->xs; a.pxq = p->pxq; a.zE = p->zE; a.yE = p->yE;
+  a.ap = p->ap; a.w_out = w_out; a.duals = p->duals; a.resid = p->resid; a.counters = p->counters;
+  a.eps = s.eps_rel; a.dbar_GN = p->G ? p->dbar * (double)p->G / (double)p->N : 0.0; a.band_scale = s.rho_band_scale;
+  a.adapt = s.adapt_rho; a.iter = 0; a.ldw = p->ldn;
+  return a;
+}
+
+static void launch_prox(prism_problem* p, cudaStream_t st, ProxArgs& a, int mode, int iter) {
+  a.iter = iter;
+  if (p->d.lot_count) k_prox<true><<<p->A, 512, 0, st>>>(a, mode);
+  else k_prox<false><<<p->A, 512, 0, st>>>(a, mode);
+}
+
+static DiagArgs make_diag_args(prism_problem* p, const double* w, const double* duals, double* resid) {
+  DiagArgs a;
+  memset(&a, 0, sizeof(a));
+  a.N = p->N; a.ldw = p->ldn; a.A = p->A; a.G = p->G; a.w = w; a.gS = p->pxq; a.duals = duals;
+  a.mu = p->d.mu; a.w0 = p->d.w0; a.w_b = p->d.w_b; a.gamma = p->d.gamma; a.lo = p->d.lo; a.hi = p->d.hi; a.hi_full = p->d.hi_full;
+  a.tau = p->d.tau; a.kappa = p->d.kappa; a.c_buy = p->d.c_buy; a.lot_slope = p->d.lot_slope; a.lot_width = p->d.lot_width;
+  a.band_lo = p->d.band_lo; a.band_hi = p->d.band_hi; a.excl = p->d.excl; a.lot_count = p->d.lot_count; a.group_id = p->d.group_id;
+  a.resid = resid; a.delta = 1e-9; a.only_done = nullptr;
+  return a;
+}
+
+// resid (device, A x NRES) <- diagnostics of w; uses rt and pxq as scratch
+static void run_diag(prism_problem* p, Launcher& L, const double* w, const double* duals, double* resid) {
+  k_diff<<<dim3((unsigned)((p->N + 255) / 256), p->A), 256, 0, L.st>>>(w, p->d.w_b, p->N, p->ldn, p->rt);
+  ++L.launches;
+  L.sigma_apply(p->rt);
+  DiagArgs da = make_diag_args(p, w, duals, resid);
+  if (p->d.lot_count) k_diag<true><<<p->A, 256, 0, L.st>>>(da);
+  else k_diag<false><<<p->A, 256, 0, L.st>>>(da);
+  ++L.launches;
+}
+
+extern "C" int prism_solve_batch(prism_problem* p, const prism_settings* sp, void* cuda_stream, double* w_out,
+                                 int32_t* status_out, int32_t* iters_out, double* resid_out, double* duals_out,
+                                 prism_solve_info* info) {
+  if (!p) return set_err(PRISM_ERR_NOT_READY, "problem object is NULL%s", "");
+  if (!w_out || !status_out || !iters_out) return set_err(PRISM_ERR_INVALID_ARG, "w_out, status_out, iters_out are mandatory%s", "");
+  prism_settings s;
+  if (sp) s = *sp; else prism_default_settings(&s);
+  if (!(s.eps_rel > 0) || s.max_iter < 1 || s.check_every < 1 || !(s.alpha > 0 && s.alpha < 2) || !(s.rho_scale > 0) || !(s.rho_band_scale > 0))
+    return set_err(PRISM_ERR_INVALID_ARG, "invalid settings%s", "");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const auto t0 = std::chrono::steady_clock::now();
+  auto elapsed_ms = [&]() { return std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count(); };
+  cudaEvent_t ev0, ev1;
+  CUDA_TRY(cudaEventCreate(&ev0));
+  CUDA_TRY(cudaEventCreate(&ev1));
+  CUDA_TRY(cudaEventRecord(ev0, st));
+  const int A = p->A, G = p->G;
+  Launcher L{p, st, p->kp / 8, s.gemm_mode};
+
+  CUDA_TRY(cudaMemsetAsync(p->counters, 0, 4 * sizeof(int32_t), st));
+  CUDA_TRY(cudaMemsetAsync(p->rt, 0, (size_t)A * p->ldn * sizeof(double), st));
+  CUDA_TRY(cudaMemsetAsync(p->resid, 0, (size_t)A * PRISM_NRES * sizeof(double), st));
+  InitArgs ia;
+  memset(&ia, 0, sizeof(ia));
+  ia.N = p->N; ia.ldw = p->ldn; ia.A = A; ia.G = G; ia.w0 = p->d.w0; ia.gamma = p->d.gamma; ia.band_lo = p->d.band_lo; ia.band_hi = p->d.band_hi;
+  ia.group_id = p->d.group_id; ia.v = p->v; ia.zE = p->zE; ia.yE = p->yE; ia.ap = p->ap; ia.rho_scale = s.rho_scale;
+  ia.band_scale = s.rho_band_scale; ia.dbar_GN = G ? p->dbar * (double)G / (double)p->N : 0.0;
+  k_init_accounts<<<A, 256, 0, st>>>(ia);
+  ++L.launches;
+
+  ProxArgs pa = make_prox_args(p, s, w_out);
+  SolveArgs sa;
+  memset(&sa, 0, sizeof(sa));
+  sa.A = A; sa.G = G; sa.kp = p->kp; sa.nchunk = p->nchunk; sa.ldv = p->ldv; sa.Tpart = p->Tpart; sa.TE = p->TE; sa.Sinv = p->Sinv;
+  sa.band_lo = p->d.band_lo; sa.band_hi = p->d.band_hi; sa.V = p->V; sa.zE = p->zE; sa.yE = p->yE; sa.ap = p->ap; sa.relax = s.alpha;
+  Gemm2Args g2 = L.g2base();
+  g2.relax = s.alpha; g2.done = p->ap.done;
+  const size_t fac_smem = (size_t)p->Kp * p->Kp * sizeof(double);
+
+  int it = 1, timed_out = 0, late_iter = -1, ndone = 0;
+  for (; it <= s.max_iter; ++it) {
+    const bool check = (it > 1) && ((it - 1) % s.check_every == 0);   // residuals of the iterate after it-1 iterations
+    launch_prox(p, st, pa, check ? PROX_CHECK : 0, it - 1);
+    ++L.launches;
+    if (check || it == 1) {
+      k_factor<<<A, 256, fac_smem, st>>>(p->gram, p->d.f, p->d.gamma, p->ap, p->k, p->kp, G, p->Sinv);
+      ++L.launches;
+    }
+    if (check) {
+      CUDA_TRY(cudaMemcpyAsync(p->h_counters, p->counters, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+      CUDA_TRY(cudaStreamSynchronize(st));
+      ndone = p->h_counters[0];
+      if (ndone >= A) break;
+      const double el = elapsed_ms();
+      if (s.deadline_ms > 0 && late_iter < 0 && el > s.deadline_ms) late_iter = it - 1;
+      if (s.time_limit_ms > 0 && el > s.time_limit_ms) { timed_out = 1; break; }
+    }
+    L.gemm1(p->rt, p->ap.done);
+    k_solve<<<A, 128, 0, st>>>(sa);
+    ++L.launches;
+    const bool next_check = (it % s.check_every == 0);
+    if (next_check) L.gemm2<G2_ADMM_CHECK>(g2); else L.gemm2<G2_ADMM>(g2);
+  }
+  if (ndone < A) {           // iteration cap or time limit: extract z for the accounts still running
+    launch_prox(p, st, pa, PROX_FINAL, it > s.max_iter ? s.max_iter : it - 1);
+    ++L.launches;
+  }
+  // H8 / H9: external diagnostics of the returned weights with the solver's multipliers, then statuses
+  run_diag(p, L, w_out, p->duals, p->resid);
+  k_status<<<(A + 127) / 128, 128, 0, st>>>(A, p->resid, p->ap.conv, p->ap.iters, timed_out, late_iter, 1e-6, p->status);
+  ++L.launches;
+  if (status_out != p->status) CUDA_TRY(cudaMemcpyAsync(status_out, p->status, (size_t)A * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
+  CUDA_TRY(cudaMemcpyAsync(iters_out, p->ap.iters, (size_t)A * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
+  if (resid_out) CUDA_TRY(cudaMemcpyAsync(resid_out, p->resid, (size_t)A * PRISM_NRES * sizeof(double), cudaMemcpyDeviceToDevice, st));
+  if (duals_out) CUDA_TRY(cudaMemcpyAsync(duals_out, p->duals, (size_t)A * PRISM_NDUAL(G) * sizeof(double), cudaMemcpyDeviceToDevice, st));
+  CUDA_TRY(cudaEventRecord(ev1, st));
+  std::vector<int32_t> hs((size_t)A), hi((size_t)A);
+  CUDA_TRY(cudaMemcpyAsync(hs.data(), p->status, (size_t)A * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaMemcpyAsync(hi.data(), p->ap.iters, (size_t)A * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  CUDA_TRY(cudaGetLastError());
+  if (info) {
+    memset(info, 0, sizeof(*info));
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, ev0, ev1);
+    info->solve_interval_ms = ms;
+    info->device_bytes = p->bytes;
+    for (int a = 0; a < A; ++a) {
+      info->iters_total += hi[(size_t)a];
+      if (hi[(size_t)a] > info->iters_max) info->iters_max = hi[(size_t)a];
+      switch (hs[(size_t)a]) {
+        case PRISM_STATUS_CERTIFIED: ++info->n_certified; break;
+        case PRISM_STATUS_FEASIBLE: ++info->n_feasible; break;
+        case PRISM_STATUS_TIMEOUT: ++info->n_timeout; break;
+        case PRISM_STATUS_LATE: ++info->n_late; break;
+        case PRISM_STATUS_NO_FEASIBLE: ++info->n_no_feasible; break;
+        default: ++info->n_failed; break;
+      }
+    }
+    info->kernel_launches = L.launches;
+    info->wall_ms = elapsed_ms();
+  }
+  cudaEventDestroy(ev0);
+  cudaEventDestroy(ev1);
+  return PRISM_OK;
+}
+
+extern "C" int prism_residuals(prism_problem* p, const double* w, const double* duals, void* cuda_stream, double* resid_out) {
+  if (!p) return set_err(PRISM_ERR_NOT_READY, "problem object is NULL%s", "");
+  if (!w || !resid_out) return set_err(PRISM_ERR_INVALID_ARG, "w and resid_out are mandatory%s", "");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  Launcher L{p, st, p->kp / 8, 0};
+  run_diag(p, L, w, duals, p->resid);
+  const double nanv = NAN;
+  std::vector<double> h((size_t)p->A * PRISM_NRES);
+  CUDA_TRY(cudaMemcpyAsync(h.data(), p->resid, h.size() * sizeof(double), cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  for (int a = 0; a < p->A; ++a) { h[(size_t)a * PRISM_NRES + PRISM_R_PRIMAL] = nanv; h[(size_t)a * PRISM_NRES + PRISM_R_DUAL] = nanv; h[(size_t)a * PRISM_NRES + PRISM_R_RHO] = nanv; h[(size_t)a * PRISM_NRES + PRISM_R_RESERVED] = 0.0; }
+  CUDA_TRY(cudaMemcpyAsync(resid_out, h.data(), h.size() * sizeof(double), cudaMemcpyHostToDevice, st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  CUDA_TRY(cudaGetLastError());
+  return PRISM_OK;
+}
+
+extern "C" int prism_solve_batch_host(prism_problem* p, const prism_settings* s, void* cuda_stream, const double* mu_host,
+                                      const double* w0_host, double* w_host, int32_t* status_host, int32_t* iters_host,
+                                      double* resid_host, prism_solve_info* info) {
+  if (!p) return set_err(PRISM_ERR_NOT_READY, "problem object is NULL%s", "");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const auto t0 = std::chrono::steady_clock::now();
+  const size_t AN = (size_t)p->A * p->N;
+  if (mu_host) CUDA_TRY(cudaMemcpyAsync((void*)p->d.mu, mu_host, AN * sizeof(double), cudaMemcpyHostToDevice, st));
+  if (w0_host) CUDA_TRY(cudaMemcpyAsync((void*)p->d.w0, w0_host, AN * sizeof(double), cudaMemcpyHostToDevice, st));
+  if (!p->w_stage) {
+    if (dev_alloc(p, &p->w_stage, AN) != PRISM_OK || dev_alloc(p, &p->i_stage, (size_t)p->A) != PRISM_OK) return PRISM_ERR_ALLOC;
+  }
+  int r = prism_solve_batch(p, s, cuda_stream, p->w_stage, p->status, p->i_stage, nullptr, nullptr, info);
+  if (r != PRISM_OK) return r;
+  if (w_host) CUDA_TRY(cudaMemcpyAsync(w_host, p->w_stage, AN * sizeof(double), cudaMemcpyDeviceToHost, st));
+  if (status_host) CUDA_TRY(cudaMemcpyAsync(status_host, p->status, (size_t)p->A * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+  if (iters_host) CUDA_TRY(cudaMemcpyAsync(iters_host, p->ap.iters, (size_t)p->A * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+  if (resid_host) CUDA_TRY(cudaMemcpyAsync(resid_host, p->resid, (size_t)p->A * PRISM_NRES * sizeof(double), cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  if (info) info->wall_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
+  return PRISM_OK;
+}

@@ -1,0 +1,314 @@
+// prox.cuh - H4 fused proximal / projection kernel, one CTA per account.
+//
+// z-update of the splitting, in trade space t = z - w0, u = v - w0, rho_i = c gamma d_i:
+//
+//   minimise  sum_i [ rho_i/2 (t_i - u_i)^2 + (kappa + c_buy) (t_i)_+ + kappa (-t_i)_+ + psi_i((-t_i)_+) ]
+//   s.t.      sum_i t_i = 1 - sum_i w0_i          (budget hyperplane, Eq. (1) row 1)
+//             lo_i <= w0_i + t_i <= hi_i          (box, exclusions as lo = hi = 0)
+//             sum_i |t_i| <= tau                  (turnover budget, D_a = I)
+//
+// With multipliers nu (budget) and theta >= 0 (turnover), alpha = nu + theta and beta = nu - theta, buys depend on
+// alpha only and sells on beta only ("L1 turnover split", BASELINE.json:north_star):
+//   buy_i(alpha)  = clip((rho_i u_i - kappa - c_buy - alpha) / rho_i, bl_i, bh_i)
+//   sell_i(beta)  = clip(sum_l clip((beta - rho_i u_i - kappa - s_il)/rho_i - Q_{i,l-1}, 0, q_il), sl_i, sh_i)
+// so the two coupled constraints become:  theta = 0: one monotone scalar equation  P(nu) - R(nu) = b;
+// cap active: two independent monotone equations  P(alpha) = (tau + b)/2,  R(beta) = (tau - b)/2.
+// Each is continuous piecewise linear; solved by safeguarded Newton (bracketed, exact on the final linear piece),
+// warm-started from the previous iteration.  All trial evaluations are block-wide reductions in this CTA.
+//
+// The same kernel then emits what the x-update needs (r~ = M^-1 r, c = r~ - z, per-group sums of r~), and on check
+// iterations the scaled residuals, the convergence mask and the per-account rho adaptation.
+#pragma once
+#include "common.cuh"
+
+struct ProxArgs {
+  int64_t N, ldw;           // ldw: leading dimension of the owned A x N arrays (v, rt, cc, xs, pxq, q)
+  int32_t A, G, kp, max_lots;
+  int64_t ldv;
+  // borrowed data
+  const double *mu, *q, *w0, *gamma, *lo, *hi, *hi_full, *tau, *kappa, *c_buy, *lot_slope, *lot_width;
+  const uint8_t *excl, *lot_count, *group_id;
+  const double* invd;
+  const double* d;
+  // iterate
+  double *v, *rt, *cc, *TE;
+  const double *xs, *pxq;
+  const double *zE, *yE;
+  AccountParams ap;
+  double* w_out;
+  double* duals;
+  double* resid;
+  int32_t* counters;
+  // settings
+  double eps, dbar_GN, band_scale;   // dbar_GN = mean(d) * G / N
+  int32_t adapt, iter;
+};
+
+enum { PROX_CHECK = 1, PROX_FINAL = 2, PROX_INIT = 4 };
+
+struct ElemConst {        // per-element quantities that do not depend on the trial thresholds
+  double rho_u, ir, bl, bh, sl, sh, w0;
+};
+
+__device__ __forceinline__ ElemConst load_elem(const ProxArgs& p, int64_t row, int64_t rowp, int64_t i, double cg,
+                                               double lo_a, double hi_a) {
+  ElemConst e;
+  const int64_t idx = row + i;
+  const double w0 = p.w0[idx];
+  const double v = p.v[rowp + i];
+  const double dinv = p.invd[i];
+  double lo = lo_a, hi = p.hi_full ? p.hi_full[idx] : hi_a;
+  if (p.excl && p.excl[idx]) { lo = 0.0; hi = 0.0; }
+  e.w0 = w0;
+  e.ir = dinv / cg;                       // 1 / rho_i
+  e.rho_u = (v - w0) * cg / dinv;         // rho_i u_i  (d_i = 1 / invd_i)
+  e.bl = fmax(lo - w0, 0.0);
+  e.bh = fmax(hi - w0, 0.0);
+  e.sl = fmax(w0 - hi, 0.0);
+  e.sh = fmax(w0 - lo, 0.0);
+  return e;
+}
+
+// buy amount at threshold alpha; mv = 1 if strictly inside its range (slope -ir)
+__device__ __forceinline__ double buy_amt(const ElemConst& e, double lam_b, double alpha, double& mv) {
+  const double raw = (e.rho_u - lam_b - alpha) * e.ir;
+  mv = (raw > e.bl && raw < e.bh) ? e.ir : 0.0;
+  return fmin(fmax(raw, e.bl), e.bh);
+}
+
+template <bool LOTS>
+__device__ __forceinline__ double sell_amt(const ElemConst& e, double kappa, double beta, const double* slope,
+                                           const double* width, int nl, double& mv) {
+  double raw, inside = 0.0;
+  double sh = e.sh;
+  if (LOTS && nl > 0) {
+    raw = 0.0;
+    double Q = 0.0;
+    for (int l = 0; l < nl; ++l) {
+      const double r = (beta - e.rho_u - kappa - slope[l]) * e.ir - Q;
+      const double ql = width[l];
+      if (r > 0.0 && r < ql) inside = 1.0;
+      raw += fmin(fmax(r, 0.0), ql);
+      Q += ql;
+    }
+    sh = fmin(sh, Q);
+  } else {
+    raw = (beta - e.rho_u - kappa) * e.ir;
+    inside = 1.0;
+  }
+  mv = (inside > 0.0 && raw > e.sl && raw < sh) ? e.ir : 0.0;
+  return fmin(fmax(raw, e.sl), sh);
+}
+
+// One bracketed Newton step on a continuous piecewise-linear monotone function.
+// dir = +1: g increasing in x, -1: decreasing.  slope = |g'| at x (0 on a flat piece).
+struct Root1D {
+  double x, lo, hi;
+  int done;
+};
+__device__ __forceinline__ void root_step(Root1D& r, double g, double slope, double target, int dir, double tol) {
+  if (r.done) return;
+  const double diff = g - target;
+  if (fabs(diff) <= tol) { r.done = 1; return; }
+  const bool too_big = (dir > 0) ? (diff > 0.0) : (diff < 0.0);   // x lies right of the root
+  if (too_big) r.hi = r.x; else r.lo = r.x;
+  double xn = (slope > 0.0) ? r.x - (double)dir * diff / slope : NAN;
+  if (!(xn > r.lo && xn < r.hi)) xn = 0.5 * (r.lo + r.hi);
+  if (xn == r.x || !(r.hi - r.lo > 0.0) || !(xn > r.lo && xn < r.hi)) { r.done = 1; r.x = (xn == xn) ? xn : r.x; return; }
+  r.x = xn;
+}
+
+template <bool LOTS>
+__global__ void __launch_bounds__(512) k_prox(ProxArgs p, int mode) {
+  __shared__ double scratch[8 * 32];
+  __shared__ double teS[PRISM_MAX_GROUPS];
+  __shared__ double eS[PRISM_MAX_GROUPS];
+  __shared__ double yES[PRISM_MAX_GROUPS];
+  const int a = blockIdx.x;
+  if (p.ap.done[a]) return;
+  const int tid = threadIdx.x, nt = blockDim.x;
+  const int64_t N = p.N, row = (int64_t)a * N, rowp = (int64_t)a * p.ldw;
+  const double gam = p.gamma[a];
+  double c = p.ap.c[a];
+  double cg = c * gam;
+  const double lo_a = p.lo[a], hi_a = p.hi[a];
+  const double kappa = p.kappa ? p.kappa[a] : 0.0;
+  const double lam_b = kappa + (p.c_buy ? p.c_buy[a] : 0.0);
+  const double tau = p.tau ? p.tau[a] : INFINITY;
+  const double b = p.ap.bsum[a];
+  const int L = PRISM_MAX_LOTS;
+
+  // ---------------------------------------------------------------- pass 0: value at the warm start + brackets
+  double alpha = p.ap.alpha[a], beta = p.ap.beta[a];
+  int amode = p.ap.mode[a];
+  if (!(amode == 1 && isfinite(tau))) { amode = 0; beta = alpha; }
+  double a_min = INFINITY, a_max = -INFINITY, b_min = INFINITY, b_max = -INFINITY;
+  double P = 0, R = 0, sP = 0, sR = 0;
+  auto eval = [&](double al, double be, bool extremes) {
+    double lP = 0, lR = 0, lsP = 0, lsR = 0, amn = INFINITY, amx = -INFINITY, bmn = INFINITY, bmx = -INFINITY;
+    for (int64_t i = tid; i < N; i += nt) {
+      const ElemConst e = load_elem(p, row, rowp, i, cg, lo_a, hi_a);
+      double mvb, mvs;
+      int nl = 0;
+      const double *sl = nullptr, *wd = nullptr;
+      if (LOTS) { nl = p.lot_count[row + i]; sl = p.lot_slope + (row + i) * L; wd = p.lot_width + (row + i) * L; }
+      lP += buy_amt(e, lam_b, al, mvb);
+      lR += sell_amt<LOTS>(e, kappa, be, sl, wd, nl, mvs);
+      lsP += mvb; lsR += mvs;
+      if (extremes) {
+        const double rho = 1.0 / e.ir;
+        if (e.bh > e.bl) { amn = fmin(amn, e.rho_u - lam_b - rho * e.bh); amx = fmax(amx, e.rho_u - lam_b - rho * e.bl); }
+        double sh = e.sh, s_first = 0.0, s_last = 0.0;
+        if (LOTS && nl > 0) { double Q = 0; for (int l = 0; l < nl; ++l) Q += wd[l]; sh = fmin(sh, Q); s_first = sl[0]; s_last = sl[nl - 1]; }
+        if (sh > e.sl) { bmn = fmin(bmn, e.rho_u + kappa + s_first + rho * e.sl); bmx = fmax(bmx, e.rho_u + kappa + s_last + rho * sh); }
+      }
+    }
+    if (extremes) {
+      double val[8] = {lP, lR, lsP, lsR, amn, amx, bmn, bmx};
+      const int op[8] = {0, 0, 0, 0, 2, 1, 2, 1};
+      block_reduce<8>(val, op, scratch);
+      P = val[0]; R = val[1]; sP = val[2]; sR = val[3];
+      a_min = val[4]; a_max = val[5]; b_min = val[6]; b_max = val[7];
+    } else {
+      double val[4] = {lP, lR, lsP, lsR};
+      const int op[4] = {0, 0, 0, 0};
+      block_reduce<4>(val, op, scratch);
+      P = val[0]; R = val[1]; sP = val[2]; sR = val[3];
+    }
+  };
+  eval(alpha, beta, true);
+  // finite brackets (with a margin so that the end values are the saturated sums)
+  const double span = fmax(fmax(fabs(a_min), fabs(a_max)), fmax(fabs(b_min), fabs(b_max)));
+  const double pad = 1e-9 * fmax(span, 1e-300) + 1e-300;
+  if (!(a_min <= a_max)) { a_min = -1.0; a_max = 1.0; }
+  if (!(b_min <= b_max)) { b_min = -1.0; b_max = 1.0; }
+  a_min -= pad; a_max += pad; b_min -= pad; b_max += pad;
+  const double tol = 2e-15 * fmax(1.0, fabs(b) + (isfinite(tau) ? tau : 0.0));
+  const double Pt = 0.5 * (tau + b), Rt = 0.5 * (tau - b);
+
+  for (int attempt = 0; attempt < 3; ++attempt) {
+    if (amode == 1) {
+      // cap active: two independent equations
+      Root1D ra = {fmin(fmax(alpha, a_min), a_max), a_min, a_max, 0};
+      Root1D rb = {fmin(fmax(beta, b_min), b_max), b_min, b_max, 0};
+      if (ra.x != alpha || rb.x != beta || attempt > 0) eval(ra.x, rb.x, false);
+      for (int it = 0; it < 80; ++it) {
+        root_step(ra, P, sP, Pt, -1, tol);
+        root_step(rb, R, sR, Rt, +1, tol);
+        if (ra.done && rb.done) break;
+        eval(ra.x, rb.x, false);
+      }
+      alpha = ra.x; beta = rb.x;
+      if (alpha >= beta) break;          // theta >= 0: accepted
+      amode = 0; alpha = beta = 0.5 * (alpha + beta);
+    } else {
+      const double lo_b = fmin(a_min, b_min), hi_b = fmax(a_max, b_max);
+      Root1D rn = {fmin(fmax(alpha, lo_b), hi_b), lo_b, hi_b, 0};
+      if (rn.x != alpha || attempt > 0 || beta != alpha) eval(rn.x, rn.x, false);
+      for (int it = 0; it < 80; ++it) {
+        root_step(rn, P - R, sP + sR, b, -1, tol);
+        if (rn.done) break;
+        eval(rn.x, rn.x, false);
+      }
+      alpha = beta = rn.x;
+      if (!isfinite(tau) || P + R <= tau + tol) break;   // cap inactive: accepted
+      amode = 1;
+    }
+  }
+
+  // ---------------------------------------------------------------- group data of the band block
+  const int G = p.G;
+  double rhoE = p.ap.rhoE[a];
+  for (int g = tid; g < G; g += nt) { teS[g] = 0.0; yES[g] = p.yE[(int64_t)a * G + g]; }
+  __syncthreads();
+
+  // ---------------------------------------------------------------- check: residuals, mask, rho adaptation
+  double rescale = 1.0;
+  int finished = 0;
+  if (mode & PROX_CHECK) {
+    double nx = 0, nz = 0, nrp = 0, nrd = 0, nPx = 0, ny = 0, nq = 0;
+    for (int64_t i = tid; i < N; i += nt) {
+      const ElemConst e = load_elem(p, row, rowp, i, cg, lo_a, hi_a);
+      double mvb, mvs; int nl = 0; const double *sl = nullptr, *wd = nullptr;
+      if (LOTS) { nl = p.lot_count[row + i]; sl = p.lot_slope + (row + i) * L; wd = p.lot_width + (row + i) * L; }
+      const double z = e.w0 + buy_amt(e, lam_b, alpha, mvb) - sell_amt<LOTS>(e, kappa, beta, sl, wd, nl, mvs);
+      const double vv = p.v[rowp + i];
+      const double y = (vv - z) / e.ir;
+      const double x = p.xs[rowp + i], pq = p.pxq[rowp + i];
+      const double qi = p.q ? p.q[rowp + i] : -p.mu[row + i];
+      const double ye = G ? yES[p.group_id[i]] : 0.0;
+      nx = fmax(nx, fabs(x)); nz = fmax(nz, fabs(z)); nrp = fmax(nrp, fabs(x - z));
+      nrd = fmax(nrd, fabs(pq + y + ye)); nPx = fmax(nPx, fabs(pq - qi)); ny = fmax(ny, fabs(y + ye)); nq = fmax(nq, fabs(qi));
+      // NaN guard: fmax drops NaN, so poison explicitly
+      if (!(z == z) || !(x == x) || !(vv == vv)) nrp = INFINITY;
+    }
+    double val[7] = {nx, nz, nrp, nrd, nPx, ny, nq};
+    const int op[7] = {1, 1, 1, 1, 1, 1, 1};
+    block_reduce<7>(val, op, scratch);
+    double rp = val[2] / fmax(fmax(val[0], val[1]), 1e-300);
+    if (G) rp = fmax(rp, p.ap.rpE[a] / fmax(p.ap.nE[a], 1e-300));
+    const double rd = val[3] / fmax(fmax(val[4], fmax(val[5], val[6])), 1e-300);
+    const bool bad = !(rp < INFINITY) || !(rd < INFINITY);
+    const bool conv = !bad && rp <= p.eps && rd <= p.eps;
+    if (tid == 0) {
+      p.resid[(int64_t)a * PRISM_NRES + PRISM_R_PRIMAL] = rp;
+      p.resid[(int64_t)a * PRISM_NRES + PRISM_R_DUAL] = rd;
+    }
+    if (conv || bad) {
+      finished = 1;
+      if (tid == 0) {
+        p.ap.conv[a] = conv ? 1 : 0;
+        if (bad) p.ap.conv[a] = -1;
+      }
+    } else if (p.adapt) {
+      const double ratio = sqrt(rp / fmax(rd, 1e-300));
+      if ((ratio > 5.0 || ratio < 0.2) && p.ap.nadapt[a] < 20) {
+        const double cn = c * fmin(fmax(ratio, 0.1), 10.0);
+        rescale = c / cn;          // v' = z + (rho/rho') (v - z) keeps y = rho (v - z) unchanged
+        c = cn; cg = c * gam;
+        rhoE = p.band_scale * c * gam * p.dbar_GN;
+        if (tid == 0) { p.ap.c[a] = c; p.ap.rhoE[a] = rhoE; p.ap.refactor[a] = 1; p.ap.nadapt[a] += 1; }
+      }
+    }
+  }
+  if (mode & PROX_FINAL) finished = 1;
+  for (int g = tid; g < G; g += nt) eS[g] = rhoE * p.zE[(int64_t)a * G + g] - yES[g];
+  __syncthreads();
+
+  // ---------------------------------------------------------------- output pass
+  const double cg_old = cg * rescale;     // rho scale the stored v refers to (c_old * gamma)
+  for (int64_t i = tid; i < N; i += nt) {
+    const ElemConst e = load_elem(p, row, rowp, i, cg_old, lo_a, hi_a);
+    double mvb, mvs; int nl = 0; const double *sl = nullptr, *wd = nullptr;
+    if (LOTS) { nl = p.lot_count[row + i]; sl = p.lot_slope + (row + i) * L; wd = p.lot_width + (row + i) * L; }
+    const double z = e.w0 + buy_amt(e, lam_b, alpha, mvb) - sell_amt<LOTS>(e, kappa, beta, sl, wd, nl, mvs);
+    if (finished) { p.w_out[row + i] = z; continue; }
+    double vv = p.v[rowp + i];
+    const double y = (vv - z) / e.ir;                      // rho_old (v - z)
+    if (rescale != 1.0) { vv = z + rescale * (vv - z); p.v[rowp + i] = vv; }
+    const double dinv = p.invd[i];
+    const double rho = cg / dinv;                          // new rho_i
+    const double qi = p.q ? p.q[rowp + i] : -p.mu[row + i];
+    const int g = G ? p.group_id[i] : 0;
+    const double r = rho * z - y - qi + (G ? eS[g] : 0.0);
+    const double rt = r * dinv / (gam * (1.0 + c));        // M_i = gamma d_i (1 + c)
+    p.rt[rowp + i] = rt;
+    p.cc[rowp + i] = rt - z;
+    if (G) atomicAdd(&teS[g], rt);
+  }
+  __syncthreads();
+  if (!finished) for (int g = tid; g < G; g += nt) p.TE[(int64_t)a * G + g] = teS[g];
+  if (tid == 0) {
+    p.ap.alpha[a] = alpha; p.ap.beta[a] = beta; p.ap.mode[a] = amode;
+    if (finished) {
+      p.ap.done[a] = 1;
+      p.ap.iters[a] = p.iter;
+      atomicAdd(&p.counters[0], 1);
+      double* du = p.duals + (int64_t)a * PRISM_NDUAL(G);
+      du[0] = 0.5 * (alpha + beta);
+      du[1] = 0.5 * (alpha - beta);
+      for (int g = 0; g < G; ++g) { du[2 + g] = fmax(yES[g], 0.0); du[2 + G + g] = fmax(-yES[g], 0.0); }
+      p.resid[(int64_t)a * PRISM_NRES + PRISM_R_RHO] = c;
+    }
+  }
+}

@@ -1,0 +1,194 @@
+// small.cuh - setup (H0), capacitance factorisation (H0/H7), per-account small solve + band block (H2),
+// external diagnostics (H8/H9: PAPER.md:142-146) and status assignment (Table 14).
+#pragma once
+#include "common.cuh"
+
+// ---------------------------------------------------------------------------------- H0: shared universe
+// Bp (N x kp asset-major), Bt (kp x ldn factor-major), invd; B given as fp64 or fp32 (configs[4] stores fp32).
+__global__ void k_setup_shared(const void* B, int is32, const double* d, int64_t N, int k, int kp, int64_t ldn,
+                               double* Bp, double* Bt, double* invd) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= N) return;
+  invd[i] = 1.0 / d[i];
+  for (int j = 0; j < kp; ++j) {
+    double b = 0.0;
+    if (j < k) b = is32 ? (double)((const float*)B)[i * k + j] : ((const double*)B)[i * k + j];
+    Bp[i * kp + j] = b;
+    Bt[(int64_t)j * ldn + i] = b;
+  }
+}
+
+// gram[r][c] = sum_i U_ir U_ic / d_i,  U = [Bp | E'] (E' = group indicators).  One CTA per (r, c), r <= c.
+__global__ void k_gram(const double* Bt, int64_t ldn, const uint8_t* gid, const double* invd, int64_t N, int kp, int G,
+                       double* gram) {
+  __shared__ double scratch[32];
+  const int Kp = kp + G;
+  const int r = blockIdx.x, c = blockIdx.y;
+  if (r > c) return;
+  double s = 0.0;
+  for (int64_t i = threadIdx.x; i < N; i += blockDim.x) {
+    const double ur = r < kp ? Bt[(int64_t)r * ldn + i] : (gid[i] == r - kp ? 1.0 : 0.0);
+    const double uc = c < kp ? Bt[(int64_t)c * ldn + i] : (gid[i] == c - kp ? 1.0 : 0.0);
+    s = fma(ur * uc, invd[i], s);
+  }
+  double val[1] = {s};
+  const int op[1] = {0};
+  block_reduce<1>(val, op, scratch);
+  if (threadIdx.x == 0) { gram[(int64_t)r * Kp + c] = val[0]; gram[(int64_t)c * Kp + r] = val[0]; }
+}
+
+// ---------------------------------------------------------------------------------- per-account cold start
+struct InitArgs {
+  int64_t N, ldw; int32_t A, G;
+  const double *w0, *gamma, *band_lo, *band_hi;
+  const uint8_t* group_id;
+  double *v, *zE, *yE;
+  AccountParams ap;
+  double rho_scale, band_scale, dbar_GN;
+};
+__global__ void k_init_accounts(InitArgs p) {
+  __shared__ double scratch[32];
+  __shared__ double gs[PRISM_MAX_GROUPS];
+  const int a = blockIdx.x, tid = threadIdx.x;
+  for (int g = tid; g < p.G; g += blockDim.x) gs[g] = 0.0;
+  __syncthreads();
+  double s = 0.0;
+  for (int64_t i = tid; i < p.N; i += blockDim.x) {
+    const double w = p.w0[(int64_t)a * p.N + i];
+    p.v[(int64_t)a * p.ldw + i] = w;            // cold start: v = w0, i.e. z = projection of w0, y = rho (w0 - z)
+    s += w;
+    if (p.G) atomicAdd(&gs[p.group_id[i]], w);
+  }
+  double val[1] = {s};
+  const int op[1] = {0};
+  block_reduce<1>(val, op, scratch);
+  for (int g = tid; g < p.G; g += blockDim.x) {
+    const int64_t e = (int64_t)a * p.G + g;
+    p.zE[e] = fmin(fmax(gs[g], p.band_lo[e]), p.band_hi[e]);
+    p.yE[e] = 0.0;
+  }
+  if (tid == 0) {
+    p.ap.bsum[a] = 1.0 - val[0];
+    p.ap.c[a] = p.rho_scale;
+    p.ap.rhoE[a] = p.band_scale * p.rho_scale * p.gamma[a] * p.dbar_GN;
+    p.ap.alpha[a] = 0.0; p.ap.beta[a] = 0.0; p.ap.mode[a] = 0;
+    p.ap.rpE[a] = 0.0; p.ap.nE[a] = 1.0;
+    p.ap.done[a] = 0; p.ap.conv[a] = 0; p.ap.iters[a] = 0; p.ap.refactor[a] = 1; p.ap.nadapt[a] = 0;
+  }
+}
+
+// ---------------------------------------------------------------------------------- H0 / H7: capacitance inverse
+// S_a = Lambda_a^-1 + gram / (gamma_a (1 + c_a)),  Lambda_a = diag(gamma_a f, [1 on padded factors], rhoE_a 1_G).
+// Inverted in shared memory by Gauss-Jordan (S is SPD, no pivoting needed).  Only accounts flagged `refactor`.
+__global__ void k_factor(const double* gram, const double* f, const double* gamma, AccountParams ap, int k, int kp,
+                         int G, double* Sinv) {
+  extern __shared__ double S[];
+  const int a = blockIdx.x, tid = threadIdx.x, nt = blockDim.x;
+  if (!ap.refactor[a] || ap.done[a]) return;
+  const int Kp = kp + G;
+  const double gam = gamma[a], c = ap.c[a], rhoE = ap.rhoE[a];
+  const double sc = 1.0 / (gam * (1.0 + c));
+  for (int e = tid; e < Kp * Kp; e += nt) {
+    const int r = e / Kp, cc = e % Kp;
+    double s = gram[e] * sc;
+    if (r == cc) s += r < k ? 1.0 / (gam * f[r]) : (r < kp ? 1.0 : 1.0 / rhoE);
+    S[e] = s;
+  }
+  __syncthreads();
+  // in-place Gauss-Jordan inversion
+  for (int p = 0; p < Kp; ++p) {
+    const double piv = 1.0 / S[p * Kp + p];
+    __syncthreads();
+    for (int cc = tid; cc < Kp; cc += nt) if (cc != p) S[p * Kp + cc] *= piv;
+    __syncthreads();
+    for (int e = tid; e < Kp * Kp; e += nt) {
+      const int r = e / Kp, cc = e % Kp;
+      if (r != p && cc != p) S[e] -= S[r * Kp + p] * S[p * Kp + cc];
+    }
+    __syncthreads();
+    for (int r = tid; r < Kp; r += nt) if (r != p) S[r * Kp + p] *= -piv;
+    if (tid == 0) S[p * Kp + p] = piv;
+    __syncthreads();
+  }
+  for (int e = tid; e < Kp * Kp; e += nt) Sinv[(int64_t)a * Kp * Kp + e] = S[e];
+  if (tid == 0) ap.refactor[a] = 0;
+}
+
+// ---------------------------------------------------------------------------------- H2: V = S^-1 T and the band block
+struct SolveArgs {
+  int32_t A, G, kp, nchunk; int64_t ldv;
+  const double *Tpart, *TE, *Sinv, *band_lo, *band_hi;
+  double *V, *zE, *yE;
+  AccountParams ap;
+  double relax;
+};
+__global__ void __launch_bounds__(128) k_solve(SolveArgs p) {
+  __shared__ double T[PRISM_MAX_KPRIME];
+  __shared__ double Vs[PRISM_MAX_KPRIME];
+  __shared__ double scratch[2 * 32];
+  const int a = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  if (p.ap.done[a]) return;
+  const int Kp = p.kp + p.G;
+  for (int j = tid; j < Kp; j += blockDim.x) {
+    double s = 0.0;
+    if (j < p.kp) for (int ch = 0; ch < p.nchunk; ++ch) s += p.Tpart[((int64_t)ch * p.A + a) * p.ldv + j];   // fixed order
+    else s = p.TE[(int64_t)a * p.G + (j - p.kp)];
+    T[j] = s;
+  }
+  __syncthreads();
+  const double* Si = p.Sinv + (int64_t)a * Kp * Kp;
+  for (int r = warp; r < Kp; r += 4) {
+    double s = 0.0;
+    for (int c = lane; c < Kp; c += 32) s = fma(Si[(int64_t)r * Kp + c], T[c], s);
+    s = warp_sum(s);
+    if (lane == 0) { Vs[r] = s; p.V[(int64_t)a * p.ldv + r] = s; }
+  }
+  __syncthreads();
+  // band block: E x = V_E / rhoE (since U'x = Lambda^-1 V);  z_E, y_E updates; its primal residual
+  const double rhoE = p.ap.rhoE[a];
+  double rp = 0.0, nrm = 0.0;
+  for (int g = tid; g < p.G; g += blockDim.x) {
+    const int64_t e = (int64_t)a * p.G + g;
+    const double Ex = Vs[p.kp + g] / rhoE;
+    const double zo = p.zE[e], yo = p.yE[e];
+    const double eh = p.relax * Ex + (1.0 - p.relax) * zo;
+    const double zn = fmin(fmax(eh + yo / rhoE, p.band_lo[e]), p.band_hi[e]);
+    p.zE[e] = zn;
+    p.yE[e] = yo + rhoE * (eh - zn);
+    rp = fmax(rp, fabs(Ex - zn));
+    nrm = fmax(nrm, fmax(fabs(Ex), fabs(zn)));
+  }
+  if (p.G) {
+    double val[2] = {rp, nrm};
+    const int op[2] = {1, 1};
+    block_reduce<2>(val, op, scratch);
+    if (tid == 0) { p.ap.rpE[a] = val[0]; p.ap.nE[a] = val[1]; }
+  }
+}
+
+// V[a][j] = gamma_a f_j * sum_ch Tpart[ch][a][j]   (Sigma-apply: B (F (B'x)) via GEMM-1 then GEMM-2)
+__global__ void k_scale_fs(const double* Tpart, int nchunk, int A, int k, int kp, int64_t ldv, const double* f,
+                           const double* gamma, double* V) {
+  const int a = blockIdx.x;
+  for (int j = threadIdx.x; j < kp; j += blockDim.x) {
+    double s = 0.0;
+    for (int ch = 0; ch < nchunk; ++ch) s += Tpart[((int64_t)ch * A + a) * ldv + j];
+    V[(int64_t)a * ldv + j] = j < k ? gamma[a] * f[j] * s : 0.0;
+  }
+}
+
+// X = w - w_b (or w) into a padded buffer
+__global__ void k_diff(const double* w, const double* wb, int64_t N, int64_t ldw, double* X) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int a = blockIdx.y;
+  if (i >= N) return;
+  const int64_t s = (int64_t)a * N + i;
+  X[(int64_t)a * ldw + i] = wb ? w[s] - wb[s] : w[s];
+}
+// q = -mu - gamma Sigma w_b  (buf holds +gamma Sigma w_b computed with X = w_b, i.e. pass w = 0 trick avoided: see api)
+__global__ void k_make_q(const double* mu, const double* gSig, int64_t N, int64_t ldw, double* q) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int a = blockIdx.y;
+  if (i >= N) return;
+  q[(int64_t)a * ldw + i] = -mu[(int64_t)a * N + i] - gSig[(int64_t)a * ldw + i];
+}
