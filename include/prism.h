@@ -123,13 +123,14 @@ typedef struct prism_settings {
   int32_t check_every;      /* residual / convergence-mask cadence in iterations (default 10)                    */
   double alpha;             /* over-relaxation in (0, 2) (default 1.6)                                           */
   double rho_scale;         /* initial c: rho_i = c gamma_a d_i (default 100)                                    */
-  double rho_band_scale;    /* band-block rho relative to the mean rho_i, per unit row norm (default 1)          */
+  double rho_band_scale;    /* unused since the bands moved into the projection; kept for ABI stability (default 1)  */
   int32_t adapt_rho;        /* 1 => per-account rho adaptation at check iterations (default 1)                   */
   int32_t gemm_mode;        /* 0 = fp64 tensor (DMMA mma.sync), 1 = fp64 FMA                                     */
   double time_limit_ms;     /* 0 => none; accounts unfinished at the limit get PRISM_STATUS_TIMEOUT              */
   double deadline_ms;       /* 0 => none; accounts finishing after it get PRISM_STATUS_LATE                      */
   int32_t use_graph;        /* 1 => replay the inner iterations as a CUDA graph (default 1)                      */
-  int32_t reserved;
+  int32_t profile;          /* 1 => bracket every kernel launch with CUDA events (read with prism_kernel_times);
+                               adds event overhead, so never combine with a throughput measurement           */
 } prism_settings;
 
 typedef struct prism_solve_info {
@@ -181,6 +182,15 @@ int prism_residuals(prism_problem* p, const double* w, const double* duals, void
 int prism_solve_batch_host(prism_problem* p, const prism_settings* s, void* cuda_stream, const double* mu_host,
                            const double* w0_host, double* w_host, int32_t* status_host, int32_t* iters_host,
                            double* resid_host, prism_solve_info* info);
+
+/* Kernel classes of the hot path: H4/H5/H6/H7 fused prox, H1 GEMM-1, H2 small solve + band
+ * block, H3 GEMM-2 + epilogue, H0/H7 capacitance factorisation, H8/H9 diagnostics, everything else. */
+enum { PRISM_K_PROX = 0, PRISM_K_GEMM1 = 1, PRISM_K_SOLVE = 2, PRISM_K_GEMM2 = 3, PRISM_K_FACTOR = 4, PRISM_K_DIAG = 5,
+       PRISM_K_OTHER = 6, PRISM_NKERN = 8 };
+
+/* Device time (ms, CUDA events on the solve stream) and launch count per kernel class of the last
+ * prism_solve_batch call that ran with settings.profile = 1.  ms_out, launches_out: host arrays of PRISM_NKERN. */
+int prism_kernel_times(const prism_problem* p, double* ms_out, int64_t* launches_out);
 
 /* Frees the workspace; never frees borrowed data.  NULL is allowed. */
 void prism_problem_destroy(prism_problem* p);

@@ -200,7 +200,10 @@ class LiftedQP:
         acc = self.acc
         a_row = self.a_row
 
-        def solve(th, r1, r2):
+        cache = {}
+
+        def factor(th):
+            # everything that depends on th only; reused by the predictor, the corrector and every refinement step
             Delta, a, cg, ct = self._theta_parts(th)
             # per-asset blocks diag(Delta_vars) + a_i s s' (s = +-1), at most (1+L) x (1+L): solved densely
             # with pivoting (a Sherman-Morrison form cancels catastrophically when an interior variable has
@@ -234,12 +237,19 @@ class LiftedQP:
             if self.has_tau:
                 rows.append(self.t_row); winv.append(1.0 / ct)
             R = np.stack(rows, axis=1)                                         # (n, nr)
-            Z = K1inv(np.concatenate([r1[:, None], R], axis=1))
-            z1, ZR = Z[:, 0], Z[:, 1:]
+            ZR = K1inv(R)
             Sc = R.T @ ZR + np.diag(winv)
+            return K1inv, R, ZR, 0.5 * (Sc + Sc.T)
+
+        def solve(th, r1, r2):
+            if cache.get("th") is not th:
+                cache["th"] = th
+                cache["f"] = factor(th)
+            K1inv, R, ZR, Sc = cache["f"]
+            z1 = K1inv(r1[:, None])[:, 0]
             rhs = R.T @ z1
             rhs[0] -= r2
-            dl = np.linalg.solve(0.5 * (Sc + Sc.T), rhs)
+            dl = np.linalg.solve(Sc, rhs)
             dv = z1 - ZR @ dl
             return dv, dl[0]
         return solve

@@ -21,7 +21,7 @@ STATUS_NAMES = ["certified", "feasible/non-certified", "timeout", "deadline exce
                 "allocation/numerical failure"]
 SYMBOLS = ["prism_default_settings", "prism_problem_create", "prism_solve_batch", "prism_residuals",
            "prism_solve_batch_host", "prism_problem_destroy", "prism_problem_device_bytes", "prism_last_error",
-           "prism_version"]
+           "prism_version", "prism_kernel_times"]
 
 
 class ConstraintSet(C.Structure):
@@ -41,7 +41,7 @@ class Settings(C.Structure):
     _fields_ = [("eps_rel", C.c_double), ("max_iter", C.c_int32), ("check_every", C.c_int32), ("alpha", C.c_double),
                 ("rho_scale", C.c_double), ("rho_band_scale", C.c_double), ("adapt_rho", C.c_int32),
                 ("gemm_mode", C.c_int32), ("time_limit_ms", C.c_double), ("deadline_ms", C.c_double),
-                ("use_graph", C.c_int32), ("reserved", C.c_int32)]
+                ("use_graph", C.c_int32), ("profile", C.c_int32)]
 
 
 class SolveInfo(C.Structure):
@@ -79,6 +79,7 @@ def load_library(path: str = LIB_PATH):
     L.prism_problem_device_bytes.argtypes = [C.c_void_p]; L.prism_problem_device_bytes.restype = C.c_int64
     L.prism_last_error.argtypes = []; L.prism_last_error.restype = C.c_char_p
     L.prism_version.argtypes = []; L.prism_version.restype = C.c_char_p
+    L.prism_kernel_times.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int64)]; L.prism_kernel_times.restype = C.c_int
     _lib = L
     return L
 
@@ -197,6 +198,13 @@ class Problem:
             _check(lib().prism_solve_batch(self.handle, C.byref(s), C.c_void_p(stream), w.data_ptr(), status.data_ptr(),
                                            iters.data_ptr(), resid.data_ptr(), duals.data_ptr(), C.byref(info)))
         return SolveResult(w, status, iters, resid, duals, self._info(info))
+
+    KERNELS = ["prox", "gemm1", "solve", "gemm2", "factor", "diag", "other"]
+
+    def kernel_times(self) -> dict:
+        ms = (C.c_double * 8)(); cnt = (C.c_int64 * 8)()
+        _check(lib().prism_kernel_times(self.handle, ms, cnt))
+        return {n: dict(ms=ms[i], launches=int(cnt[i])) for i, n in enumerate(self.KERNELS)}
 
     def residuals(self, w, duals=None):
         torch = self.torch

@@ -15,13 +15,10 @@
 
 struct AccountParams {            // per-account scalars, struct of arrays on the device (A entries each)
   double* c;        // rho scale: rho_i = c gamma d_i
-  double* rhoE;     // band-block rho
   double* alpha;    // buy threshold  nu + theta   (warm start of the root find)
   double* beta;     // sell threshold nu - theta
   int32_t* mode;    // 0: turnover inactive (alpha == beta == nu), 1: cap active
   double* bsum;     // 1 - sum_i w0_i : budget in trade space
-  double* rpE;      // band-block primal residual |E x - z_E|_inf and its scale (set by the small-solve kernel)
-  double* nE;
   int32_t* done;    // convergence mask (H6)
   int32_t* conv;    // 1 if own tolerance met
   int32_t* iters;
@@ -31,7 +28,7 @@ struct AccountParams {            // per-account scalars, struct of arrays on th
 
 struct prism_problem {
   int64_t N;
-  int32_t k, kp, A, G, Kp;       // kp: k padded to 8; Kp = kp + G: rows of T and V per account
+  int32_t k, kp, A, G, Kp;       // kp: k padded to 8 * MT; Kp = kp: rows of T and V per account (U = Bp)
   int64_t ldv;                   // leading dimension of V / T rows (Kp padded to 8)
   uint32_t flags;
   int32_t max_lots;
@@ -41,17 +38,16 @@ struct prism_problem {
   double* Bt;       // kp x ldn, factor-major                      (GEMM-1 operand)
   int64_t ldn;      // N padded to 32
   double* invd;     // N
-  double* gram;     // Kp x Kp : U' D^-1 U with U = [Bp | E']
+  double* gram;     // Kp x Kp : Bp' D^-1 Bp
   double* q;        // A x N : -mu - gamma Sigma w_b, only with a benchmark shift (else NULL and q = -mu)
   // iterate (owned)
   double *v, *rt, *cc, *xs, *pxq;          // A x N each
   double* Tpart;    // nchunk x A x ldv  split-K partials of GEMM-1
   int32_t nchunk;
   int64_t chunk;    // assets per split-K chunk
-  double *TE;       // A x G   group sums of r~
   double *V;        // A x ldv
   double *Sinv;     // A x Kp x Kp
-  double *zE, *yE, *eE;   // A x G
+  double *gw0, *lamG;     // A x G: group sums of w0; band multipliers
   double *resid;    // A x PRISM_NRES (internal copy)
   double *duals;    // A x PRISM_NDUAL(G)
   int32_t* status;  // A
@@ -63,6 +59,8 @@ struct prism_problem {
   int64_t bytes;
   int sm_count;
   double dbar;            // mean of d (host copy at create)
+  double prof_ms[PRISM_NKERN];   // per-kernel-class device time of the last profiled solve
+  int64_t prof_cnt[PRISM_NKERN];
 };
 
 static thread_local char g_err[512] = "";
@@ -117,4 +115,29 @@ __device__ __forceinline__ void block_reduce(double (&val)[NV], const int (&op)[
 #pragma unroll
   for (int q = 0; q < NV; ++q) val[q] = scratch[q * 32];
   __syncthreads();
+}
+
+// Deterministic per-group accumulation (replaces shared-memory atomics, whose order is unspecified):
+// lanes holding the same group are summed in ascending lane order, the lowest lane adds the sum to THIS WARP's bin.
+// Call from warp-uniform control flow (every lane of the warp, `valid` masks the tail).  bins: [nwarps][ngroups].
+__device__ __forceinline__ void warp_group_add(double* bins, int ngroups, int g, double val, bool valid) {
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  const int key = valid ? g : (0x40000000 + lane);
+  const unsigned m = __match_any_sync(0xffffffffu, key);
+  unsigned rem = m;
+  double s = 0.0;
+  while (__any_sync(0xffffffffu, rem != 0u)) {
+    const int src = rem ? (__ffs(rem) - 1) : lane;
+    const double x = __shfl_sync(0xffffffffu, val, src);
+    if (rem) { s += x; rem &= rem - 1u; }
+  }
+  if (valid && lane == __ffs(m) - 1) bins[wid * ngroups + g] += s;
+  __syncwarp();
+}
+// sum of the per-warp bins in warp order; call after __syncthreads()
+__device__ __forceinline__ double group_total(const double* bins, int ngroups, int g) {
+  const int nw = (blockDim.x + 31) >> 5;
+  double s = 0.0;
+  for (int w = 0; w < nw; ++w) s += bins[w * ngroups + g];
+  return s;
 }

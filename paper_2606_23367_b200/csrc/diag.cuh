@@ -19,6 +19,7 @@ struct DiagArgs {
 template <bool LOTS>
 __global__ void __launch_bounds__(256) k_diag(DiagArgs p) {
   __shared__ double scratch[8 * 32];
+  __shared__ double gbin[8 * PRISM_MAX_GROUPS];
   __shared__ double gsum[PRISM_MAX_GROUPS];
   __shared__ double lam[PRISM_MAX_GROUPS];
   const int a = blockIdx.x, tid = threadIdx.x, nt = blockDim.x;
@@ -27,7 +28,8 @@ __global__ void __launch_bounds__(256) k_diag(DiagArgs p) {
   const bool have = p.duals != nullptr;
   const double* du = have ? p.duals + (int64_t)a * PRISM_NDUAL(G) : nullptr;
   const double nu = have ? du[0] : 0.0, theta = have ? du[1] : 0.0;
-  for (int g = tid; g < G; g += nt) { gsum[g] = 0.0; lam[g] = have ? du[2 + g] - du[2 + G + g] : 0.0; }
+  for (int g = tid; g < 8 * G; g += nt) gbin[g] = 0.0;
+  for (int g = tid; g < G; g += nt) lam[g] = have ? du[2 + g] - du[2 + G + g] : 0.0;
   __syncthreads();
   const double lo_a = p.lo[a], hi_a = p.hi[a];
   const double kappa = p.kappa ? p.kappa[a] : 0.0, cb = p.c_buy ? p.c_buy[a] : 0.0;
@@ -35,7 +37,11 @@ __global__ void __launch_bounds__(256) k_diag(DiagArgs p) {
   const double lamt = kappa + theta, dl = p.delta;
   double sw = 0, rbox = 0, turn = 0, fobj = 0, rstat = 0;
   bool bad = false;
-  for (int64_t i = tid; i < N; i += nt) {
+  for (int64_t i0 = 0; i0 < N; i0 += nt) {
+    const int64_t i = i0 + tid;
+    const bool valid = i < N;
+    if (G) warp_group_add(gbin, G, valid ? p.group_id[i] : 0, valid ? p.w[row + i] : 0.0, valid);
+    if (!valid) continue;
     const double w = p.w[row + i], w0 = p.w0[row + i], mu = p.mu[row + i];
     double lo = lo_a, hi = p.hi_full ? p.hi_full[row + i] : hi_a;
     if (p.excl && p.excl[row + i]) { lo = 0.0; hi = 0.0; }
@@ -44,7 +50,6 @@ __global__ void __launch_bounds__(256) k_diag(DiagArgs p) {
     sw += w;
     turn += fabs(dw);
     rbox = fmax(rbox, fmax(lo - w, w - hi));
-    if (G) atomicAdd(&gsum[p.group_id[i]], w);
     // objective f(w) (PAPER.md:109 in the SURVEY 8.0 form)
     const double x = p.w_b ? w - p.w_b[row + i] : w;
     const double gs = p.gS[rowp + i];
@@ -82,6 +87,8 @@ __global__ void __launch_bounds__(256) k_diag(DiagArgs p) {
       rstat = fmax(rstat, fmax(fmax(Slo + g, -g - Shi), 0.0));
     }
   }
+  __syncthreads();
+  for (int g = tid; g < G; g += nt) gsum[g] = group_total(gbin, G, g);
   __syncthreads();
   double val[5] = {sw, turn, fobj, rbox, rstat};
   const int op[5] = {0, 0, 0, 1, 1};

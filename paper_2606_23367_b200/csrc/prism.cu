@@ -55,9 +55,9 @@ static int dev_alloc(prism_problem* p, T** ptr, size_t count, bool zero = true) 
 
 extern "C" void prism_problem_destroy(prism_problem* p) {
   if (!p) return;
-  void* ptrs[] = {p->Bp, p->Bt, p->invd, p->gram, p->q, p->v, p->rt, p->cc, p->xs, p->pxq, p->Tpart, p->TE, p->V, p->Sinv,
-                  p->zE, p->yE, p->eE, p->resid, p->duals, p->status, p->ap.c, p->ap.rhoE, p->ap.alpha, p->ap.beta,
-                  p->ap.mode, p->ap.bsum, p->ap.rpE, p->ap.nE, p->ap.done, p->ap.conv, p->ap.iters, p->ap.refactor,
+  void* ptrs[] = {p->Bp, p->Bt, p->invd, p->gram, p->q, p->v, p->rt, p->cc, p->xs, p->pxq, p->Tpart, p->V, p->Sinv,
+                  p->gw0, p->lamG, p->resid, p->duals, p->status, p->ap.c, p->ap.alpha, p->ap.beta,
+                  p->ap.mode, p->ap.bsum, p->ap.done, p->ap.conv, p->ap.iters, p->ap.refactor,
                   p->ap.nadapt, p->counters, p->w_stage, p->i_stage};
   for (void* q : ptrs) if (q) cudaFree(q);
   if (p->h_counters) cudaFreeHost(p->h_counters);
@@ -71,6 +71,31 @@ struct Launcher {
   int mt;
   int gemm_mode;
   int64_t launches = 0;
+  bool prof = false;
+  struct Ev { cudaEvent_t a, b; int cls; };
+  std::vector<Ev> evs;
+  void begin(int cls) {
+    if (!prof) return;
+    Ev e; e.cls = cls;
+    cudaEventCreate(&e.a); cudaEventCreate(&e.b);
+    cudaEventRecord(e.a, st);
+    evs.push_back(e);
+  }
+  void end() {
+    if (prof) cudaEventRecord(evs.back().b, st);
+    ++launches;
+  }
+  // after a stream synchronize: per-class device time and launch counts
+  void collect(double* ms, int64_t* cnt) {
+    for (int i = 0; i < PRISM_NKERN; ++i) { ms[i] = 0.0; cnt[i] = 0; }
+    for (auto& e : evs) {
+      float t = 0.f;
+      cudaEventElapsedTime(&t, e.a, e.b);
+      ms[e.cls] += t; cnt[e.cls] += 1;
+      cudaEventDestroy(e.a); cudaEventDestroy(e.b);
+    }
+    evs.clear();
+  }
 
   Gemm1Args g1args(const double* X, const int32_t* done) const {
     Gemm1Args a;
@@ -80,6 +105,7 @@ struct Launcher {
   }
   void gemm1(const double* X, const int32_t* done) {
     Gemm1Args a = g1args(X, done);
+    begin(PRISM_K_GEMM1);
     if (gemm_mode == 1) {
       const int kp = p->kp;
       dim3 grid(p->nchunk, (unsigned)(((int64_t)p->A * kp + 127) / 128));
@@ -88,10 +114,11 @@ struct Launcher {
       dim3 grid(p->nchunk, (p->A + G1_TA - 1) / G1_TA);
       MT_SWITCH(mt, k_gemm1<MT><<<grid, 256, g1_smem(MT), st>>>(a));
     }
-    ++launches;
+    end();
   }
   template <int MODE>
   void gemm2(const Gemm2Args& a) {
+    begin(PRISM_K_GEMM2);
     if (gemm_mode == 1) {
       dim3 grid((unsigned)((p->N + 127) / 128), p->A);
       k_gemm2_ref<MODE><<<grid, 128, 0, st>>>(a);
@@ -99,13 +126,13 @@ struct Launcher {
       dim3 grid((unsigned)((p->N + G2_TN - 1) / G2_TN), (p->A + G2_TM - 1) / G2_TM);
       MT_SWITCH(mt, k_gemm2<MT, MODE><<<grid, 256, g2_smem(MT), st>>>(a));
     }
-    ++launches;
+    end();
   }
   Gemm2Args g2base() const {
     Gemm2Args a;
     memset(&a, 0, sizeof(a));
-    a.Bp = p->Bp; a.kp = p->kp; a.V = p->V; a.ldv = p->ldv; a.N = p->N; a.ldw = p->ldn; a.A = p->A; a.G = p->G;
-    a.group_id = p->d.group_id; a.invd = p->invd; a.d = p->d.d; a.gamma = p->d.gamma; a.c = p->ap.c;
+    a.Bp = p->Bp; a.kp = p->kp; a.V = p->V; a.ldv = p->ldv; a.N = p->N; a.ldw = p->ldn; a.A = p->A; a.G = 0;     // no consensus rows in the x-update: U = Bp
+    a.group_id = nullptr; a.invd = p->invd; a.d = p->d.d; a.gamma = p->d.gamma; a.c = p->ap.c;
     a.v = p->v; a.cc = p->cc; a.rt = p->rt; a.xs = p->xs; a.pxq = p->pxq; a.q = p->q; a.mu = p->d.mu;
     a.relax = 1.0; a.done = nullptr;
     return a;
@@ -113,8 +140,9 @@ struct Launcher {
   // pxq <- gamma Sigma X   (H8: Sigma W = B (F (B'W)) + D o W, fp64)
   void sigma_apply(const double* X) {
     gemm1(X, nullptr);
+    begin(PRISM_K_OTHER);
     k_scale_fs<<<p->A, 128, 0, st>>>(p->Tpart, p->nchunk, p->A, p->k, p->kp, p->ldv, p->d.f, p->d.gamma, p->V);
-    ++launches;
+    end();
     Gemm2Args a = g2base();
     a.X = X;
     gemm2<G2_SIGMA>(a);
@@ -142,7 +170,7 @@ extern "C" int prism_problem_create(int64_t N, int32_t k, int32_t accounts, cons
   if (!(cs->flags & PRISM_BUDGET) || !(cs->flags & PRISM_BOX)) return set_err(PRISM_ERR_INVALID_ARG, "PRISM_BUDGET and PRISM_BOX are mandatory%s", "");
   const int mt = pick_mt(k);
   if (mt < 0 || k > PRISM_MAX_FACTORS) return set_err(PRISM_ERR_INVALID_ARG, "k = %s%lld exceeds the supported factor count (128)", "", k);
-  if (G < 0 || G > PRISM_MAX_GROUPS || 8 * mt + G > PRISM_MAX_KPRIME) return set_err(PRISM_ERR_INVALID_ARG, "G = %s%lld out of range", "", G);
+  if (G < 0 || G > PRISM_MAX_GROUPS || 8 * mt > PRISM_MAX_KPRIME) return set_err(PRISM_ERR_INVALID_ARG, "G = %s%lld out of range", "", G);
   if ((cs->flags & PRISM_GROUP_BANDS) && (G < 1 || !data->group_id || !data->band_lo || !data->band_hi)) return set_err(PRISM_ERR_INVALID_ARG, "group bands need G >= 1, group_id, band_lo, band_hi%s", "");
   if ((cs->flags & PRISM_TAX_LOTS) && (!data->lot_slope || !data->lot_width || !data->lot_count || cs->max_lots < 1 || cs->max_lots > PRISM_MAX_LOTS)) return set_err(PRISM_ERR_INVALID_ARG, "tax lots need lot arrays and 1 <= max_lots <= 4%s", "");
   if (!data->B || !data->f || !data->d || !data->mu || !data->gamma || !data->w0 || !data->lo || !data->hi) return set_err(PRISM_ERR_INVALID_ARG, "missing mandatory data pointer%s", "");
@@ -152,7 +180,7 @@ extern "C" int prism_problem_create(int64_t N, int32_t k, int32_t accounts, cons
   prism_problem* p = new (std::nothrow) prism_problem();
   if (!p) return set_err(PRISM_ERR_ALLOC, "host allocation failed%s", "");
   memset(p, 0, sizeof(*p));
-  p->N = N; p->k = k; p->kp = 8 * mt; p->A = A; p->G = G; p->Kp = p->kp + G; p->ldv = (p->Kp + 7) / 8 * 8;
+  p->N = N; p->k = k; p->kp = 8 * mt; p->A = A; p->G = G; p->Kp = p->kp; p->ldv = (p->Kp + 7) / 8 * 8;
   p->flags = cs->flags; p->max_lots = (cs->flags & PRISM_TAX_LOTS) ? cs->max_lots : 0;
   p->d = *data;
   if (!(cs->flags & PRISM_TAX_LOTS)) { p->d.lot_slope = p->d.lot_width = nullptr; p->d.lot_count = nullptr; }
@@ -188,22 +216,18 @@ extern "C" int prism_problem_create(int64_t N, int32_t k, int32_t accounts, cons
   ALLOC_TRY(dev_alloc(p, &p->xs, AN));
   ALLOC_TRY(dev_alloc(p, &p->pxq, AN));
   ALLOC_TRY(dev_alloc(p, &p->Tpart, (size_t)p->nchunk * A * p->ldv));
-  ALLOC_TRY(dev_alloc(p, &p->TE, (size_t)A * (G ? G : 1)));
   ALLOC_TRY(dev_alloc(p, &p->V, (size_t)A * p->ldv));
   ALLOC_TRY(dev_alloc(p, &p->Sinv, (size_t)A * p->Kp * p->Kp));
-  ALLOC_TRY(dev_alloc(p, &p->zE, (size_t)A * (G ? G : 1)));
-  ALLOC_TRY(dev_alloc(p, &p->yE, (size_t)A * (G ? G : 1)));
+  ALLOC_TRY(dev_alloc(p, &p->gw0, (size_t)A * (G ? G : 1)));
+  ALLOC_TRY(dev_alloc(p, &p->lamG, (size_t)A * (G ? G : 1)));
   ALLOC_TRY(dev_alloc(p, &p->resid, (size_t)A * PRISM_NRES));
   ALLOC_TRY(dev_alloc(p, &p->duals, (size_t)A * PRISM_NDUAL(G)));
   ALLOC_TRY(dev_alloc(p, &p->status, (size_t)A));
   ALLOC_TRY(dev_alloc(p, &p->ap.c, (size_t)A));
-  ALLOC_TRY(dev_alloc(p, &p->ap.rhoE, (size_t)A));
   ALLOC_TRY(dev_alloc(p, &p->ap.alpha, (size_t)A));
   ALLOC_TRY(dev_alloc(p, &p->ap.beta, (size_t)A));
   ALLOC_TRY(dev_alloc(p, &p->ap.mode, (size_t)A));
   ALLOC_TRY(dev_alloc(p, &p->ap.bsum, (size_t)A));
-  ALLOC_TRY(dev_alloc(p, &p->ap.rpE, (size_t)A));
-  ALLOC_TRY(dev_alloc(p, &p->ap.nE, (size_t)A));
   ALLOC_TRY(dev_alloc(p, &p->ap.done, (size_t)A));
   ALLOC_TRY(dev_alloc(p, &p->ap.conv, (size_t)A));
   ALLOC_TRY(dev_alloc(p, &p->ap.iters, (size_t)A));
@@ -215,7 +239,7 @@ extern "C" int prism_problem_create(int64_t N, int32_t k, int32_t accounts, cons
   { int r = set_kernel_attrs(mt, p->Kp); if (r != PRISM_OK) { prism_problem_destroy(p); return r; } }
 
   k_setup_shared<<<(unsigned)((N + 127) / 128), 128, 0, st>>>(data->B, data->B_is_fp32, data->d, N, k, p->kp, p->ldn, p->Bp, p->Bt, p->invd);
-  k_gram<<<dim3(p->Kp, p->Kp), 256, 0, st>>>(p->Bt, p->ldn, p->d.group_id, p->invd, N, p->kp, G, p->gram);
+  k_gram<<<dim3(p->Kp, p->Kp), 256, 0, st>>>(p->Bt, p->ldn, nullptr, p->invd, N, p->kp, 0, p->gram);
   if (p->d.w_b) {            // q = -mu - gamma Sigma w_b
     Launcher L{p, st, mt, 0};
     k_diff<<<dim3((unsigned)((N + 255) / 256), A), 256, 0, st>>>(p->d.w_b, nullptr, N, p->ldn, p->rt);
@@ -246,9 +270,10 @@ static ProxArgs make_prox_args(prism_problem* p, const prism_settings& s, double
   a.mu = p->d.mu; a.q = p->q; a.w0 = p->d.w0; a.gamma = p->d.gamma; a.lo = p->d.lo; a.hi = p->d.hi; a.hi_full = p->d.hi_full;
   a.tau = p->d.tau; a.kappa = p->d.kappa; a.c_buy = p->d.c_buy; a.lot_slope = p->d.lot_slope; a.lot_width = p->d.lot_width;
   a.excl = p->d.excl; a.lot_count = p->d.lot_count; a.group_id = p->d.group_id; a.invd = p->invd; a.d = p->d.d;
-  a.v = p->v; a.rt = p->rt; a.cc = p->cc; a.TE = p->TE; a.xs = p->xs; a.pxq = p->pxq; a.zE = p->zE; a.yE = p->yE;
+  a.v = p->v; a.rt = p->rt; a.cc = p->cc; a.xs = p->xs; a.pxq = p->pxq; a.band_lo = p->d.band_lo; a.band_hi = p->d.band_hi;
+  a.lamG = p->lamG; a.gw0 = p->gw0;
   a.ap = p->ap; a.w_out = w_out; a.duals = p->duals; a.resid = p->resid; a.counters = p->counters;
-  a.eps = s.eps_rel; a.dbar_GN = p->G ? p->dbar * (double)p->G / (double)p->N : 0.0; a.band_scale = s.rho_band_scale;
+  a.eps = s.eps_rel;
   a.adapt = s.adapt_rho; a.iter = 0; a.ldw = p->ldn;
   return a;
 }
@@ -272,13 +297,15 @@ static DiagArgs make_diag_args(prism_problem* p, const double* w, const double* 
 
 // resid (device, A x NRES) <- diagnostics of w; uses rt and pxq as scratch
 static void run_diag(prism_problem* p, Launcher& L, const double* w, const double* duals, double* resid) {
+  L.begin(PRISM_K_OTHER);
   k_diff<<<dim3((unsigned)((p->N + 255) / 256), p->A), 256, 0, L.st>>>(w, p->d.w_b, p->N, p->ldn, p->rt);
-  ++L.launches;
+  L.end();
   L.sigma_apply(p->rt);
   DiagArgs da = make_diag_args(p, w, duals, resid);
+  L.begin(PRISM_K_DIAG);
   if (p->d.lot_count) k_diag<true><<<p->A, 256, 0, L.st>>>(da);
   else k_diag<false><<<p->A, 256, 0, L.st>>>(da);
-  ++L.launches;
+  L.end();
 }
 
 extern "C" int prism_solve_batch(prism_problem* p, const prism_settings* sp, void* cuda_stream, double* w_out,
@@ -305,17 +332,18 @@ extern "C" int prism_solve_batch(prism_problem* p, const prism_settings* sp, voi
   CUDA_TRY(cudaMemsetAsync(p->resid, 0, (size_t)A * PRISM_NRES * sizeof(double), st));
   InitArgs ia;
   memset(&ia, 0, sizeof(ia));
-  ia.N = p->N; ia.ldw = p->ldn; ia.A = A; ia.G = G; ia.w0 = p->d.w0; ia.gamma = p->d.gamma; ia.band_lo = p->d.band_lo; ia.band_hi = p->d.band_hi;
-  ia.group_id = p->d.group_id; ia.v = p->v; ia.zE = p->zE; ia.yE = p->yE; ia.ap = p->ap; ia.rho_scale = s.rho_scale;
-  ia.band_scale = s.rho_band_scale; ia.dbar_GN = G ? p->dbar * (double)G / (double)p->N : 0.0;
+  ia.N = p->N; ia.ldw = p->ldn; ia.A = A; ia.G = G; ia.w0 = p->d.w0; ia.gamma = p->d.gamma;
+  ia.group_id = p->d.group_id; ia.v = p->v; ia.gw0 = p->gw0; ia.lamG = p->lamG; ia.ap = p->ap; ia.rho_scale = s.rho_scale;
+  L.prof = s.profile != 0;
+  L.begin(PRISM_K_OTHER);
   k_init_accounts<<<A, 256, 0, st>>>(ia);
-  ++L.launches;
+  L.end();
 
   ProxArgs pa = make_prox_args(p, s, w_out);
   SolveArgs sa;
   memset(&sa, 0, sizeof(sa));
-  sa.A = A; sa.G = G; sa.kp = p->kp; sa.nchunk = p->nchunk; sa.ldv = p->ldv; sa.Tpart = p->Tpart; sa.TE = p->TE; sa.Sinv = p->Sinv;
-  sa.band_lo = p->d.band_lo; sa.band_hi = p->d.band_hi; sa.V = p->V; sa.zE = p->zE; sa.yE = p->yE; sa.ap = p->ap; sa.relax = s.alpha;
+  sa.A = A; sa.kp = p->kp; sa.nchunk = p->nchunk; sa.ldv = p->ldv; sa.Tpart = p->Tpart; sa.Sinv = p->Sinv;
+  sa.V = p->V; sa.ap = p->ap;
   Gemm2Args g2 = L.g2base();
   g2.relax = s.alpha; g2.done = p->ap.done;
   const size_t fac_smem = (size_t)p->Kp * p->Kp * sizeof(double);
@@ -323,11 +351,13 @@ extern "C" int prism_solve_batch(prism_problem* p, const prism_settings* sp, voi
   int it = 1, timed_out = 0, late_iter = -1, ndone = 0;
   for (; it <= s.max_iter; ++it) {
     const bool check = (it > 1) && ((it - 1) % s.check_every == 0);   // residuals of the iterate after it-1 iterations
+    L.begin(PRISM_K_PROX);
     launch_prox(p, st, pa, check ? PROX_CHECK : 0, it - 1);
-    ++L.launches;
+    L.end();
     if (check || it == 1) {
-      k_factor<<<A, 256, fac_smem, st>>>(p->gram, p->d.f, p->d.gamma, p->ap, p->k, p->kp, G, p->Sinv);
-      ++L.launches;
+      L.begin(PRISM_K_FACTOR);
+      k_factor<<<A, 256, fac_smem, st>>>(p->gram, p->d.f, p->d.gamma, p->ap, p->k, p->kp, 0, p->Sinv);
+      L.end();
     }
     if (check) {
       CUDA_TRY(cudaMemcpyAsync(p->h_counters, p->counters, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
@@ -339,19 +369,22 @@ extern "C" int prism_solve_batch(prism_problem* p, const prism_settings* sp, voi
       if (s.time_limit_ms > 0 && el > s.time_limit_ms) { timed_out = 1; break; }
     }
     L.gemm1(p->rt, p->ap.done);
+    L.begin(PRISM_K_SOLVE);
     k_solve<<<A, 128, 0, st>>>(sa);
-    ++L.launches;
+    L.end();
     const bool next_check = (it % s.check_every == 0);
     if (next_check) L.gemm2<G2_ADMM_CHECK>(g2); else L.gemm2<G2_ADMM>(g2);
   }
   if (ndone < A) {           // iteration cap or time limit: extract z for the accounts still running
+    L.begin(PRISM_K_PROX);
     launch_prox(p, st, pa, PROX_FINAL, it > s.max_iter ? s.max_iter : it - 1);
-    ++L.launches;
+    L.end();
   }
   // H8 / H9: external diagnostics of the returned weights with the solver's multipliers, then statuses
   run_diag(p, L, w_out, p->duals, p->resid);
+  L.begin(PRISM_K_OTHER);
   k_status<<<(A + 127) / 128, 128, 0, st>>>(A, p->resid, p->ap.conv, p->ap.iters, timed_out, late_iter, 1e-6, p->status);
-  ++L.launches;
+  L.end();
   if (status_out != p->status) CUDA_TRY(cudaMemcpyAsync(status_out, p->status, (size_t)A * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
   CUDA_TRY(cudaMemcpyAsync(iters_out, p->ap.iters, (size_t)A * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
   if (resid_out) CUDA_TRY(cudaMemcpyAsync(resid_out, p->resid, (size_t)A * PRISM_NRES * sizeof(double), cudaMemcpyDeviceToDevice, st));
@@ -362,6 +395,7 @@ extern "C" int prism_solve_batch(prism_problem* p, const prism_settings* sp, voi
   CUDA_TRY(cudaMemcpyAsync(hi.data(), p->ap.iters, (size_t)A * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
   CUDA_TRY(cudaStreamSynchronize(st));
   CUDA_TRY(cudaGetLastError());
+  if (L.prof) L.collect(p->prof_ms, p->prof_cnt);
   if (info) {
     memset(info, 0, sizeof(*info));
     float ms = 0.f;
@@ -385,6 +419,12 @@ extern "C" int prism_solve_batch(prism_problem* p, const prism_settings* sp, voi
   }
   cudaEventDestroy(ev0);
   cudaEventDestroy(ev1);
+  return PRISM_OK;
+}
+
+extern "C" int prism_kernel_times(const prism_problem* p, double* ms_out, int64_t* launches_out) {
+  if (!p || !ms_out || !launches_out) return set_err(PRISM_ERR_INVALID_ARG, "null argument%s", "");
+  for (int i = 0; i < PRISM_NKERN; ++i) { ms_out[i] = p->prof_ms[i]; launches_out[i] = p->prof_cnt[i]; }
   return PRISM_OK;
 }
 

@@ -16,6 +16,15 @@
 // Each is continuous piecewise linear; solved by safeguarded Newton (bracketed, exact on the final linear piece),
 // warm-started from the previous iteration.  All trial evaluations are block-wide reductions in this CTA.
 //
+// Group bands (Eq. (1) row 3 with A_a = group indicators) are handled in the same projection: with
+// multipliers lambda_g (> 0: upper band active, < 0: lower band active) the thresholds of an asset of group g
+// become alpha + lambda_g and beta + lambda_g.  For fixed lambda the (alpha, beta) equations keep their form; the
+// group sums S_g(lambda_g) (with alpha, beta re-solved) are monotone, so violated / active groups are fixed one
+// at a time by a bracketed scalar Newton iteration on lambda_g (Gauss-Seidel over groups, usually 0 or 1 group).
+// Putting ALL polyhedral constraints into this projection (instead of a consensus block in the x-update) is what
+// makes the splitting converge in a few hundred iterations: a consensus row's dual moves at rate
+// (#moving assets)/(#assets in the row) per iteration ("why the bands live in the prox").
+//
 // The same kernel then emits what the x-update needs (r~ = M^-1 r, c = r~ - z, per-group sums of r~), and on check
 // iterations the scaled residuals, the convergence mask and the per-account rho adaptation.
 #pragma once
@@ -31,16 +40,18 @@ struct ProxArgs {
   const double* invd;
   const double* d;
   // iterate
-  double *v, *rt, *cc, *TE;
+  double *v, *rt, *cc;
   const double *xs, *pxq;
-  const double *zE, *yE;
+  const double *band_lo, *band_hi;
+  double *lamG;             // A x G band multipliers (warm start, persists across iterations)
+  const double *gw0;        // A x G group sums of w0
   AccountParams ap;
   double* w_out;
   double* duals;
   double* resid;
   int32_t* counters;
   // settings
-  double eps, dbar_GN, band_scale;   // dbar_GN = mean(d) * G / N
+  double eps;
   int32_t adapt, iter;
 };
 
@@ -121,9 +132,10 @@ __device__ __forceinline__ void root_step(Root1D& r, double g, double slope, dou
 template <bool LOTS>
 __global__ void __launch_bounds__(512) k_prox(ProxArgs p, int mode) {
   __shared__ double scratch[8 * 32];
-  __shared__ double teS[PRISM_MAX_GROUPS];
-  __shared__ double eS[PRISM_MAX_GROUPS];
-  __shared__ double yES[PRISM_MAX_GROUPS];
+  __shared__ double gbin[16 * PRISM_MAX_GROUPS];    // per-warp group bins (deterministic accumulation)
+  __shared__ double lamS[PRISM_MAX_GROUPS];
+  __shared__ double gsum[PRISM_MAX_GROUPS];
+  __shared__ int selS[2];
   const int a = blockIdx.x;
   if (p.ap.done[a]) return;
   const int tid = threadIdx.x, nt = blockDim.x;
@@ -136,48 +148,52 @@ __global__ void __launch_bounds__(512) k_prox(ProxArgs p, int mode) {
   const double lam_b = kappa + (p.c_buy ? p.c_buy[a] : 0.0);
   const double tau = p.tau ? p.tau[a] : INFINITY;
   const double b = p.ap.bsum[a];
-  const int L = PRISM_MAX_LOTS;
+  const int L = PRISM_MAX_LOTS, G = p.G;
+  for (int g = tid; g < G; g += nt) lamS[g] = p.lamG[(int64_t)a * G + g];
+  __syncthreads();
 
-  // ---------------------------------------------------------------- pass 0: value at the warm start + brackets
   double alpha = p.ap.alpha[a], beta = p.ap.beta[a];
   int amode = p.ap.mode[a];
   if (!(amode == 1 && isfinite(tau))) { amode = 0; beta = alpha; }
   double a_min = INFINITY, a_max = -INFINITY, b_min = INFINITY, b_max = -INFINITY;
-  double P = 0, R = 0, sP = 0, sR = 0;
-  auto eval = [&](double al, double be, bool extremes) {
-    double lP = 0, lR = 0, lsP = 0, lsR = 0, amn = INFINITY, amx = -INFINITY, bmn = INFINITY, bmx = -INFINITY;
+  double P = 0, R = 0, sP = 0, sR = 0, Pa = 0, Ra = 0, pa = 0, ra = 0;
+  // one pass over the account: totals at thresholds (al, be) shifted by the group multipliers; with sel >= 0 also
+  // the sums of group `sel`; with extremes the range of the breakpoints (brackets).
+  auto eval = [&](double al, double be, int sel, bool extremes) {
+    double lP = 0, lR = 0, lsP = 0, lsR = 0, x4 = 0, x5 = 0, x6 = 0, x7 = 0;
+    if (extremes) { x4 = INFINITY; x5 = -INFINITY; x6 = INFINITY; x7 = -INFINITY; }
     for (int64_t i = tid; i < N; i += nt) {
       const ElemConst e = load_elem(p, row, rowp, i, cg, lo_a, hi_a);
       double mvb, mvs;
       int nl = 0;
       const double *sl = nullptr, *wd = nullptr;
       if (LOTS) { nl = p.lot_count[row + i]; sl = p.lot_slope + (row + i) * L; wd = p.lot_width + (row + i) * L; }
-      lP += buy_amt(e, lam_b, al, mvb);
-      lR += sell_amt<LOTS>(e, kappa, be, sl, wd, nl, mvs);
-      lsP += mvb; lsR += mvs;
+      const int g = G ? p.group_id[i] : 0;
+      const double lg = G ? lamS[g] : 0.0;
+      const double pb = buy_amt(e, lam_b, al + lg, mvb);
+      const double ps = sell_amt<LOTS>(e, kappa, be + lg, sl, wd, nl, mvs);
+      lP += pb; lR += ps; lsP += mvb; lsR += mvs;
       if (extremes) {
         const double rho = 1.0 / e.ir;
-        if (e.bh > e.bl) { amn = fmin(amn, e.rho_u - lam_b - rho * e.bh); amx = fmax(amx, e.rho_u - lam_b - rho * e.bl); }
+        if (e.bh > e.bl) { x4 = fmin(x4, e.rho_u - lam_b - rho * e.bh); x5 = fmax(x5, e.rho_u - lam_b - rho * e.bl); }
         double sh = e.sh, s_first = 0.0, s_last = 0.0;
         if (LOTS && nl > 0) { double Q = 0; for (int l = 0; l < nl; ++l) Q += wd[l]; sh = fmin(sh, Q); s_first = sl[0]; s_last = sl[nl - 1]; }
-        if (sh > e.sl) { bmn = fmin(bmn, e.rho_u + kappa + s_first + rho * e.sl); bmx = fmax(bmx, e.rho_u + kappa + s_last + rho * sh); }
-      }
+        if (sh > e.sl) { x6 = fmin(x6, e.rho_u + kappa + s_first + rho * e.sl); x7 = fmax(x7, e.rho_u + kappa + s_last + rho * sh); }
+      } else if (g == sel) { x4 += pb; x5 += ps; x6 += mvb; x7 += mvs; }
     }
+    double val[8] = {lP, lR, lsP, lsR, x4, x5, x6, x7};
     if (extremes) {
-      double val[8] = {lP, lR, lsP, lsR, amn, amx, bmn, bmx};
       const int op[8] = {0, 0, 0, 0, 2, 1, 2, 1};
       block_reduce<8>(val, op, scratch);
-      P = val[0]; R = val[1]; sP = val[2]; sR = val[3];
       a_min = val[4]; a_max = val[5]; b_min = val[6]; b_max = val[7];
     } else {
-      double val[4] = {lP, lR, lsP, lsR};
-      const int op[4] = {0, 0, 0, 0};
-      block_reduce<4>(val, op, scratch);
-      P = val[0]; R = val[1]; sP = val[2]; sR = val[3];
+      const int op[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+      block_reduce<8>(val, op, scratch);
+      Pa = val[4]; Ra = val[5]; pa = val[6]; ra = val[7];
     }
+    P = val[0]; R = val[1]; sP = val[2]; sR = val[3];
   };
-  eval(alpha, beta, true);
-  // finite brackets (with a margin so that the end values are the saturated sums)
+  eval(alpha, beta, -1, true);
   const double span = fmax(fmax(fabs(a_min), fabs(a_max)), fmax(fabs(b_min), fabs(b_max)));
   const double pad = 1e-9 * fmax(span, 1e-300) + 1e-300;
   if (!(a_min <= a_max)) { a_min = -1.0; a_max = 1.0; }
@@ -185,41 +201,110 @@ __global__ void __launch_bounds__(512) k_prox(ProxArgs p, int mode) {
   a_min -= pad; a_max += pad; b_min -= pad; b_max += pad;
   const double tol = 2e-15 * fmax(1.0, fabs(b) + (isfinite(tau) ? tau : 0.0));
   const double Pt = 0.5 * (tau + b), Rt = 0.5 * (tau - b);
+  const double Lmax = 2.0 * (fmax(a_max, b_max) - fmin(a_min, b_min)) + 1.0;
+  bool fresh = true;     // P, R, ... correspond to (alpha, beta, lamS, sel = -1)
 
-  for (int attempt = 0; attempt < 3; ++attempt) {
-    if (amode == 1) {
-      // cap active: two independent equations
-      Root1D ra = {fmin(fmax(alpha, a_min), a_max), a_min, a_max, 0};
-      Root1D rb = {fmin(fmax(beta, b_min), b_max), b_min, b_max, 0};
-      if (ra.x != alpha || rb.x != beta || attempt > 0) eval(ra.x, rb.x, false);
-      for (int it = 0; it < 80; ++it) {
-        root_step(ra, P, sP, Pt, -1, tol);
-        root_step(rb, R, sR, Rt, +1, tol);
-        if (ra.done && rb.done) break;
-        eval(ra.x, rb.x, false);
+  // (alpha, beta) for the current group multipliers; leaves the sums of the final thresholds (and of group sel)
+  auto solve_ab = [&](int sel) {
+    double lmin = 0.0, lmax = 0.0;
+    for (int g = 0; g < G; ++g) { lmin = fmin(lmin, lamS[g]); lmax = fmax(lmax, lamS[g]); }
+    const double alo = a_min - lmax, ahi = a_max - lmin, blo = b_min - lmax, bhi = b_max - lmin;
+    for (int attempt = 0; attempt < 3; ++attempt) {
+      if (amode == 1) {
+        Root1D ra_ = {fmin(fmax(alpha, alo), ahi), alo, ahi, 0};
+        Root1D rb_ = {fmin(fmax(beta, blo), bhi), blo, bhi, 0};
+        if (!fresh || sel >= 0 || ra_.x != alpha || rb_.x != beta) eval(ra_.x, rb_.x, sel, false);
+        fresh = false;
+        for (int it = 0; it < 80; ++it) {
+          root_step(ra_, P, sP, Pt, -1, tol);
+          root_step(rb_, R, sR, Rt, +1, tol);
+          if (ra_.done && rb_.done) break;
+          eval(ra_.x, rb_.x, sel, false);
+        }
+        alpha = ra_.x; beta = rb_.x;
+        if (alpha >= beta) break;
+        amode = 0; alpha = beta = 0.5 * (alpha + beta);
+      } else {
+        const double lo_b = fmin(alo, blo), hi_b = fmax(ahi, bhi);
+        Root1D rn = {fmin(fmax(alpha, lo_b), hi_b), lo_b, hi_b, 0};
+        if (!fresh || sel >= 0 || rn.x != alpha || beta != alpha) eval(rn.x, rn.x, sel, false);
+        fresh = false;
+        for (int it = 0; it < 80; ++it) {
+          root_step(rn, P - R, sP + sR, b, -1, tol);
+          if (rn.done) break;
+          eval(rn.x, rn.x, sel, false);
+        }
+        alpha = beta = rn.x;
+        if (!isfinite(tau) || P + R <= tau + tol) break;
+        amode = 1;
       }
-      alpha = ra.x; beta = rb.x;
-      if (alpha >= beta) break;          // theta >= 0: accepted
-      amode = 0; alpha = beta = 0.5 * (alpha + beta);
-    } else {
-      const double lo_b = fmin(a_min, b_min), hi_b = fmax(a_max, b_max);
-      Root1D rn = {fmin(fmax(alpha, lo_b), hi_b), lo_b, hi_b, 0};
-      if (rn.x != alpha || attempt > 0 || beta != alpha) eval(rn.x, rn.x, false);
-      for (int it = 0; it < 80; ++it) {
-        root_step(rn, P - R, sP + sR, b, -1, tol);
-        if (rn.done) break;
-        eval(rn.x, rn.x, false);
-      }
-      alpha = beta = rn.x;
-      if (!isfinite(tau) || P + R <= tau + tol) break;   // cap inactive: accepted
-      amode = 1;
     }
-  }
+  };
 
-  // ---------------------------------------------------------------- group data of the band block
-  const int G = p.G;
-  double rhoE = p.ap.rhoE[a];
-  for (int g = tid; g < G; g += nt) { teS[g] = 0.0; yES[g] = p.yE[(int64_t)a * G + g]; }
+  for (int round = 0; round < 2 * G + 2; ++round) {
+    solve_ab(-1);
+    if (G == 0) break;
+    // all group sums at the current solution (deterministic binned pass)
+    for (int g = tid; g < 16 * G; g += nt) gbin[g] = 0.0;
+    __syncthreads();
+    for (int64_t i0 = 0; i0 < N; i0 += nt) {
+      const int64_t i = i0 + tid;
+      const bool valid = i < N;
+      double t = 0.0; int g = 0;
+      if (valid) {
+        const ElemConst e = load_elem(p, row, rowp, i, cg, lo_a, hi_a);
+        double mvb, mvs; int nl = 0; const double *sl = nullptr, *wd = nullptr;
+        if (LOTS) { nl = p.lot_count[row + i]; sl = p.lot_slope + (row + i) * L; wd = p.lot_width + (row + i) * L; }
+        g = p.group_id[i];
+        t = buy_amt(e, lam_b, alpha + lamS[g], mvb) - sell_amt<LOTS>(e, kappa, beta + lamS[g], sl, wd, nl, mvs);
+      }
+      warp_group_add(gbin, G, g, t, valid);
+    }
+    __syncthreads();
+    for (int g = tid; g < G; g += nt) gsum[g] = p.gw0[(int64_t)a * G + g] + group_total(gbin, G, g);
+    __syncthreads();
+    if (tid == 0) {
+      int sel = -1, sgn = 0; double worst = 8.0 * tol;
+      for (int g = 0; g < G; ++g) {
+        const double bl_ = p.band_lo[(int64_t)a * G + g], bh_ = p.band_hi[(int64_t)a * G + g];
+        double viol; int sg;
+        if (lamS[g] > 0.0) { viol = fabs(gsum[g] - bh_); sg = +1; }
+        else if (lamS[g] < 0.0) { viol = fabs(gsum[g] - bl_); sg = -1; }
+        else if (gsum[g] > bh_) { viol = gsum[g] - bh_; sg = +1; }
+        else { viol = bl_ - gsum[g]; sg = -1; }
+        if (viol > worst) { worst = viol; sel = g; sgn = sg; }
+      }
+      selS[0] = sel; selS[1] = sgn;
+    }
+    __syncthreads();
+    const int sel = selS[0], sgn = selS[1];
+    if (sel < 0) break;
+    // scalar problem in m = sgn * lambda_sel >= 0:  h(m) = sgn * (S_sel - bound) is non-increasing, want h = 0 or m = 0
+    const double bound = sgn > 0 ? p.band_hi[(int64_t)a * G + sel] : p.band_lo[(int64_t)a * G + sel];
+    const double gw = p.gw0[(int64_t)a * G + sel];
+    double m = sgn * lamS[sel], mlo = 0.0, mhi = Lmax;
+    bool lo_known = false;      // h(mlo) > 0 established
+    for (int it = 0; it < 60; ++it) {
+      __syncthreads();
+      if (tid == 0) lamS[sel] = sgn * m;
+      __syncthreads();
+      solve_ab(sel);
+      const double h = sgn * (gw + Pa - Ra - bound);
+      if (fabs(h) <= tol) break;
+      if (m == 0.0 && h < 0.0) break;                    // band inactive at lambda = 0
+      double slope = pa + ra;
+      if (amode == 1) slope -= (sP > 0.0 ? pa * pa / sP : 0.0) + (sR > 0.0 ? ra * ra / sR : 0.0);
+      else slope -= (sP + sR > 0.0 ? (pa + ra) * (pa + ra) / (sP + sR) : 0.0);
+      if (h > 0.0) { mlo = m; lo_known = true; } else mhi = m;
+      double mn = slope > 1e-300 ? m + h / slope : NAN;
+      if (!(mn == mn)) mn = lo_known || mlo > 0.0 ? 0.5 * (mlo + mhi) : 0.0;
+      if (mn <= mlo) mn = lo_known ? 0.5 * (mlo + mhi) : 0.0;
+      if (mn >= mhi) mn = 0.5 * (mlo + mhi);
+      if (mn == m) break;
+      m = mn;
+    }
+    fresh = false;
+  }
   __syncthreads();
 
   // ---------------------------------------------------------------- check: residuals, mask, rho adaptation
@@ -231,22 +316,20 @@ __global__ void __launch_bounds__(512) k_prox(ProxArgs p, int mode) {
       const ElemConst e = load_elem(p, row, rowp, i, cg, lo_a, hi_a);
       double mvb, mvs; int nl = 0; const double *sl = nullptr, *wd = nullptr;
       if (LOTS) { nl = p.lot_count[row + i]; sl = p.lot_slope + (row + i) * L; wd = p.lot_width + (row + i) * L; }
-      const double z = e.w0 + buy_amt(e, lam_b, alpha, mvb) - sell_amt<LOTS>(e, kappa, beta, sl, wd, nl, mvs);
+      const double lg = G ? lamS[p.group_id[i]] : 0.0;
+      const double z = e.w0 + buy_amt(e, lam_b, alpha + lg, mvb) - sell_amt<LOTS>(e, kappa, beta + lg, sl, wd, nl, mvs);
       const double vv = p.v[rowp + i];
       const double y = (vv - z) / e.ir;
       const double x = p.xs[rowp + i], pq = p.pxq[rowp + i];
       const double qi = p.q ? p.q[rowp + i] : -p.mu[row + i];
-      const double ye = G ? yES[p.group_id[i]] : 0.0;
       nx = fmax(nx, fabs(x)); nz = fmax(nz, fabs(z)); nrp = fmax(nrp, fabs(x - z));
-      nrd = fmax(nrd, fabs(pq + y + ye)); nPx = fmax(nPx, fabs(pq - qi)); ny = fmax(ny, fabs(y + ye)); nq = fmax(nq, fabs(qi));
-      // NaN guard: fmax drops NaN, so poison explicitly
-      if (!(z == z) || !(x == x) || !(vv == vv)) nrp = INFINITY;
+      nrd = fmax(nrd, fabs(pq + y)); nPx = fmax(nPx, fabs(pq - qi)); ny = fmax(ny, fabs(y)); nq = fmax(nq, fabs(qi));
+      if (!(z == z) || !(x == x) || !(vv == vv)) nrp = INFINITY;     // fmax drops NaN: poison explicitly
     }
     double val[7] = {nx, nz, nrp, nrd, nPx, ny, nq};
     const int op[7] = {1, 1, 1, 1, 1, 1, 1};
     block_reduce<7>(val, op, scratch);
-    double rp = val[2] / fmax(fmax(val[0], val[1]), 1e-300);
-    if (G) rp = fmax(rp, p.ap.rpE[a] / fmax(p.ap.nE[a], 1e-300));
+    const double rp = val[2] / fmax(fmax(val[0], val[1]), 1e-300);
     const double rd = val[3] / fmax(fmax(val[4], fmax(val[5], val[6])), 1e-300);
     const bool bad = !(rp < INFINITY) || !(rd < INFINITY);
     const bool conv = !bad && rp <= p.eps && rd <= p.eps;
@@ -256,24 +339,18 @@ __global__ void __launch_bounds__(512) k_prox(ProxArgs p, int mode) {
     }
     if (conv || bad) {
       finished = 1;
-      if (tid == 0) {
-        p.ap.conv[a] = conv ? 1 : 0;
-        if (bad) p.ap.conv[a] = -1;
-      }
+      if (tid == 0) p.ap.conv[a] = bad ? -1 : 1;
     } else if (p.adapt) {
       const double ratio = sqrt(rp / fmax(rd, 1e-300));
       if ((ratio > 5.0 || ratio < 0.2) && p.ap.nadapt[a] < 20) {
         const double cn = c * fmin(fmax(ratio, 0.1), 10.0);
         rescale = c / cn;          // v' = z + (rho/rho') (v - z) keeps y = rho (v - z) unchanged
         c = cn; cg = c * gam;
-        rhoE = p.band_scale * c * gam * p.dbar_GN;
-        if (tid == 0) { p.ap.c[a] = c; p.ap.rhoE[a] = rhoE; p.ap.refactor[a] = 1; p.ap.nadapt[a] += 1; }
+        if (tid == 0) { p.ap.c[a] = c; p.ap.refactor[a] = 1; p.ap.nadapt[a] += 1; }
       }
     }
   }
   if (mode & PROX_FINAL) finished = 1;
-  for (int g = tid; g < G; g += nt) eS[g] = rhoE * p.zE[(int64_t)a * G + g] - yES[g];
-  __syncthreads();
 
   // ---------------------------------------------------------------- output pass
   const double cg_old = cg * rescale;     // rho scale the stored v refers to (c_old * gamma)
@@ -281,7 +358,8 @@ __global__ void __launch_bounds__(512) k_prox(ProxArgs p, int mode) {
     const ElemConst e = load_elem(p, row, rowp, i, cg_old, lo_a, hi_a);
     double mvb, mvs; int nl = 0; const double *sl = nullptr, *wd = nullptr;
     if (LOTS) { nl = p.lot_count[row + i]; sl = p.lot_slope + (row + i) * L; wd = p.lot_width + (row + i) * L; }
-    const double z = e.w0 + buy_amt(e, lam_b, alpha, mvb) - sell_amt<LOTS>(e, kappa, beta, sl, wd, nl, mvs);
+    const double lg = G ? lamS[p.group_id[i]] : 0.0;
+    const double z = e.w0 + buy_amt(e, lam_b, alpha + lg, mvb) - sell_amt<LOTS>(e, kappa, beta + lg, sl, wd, nl, mvs);
     if (finished) { p.w_out[row + i] = z; continue; }
     double vv = p.v[rowp + i];
     const double y = (vv - z) / e.ir;                      // rho_old (v - z)
@@ -289,15 +367,12 @@ __global__ void __launch_bounds__(512) k_prox(ProxArgs p, int mode) {
     const double dinv = p.invd[i];
     const double rho = cg / dinv;                          // new rho_i
     const double qi = p.q ? p.q[rowp + i] : -p.mu[row + i];
-    const int g = G ? p.group_id[i] : 0;
-    const double r = rho * z - y - qi + (G ? eS[g] : 0.0);
+    const double r = rho * z - y - qi;
     const double rt = r * dinv / (gam * (1.0 + c));        // M_i = gamma d_i (1 + c)
     p.rt[rowp + i] = rt;
     p.cc[rowp + i] = rt - z;
-    if (G) atomicAdd(&teS[g], rt);
   }
-  __syncthreads();
-  if (!finished) for (int g = tid; g < G; g += nt) p.TE[(int64_t)a * G + g] = teS[g];
+  for (int g = tid; g < G; g += nt) p.lamG[(int64_t)a * G + g] = lamS[g];
   if (tid == 0) {
     p.ap.alpha[a] = alpha; p.ap.beta[a] = beta; p.ap.mode[a] = amode;
     if (finished) {
@@ -307,7 +382,7 @@ __global__ void __launch_bounds__(512) k_prox(ProxArgs p, int mode) {
       double* du = p.duals + (int64_t)a * PRISM_NDUAL(G);
       du[0] = 0.5 * (alpha + beta);
       du[1] = 0.5 * (alpha - beta);
-      for (int g = 0; g < G; ++g) { du[2 + g] = fmax(yES[g], 0.0); du[2 + G + g] = fmax(-yES[g], 0.0); }
+      for (int g = 0; g < G; ++g) { du[2 + g] = fmax(lamS[g], 0.0); du[2 + G + g] = fmax(-lamS[g], 0.0); }
       p.resid[(int64_t)a * PRISM_NRES + PRISM_R_RHO] = c;
     }
   }

@@ -40,45 +40,48 @@ __global__ void k_gram(const double* Bt, int64_t ldn, const uint8_t* gid, const 
 // ---------------------------------------------------------------------------------- per-account cold start
 struct InitArgs {
   int64_t N, ldw; int32_t A, G;
-  const double *w0, *gamma, *band_lo, *band_hi;
+  const double *w0, *gamma;
   const uint8_t* group_id;
-  double *v, *zE, *yE;
+  double *v, *gw0, *lamG;
   AccountParams ap;
-  double rho_scale, band_scale, dbar_GN;
+  double rho_scale;
 };
 __global__ void k_init_accounts(InitArgs p) {
   __shared__ double scratch[32];
-  __shared__ double gs[PRISM_MAX_GROUPS];
+  __shared__ double gs[8 * PRISM_MAX_GROUPS];
   const int a = blockIdx.x, tid = threadIdx.x;
-  for (int g = tid; g < p.G; g += blockDim.x) gs[g] = 0.0;
+  for (int g = tid; g < 8 * p.G; g += blockDim.x) gs[g] = 0.0;
   __syncthreads();
   double s = 0.0;
-  for (int64_t i = tid; i < p.N; i += blockDim.x) {
-    const double w = p.w0[(int64_t)a * p.N + i];
-    p.v[(int64_t)a * p.ldw + i] = w;            // cold start: v = w0, i.e. z = projection of w0, y = rho (w0 - z)
-    s += w;
-    if (p.G) atomicAdd(&gs[p.group_id[i]], w);
+  for (int64_t i0 = 0; i0 < p.N; i0 += blockDim.x) {
+    const int64_t i = i0 + tid;
+    const bool valid = i < p.N;
+    double w = 0.0;
+    if (valid) {
+      w = p.w0[(int64_t)a * p.N + i];
+      p.v[(int64_t)a * p.ldw + i] = w;          // cold start: v = w0, i.e. z = projection of w0, y = rho (w0 - z)
+      s += w;
+    }
+    if (p.G) warp_group_add(gs, p.G, valid ? p.group_id[i] : 0, w, valid);
   }
   double val[1] = {s};
   const int op[1] = {0};
   block_reduce<1>(val, op, scratch);
   for (int g = tid; g < p.G; g += blockDim.x) {
     const int64_t e = (int64_t)a * p.G + g;
-    p.zE[e] = fmin(fmax(gs[g], p.band_lo[e]), p.band_hi[e]);
-    p.yE[e] = 0.0;
+    p.gw0[e] = group_total(gs, p.G, g);     // group sums of w0: S_g = gw0_g + sum of the group's trades
+    p.lamG[e] = 0.0;
   }
   if (tid == 0) {
     p.ap.bsum[a] = 1.0 - val[0];
     p.ap.c[a] = p.rho_scale;
-    p.ap.rhoE[a] = p.band_scale * p.rho_scale * p.gamma[a] * p.dbar_GN;
     p.ap.alpha[a] = 0.0; p.ap.beta[a] = 0.0; p.ap.mode[a] = 0;
-    p.ap.rpE[a] = 0.0; p.ap.nE[a] = 1.0;
     p.ap.done[a] = 0; p.ap.conv[a] = 0; p.ap.iters[a] = 0; p.ap.refactor[a] = 1; p.ap.nadapt[a] = 0;
   }
 }
 
 // ---------------------------------------------------------------------------------- H0 / H7: capacitance inverse
-// S_a = Lambda_a^-1 + gram / (gamma_a (1 + c_a)),  Lambda_a = diag(gamma_a f, [1 on padded factors], rhoE_a 1_G).
+// S_a = Lambda_a^-1 + gram / (gamma_a (1 + c_a)),  Lambda_a = diag(gamma_a f, [1 on padded factors]); U = Bp.
 // Inverted in shared memory by Gauss-Jordan (S is SPD, no pivoting needed).  Only accounts flagged `refactor`.
 __global__ void k_factor(const double* gram, const double* f, const double* gamma, AccountParams ap, int k, int kp,
                          int G, double* Sinv) {
@@ -86,12 +89,12 @@ __global__ void k_factor(const double* gram, const double* f, const double* gamm
   const int a = blockIdx.x, tid = threadIdx.x, nt = blockDim.x;
   if (!ap.refactor[a] || ap.done[a]) return;
   const int Kp = kp + G;
-  const double gam = gamma[a], c = ap.c[a], rhoE = ap.rhoE[a];
+  const double gam = gamma[a], c = ap.c[a];
   const double sc = 1.0 / (gam * (1.0 + c));
   for (int e = tid; e < Kp * Kp; e += nt) {
     const int r = e / Kp, cc = e % Kp;
     double s = gram[e] * sc;
-    if (r == cc) s += r < k ? 1.0 / (gam * f[r]) : (r < kp ? 1.0 : 1.0 / rhoE);
+    if (r == cc) s += r < k ? 1.0 / (gam * f[r]) : 1.0;
     S[e] = s;
   }
   __syncthreads();
@@ -114,25 +117,21 @@ __global__ void k_factor(const double* gram, const double* f, const double* gamm
   if (tid == 0) ap.refactor[a] = 0;
 }
 
-// ---------------------------------------------------------------------------------- H2: V = S^-1 T and the band block
+// ---------------------------------------------------------------------------------- H2: V = S^-1 T
 struct SolveArgs {
-  int32_t A, G, kp, nchunk; int64_t ldv;
-  const double *Tpart, *TE, *Sinv, *band_lo, *band_hi;
-  double *V, *zE, *yE;
+  int32_t A, kp, nchunk; int64_t ldv;
+  const double *Tpart, *Sinv;
+  double *V;
   AccountParams ap;
-  double relax;
 };
 __global__ void __launch_bounds__(128) k_solve(SolveArgs p) {
   __shared__ double T[PRISM_MAX_KPRIME];
-  __shared__ double Vs[PRISM_MAX_KPRIME];
-  __shared__ double scratch[2 * 32];
   const int a = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   if (p.ap.done[a]) return;
-  const int Kp = p.kp + p.G;
+  const int Kp = p.kp;
   for (int j = tid; j < Kp; j += blockDim.x) {
     double s = 0.0;
-    if (j < p.kp) for (int ch = 0; ch < p.nchunk; ++ch) s += p.Tpart[((int64_t)ch * p.A + a) * p.ldv + j];   // fixed order
-    else s = p.TE[(int64_t)a * p.G + (j - p.kp)];
+    for (int ch = 0; ch < p.nchunk; ++ch) s += p.Tpart[((int64_t)ch * p.A + a) * p.ldv + j];   // fixed order => deterministic
     T[j] = s;
   }
   __syncthreads();
@@ -141,28 +140,7 @@ __global__ void __launch_bounds__(128) k_solve(SolveArgs p) {
     double s = 0.0;
     for (int c = lane; c < Kp; c += 32) s = fma(Si[(int64_t)r * Kp + c], T[c], s);
     s = warp_sum(s);
-    if (lane == 0) { Vs[r] = s; p.V[(int64_t)a * p.ldv + r] = s; }
-  }
-  __syncthreads();
-  // band block: E x = V_E / rhoE (since U'x = Lambda^-1 V);  z_E, y_E updates; its primal residual
-  const double rhoE = p.ap.rhoE[a];
-  double rp = 0.0, nrm = 0.0;
-  for (int g = tid; g < p.G; g += blockDim.x) {
-    const int64_t e = (int64_t)a * p.G + g;
-    const double Ex = Vs[p.kp + g] / rhoE;
-    const double zo = p.zE[e], yo = p.yE[e];
-    const double eh = p.relax * Ex + (1.0 - p.relax) * zo;
-    const double zn = fmin(fmax(eh + yo / rhoE, p.band_lo[e]), p.band_hi[e]);
-    p.zE[e] = zn;
-    p.yE[e] = yo + rhoE * (eh - zn);
-    rp = fmax(rp, fabs(Ex - zn));
-    nrm = fmax(nrm, fmax(fabs(Ex), fabs(zn)));
-  }
-  if (p.G) {
-    double val[2] = {rp, nrm};
-    const int op[2] = {1, 1};
-    block_reduce<2>(val, op, scratch);
-    if (tid == 0) { p.ap.rpE[a] = val[0]; p.ap.nE[a] = val[1]; }
+    if (lane == 0) p.V[(int64_t)a * p.ldv + r] = s;
   }
 }
 
