@@ -23,7 +23,7 @@ struct AccountParams {            // per-account scalars, struct of arrays on th
   int32_t* conv;    // 1 if own tolerance met
   int32_t* iters;
   int32_t* refactor;// capacitance must be rebuilt (rho changed)
-  int32_t* nadapt;
+  int32_t* nadapt;  // iteration of the account's last rho adaptation
 };
 
 struct prism_problem {

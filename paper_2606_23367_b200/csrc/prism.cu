@@ -27,6 +27,7 @@ static int pick_mt(int k) {
     default: { constexpr int MT = 16; __VA_ARGS__; } break;           \
   }
 
+#define PROX_SMEM_MAX (200 * 1024)   // dynamic shared memory budget of k_prox_smem (plus ~11 KB static)
 static size_t g1_smem(int mt) { return (size_t)G1_STAGES * (8 * mt + G1_TA) * G1_LD * sizeof(double); }
 static size_t g2_smem(int mt) { return (size_t)(G2_TM + G2_TN) * (8 * mt + 4) * sizeof(double); }
 
@@ -156,6 +157,7 @@ static int set_kernel_attrs(int mt, int Kp) {
     CUDA_TRY(cudaFuncSetAttribute(k_gemm2<MT, G2_ADMM_CHECK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g2_smem(MT)));
     CUDA_TRY(cudaFuncSetAttribute(k_gemm2<MT, G2_SIGMA>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g2_smem(MT)));
   });
+  CUDA_TRY(cudaFuncSetAttribute(k_prox_smem, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PROX_SMEM_MAX));
   CUDA_TRY(cudaFuncSetAttribute(k_factor, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)((size_t)Kp * Kp * sizeof(double))));
   return PRISM_OK;
 }
@@ -281,7 +283,8 @@ static ProxArgs make_prox_args(prism_problem* p, const prism_settings& s, double
 static void launch_prox(prism_problem* p, cudaStream_t st, ProxArgs& a, int mode, int iter) {
   a.iter = iter;
   if (p->d.lot_count) k_prox<true><<<p->A, 512, 0, st>>>(a, mode);
-  else k_prox<false><<<p->A, 512, 0, st>>>(a, mode);
+  else if (p->d.hi_full || (size_t)p->N * 16 > PROX_SMEM_MAX) k_prox<false><<<p->A, 512, 0, st>>>(a, mode);
+  else k_prox_smem<<<p->A, 512, (size_t)p->N * 16, st>>>(a, mode);
 }
 
 static DiagArgs make_diag_args(prism_problem* p, const double* w, const double* duals, double* resid) {

@@ -56,39 +56,29 @@ struct ProxArgs {
 };
 
 enum { PROX_CHECK = 1, PROX_FINAL = 2, PROX_INIT = 4 };
+#define PRISM_ADAPT_START 200   // first iteration at which an account's rho may be adapted
+#define PRISM_ADAPT_EVERY 100   // minimum iterations between two adaptations of one account
 
 struct ElemConst {        // per-element quantities that do not depend on the trial thresholds
-  double rho_u, ir, bl, bh, sl, sh, w0;
+  double u, ir, bl, bh, sl, sh, w0;     // u = v - w0, ir = 1 / rho_i, buy range [bl, bh], sell range [sl, sh]
 };
 
-__device__ __forceinline__ ElemConst load_elem(const ProxArgs& p, int64_t row, int64_t rowp, int64_t i, double cg,
-                                               double lo_a, double hi_a) {
-  ElemConst e;
-  const int64_t idx = row + i;
-  const double w0 = p.w0[idx];
-  const double v = p.v[rowp + i];
-  const double dinv = p.invd[i];
-  double lo = lo_a, hi = p.hi_full ? p.hi_full[idx] : hi_a;
-  if (p.excl && p.excl[idx]) { lo = 0.0; hi = 0.0; }
-  e.w0 = w0;
-  e.ir = dinv / cg;                       // 1 / rho_i
-  e.rho_u = (v - w0) * cg / dinv;         // rho_i u_i  (d_i = 1 / invd_i)
-  e.bl = fmax(lo - w0, 0.0);
-  e.bh = fmax(hi - w0, 0.0);
-  e.sl = fmax(w0 - hi, 0.0);
-  e.sh = fmax(w0 - lo, 0.0);
-  return e;
+__device__ __forceinline__ void elem_ranges(ElemConst& e, double lo, double hi) {
+  e.bl = fmax(lo - e.w0, 0.0);
+  e.bh = fmax(hi - e.w0, 0.0);
+  e.sl = fmax(e.w0 - hi, 0.0);
+  e.sh = fmax(e.w0 - lo, 0.0);
 }
 
-// buy amount at threshold alpha; mv = 1 if strictly inside its range (slope -ir)
-__device__ __forceinline__ double buy_amt(const ElemConst& e, double lam_b, double alpha, double& mv) {
-  const double raw = (e.rho_u - lam_b - alpha) * e.ir;
+// buy amount at threshold a = alpha + lambda_g; mv = 1/rho_i if strictly inside its range (|slope| of the piece)
+__device__ __forceinline__ double buy_amt(const ElemConst& e, double lam_b, double a, double& mv) {
+  const double raw = e.u - (lam_b + a) * e.ir;
   mv = (raw > e.bl && raw < e.bh) ? e.ir : 0.0;
   return fmin(fmax(raw, e.bl), e.bh);
 }
 
 template <bool LOTS>
-__device__ __forceinline__ double sell_amt(const ElemConst& e, double kappa, double beta, const double* slope,
+__device__ __forceinline__ double sell_amt(const ElemConst& e, double kappa, double bt, const double* slope,
                                            const double* width, int nl, double& mv) {
   double raw, inside = 0.0;
   double sh = e.sh;
@@ -96,7 +86,7 @@ __device__ __forceinline__ double sell_amt(const ElemConst& e, double kappa, dou
     raw = 0.0;
     double Q = 0.0;
     for (int l = 0; l < nl; ++l) {
-      const double r = (beta - e.rho_u - kappa - slope[l]) * e.ir - Q;
+      const double r = (bt - kappa - slope[l]) * e.ir - e.u - Q;
       const double ql = width[l];
       if (r > 0.0 && r < ql) inside = 1.0;
       raw += fmin(fmax(r, 0.0), ql);
@@ -104,7 +94,7 @@ __device__ __forceinline__ double sell_amt(const ElemConst& e, double kappa, dou
     }
     sh = fmin(sh, Q);
   } else {
-    raw = (beta - e.rho_u - kappa) * e.ir;
+    raw = (bt - kappa) * e.ir - e.u;
     inside = 1.0;
   }
   mv = (inside > 0.0 && raw > e.sl && raw < sh) ? e.ir : 0.0;
@@ -129,71 +119,163 @@ __device__ __forceinline__ void root_step(Root1D& r, double g, double slope, dou
   r.x = xn;
 }
 
+// ---------------------------------------------------------------------------------------------- element sources
+// Generic source: every pass re-reads the account from global memory (any N, lots, per-asset caps).
 template <bool LOTS>
-__global__ void __launch_bounds__(512) k_prox(ProxArgs p, int mode) {
+struct SrcGlobal {
+  const ProxArgs& p;
+  int64_t row, rowp;
+  double icg, lo_a, hi_a;
+  __device__ SrcGlobal(const ProxArgs& p_, int a, double cg, double lo, double hi)
+      : p(p_), row((int64_t)a * p_.N), rowp((int64_t)a * p_.ldw), icg(1.0 / cg), lo_a(lo), hi_a(hi) {}
+  __device__ __forceinline__ void set_scale(double cg) { icg = 1.0 / cg; }
+  __device__ __forceinline__ void load(int64_t i, ElemConst& e, int& g, int& nl, const double*& sl, const double*& wd) const {
+    const int64_t idx = row + i;
+    e.w0 = p.w0[idx];
+    e.u = p.v[rowp + i] - e.w0;
+    e.ir = p.invd[i] * icg;
+    double lo = lo_a, hi = p.hi_full ? p.hi_full[idx] : hi_a;
+    if (p.excl && p.excl[idx]) { lo = 0.0; hi = 0.0; }
+    elem_ranges(e, lo, hi);
+    g = p.G ? p.group_id[i] : 0;
+    nl = 0; sl = nullptr; wd = nullptr;
+    if (LOTS) { nl = p.lot_count[idx]; sl = p.lot_slope + idx * PRISM_MAX_LOTS; wd = p.lot_width + idx * PRISM_MAX_LOTS; }
+  }
+  template <class F>
+  __device__ __forceinline__ void for_each(F f) const {          // f(i, e, g, nl, sl, wd)
+    for (int64_t i = threadIdx.x; i < p.N; i += blockDim.x) {
+      ElemConst e; int g, nl; const double *sl, *wd;
+      load(i, e, g, nl, sl, wd);
+      f(i, e, g, nl, sl, wd);
+    }
+  }
+  template <class F>
+  __device__ __forceinline__ void for_each_uniform(F f) const {  // f(valid, i, e, g, nl, sl, wd), warp-uniform trip count
+    for (int64_t i0 = 0; i0 < p.N; i0 += blockDim.x) {
+      const int64_t i = i0 + threadIdx.x;
+      const bool valid = i < p.N;
+      ElemConst e; int g = 0, nl = 0; const double *sl = nullptr, *wd = nullptr;
+      if (valid) load(i, e, g, nl, sl, wd);
+      f(valid, i, e, g, nl, sl, wd);
+    }
+  }
+  __device__ __forceinline__ void store_v(int64_t i, double vv) const { p.v[rowp + i] = vv; }
+};
+
+// Shared-memory source: u = v - w0 and w0 of the whole account stay in shared memory for the kernel (2 x 8 B x N),
+// so a trial evaluation touches no HBM: only 1/d_i, the exclusion byte and the group id (shared by many CTAs or
+// tiny; L1/L2 resident).  Each thread reads back only what it wrote: no barrier needed.  No lots, no per-asset caps.
+struct SrcSmem {
+  const ProxArgs& p;
+  int64_t row, rowp;
+  double icg, lo_a, hi_a;
+  double *us, *ws;
+  __device__ SrcSmem(const ProxArgs& p_, int a, double cg, double lo, double hi, double* smem)
+      : p(p_), row((int64_t)a * p_.N), rowp((int64_t)a * p_.ldw), icg(1.0 / cg), lo_a(lo), hi_a(hi), us(smem), ws(smem + p_.N) {
+    for (int64_t i = threadIdx.x; i < p.N; i += blockDim.x) {
+      const double w = p.w0[row + i];
+      ws[i] = w;
+      us[i] = p.v[rowp + i] - w;
+    }
+  }
+  __device__ __forceinline__ void load(int64_t i, ElemConst& e, int& g) const {
+    e.w0 = ws[i]; e.u = us[i];
+    e.ir = p.invd[i] * icg;
+    const bool ex = p.excl && p.excl[row + i];
+    elem_ranges(e, ex ? 0.0 : lo_a, ex ? 0.0 : hi_a);
+    g = p.G ? p.group_id[i] : 0;
+  }
+  template <class F>
+  __device__ __forceinline__ void for_each(F f) const {
+    for (int64_t i = threadIdx.x; i < p.N; i += blockDim.x) {
+      ElemConst e; int g;
+      load(i, e, g);
+      f(i, e, g, 0, (const double*)nullptr, (const double*)nullptr);
+    }
+  }
+  template <class F>
+  __device__ __forceinline__ void for_each_uniform(F f) const {
+    for (int64_t i0 = 0; i0 < p.N; i0 += blockDim.x) {
+      const int64_t i = i0 + threadIdx.x;
+      const bool valid = i < p.N;
+      ElemConst e; int g = 0;
+      if (valid) load(i, e, g);
+      f(valid, i, e, g, 0, (const double*)nullptr, (const double*)nullptr);
+    }
+  }
+  __device__ __forceinline__ void store_v(int64_t i, double vv) const { p.v[rowp + i] = vv; }
+};
+
+template <bool LOTS, class Src>
+__device__ __forceinline__ void prox_body(const ProxArgs& p, int mode, Src& src, int a, double gam, double c) {
   __shared__ double scratch[8 * 32];
   __shared__ double gbin[16 * PRISM_MAX_GROUPS];    // per-warp group bins (deterministic accumulation)
   __shared__ double lamS[PRISM_MAX_GROUPS];
   __shared__ double gsum[PRISM_MAX_GROUPS];
   __shared__ int selS[2];
-  const int a = blockIdx.x;
-  if (p.ap.done[a]) return;
   const int tid = threadIdx.x, nt = blockDim.x;
   const int64_t N = p.N, row = (int64_t)a * N, rowp = (int64_t)a * p.ldw;
-  const double gam = p.gamma[a];
-  double c = p.ap.c[a];
   double cg = c * gam;
-  const double lo_a = p.lo[a], hi_a = p.hi[a];
   const double kappa = p.kappa ? p.kappa[a] : 0.0;
   const double lam_b = kappa + (p.c_buy ? p.c_buy[a] : 0.0);
   const double tau = p.tau ? p.tau[a] : INFINITY;
   const double b = p.ap.bsum[a];
-  const int L = PRISM_MAX_LOTS, G = p.G;
+  const int G = p.G;
   for (int g = tid; g < G; g += nt) lamS[g] = p.lamG[(int64_t)a * G + g];
   __syncthreads();
 
   double alpha = p.ap.alpha[a], beta = p.ap.beta[a];
   int amode = p.ap.mode[a];
   if (!(amode == 1 && isfinite(tau))) { amode = 0; beta = alpha; }
-  double a_min = INFINITY, a_max = -INFINITY, b_min = INFINITY, b_max = -INFINITY;
+  double a_min, a_max, b_min, b_max;
   double P = 0, R = 0, sP = 0, sR = 0, Pa = 0, Ra = 0, pa = 0, ra = 0;
-  // one pass over the account: totals at thresholds (al, be) shifted by the group multipliers; with sel >= 0 also
-  // the sums of group `sel`; with extremes the range of the breakpoints (brackets).
-  auto eval = [&](double al, double be, int sel, bool extremes) {
-    double lP = 0, lR = 0, lsP = 0, lsR = 0, x4 = 0, x5 = 0, x6 = 0, x7 = 0;
-    if (extremes) { x4 = INFINITY; x5 = -INFINITY; x6 = INFINITY; x7 = -INFINITY; }
-    for (int64_t i = tid; i < N; i += nt) {
-      const ElemConst e = load_elem(p, row, rowp, i, cg, lo_a, hi_a);
+
+  // pass 0: totals at the warm start and the range of the breakpoints (brackets)
+  {
+    double lP = 0, lR = 0, lsP = 0, lsR = 0, x4 = INFINITY, x5 = -INFINITY, x6 = INFINITY, x7 = -INFINITY;
+    src.for_each([&](int64_t, const ElemConst& e, int g, int nl, const double* sl, const double* wd) {
       double mvb, mvs;
-      int nl = 0;
-      const double *sl = nullptr, *wd = nullptr;
-      if (LOTS) { nl = p.lot_count[row + i]; sl = p.lot_slope + (row + i) * L; wd = p.lot_width + (row + i) * L; }
-      const int g = G ? p.group_id[i] : 0;
+      const double lg = G ? lamS[g] : 0.0;
+      lP += buy_amt(e, lam_b, alpha + lg, mvb);
+      lR += sell_amt<LOTS>(e, kappa, beta + lg, sl, wd, nl, mvs);
+      lsP += mvb; lsR += mvs;
+      const double rho = 1.0 / e.ir;
+      if (e.bh > e.bl) { x4 = fmin(x4, rho * (e.u - e.bh) - lam_b); x5 = fmax(x5, rho * (e.u - e.bl) - lam_b); }
+      double sh = e.sh, s_first = 0.0, s_last = 0.0;
+      if (LOTS && nl > 0) { double Q = 0; for (int l = 0; l < nl; ++l) Q += wd[l]; sh = fmin(sh, Q); s_first = sl[0]; s_last = sl[nl - 1]; }
+      if (sh > e.sl) { x6 = fmin(x6, rho * (e.u + e.sl) + kappa + s_first); x7 = fmax(x7, rho * (e.u + sh) + kappa + s_last); }
+    });
+    double val[8] = {lP, lR, lsP, lsR, x4, x5, x6, x7};
+    const int op[8] = {0, 0, 0, 0, 2, 1, 2, 1};
+    block_reduce<8>(val, op, scratch);
+    P = val[0]; R = val[1]; sP = val[2]; sR = val[3];
+    a_min = val[4]; a_max = val[5]; b_min = val[6]; b_max = val[7];
+  }
+  // one pass: totals at thresholds (al, be) shifted by the group multipliers; with sel >= 0 also the sums of group sel
+  int n_eval = 1;
+  auto eval = [&](double al, double be, int sel) {
+    ++n_eval;
+    double lP = 0, lR = 0, lsP = 0, lsR = 0, x4 = 0, x5 = 0, x6 = 0, x7 = 0;
+    src.for_each([&](int64_t, const ElemConst& e, int g, int nl, const double* sl, const double* wd) {
+      double mvb, mvs;
       const double lg = G ? lamS[g] : 0.0;
       const double pb = buy_amt(e, lam_b, al + lg, mvb);
       const double ps = sell_amt<LOTS>(e, kappa, be + lg, sl, wd, nl, mvs);
       lP += pb; lR += ps; lsP += mvb; lsR += mvs;
-      if (extremes) {
-        const double rho = 1.0 / e.ir;
-        if (e.bh > e.bl) { x4 = fmin(x4, e.rho_u - lam_b - rho * e.bh); x5 = fmax(x5, e.rho_u - lam_b - rho * e.bl); }
-        double sh = e.sh, s_first = 0.0, s_last = 0.0;
-        if (LOTS && nl > 0) { double Q = 0; for (int l = 0; l < nl; ++l) Q += wd[l]; sh = fmin(sh, Q); s_first = sl[0]; s_last = sl[nl - 1]; }
-        if (sh > e.sl) { x6 = fmin(x6, e.rho_u + kappa + s_first + rho * e.sl); x7 = fmax(x7, e.rho_u + kappa + s_last + rho * sh); }
-      } else if (g == sel) { x4 += pb; x5 += ps; x6 += mvb; x7 += mvs; }
-    }
-    double val[8] = {lP, lR, lsP, lsR, x4, x5, x6, x7};
-    if (extremes) {
-      const int op[8] = {0, 0, 0, 0, 2, 1, 2, 1};
-      block_reduce<8>(val, op, scratch);
-      a_min = val[4]; a_max = val[5]; b_min = val[6]; b_max = val[7];
-    } else {
+      if (g == sel) { x4 += pb; x5 += ps; x6 += mvb; x7 += mvs; }
+    });
+    if (sel >= 0) {
+      double val[8] = {lP, lR, lsP, lsR, x4, x5, x6, x7};
       const int op[8] = {0, 0, 0, 0, 0, 0, 0, 0};
       block_reduce<8>(val, op, scratch);
-      Pa = val[4]; Ra = val[5]; pa = val[6]; ra = val[7];
+      P = val[0]; R = val[1]; sP = val[2]; sR = val[3]; Pa = val[4]; Ra = val[5]; pa = val[6]; ra = val[7];
+    } else {
+      double val[4] = {lP, lR, lsP, lsR};
+      const int op[4] = {0, 0, 0, 0};
+      block_reduce<4>(val, op, scratch);
+      P = val[0]; R = val[1]; sP = val[2]; sR = val[3];
     }
-    P = val[0]; R = val[1]; sP = val[2]; sR = val[3];
   };
-  eval(alpha, beta, -1, true);
   const double span = fmax(fmax(fabs(a_min), fabs(a_max)), fmax(fabs(b_min), fabs(b_max)));
   const double pad = 1e-9 * fmax(span, 1e-300) + 1e-300;
   if (!(a_min <= a_max)) { a_min = -1.0; a_max = 1.0; }
@@ -213,13 +295,13 @@ __global__ void __launch_bounds__(512) k_prox(ProxArgs p, int mode) {
       if (amode == 1) {
         Root1D ra_ = {fmin(fmax(alpha, alo), ahi), alo, ahi, 0};
         Root1D rb_ = {fmin(fmax(beta, blo), bhi), blo, bhi, 0};
-        if (!fresh || sel >= 0 || ra_.x != alpha || rb_.x != beta) eval(ra_.x, rb_.x, sel, false);
+        if (!fresh || sel >= 0 || ra_.x != alpha || rb_.x != beta) eval(ra_.x, rb_.x, sel);
         fresh = false;
         for (int it = 0; it < 80; ++it) {
           root_step(ra_, P, sP, Pt, -1, tol);
           root_step(rb_, R, sR, Rt, +1, tol);
           if (ra_.done && rb_.done) break;
-          eval(ra_.x, rb_.x, sel, false);
+          eval(ra_.x, rb_.x, sel);
         }
         alpha = ra_.x; beta = rb_.x;
         if (alpha >= beta) break;
@@ -227,12 +309,12 @@ __global__ void __launch_bounds__(512) k_prox(ProxArgs p, int mode) {
       } else {
         const double lo_b = fmin(alo, blo), hi_b = fmax(ahi, bhi);
         Root1D rn = {fmin(fmax(alpha, lo_b), hi_b), lo_b, hi_b, 0};
-        if (!fresh || sel >= 0 || rn.x != alpha || beta != alpha) eval(rn.x, rn.x, sel, false);
+        if (!fresh || sel >= 0 || rn.x != alpha || beta != alpha) eval(rn.x, rn.x, sel);
         fresh = false;
         for (int it = 0; it < 80; ++it) {
           root_step(rn, P - R, sP + sR, b, -1, tol);
           if (rn.done) break;
-          eval(rn.x, rn.x, sel, false);
+          eval(rn.x, rn.x, sel);
         }
         alpha = beta = rn.x;
         if (!isfinite(tau) || P + R <= tau + tol) break;
@@ -247,19 +329,14 @@ __global__ void __launch_bounds__(512) k_prox(ProxArgs p, int mode) {
     // all group sums at the current solution (deterministic binned pass)
     for (int g = tid; g < 16 * G; g += nt) gbin[g] = 0.0;
     __syncthreads();
-    for (int64_t i0 = 0; i0 < N; i0 += nt) {
-      const int64_t i = i0 + tid;
-      const bool valid = i < N;
-      double t = 0.0; int g = 0;
+    src.for_each_uniform([&](bool valid, int64_t, const ElemConst& e, int g, int nl, const double* sl, const double* wd) {
+      double t = 0.0;
       if (valid) {
-        const ElemConst e = load_elem(p, row, rowp, i, cg, lo_a, hi_a);
-        double mvb, mvs; int nl = 0; const double *sl = nullptr, *wd = nullptr;
-        if (LOTS) { nl = p.lot_count[row + i]; sl = p.lot_slope + (row + i) * L; wd = p.lot_width + (row + i) * L; }
-        g = p.group_id[i];
+        double mvb, mvs;
         t = buy_amt(e, lam_b, alpha + lamS[g], mvb) - sell_amt<LOTS>(e, kappa, beta + lamS[g], sl, wd, nl, mvs);
       }
-      warp_group_add(gbin, G, g, t, valid);
-    }
+      warp_group_add(gbin, G, valid ? g : 0, t, valid);
+    });
     __syncthreads();
     for (int g = tid; g < G; g += nt) gsum[g] = p.gw0[(int64_t)a * G + g] + group_total(gbin, G, g);
     __syncthreads();
@@ -312,20 +389,18 @@ __global__ void __launch_bounds__(512) k_prox(ProxArgs p, int mode) {
   int finished = 0;
   if (mode & PROX_CHECK) {
     double nx = 0, nz = 0, nrp = 0, nrd = 0, nPx = 0, ny = 0, nq = 0;
-    for (int64_t i = tid; i < N; i += nt) {
-      const ElemConst e = load_elem(p, row, rowp, i, cg, lo_a, hi_a);
-      double mvb, mvs; int nl = 0; const double *sl = nullptr, *wd = nullptr;
-      if (LOTS) { nl = p.lot_count[row + i]; sl = p.lot_slope + (row + i) * L; wd = p.lot_width + (row + i) * L; }
-      const double lg = G ? lamS[p.group_id[i]] : 0.0;
-      const double z = e.w0 + buy_amt(e, lam_b, alpha + lg, mvb) - sell_amt<LOTS>(e, kappa, beta + lg, sl, wd, nl, mvs);
-      const double vv = p.v[rowp + i];
-      const double y = (vv - z) / e.ir;
+    src.for_each([&](int64_t i, const ElemConst& e, int g, int nl, const double* sl, const double* wd) {
+      double mvb, mvs;
+      const double lg = G ? lamS[g] : 0.0;
+      const double tr = buy_amt(e, lam_b, alpha + lg, mvb) - sell_amt<LOTS>(e, kappa, beta + lg, sl, wd, nl, mvs);
+      const double z = e.w0 + tr;
+      const double y = (e.u - tr) / e.ir;                 // rho (v - z)
       const double x = p.xs[rowp + i], pq = p.pxq[rowp + i];
       const double qi = p.q ? p.q[rowp + i] : -p.mu[row + i];
       nx = fmax(nx, fabs(x)); nz = fmax(nz, fabs(z)); nrp = fmax(nrp, fabs(x - z));
       nrd = fmax(nrd, fabs(pq + y)); nPx = fmax(nPx, fabs(pq - qi)); ny = fmax(ny, fabs(y)); nq = fmax(nq, fabs(qi));
-      if (!(z == z) || !(x == x) || !(vv == vv)) nrp = INFINITY;     // fmax drops NaN: poison explicitly
-    }
+      if (!(z == z) || !(x == x) || !(e.u == e.u)) nrp = INFINITY;     // fmax drops NaN: poison explicitly
+    });
     double val[7] = {nx, nz, nrp, nrd, nPx, ny, nq};
     const int op[7] = {1, 1, 1, 1, 1, 1, 1};
     block_reduce<7>(val, op, scratch);
@@ -340,40 +415,42 @@ __global__ void __launch_bounds__(512) k_prox(ProxArgs p, int mode) {
     if (conv || bad) {
       finished = 1;
       if (tid == 0) p.ap.conv[a] = bad ? -1 : 1;
-    } else if (p.adapt) {
+    } else if (p.adapt && p.iter >= PRISM_ADAPT_START && p.iter - p.ap.nadapt[a] >= PRISM_ADAPT_EVERY) {
+      // H7: only accounts that are unusually slow are re-scaled (typical accounts finish before PRISM_ADAPT_START);
+      // rho <- rho sqrt(r_p / r_d), clipped, applied when the two scaled residuals are out of balance
       const double ratio = sqrt(rp / fmax(rd, 1e-300));
-      if ((ratio > 5.0 || ratio < 0.2) && p.ap.nadapt[a] < 20) {
-        const double cn = c * fmin(fmax(ratio, 0.1), 10.0);
+      if (ratio > 3.0 || ratio < 1.0 / 3.0) {
+        const double cn = c * fmin(fmax(ratio, 0.2), 5.0);
         rescale = c / cn;          // v' = z + (rho/rho') (v - z) keeps y = rho (v - z) unchanged
         c = cn; cg = c * gam;
-        if (tid == 0) { p.ap.c[a] = c; p.ap.refactor[a] = 1; p.ap.nadapt[a] += 1; }
+        if (tid == 0) { p.ap.c[a] = c; p.ap.refactor[a] = 1; }
       }
+      if (tid == 0) p.ap.nadapt[a] = p.iter;
     }
   }
   if (mode & PROX_FINAL) finished = 1;
 
-  // ---------------------------------------------------------------- output pass
-  const double cg_old = cg * rescale;     // rho scale the stored v refers to (c_old * gamma)
-  for (int64_t i = tid; i < N; i += nt) {
-    const ElemConst e = load_elem(p, row, rowp, i, cg_old, lo_a, hi_a);
-    double mvb, mvs; int nl = 0; const double *sl = nullptr, *wd = nullptr;
-    if (LOTS) { nl = p.lot_count[row + i]; sl = p.lot_slope + (row + i) * L; wd = p.lot_width + (row + i) * L; }
-    const double lg = G ? lamS[p.group_id[i]] : 0.0;
-    const double z = e.w0 + buy_amt(e, lam_b, alpha + lg, mvb) - sell_amt<LOTS>(e, kappa, beta + lg, sl, wd, nl, mvs);
-    if (finished) { p.w_out[row + i] = z; continue; }
-    double vv = p.v[rowp + i];
-    const double y = (vv - z) / e.ir;                      // rho_old (v - z)
-    if (rescale != 1.0) { vv = z + rescale * (vv - z); p.v[rowp + i] = vv; }
+  // ---------------------------------------------------------------- output pass (e.ir still refers to the old rho)
+  const double igc = 1.0 / (gam * (1.0 + c));
+  src.for_each([&](int64_t i, const ElemConst& e, int g, int nl, const double* sl, const double* wd) {
+    double mvb, mvs;
+    const double lg = G ? lamS[g] : 0.0;
+    const double tr = buy_amt(e, lam_b, alpha + lg, mvb) - sell_amt<LOTS>(e, kappa, beta + lg, sl, wd, nl, mvs);
+    const double z = e.w0 + tr;
+    if (finished) { p.w_out[row + i] = z; return; }
+    const double y = (e.u - tr) / e.ir;                    // rho_old (v - z)
+    if (rescale != 1.0) src.store_v(i, z + rescale * (e.u - tr));
     const double dinv = p.invd[i];
     const double rho = cg / dinv;                          // new rho_i
     const double qi = p.q ? p.q[rowp + i] : -p.mu[row + i];
     const double r = rho * z - y - qi;
-    const double rt = r * dinv / (gam * (1.0 + c));        // M_i = gamma d_i (1 + c)
+    const double rt = r * dinv * igc;                      // M_i = gamma d_i (1 + c)
     p.rt[rowp + i] = rt;
     p.cc[rowp + i] = rt - z;
-  }
+  });
   for (int g = tid; g < G; g += nt) p.lamG[(int64_t)a * G + g] = lamS[g];
   if (tid == 0) {
+    p.resid[(int64_t)a * PRISM_NRES + PRISM_R_RESERVED] += (double)n_eval;   // trial evaluations (passes) so far
     p.ap.alpha[a] = alpha; p.ap.beta[a] = beta; p.ap.mode[a] = amode;
     if (finished) {
       p.ap.done[a] = 1;
@@ -386,4 +463,24 @@ __global__ void __launch_bounds__(512) k_prox(ProxArgs p, int mode) {
       p.resid[(int64_t)a * PRISM_NRES + PRISM_R_RHO] = c;
     }
   }
+}
+
+// generic kernel: any N, lots, per-asset caps
+template <bool LOTS>
+__global__ void __launch_bounds__(512) k_prox(ProxArgs p, int mode) {
+  const int a = blockIdx.x;
+  if (p.ap.done[a]) return;
+  const double gam = p.gamma[a], c = p.ap.c[a];
+  SrcGlobal<LOTS> src(p, a, c * gam, p.lo[a], p.hi[a]);
+  prox_body<LOTS>(p, mode, src, a, gam, c);
+}
+
+// shared-memory-resident kernel: 16 N bytes of dynamic shared memory, no lots, no per-asset caps
+__global__ void __launch_bounds__(512, 1) k_prox_smem(ProxArgs p, int mode) {
+  extern __shared__ __align__(16) double prox_smem[];
+  const int a = blockIdx.x;
+  if (p.ap.done[a]) return;
+  const double gam = p.gamma[a], c = p.ap.c[a];
+  SrcSmem src(p, a, c * gam, p.lo[a], p.hi[a], prox_smem);
+  prox_body<false>(p, mode, src, a, gam, c);
 }
