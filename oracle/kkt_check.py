@@ -74,28 +74,19 @@ def _phi_interval(acc: Account, w: np.ndarray, delta: float):
             else:
                 lo[i], hi[i] = 0.0, acc.c_buy
             continue
-        # derivative of phi wrt w on the sell side is -slope of the lot being consumed
+        # derivative of phi wrt w on the sell side is -slope of the lot being consumed.  Activity with threshold
+        # delta (reading R19): every lot whose range [Q_l, Q_l + q_l] comes within delta of s is "touched" (lots can
+        # be narrower than delta), and the subdifferential is [-max touched slope, -min touched slope]; at s <= delta
+        # the buy side joins (upper end c_buy); at the end of the last lot no further selling is possible (-inf).
         Q = 0.0
-        left = None; right = None        # slopes just below / just above the sell amount s
+        touched = []
         for l in range(Li):
-            q = acc.lot_width[i, l]; sl = acc.lot_slope[i, l]
-            if s > Q + delta and s < Q + q - delta:
-                left = right = sl
-                break
-            if abs(s - Q) <= delta:      # at the start of lot l
-                right = sl
-                if l > 0:
-                    left = acc.lot_slope[i, l - 1]
-                break
+            q = acc.lot_width[i, l]
+            if Q - delta <= s <= Q + q + delta:
+                touched.append(acc.lot_slope[i, l])
             Q += q
-        else:
-            # at (or beyond) the end of the last lot: no further selling possible
-            left = acc.lot_slope[i, Li - 1]; right = np.inf
-        if abs(s) <= delta:              # kink at w0: buy side slope c_buy, sell side slope -s_1
-            lo[i], hi[i] = -acc.lot_slope[i, 0], acc.c_buy
-        else:
-            # d phi / d w in [-right, -left]
-            lo[i] = -right; hi[i] = -left
+        lo[i] = -np.inf if s >= Q - delta else -max(touched)
+        hi[i] = acc.c_buy if s <= delta else -min(touched)
     return lo, hi
 
 

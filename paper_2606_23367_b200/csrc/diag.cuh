@@ -62,18 +62,18 @@ __global__ void __launch_bounds__(256) k_diag(DiagArgs p) {
     if (dw > dl) { plo = phi_ = cb; }
     else if (nl == 0) { if (s > dl) { plo = phi_ = 0.0; } else { plo = 0.0; phi_ = cb; } }
     else {
-      double Q = 0.0, tax = 0.0;
-      bool found = false;
-      plo = -INFINITY; phi_ = -sl[nl - 1];        // default: at / beyond the end of the last lot
+      // lots whose range [Q_l, Q_l + q_l] comes within delta of the sell amount s are "touched": the subdifferential
+      // of the penalty is [-max touched slope, -min touched slope]; at s <= delta the buy side (c_buy) joins, at the
+      // end of the last lot no further selling is possible (lower end -inf).
+      double Q = 0.0, tax = 0.0, smin = INFINITY, smax = -INFINITY;
       for (int l = 0; l < nl; ++l) {
         const double ql = wd[l];
         tax += sl[l] * fmin(fmax(s - Q, 0.0), ql);
-        if (!found) {
-          if (s > Q + dl && s < Q + ql - dl) { plo = phi_ = -sl[l]; found = true; }
-          else if (fabs(s - Q) <= dl) { plo = -sl[l]; phi_ = l > 0 ? -sl[l - 1] : cb; found = true; }
-        }
+        if (s >= Q - dl && s <= Q + ql + dl) { smin = fmin(smin, sl[l]); smax = fmax(smax, sl[l]); }
         Q += ql;
       }
+      plo = (s >= Q - dl) ? -INFINITY : -smax;
+      phi_ = (s <= dl) ? cb : -smin;
       pen += tax;
       rbox = fmax(rbox, (w0 - Q) - w);            // cannot sell more than the lots held
     }

@@ -1,0 +1,125 @@
+"""CPU-side checks of the boundary: the C-ABI library builds for sm_100a, loads without a GPU and exports every
+symbol include/prism.h declares; settings defaults; struct layouts of the binding match the header; the product
+path has no CPU fallback.  No compute calls (there is no GPU here)."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2606_23367_b200 import build, binding
+    build.build()
+    return binding.load_library()
+
+
+def _header():
+    with open(os.path.join(ROOT, "include", "prism.h")) as f:
+        return f.read()
+
+
+def test_every_declared_symbol_is_exported(lib):
+    h = _header()
+    names = set(re.findall(r"\b(prism_[a-z_]+)\s*\(", h))
+    names -= {"prism_problem", "prism_settings", "prism_data", "prism_constraint_set", "prism_solve_info"}
+    assert {"prism_problem_create", "prism_solve_batch", "prism_residuals"} <= names      # BASELINE.json:north_star
+    for n in sorted(names):
+        assert hasattr(lib, n), f"{n} declared in prism.h but not exported"
+    from paper_2606_23367_b200 import binding
+    assert set(binding.SYMBOLS) == names
+
+
+def test_default_settings_and_version(lib):
+    from paper_2606_23367_b200 import binding
+    s = binding.default_settings()
+    assert s.eps_rel == 1e-6 and s.max_iter == 4000 and s.check_every == 10 and s.alpha == 1.6 and s.rho_scale == 100.0
+    assert s.adapt_rho == 1 and s.gemm_mode == 0 and s.profile == 0
+    assert "sm_100a" in binding.version()
+
+
+def test_header_constants_match_binding():
+    from paper_2606_23367_b200 import binding
+    from instances import gen
+    h = _header()
+    assert int(re.search(r"PRISM_NRES = (\d+)", h).group(1)) == binding.NRES
+    for name, val in [("PRISM_R_BUDGET", binding.RES["budget"]), ("PRISM_R_STAT", binding.RES["stat"]),
+                      ("PRISM_R_OBJECTIVE", binding.RES["objective"]), ("PRISM_R_DUAL", binding.RES["dual"])]:
+        assert int(re.search(name + r" = (\d+)", h).group(1)) == val
+    flags = dict(re.findall(r"(PRISM_[A-Z_]+) = (\d+)", h))
+    assert int(flags["PRISM_GROUP_BANDS"]) == gen.F_GROUP_BANDS and int(flags["PRISM_TAX_LOTS"]) == gen.F_TAX_LOTS
+    assert int(flags["PRISM_BENCHMARK_SHIFT"]) == gen.F_BENCHMARK_SHIFT and int(flags["PRISM_EXCLUSION"]) == gen.F_EXCLUSION
+    assert len(binding.STATUS_NAMES) == 6                                               # Table 14
+    # struct sizes (natural alignment) as the C compiler lays them out
+    assert C.sizeof(binding.Settings) == 72 and C.sizeof(binding.ConstraintSet) == 12
+    assert C.sizeof(binding.Data) == 22 * 8
+
+
+def test_invalid_arguments_are_errors_not_crashes(lib):
+    from paper_2606_23367_b200 import binding
+    out = C.c_void_p()
+    rc = lib.prism_problem_create(10, 2, 1, None, None, None, C.byref(out))
+    assert rc == 1 and not out.value and b"null" in lib.prism_last_error()
+    cs = binding.ConstraintSet(flags=0, G=0, max_lots=0)
+    d = binding.Data()
+    rc = lib.prism_problem_create(10, 2, 1, C.byref(cs), C.byref(d), None, C.byref(out))
+    assert rc == 1 and b"mandatory" in lib.prism_last_error()
+    cs = binding.ConstraintSet(flags=3, G=0, max_lots=0)
+    rc = lib.prism_problem_create(0, 2, 1, C.byref(cs), C.byref(d), None, C.byref(out))
+    assert rc == 1
+    rc = lib.prism_problem_create(10, 1000, 1, C.byref(cs), C.byref(d), None, C.byref(out))
+    assert rc == 1
+    assert lib.prism_solve_batch(None, None, None, None, None, None, None, None, None) == 4    # PRISM_ERR_NOT_READY
+    assert lib.prism_residuals(None, None, None, None, None) == 4
+    lib.prism_problem_destroy(None)                                                         # NULL is allowed
+    assert lib.prism_problem_device_bytes(None) == 0
+
+
+def test_product_path_does_not_touch_the_oracle_or_any_cpu_fallback():
+    pkg = os.path.join(ROOT, "paper_2606_23367_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for fn in files:
+            if fn.endswith((".py", ".cu", ".cuh", ".h")):
+                src = open(os.path.join(dirpath, fn)).read()
+                assert "oracle" not in src.replace("no CPU fallback", ""), f"{fn} mentions the oracle"
+    from paper_2606_23367_b200 import binding
+    with pytest.raises(RuntimeError):
+        binding._lib = None
+        try:
+            binding.load_library("/nonexistent/libprism.so")
+        finally:
+            binding._lib = None
+
+
+def test_sharding_plan_world_size_2_gloo(tmp_path):
+    """Multi-GPU path: accounts shard with no data-path collective; the only communication is
+    the barrier and the max-reduction of the timing, exercised here with gloo on CPU, world size 2."""
+    import subprocess, sys, textwrap
+    code = textwrap.dedent("""
+        import os, sys, torch, torch.distributed as dist
+        sys.path.insert(0, %r)
+        from instances import gen
+        dist.init_process_group('gloo')
+        r, w = dist.get_rank(), dist.get_world_size()
+        inst = gen.config1(seed=r, N=64, k=4, A=3)          # every rank draws its own batch (weak scaling)
+        t = torch.tensor([float(10 + r)], dtype=torch.float64)
+        dist.barrier()
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        s = torch.tensor([float(inst.mu.sum())], dtype=torch.float64)
+        g = [torch.zeros(1, dtype=torch.float64) for _ in range(w)]
+        dist.all_gather(g, s)
+        assert t.item() == 10 + w - 1
+        assert g[0].item() != g[1].item()                    # different seeds -> different batches
+        dist.destroy_process_group()
+        print('rank' + str(r) + 'done', flush=True)
+    """ % ROOT)
+    script = tmp_path / "worker.py"
+    script.write_text(code)
+    res = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2",
+                          "--master-addr", "127.0.0.1", "--master-port", "29532", str(script)],
+                         capture_output=True, text=True, timeout=300)
+    assert res.returncode == 0, res.stderr[-2000:]
+    assert "rank0done" in res.stdout and "rank1done" in res.stdout

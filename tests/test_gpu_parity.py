@@ -1,0 +1,188 @@
+"""Parity of the CUDA path (through the C ABI) with the CPU oracle, element by element on the same seeded inputs.
+
+Tolerances are BASELINE.json:north_star's: ||dw||_inf <= 1e-4, relative objective gap <= 1e-6, scaled primal/dual
+residuals <= 1e-6, every constraint verified externally (independent checker oracle/kkt_check.py AND the library's
+own prism_residuals), statuses from the Table 14 vocabulary."""
+import numpy as np
+import pytest
+
+from instances import gen
+
+pytestmark = pytest.mark.gpu
+
+TOL_W, TOL_GAP, TOL_RES, TOL_GATE = 1e-4, 1e-6, 1e-6, 1e-6
+
+
+def _solve_gpu(inst, **kw):
+    import paper_2606_23367_b200 as pr
+    P = pr.Problem(inst)
+    r = P.solve(**kw)
+    return P, r
+
+
+def _oracle(inst, accounts=None):
+    from oracle import ipm
+    return ipm.solve_instance(inst, accounts=accounts)
+
+
+def _check_against_oracle(inst, r, W, res, accounts=None):
+    from oracle import kkt_check, problem
+    accounts = list(range(inst.A)) if accounts is None else list(accounts)
+    w = r.w.cpu().numpy(); st = r.status.cpu().numpy(); rs = r.resid.cpu().numpy(); du = r.duals.cpu().numpy()
+    G = inst.G
+    for j, a in enumerate(accounts):
+        acc = problem.account_from_instance(inst, a)
+        assert st[a] == 0, f"account {a}: status {st[a]}"
+        assert np.max(np.abs(w[a] - W[j])) <= TOL_W, f"account {a}: dw {np.max(np.abs(w[a] - W[j])):.2e}"
+        fo = problem.objective(acc, W[j]); fg = problem.objective(acc, w[a])
+        assert abs(fg - fo) / max(abs(fo), 1e-12) <= TOL_GAP, f"account {a}: gap {(fg - fo) / abs(fo):.2e}"
+        assert rs[a, 7] <= TOL_RES and rs[a, 8] <= TOL_RES
+        # every constraint verified externally (independent checker)
+        feas = kkt_check.feasibility(acc, w[a])
+        assert max(feas.values()) <= TOL_GATE, feas
+        # the library's own diagnostics agree with the independent checker
+        assert abs(rs[a, 0] - feas["r_budget"]) <= 1e-12 and abs(rs[a, 1] - feas["r_box"]) <= 1e-12
+        assert abs(rs[a, 2] - feas["r_exposure"]) <= 1e-12 and abs(rs[a, 3] - feas["r_turnover"]) <= 1e-12
+        assert abs(rs[a, 6] - fg) <= 1e-12 * max(1.0, abs(fg))
+        # KKT certificate of the returned weights with the returned multipliers
+        mult = dict(nu=du[a, 0], theta=du[a, 1], lam_hi=du[a, 2:2 + G], lam_lo=du[a, 2 + G:2 + 2 * G])
+        k = kkt_check.kkt(acc, w[a], mult, delta=1e-9)
+        scale = max(np.max(np.abs(acc.mu)), 1e-12)
+        assert k["r_stat"] <= 1e-5 * scale * 10 and k["r_comp"] <= 1e-9 and k["min_multiplier"] >= -1e-15, k
+        assert abs(rs[a, 4] - k["r_stat"]) <= 1e-10 and abs(rs[a, 5] - k["r_comp"]) <= 1e-12
+
+
+CASES = {
+    "cfg0": lambda: gen.config0(),
+    "cfg1_small": lambda: gen.config1(N=500, k=12, A=5),
+    "cfg1_ragged": lambda: gen.config1(N=333, k=9, A=3),                       # odd N, ragged tiles
+    "cfg1_multi_tile": lambda: gen.config1(N=1100, k=30, A=70),               # > 64 accounts: two account tiles
+    "cfg2_small": lambda: gen.config2(N=1000, k=20, A=6, G=5, band_half=0.005),  # bands certainly active (R9 variant)
+    "cfg2_mid": lambda: gen.config2(N=2500, k=50, A=9),
+    "cfg3_small": lambda: gen.config3(N=600, k=12, A=4),
+    "cfg4_small": lambda: gen.config4(N=4000, k=100, A=3, hi=0.001),          # fp32 loadings, k = 100 (13 factor tiles)
+    "sec9": lambda: gen.section9(N=481, k=20, A=2),                           # PAPER.md:378 transition objective (R14)
+    "benchmark_shift": lambda: gen.make_instance("wb", 7, 400, 8, 3, hi_fixed=0.05, tau_range=(0.2, 0.5), benchmark_in_risk=True),
+}
+
+
+@pytest.mark.parametrize("name", sorted(CASES))
+@pytest.mark.parametrize("gemm_mode", [0, 1])
+def test_parity_with_oracle(name, gemm_mode):
+    inst = CASES[name]()
+    W, res = _oracle(inst)
+    P, r = _solve_gpu(inst, gemm_mode=gemm_mode)
+    _check_against_oracle(inst, r, W, res)
+    P.close()
+
+
+def test_dmma_and_fma_gemms_agree():
+    """The tensor-pipe GEMMs against the plain-FMA kernels of the same contract: same iterations, same weights."""
+    inst = gen.config1(N=700, k=30, A=10)
+    P, r0 = _solve_gpu(inst, gemm_mode=0)
+    r1 = P.solve(gemm_mode=1)
+    assert (r0.iters == r1.iters).all()
+    assert float((r0.w - r1.w).abs().max()) <= 1e-12
+    P.close()
+
+
+def test_batch_equals_single_accounts_and_identical_accounts():
+    inst = gen.config1(N=400, k=10, A=4)
+    P, r = _solve_gpu(inst)
+    for a in range(inst.A):
+        Pa, ra = _solve_gpu(inst.subset([a]))
+        assert float((ra.w[0] - r.w[a]).abs().max()) <= 1e-12
+        Pa.close()
+    twin = inst.subset([2, 2, 2])
+    Pt, rt = _solve_gpu(twin)
+    assert float((rt.w[0] - rt.w[1]).abs().max()) == 0.0 and float((rt.w[0] - rt.w[2]).abs().max()) == 0.0
+    Pt.close(); P.close()
+
+
+def test_run_to_run_determinism():
+    inst = gen.config2(N=1500, k=20, A=5, G=7, band_half=0.01)
+    P, r1 = _solve_gpu(inst)
+    r2 = P.solve()
+    assert (r1.w == r2.w).all() and (r1.iters == r2.iters).all()
+    P.close()
+
+
+def test_residuals_call_is_external_and_matches_checker():
+    """prism_residuals depends only on data + given w (+ multipliers): applied to the ORACLE's weights and duals."""
+    from oracle import kkt_check, problem
+    inst = gen.config2(N=800, k=16, A=3, G=4, band_half=0.01)
+    W, res = _oracle(inst)
+    import paper_2606_23367_b200 as pr
+    P = pr.Problem(inst)
+    G = inst.G
+    du = np.zeros((inst.A, 2 + 2 * G))
+    for a in range(inst.A):
+        m = res[a]["mult"]
+        du[a, 0], du[a, 1] = m["nu"], m["theta"]
+        du[a, 2:2 + G] = m["lam_hi"]; du[a, 2 + G:] = m["lam_lo"]
+    rs = P.residuals(W, du).cpu().numpy()
+    rn = P.residuals(W, None).cpu().numpy()
+    for a in range(inst.A):
+        acc = problem.account_from_instance(inst, a)
+        k = kkt_check.kkt(acc, W[a], res[a]["mult"], delta=1e-9)
+        assert abs(rs[a, 4] - k["r_stat"]) <= 1e-10 and abs(rs[a, 5] - k["r_comp"]) <= 1e-12
+        assert abs(rs[a, 6] - problem.objective(acc, W[a])) <= 1e-14
+        assert max(rs[a, 0:4]) <= 1e-9
+        assert np.isnan(rn[a, 4]) and np.isnan(rn[a, 5]) and np.isnan(rs[a, 7])
+    # a wrong weight vector is flagged
+    Wb = W.copy(); Wb[:, 0] += 1e-3
+    rb = P.residuals(Wb, du).cpu().numpy()
+    assert np.all(np.abs(rb[:, 0] - 1e-3) < 1e-12)
+    P.close()
+
+
+def test_status_vocabulary():
+    inst = gen.config1(N=400, k=10, A=4)
+    P, r = _solve_gpu(inst, max_iter=20)                     # iteration cap -> feasible / non-certified
+    st = r.status.cpu().numpy()
+    assert set(st.tolist()) <= {0, 1} and (st == 1).any()
+    assert float(r.resid[:, 0:4].max()) <= 1e-6               # gates pass: returned point is exactly feasible
+    r = P.solve(time_limit_ms=1e-3)                          # timeout
+    assert set(r.status.cpu().numpy().tolist()) <= {2}
+    r = P.solve(deadline_ms=1e-3)                            # finished after the deadline -> late
+    assert set(r.status.cpu().numpy().tolist()) == {3}
+    P.close()
+    bad = gen.config1(N=400, k=10, A=3)
+    bad.mu[1, 5] = np.nan                                    # numerical failure is a status, not an error
+    Pb, rb = _solve_gpu(bad)
+    sb = rb.status.cpu().numpy()
+    assert sb[1] == 5 and sb[0] == 0 and sb[2] == 0
+    Pb.close()
+    inf = gen.config1(N=400, k=10, A=2)
+    inf.tau[0] = 1e-6                                        # infeasible with exclusions held: no accepted feasible return
+    Pi, ri = _solve_gpu(inf, max_iter=200)
+    assert ri.status.cpu().numpy()[0] == 4 and ri.status.cpu().numpy()[1] == 0
+    Pi.close()
+
+
+def test_edge_cases():
+    # single account, single factor tile, tiny N; tau = inf (no cap); kappa-only
+    for inst in [gen.make_instance("tiny", 1, 8, 2, 1, hi_fixed=0.5, tau_fixed=0.5),
+                 gen.make_instance("nocap", 2, 200, 5, 2, hi_fixed=0.05),
+                 gen.make_instance("pen", 3, 200, 5, 2, hi_fixed=0.05, kappa_fixed=0.003, c_buy=0.001)]:
+        W, res = _oracle(inst)
+        P, r = _solve_gpu(inst)
+        _check_against_oracle(inst, r, W, res)
+        P.close()
+
+
+@pytest.mark.parametrize("cfg,n_sample", [("cfg2", 3), ("cfg3", 2)])
+def test_full_size_sampled_accounts(cfg, n_sample):
+    """BASELINE.json full sizes in the launch configuration bench.py times; the oracle solves a sample of accounts
+    one by one, the rest are certified through properties that hold at any size (gates, KKT residuals, statuses)."""
+    inst = gen.by_name(cfg)
+    P, r = _solve_gpu(inst)
+    st = r.status.cpu().numpy(); rs = r.resid.cpu().numpy()
+    assert (st == 0).all(), np.bincount(st)
+    assert rs[:, 0:4].max() <= TOL_GATE and rs[:, 7].max() <= TOL_RES and rs[:, 8].max() <= TOL_RES
+    assert rs[:, 4].max() <= 1e-5 and rs[:, 5].max() <= 1e-9
+    rng = np.random.default_rng(0)
+    sample = sorted(rng.choice(inst.A, size=n_sample, replace=False).tolist())
+    W, res = _oracle(inst, accounts=sample)
+    _check_against_oracle(inst, r, W, res, accounts=sample)
+    P.close()
