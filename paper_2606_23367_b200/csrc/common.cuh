@@ -24,6 +24,7 @@ struct AccountParams {            // per-account scalars, struct of arrays on th
   int32_t* iters;
   int32_t* refactor;// capacitance must be rebuilt (rho changed)
   int32_t* nadapt;  // iteration of the account's last rho adaptation
+  double* win;      // live-list window of the prox for the next launch (threshold units)
 };
 
 struct prism_problem {
@@ -54,6 +55,7 @@ struct prism_problem {
   double* w_stage;  // A x N, allocated on the first prism_solve_batch_host call
   int32_t* i_stage; // A
   AccountParams ap;
+  long long* xs_dbg;      // debug phase timers (PRISM_DBG)
   int32_t* counters;      // [0] number of done accounts
   int32_t* h_counters;    // pinned host mirror
   int64_t bytes;
@@ -91,30 +93,30 @@ __device__ __forceinline__ double warp_min(double x) {
   return x;
 }
 
-// Block-wide reduction of NV values per thread; OP: 0 sum, 1 max, 2 min.  Result broadcast to all threads.
-// `scratch` needs NV * 32 doubles.  Fixed order => deterministic.
-template <int NV>
-__device__ __forceinline__ void block_reduce(double (&val)[NV], const int (&op)[NV], double* scratch) {
+// Block-wide reduction of NV values per thread with one compile-time operation OP (0 sum, 1 max); the result is
+// broadcast to all threads.  `scratch` needs NV * 32 doubles.  Fixed order => deterministic.
+template <int OP>
+__device__ __forceinline__ double red_op(double a, double b) { return OP == 0 ? a + b : fmax(a, b); }
+template <int NV, int OP>
+__device__ __forceinline__ void block_reduce(double (&val)[NV], double* scratch) {
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
 #pragma unroll
   for (int q = 0; q < NV; ++q) {
     double x = val[q];
-    x = op[q] == 0 ? warp_sum(x) : (op[q] == 1 ? warp_max(x) : warp_min(x));
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) x = red_op<OP>(x, __shfl_xor_sync(0xffffffffu, x, o));
     if (lane == 0) scratch[q * 32 + wid] = x;
   }
   __syncthreads();
-  if (wid == 0) {
+  // every warp reduces the per-warp partials itself (no second barrier, no broadcast step)
 #pragma unroll
-    for (int q = 0; q < NV; ++q) {
-      double x = lane < nw ? scratch[q * 32 + lane] : (op[q] == 0 ? 0.0 : (op[q] == 1 ? -INFINITY : INFINITY));
-      x = op[q] == 0 ? warp_sum(x) : (op[q] == 1 ? warp_max(x) : warp_min(x));
-      if (lane == 0) scratch[q * 32] = x;
-    }
+  for (int q = 0; q < NV; ++q) {
+    double x = lane < nw ? scratch[q * 32 + lane] : (OP == 0 ? 0.0 : -INFINITY);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) x = red_op<OP>(x, __shfl_xor_sync(0xffffffffu, x, o));
+    val[q] = x;
   }
-  __syncthreads();
-#pragma unroll
-  for (int q = 0; q < NV; ++q) val[q] = scratch[q * 32];
-  __syncthreads();
+  __syncthreads();      // scratch may be reused by the next call
 }
 
 // Deterministic per-group accumulation (replaces shared-memory atomics, whose order is unspecified):

@@ -90,15 +90,16 @@ __global__ void __launch_bounds__(256) k_diag(DiagArgs p) {
   __syncthreads();
   for (int g = tid; g < G; g += nt) gsum[g] = group_total(gbin, G, g);
   __syncthreads();
-  double val[5] = {sw, turn, fobj, rbox, rstat};
-  const int op[5] = {0, 0, 0, 1, 1};
-  block_reduce<5>(val, op, scratch);
+  double val[3] = {sw, turn, fobj};
+  block_reduce<3, 0>(val, scratch);
+  double vmx[2] = {rbox, rstat};
+  block_reduce<2, 1>(vmx, scratch);
   const int any_bad = __syncthreads_or(bad ? 1 : 0);
   if (tid == 0) {
     double* r = p.resid + (int64_t)a * PRISM_NRES;
     const double nan = any_bad ? NAN : 0.0;
     r[PRISM_R_BUDGET] = fabs(val[0] - 1.0) + nan;
-    r[PRISM_R_BOX] = fmax(val[3], 0.0) + nan;
+    r[PRISM_R_BOX] = fmax(vmx[0], 0.0) + nan;
     double rexp = 0.0, rcomp = 0.0;
     for (int g = 0; g < G; ++g) {
       const double bl = p.band_lo[(int64_t)a * G + g], bh = p.band_hi[(int64_t)a * G + g];
@@ -108,7 +109,7 @@ __global__ void __launch_bounds__(256) k_diag(DiagArgs p) {
     r[PRISM_R_EXPOSURE] = fmax(rexp, 0.0);
     r[PRISM_R_TURNOVER] = isfinite(tau) ? fmax(val[1] - tau, 0.0) : 0.0;
     if (have && isfinite(tau)) rcomp = fmax(rcomp, fabs(theta * (val[1] - tau)));
-    r[PRISM_R_STAT] = have ? val[4] : NAN;
+    r[PRISM_R_STAT] = have ? vmx[1] : NAN;
     r[PRISM_R_COMP] = have ? rcomp : NAN;
     r[PRISM_R_OBJECTIVE] = val[2] + nan;
     r[PRISM_R_TURNOVER_VALUE] = val[1];

@@ -3,6 +3,7 @@
 #include <chrono>
 #include <new>
 #include <vector>
+#include <cstdlib>
 
 #include "common.cuh"
 #include "diag.cuh"
@@ -27,7 +28,7 @@ static int pick_mt(int k) {
     default: { constexpr int MT = 16; __VA_ARGS__; } break;           \
   }
 
-#define PROX_SMEM_MAX (200 * 1024)   // dynamic shared memory budget of k_prox_smem (plus ~11 KB static)
+#define PROX_SMEM_MAX (208 * 1024)   // dynamic shared memory budget of k_prox_smem (plus ~11 KB static)
 static size_t g1_smem(int mt) { return (size_t)G1_STAGES * (8 * mt + G1_TA) * G1_LD * sizeof(double); }
 static size_t g2_smem(int mt) { return (size_t)(G2_TM + G2_TN) * (8 * mt + 4) * sizeof(double); }
 
@@ -59,7 +60,7 @@ extern "C" void prism_problem_destroy(prism_problem* p) {
   void* ptrs[] = {p->Bp, p->Bt, p->invd, p->gram, p->q, p->v, p->rt, p->cc, p->xs, p->pxq, p->Tpart, p->V, p->Sinv,
                   p->gw0, p->lamG, p->resid, p->duals, p->status, p->ap.c, p->ap.alpha, p->ap.beta,
                   p->ap.mode, p->ap.bsum, p->ap.done, p->ap.conv, p->ap.iters, p->ap.refactor,
-                  p->ap.nadapt, p->counters, p->w_stage, p->i_stage};
+                  p->ap.nadapt, p->ap.win, p->counters, p->w_stage, p->i_stage, p->xs_dbg};
   for (void* q : ptrs) if (q) cudaFree(q);
   if (p->h_counters) cudaFreeHost(p->h_counters);
   delete p;
@@ -235,7 +236,9 @@ extern "C" int prism_problem_create(int64_t N, int32_t k, int32_t accounts, cons
   ALLOC_TRY(dev_alloc(p, &p->ap.iters, (size_t)A));
   ALLOC_TRY(dev_alloc(p, &p->ap.refactor, (size_t)A));
   ALLOC_TRY(dev_alloc(p, &p->ap.nadapt, (size_t)A));
+  ALLOC_TRY(dev_alloc(p, &p->ap.win, (size_t)A));
   ALLOC_TRY(dev_alloc(p, &p->counters, (size_t)4));
+  ALLOC_TRY(dev_alloc(p, &p->xs_dbg, (size_t)A * 12));
   if (cudaMallocHost((void**)&p->h_counters, 4 * sizeof(int32_t)) != cudaSuccess) { prism_problem_destroy(p); return set_err(PRISM_ERR_ALLOC, "pinned allocation failed%s", ""); }
   if (p->d.w_b) ALLOC_TRY(dev_alloc(p, &p->q, AN));
   { int r = set_kernel_attrs(mt, p->Kp); if (r != PRISM_OK) { prism_problem_destroy(p); return r; } }
@@ -277,14 +280,15 @@ static ProxArgs make_prox_args(prism_problem* p, const prism_settings& s, double
   a.ap = p->ap; a.w_out = w_out; a.duals = p->duals; a.resid = p->resid; a.counters = p->counters;
   a.eps = s.eps_rel;
   a.adapt = s.adapt_rho; a.iter = 0; a.ldw = p->ldn;
+  a.dbg = getenv("PRISM_DBG") ? (long long*)p->xs_dbg : nullptr;
   return a;
 }
 
 static void launch_prox(prism_problem* p, cudaStream_t st, ProxArgs& a, int mode, int iter) {
   a.iter = iter;
   if (p->d.lot_count) k_prox<true><<<p->A, 512, 0, st>>>(a, mode);
-  else if (p->d.hi_full || (size_t)p->N * 16 > PROX_SMEM_MAX) k_prox<false><<<p->A, 512, 0, st>>>(a, mode);
-  else k_prox_smem<<<p->A, 512, (size_t)p->N * 16, st>>>(a, mode);
+  else if (p->d.hi_full || (size_t)p->N * 20 + 16 > PROX_SMEM_MAX) k_prox<false><<<p->A, 512, 0, st>>>(a, mode);
+  else k_prox_smem<<<p->A, 512, (size_t)p->N * 20 + 16, st>>>(a, mode);
 }
 
 static DiagArgs make_diag_args(prism_problem* p, const double* w, const double* duals, double* resid) {
@@ -423,6 +427,12 @@ extern "C" int prism_solve_batch(prism_problem* p, const prism_settings* sp, voi
   cudaEventDestroy(ev0);
   cudaEventDestroy(ev1);
   return PRISM_OK;
+}
+
+extern "C" int prism_debug_timers(const prism_problem* p, long long* out) {
+  cudaMemcpy(out, p->xs_dbg, (size_t)p->A * 12 * sizeof(long long), cudaMemcpyDeviceToHost);
+  cudaMemset(p->xs_dbg, 0, (size_t)p->A * 12 * sizeof(long long));
+  return 0;
 }
 
 extern "C" int prism_kernel_times(const prism_problem* p, double* ms_out, int64_t* launches_out) {

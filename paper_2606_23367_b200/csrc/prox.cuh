@@ -53,70 +53,84 @@ struct ProxArgs {
   // settings
   double eps;
   int32_t adapt, iter;
+  long long* dbg;          // optional per-account phase timers (8 per account), NULL in production
 };
 
 enum { PROX_CHECK = 1, PROX_FINAL = 2, PROX_INIT = 4 };
 #define PRISM_ADAPT_START 200   // first iteration at which an account's rho may be adapted
 #define PRISM_ADAPT_EVERY 100   // minimum iterations between two adaptations of one account
 
-struct ElemConst {        // per-element quantities that do not depend on the trial thresholds
-  double u, ir, bl, bh, sl, sh, w0;     // u = v - w0, ir = 1 / rho_i, buy range [bl, bh], sell range [sl, sh]
+// Per-element constants of one launch, in "threshold space":  T = rho u - (kappa + c_buy),  Delta = 2 kappa + c_buy:
+//   buy_i(a)  = bl + clamp((T - a) / rho - bl, 0, wB)            a  = alpha + lambda_g
+//   sell_i(b) = sl + clamp((b - Delta - T) / rho - sl, 0, wS)    b  = beta + lambda_g
+// (with lots: sum over lots of clamp((b - Delta - s_l - T)/rho - Q_{l-1}, 0, q_l), clipped to [sl, min(sl + wS, Q_L)]).
+struct ElemConst {
+  double T, ir, bl, wB, sl, wS, w0;      // ir = 1 / rho_i; buy range [bl, bl + wB]; sell range [sl, sl + wS]
 };
 
 __device__ __forceinline__ void elem_ranges(ElemConst& e, double lo, double hi) {
+  const double bh = fmax(hi - e.w0, 0.0), sh = fmax(e.w0 - lo, 0.0);
   e.bl = fmax(lo - e.w0, 0.0);
-  e.bh = fmax(hi - e.w0, 0.0);
   e.sl = fmax(e.w0 - hi, 0.0);
-  e.sh = fmax(e.w0 - lo, 0.0);
+  e.wB = bh - e.bl;
+  e.wS = sh - e.sl;
 }
 
-// buy amount at threshold a = alpha + lambda_g; mv = 1/rho_i if strictly inside its range (|slope| of the piece)
-__device__ __forceinline__ double buy_amt(const ElemConst& e, double lam_b, double a, double& mv) {
-  const double raw = e.u - (lam_b + a) * e.ir;
-  mv = (raw > e.bl && raw < e.bh) ? e.ir : 0.0;
-  return fmin(fmax(raw, e.bl), e.bh);
+// buy amount at threshold a; mv = 1/rho_i if strictly inside its range (|slope| of the piece), else 0
+__device__ __forceinline__ double buy_amt(const ElemConst& e, double a, double& mv) {
+  const double tb = (e.T - a) * e.ir - e.bl;
+  mv = 0.0;
+  if (tb <= 0.0) return e.bl;
+  if (tb >= e.wB) return e.bl + e.wB;
+  mv = e.ir;
+  return e.bl + tb;
 }
 
 template <bool LOTS>
-__device__ __forceinline__ double sell_amt(const ElemConst& e, double kappa, double bt, const double* slope,
-                                           const double* width, int nl, double& mv) {
-  double raw, inside = 0.0;
-  double sh = e.sh;
+__device__ __forceinline__ double sell_amt(const ElemConst& e, double bd, const double* slope, const double* width,
+                                           int nl, double& mv) {   // bd = beta + lambda_g - Delta
+  mv = 0.0;
   if (LOTS && nl > 0) {
-    raw = 0.0;
-    double Q = 0.0;
+    double raw = 0.0, Q = 0.0, inside = 0.0;
     for (int l = 0; l < nl; ++l) {
-      const double r = (bt - kappa - slope[l]) * e.ir - e.u - Q;
+      const double r = (bd - slope[l] - e.T) * e.ir - Q;
       const double ql = width[l];
       if (r > 0.0 && r < ql) inside = 1.0;
       raw += fmin(fmax(r, 0.0), ql);
       Q += ql;
     }
-    sh = fmin(sh, Q);
-  } else {
-    raw = (bt - kappa) * e.ir - e.u;
-    inside = 1.0;
+    const double sh = fmin(e.sl + e.wS, Q);
+    if (inside > 0.0 && raw > e.sl && raw < sh) mv = e.ir;
+    return fmin(fmax(raw, e.sl), sh);
   }
-  mv = (inside > 0.0 && raw > e.sl && raw < sh) ? e.ir : 0.0;
-  return fmin(fmax(raw, e.sl), sh);
+  const double ts = (bd - e.T) * e.ir - e.sl;
+  if (ts <= 0.0) return e.sl;
+  if (ts >= e.wS) return e.sl + e.wS;
+  mv = e.ir;
+  return e.sl + ts;
 }
 
 // One bracketed Newton step on a continuous piecewise-linear monotone function.
-// dir = +1: g increasing in x, -1: decreasing.  slope = |g'| at x (0 on a flat piece).
+// dir = +1: g increasing in x, -1: decreasing.  slope = |g'| at x (0 on a flat piece).  Brackets may be infinite
+// (lazy): then a step that needs bisection reports need_bracket instead.
 struct Root1D {
   double x, lo, hi;
   int done;
 };
-__device__ __forceinline__ void root_step(Root1D& r, double g, double slope, double target, int dir, double tol) {
-  if (r.done) return;
+__device__ __forceinline__ bool root_step(Root1D& r, double g, double slope, double target, int dir, double tol) {
+  if (r.done) return false;
   const double diff = g - target;
-  if (fabs(diff) <= tol) { r.done = 1; return; }
+  if (fabs(diff) <= tol) { r.done = 1; return false; }
   const bool too_big = (dir > 0) ? (diff > 0.0) : (diff < 0.0);   // x lies right of the root
   if (too_big) r.hi = r.x; else r.lo = r.x;
   double xn = (slope > 0.0) ? r.x - (double)dir * diff / slope : NAN;
-  if (!(xn > r.lo && xn < r.hi)) xn = 0.5 * (r.lo + r.hi);
-  if (xn == r.x || !(r.hi - r.lo > 0.0) || !(xn > r.lo && xn < r.hi)) { r.done = 1; r.x = (xn == xn) ? xn : r.x; return; }
+  if (!(xn > r.lo && xn < r.hi)) {
+    if (!(r.lo > -INFINITY) || !(r.hi < INFINITY)) return true;   // bisection needs finite brackets
+    xn = 0.5 * (r.lo + r.hi);
+  }
+  if (xn == r.x || !(r.hi - r.lo > 0.0) || !(xn > r.lo && xn < r.hi)) { r.done = 1; r.x = (xn == xn) ? xn : r.x; return false; }
   r.x = xn;
+  return false;
 }
 
 // ---------------------------------------------------------------------------------------------- element sources
@@ -125,14 +139,13 @@ template <bool LOTS>
 struct SrcGlobal {
   const ProxArgs& p;
   int64_t row, rowp;
-  double icg, lo_a, hi_a;
-  __device__ SrcGlobal(const ProxArgs& p_, int a, double cg, double lo, double hi)
-      : p(p_), row((int64_t)a * p_.N), rowp((int64_t)a * p_.ldw), icg(1.0 / cg), lo_a(lo), hi_a(hi) {}
-  __device__ __forceinline__ void set_scale(double cg) { icg = 1.0 / cg; }
+  double cg, icg, lo_a, hi_a, lam_b;
+  __device__ SrcGlobal(const ProxArgs& p_, int a, double cg_, double lo, double hi, double lam_b_)
+      : p(p_), row((int64_t)a * p_.N), rowp((int64_t)a * p_.ldw), cg(cg_), icg(1.0 / cg_), lo_a(lo), hi_a(hi), lam_b(lam_b_) {}
   __device__ __forceinline__ void load(int64_t i, ElemConst& e, int& g, int& nl, const double*& sl, const double*& wd) const {
     const int64_t idx = row + i;
     e.w0 = p.w0[idx];
-    e.u = p.v[rowp + i] - e.w0;
+    e.T = (p.v[rowp + i] - e.w0) * (cg * p.d[i]) - lam_b;
     e.ir = p.invd[i] * icg;
     double lo = lo_a, hi = p.hi_full ? p.hi_full[idx] : hi_a;
     if (p.excl && p.excl[idx]) { lo = 0.0; hi = 0.0; }
@@ -159,35 +172,118 @@ struct SrcGlobal {
       f(valid, i, e, g, nl, sl, wd);
     }
   }
-  __device__ __forceinline__ void store_v(int64_t i, double vv) const { p.v[rowp + i] = vv; }
+  template <class F>
+  __device__ __forceinline__ void for_each_all(F f) const { for_each(f); }
+  __device__ __forceinline__ void classify(double, double, const double*, double, int*) {}
+  __device__ __forceinline__ bool window_ok(double, double, const double*) const { return true; }
+  static constexpr bool kWindowed = false;
 };
 
-// Shared-memory source: u = v - w0 and w0 of the whole account stay in shared memory for the kernel (2 x 8 B x N),
-// so a trial evaluation touches no HBM: only 1/d_i, the exclusion byte and the group id (shared by many CTAs or
-// tiny; L1/L2 resident).  Each thread reads back only what it wrote: no barrier needed.  No lots, no per-asset caps.
+// Shared-memory source: T and w0 of the whole account (2 x 8 B x N) plus a class byte and the group id per asset
+// stay in shared memory for the kernel, so a trial evaluation touches no HBM: only 1/d_i (shared by all accounts,
+// L2 resident).  No lots, no per-asset caps.
+//
+// Live list.  Most assets sit on the kink (no trade) and stay there while the thresholds move a little, so the
+// root-finding passes only visit the assets that can trade for thresholds inside a WINDOW around the warm start:
+// a regular asset is dead if  T <= (alpha_w + lambda_w,g) - W  and  T + Delta >= (beta_w + lambda_w,g) + W;  then its
+// buy and sell amounts are exactly 0 whenever |alpha - alpha_w|, |beta - beta_w|, |lambda_g - lambda_w,g| <= W / 2.
+// The solve runs on the live list; if its result leaves the window it is repeated with W = inf (all assets).
+// The list is compacted in (thread, slot) order by a block scan, so every sum keeps a fixed order (deterministic).
 struct SrcSmem {
   const ProxArgs& p;
   int64_t row, rowp;
-  double icg, lo_a, hi_a;
-  double *us, *ws;
-  __device__ SrcSmem(const ProxArgs& p_, int a, double cg, double lo, double hi, double* smem)
-      : p(p_), row((int64_t)a * p_.N), rowp((int64_t)a * p_.ldw), icg(1.0 / cg), lo_a(lo), hi_a(hi), us(smem), ws(smem + p_.N) {
-    for (int64_t i = threadIdx.x; i < p.N; i += blockDim.x) {
-      const double w = p.w0[row + i];
-      ws[i] = w;
-      us[i] = p.v[rowp + i] - w;
+  double icg, lo_a, hi_a, Delta;
+  double *Ts, *ws;
+  uint8_t *cls, *gid;      // cls: 0 regular (lo <= w0 <= hi, not excluded), 1 excluded, 2 outside the box
+  static constexpr bool kWindowed = true;
+  uint16_t* live;
+  int n_live;
+  double aw, bw, W;        // warm-start thresholds and window
+  const double* lam_w;     // warm-start band multipliers (global, G entries)
+  __device__ SrcSmem(const ProxArgs& p_, int a, double cg, double lo, double hi, double lam_b, double Delta_, double* smem)
+      : p(p_), row((int64_t)a * p_.N), rowp((int64_t)a * p_.ldw), icg(1.0 / cg), lo_a(lo), hi_a(hi), Delta(Delta_), Ts(smem),
+        ws(smem + p_.N), cls((uint8_t*)(smem + 2 * p_.N)), gid((uint8_t*)(smem + 2 * p_.N) + p_.N),
+        live((uint16_t*)((uint8_t*)(smem + 2 * p_.N) + 2 * p_.N)), n_live(0), aw(0), bw(0), W(INFINITY), lam_w(nullptr) {
+    constexpr int CB = 8;                              // loads of CB slots are issued together (memory-level parallelism)
+    const int64_t nt = blockDim.x;
+    for (int64_t i0 = threadIdx.x; i0 < p.N; i0 += CB * nt) {
+      double v8[CB], w8[CB], d8[CB]; uint8_t e8[CB], g8[CB];
+#pragma unroll
+      for (int u = 0; u < CB; ++u) {
+        const int64_t i = i0 + u * nt;
+        if (i < p.N) {
+          w8[u] = p.w0[row + i]; v8[u] = p.v[rowp + i]; d8[u] = p.d[i];
+          e8[u] = p.excl ? p.excl[row + i] : 0; g8[u] = p.G ? p.group_id[i] : 0;
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < CB; ++u) {
+        const int64_t i = i0 + u * nt;
+        if (i < p.N) {
+          ws[i] = w8[u];
+          Ts[i] = (v8[u] - w8[u]) * (cg * d8[u]) - lam_b;
+          cls[i] = e8[u] ? 1 : ((w8[u] >= lo && w8[u] <= hi) ? 0 : 2);
+          gid[i] = g8[u];
+        }
+      }
     }
   }
-  __device__ __forceinline__ void load(int64_t i, ElemConst& e, int& g) const {
-    e.w0 = ws[i]; e.u = us[i];
-    e.ir = p.invd[i] * icg;
-    const bool ex = p.excl && p.excl[row + i];
-    elem_ranges(e, ex ? 0.0 : lo_a, ex ? 0.0 : hi_a);
-    g = p.G ? p.group_id[i] : 0;
+  // (Re)build the live list for the window W around (aw_, bw_, lam_w_).  scratch: >= 64 ints of shared memory.
+  __device__ void classify(double aw_, double bw_, const double* lam_w_, double W_, int* scratch) {
+    aw = aw_; bw = bw_; lam_w = lam_w_; W = W_;
+    const int tid = threadIdx.x, nt = blockDim.x, lane = tid & 31, wid = tid >> 5, nw = (nt + 31) >> 5;
+    const bool all = !(W < INFINITY);
+    auto is_live = [&](int64_t i) -> bool {
+      if (all || cls[i] != 0) return true;
+      const double lg = p.G ? lam_w[gid[i]] : 0.0;
+      const double T = Ts[i];
+      return !(T <= aw + lg - W && T + Delta >= bw + lg + W);
+    };
+    // index-ordered compaction (keeps shared-memory and global accesses of the live passes coalesced):
+    // per (slot, warp) counts by ballot -> serial exclusive scan of the small table -> ballot again and write
+    const int nslot = (int)((p.N + nt - 1) / nt);
+    __syncthreads();                                   // scratch may still be in use by an earlier reduction
+    for (int sl = 0; sl < nslot; ++sl) {
+      const int64_t i = (int64_t)sl * nt + tid;
+      const unsigned m = __ballot_sync(0xffffffffu, i < p.N && is_live(i));
+      if (lane == 0) scratch[sl * nw + wid] = __popc(m);
+    }
+    __syncthreads();
+    if (tid == 0) {
+      int run = 0;
+      for (int q = 0; q < nslot * nw; ++q) { const int t = scratch[q]; scratch[q] = run; run += t; }
+      scratch[nslot * nw] = run;
+    }
+    __syncthreads();
+    for (int sl = 0; sl < nslot; ++sl) {
+      const int64_t i = (int64_t)sl * nt + tid;
+      const bool lv = i < p.N && is_live(i);
+      const unsigned m = __ballot_sync(0xffffffffu, lv);
+      if (lv) live[scratch[sl * nw + wid] + __popc(m & ((1u << lane) - 1u))] = (uint16_t)i;
+    }
+    n_live = scratch[nslot * nw];
+    __syncthreads();
   }
+  __device__ __forceinline__ bool window_ok(double al, double be, const double* lamS) const {
+    if (!(W < INFINITY)) return true;
+    bool ok = fabs(al - aw) <= 0.5 * W && fabs(be - bw) <= 0.5 * W;
+    for (int g = 0; g < p.G; ++g) ok = ok && fabs(lamS[g] - lam_w[g]) <= 0.5 * W;
+    return ok;
+  }
+  __device__ __forceinline__ void load(int64_t i, ElemConst& e, int& g) const {
+    e.w0 = ws[i]; e.T = Ts[i];
+    e.ir = p.invd[i] * icg;
+    const int c = cls[i];
+    g = gid[i];
+    if (c == 0) { e.bl = 0.0; e.sl = 0.0; e.wB = hi_a - e.w0; e.wS = e.w0 - lo_a; }
+    else elem_ranges(e, c == 1 ? 0.0 : lo_a, c == 1 ? 0.0 : hi_a);
+  }
+  // live assets only (root-finding passes)
   template <class F>
   __device__ __forceinline__ void for_each(F f) const {
-    for (int64_t i = threadIdx.x; i < p.N; i += blockDim.x) {
+#pragma unroll 2
+    for (int j = threadIdx.x; j < n_live; j += blockDim.x) {
+      const int64_t i = live[j];
       ElemConst e; int g;
       load(i, e, g);
       f(i, e, g, 0, (const double*)nullptr, (const double*)nullptr);
@@ -195,20 +291,169 @@ struct SrcSmem {
   }
   template <class F>
   __device__ __forceinline__ void for_each_uniform(F f) const {
-    for (int64_t i0 = 0; i0 < p.N; i0 += blockDim.x) {
-      const int64_t i = i0 + threadIdx.x;
-      const bool valid = i < p.N;
+    for (int j0 = 0; j0 < n_live; j0 += blockDim.x) {
+      const int j = j0 + threadIdx.x;
+      const bool valid = j < n_live;
+      const int64_t i = valid ? live[j] : 0;
       ElemConst e; int g = 0;
       if (valid) load(i, e, g);
       f(valid, i, e, g, 0, (const double*)nullptr, (const double*)nullptr);
     }
   }
-  __device__ __forceinline__ void store_v(int64_t i, double vv) const { p.v[rowp + i] = vv; }
+  // every asset (check and output passes), loads batched
+  template <class F>
+  __device__ __forceinline__ void for_each_all(F f) const {
+    constexpr int PB = 4;
+    const int64_t nt = blockDim.x;
+    for (int64_t i0 = threadIdx.x; i0 < p.N; i0 += PB * nt) {
+      double T4[PB], w4[PB], iv4[PB]; int c4[PB], g4[PB];
+#pragma unroll
+      for (int u = 0; u < PB; ++u) {
+        const int64_t i = i0 + u * nt;
+        if (i < p.N) { T4[u] = Ts[i]; w4[u] = ws[i]; iv4[u] = p.invd[i]; c4[u] = cls[i]; g4[u] = gid[i]; }
+      }
+#pragma unroll
+      for (int u = 0; u < PB; ++u) {
+        const int64_t i = i0 + u * nt;
+        if (i < p.N) {
+          ElemConst e;
+          e.w0 = w4[u]; e.T = T4[u]; e.ir = iv4[u] * icg;
+          if (c4[u] == 0) { e.bl = 0.0; e.sl = 0.0; e.wB = hi_a - e.w0; e.wS = e.w0 - lo_a; }
+          else elem_ranges(e, c4[u] == 1 ? 0.0 : lo_a, c4[u] == 1 ? 0.0 : hi_a);
+          f(i, e, g4[u], 0, (const double*)nullptr, (const double*)nullptr);
+        }
+      }
+    }
+  }
 };
 
+// One pass over the account: totals P, R and their slopes at thresholds (al, bd + Delta) shifted by the group
+// multipliers, plus the same four sums restricted to up to two selected groups s1, s2 (-1 = none).
+// out[0..3] = P, R, sP, sR;  out[4..7] = group s1;  out[8..11] = group s2.   Not inlined: it is called from many places.
 template <bool LOTS, class Src>
-__device__ __forceinline__ void prox_body(const ProxArgs& p, int mode, Src& src, int a, double gam, double c) {
-  __shared__ double scratch[8 * 32];
+__device__ __noinline__ void prox_eval(const Src& src, const double* lamS, int G, double al, double bd, int s1, int s2,
+                                       double* scratch, double* out) {
+  double lP = 0, lR = 0, lsP = 0, lsR = 0, x[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+  const long long tq0 = clock64();
+  src.for_each([&](int64_t, const ElemConst& e, int g, int nl, const double* sl, const double* wd) {
+    double mvb, mvs;
+    const double lg = G ? lamS[g] : 0.0;
+    const double pb = buy_amt(e, al + lg, mvb);
+    const double ps = sell_amt<LOTS>(e, bd + lg, sl, wd, nl, mvs);
+    lP += pb; lR += ps; lsP += mvb; lsR += mvs;
+    if (g == s1) { x[0] += pb; x[1] += ps; x[2] += mvb; x[3] += mvs; }
+    if (g == s2) { x[4] += pb; x[5] += ps; x[6] += mvb; x[7] += mvs; }
+  });
+  const long long tq1 = clock64();
+  if (src.p.dbg && threadIdx.x == 0) { src.p.dbg[(int64_t)blockIdx.x * 12 + 10] += tq1 - tq0; }
+  if (s1 >= 0 || s2 >= 0) {
+    double val[12] = {lP, lR, lsP, lsR, x[0], x[1], x[2], x[3], x[4], x[5], x[6], x[7]};
+    block_reduce<12, 0>(val, scratch);
+#pragma unroll
+    for (int q = 0; q < 12; ++q) out[q] = val[q];
+  } else {
+    double val[4] = {lP, lR, lsP, lsR};
+    block_reduce<4, 0>(val, scratch);
+#pragma unroll
+    for (int q = 0; q < 4; ++q) out[q] = val[q];
+  }
+  if (src.p.dbg && threadIdx.x == 0) { src.p.dbg[(int64_t)blockIdx.x * 12 + 11] += clock64() - tq1; }
+}
+
+// Range of the breakpoints in threshold space: out = {a_min, a_max, b_min, b_max} (only when bisection is needed).
+template <bool LOTS, class Src>
+__device__ __noinline__ void prox_brackets(const Src& src, double Delta, double* scratch, double* out) {
+  double x4 = INFINITY, x5 = -INFINITY, x6 = INFINITY, x7 = -INFINITY;
+  src.for_each([&](int64_t, const ElemConst& e, int, int nl, const double* sl, const double* wd) {
+    const double rho = 1.0 / e.ir;
+    if (e.wB > 0.0) { x4 = fmin(x4, e.T - rho * (e.bl + e.wB)); x5 = fmax(x5, e.T - rho * e.bl); }
+    double sh = e.sl + e.wS, s_first = 0.0, s_last = 0.0;
+    if (LOTS && nl > 0) { double Q = 0; for (int l = 0; l < nl; ++l) Q += wd[l]; sh = fmin(sh, Q); s_first = sl[0]; s_last = sl[nl - 1]; }
+    if (sh > e.sl) { x6 = fmin(x6, e.T + Delta + s_first + rho * e.sl); x7 = fmax(x7, e.T + Delta + s_last + rho * sh); }
+  });
+  double val[4] = {-x4, x5, -x6, x7};          // min via max of the negation: one uniform reduction
+  block_reduce<4, 1>(val, scratch);
+  out[0] = -val[0]; out[1] = val[1]; out[2] = -val[2]; out[3] = val[3];
+}
+
+// Sums of the trades per group at the final thresholds -> gsum[g] = gw0[g] + sum (deterministic binned pass).
+template <bool LOTS, class Src>
+__device__ __noinline__ void prox_group_sums(const Src& src, const double* lamS, int G, double al, double bd,
+                                             const double* gw0, double* gbin, double* gsum) {
+  const int tid = threadIdx.x, nt = blockDim.x;
+  for (int g = tid; g < 16 * G; g += nt) gbin[g] = 0.0;
+  __syncthreads();
+  src.for_each_uniform([&](bool valid, int64_t, const ElemConst& e, int g, int nl, const double* sl, const double* wd) {
+    double t = 0.0;
+    if (valid) {
+      double mvb, mvs;
+      t = buy_amt(e, al + lamS[g], mvb) - sell_amt<LOTS>(e, bd + lamS[g], sl, wd, nl, mvs);
+    }
+    warp_group_add(gbin, G, valid ? g : 0, t, valid);
+  });
+  __syncthreads();
+  for (int g = tid; g < G; g += nt) gsum[g] = gw0[g] + group_total(gbin, G, g);
+  __syncthreads();
+}
+
+// Scaled residuals of the splitting (reading R13) from the stored x and P x + q: out = {r_p, r_d}.
+template <bool LOTS, class Src>
+__device__ __noinline__ void prox_check(const ProxArgs& p, const Src& src, const double* lamS, int a, double al, double bd,
+                                        double lam_b, double cg, double* scratch, double* out) {
+  const int G = p.G;
+  const int64_t row = (int64_t)a * p.N, rowp = (int64_t)a * p.ldw;
+  double nx = 0, nz = 0, nrp = 0, nrd = 0, nPx = 0, ny = 0, nq = 0;
+  src.for_each_all([&](int64_t i, const ElemConst& e, int g, int nl, const double* sl, const double* wd) {
+    double mvb, mvs;
+    const double lg = G ? lamS[g] : 0.0;
+    const double tr = buy_amt(e, al + lg, mvb) - sell_amt<LOTS>(e, bd + lg, sl, wd, nl, mvs);
+    const double z = e.w0 + tr;
+    const double y = e.T + lam_b - tr * (cg * p.d[i]);  // rho (v - z) = rho u - rho t
+    const double x = p.xs[rowp + i], pq = p.pxq[rowp + i];
+    const double qi = p.q ? p.q[rowp + i] : -p.mu[row + i];
+    nx = fmax(nx, fabs(x)); nz = fmax(nz, fabs(z)); nrp = fmax(nrp, fabs(x - z));
+    nrd = fmax(nrd, fabs(pq + y)); nPx = fmax(nPx, fabs(pq - qi)); ny = fmax(ny, fabs(y)); nq = fmax(nq, fabs(qi));
+    if (!(z == z) || !(x == x) || !(e.T == e.T)) nrp = INFINITY;     // fmax drops NaN: poison explicitly
+  });
+  double val[7] = {nx, nz, nrp, nrd, nPx, ny, nq};
+  block_reduce<7, 1>(val, scratch);
+  out[0] = val[2] / fmax(fmax(val[0], val[1]), 1e-300);
+  out[1] = val[3] / fmax(fmax(val[4], fmax(val[5], val[6])), 1e-300);
+}
+
+// Output pass: either the returned weights (finished) or what the x-update needs: r~ = M^-1 r, c = r~ - z,
+// and v re-expressed in the new rho when it changed.  (e.T, e.ir refer to the old rho.)
+template <bool LOTS, class Src>
+__device__ __noinline__ void prox_output(const ProxArgs& p, const Src& src, const double* lamS, int a, double al, double bd,
+                                         double lam_b, double gam, double c_old, double c_new, int finished) {
+  const int G = p.G;
+  const int64_t row = (int64_t)a * p.N, rowp = (int64_t)a * p.ldw;
+  const double cg = c_old * gam, cgn = c_new * gam, igc = 1.0 / (gam * (1.0 + c_new)), icgn = 1.0 / cgn;
+  const bool rescale = c_new != c_old;
+  src.for_each_all([&](int64_t i, const ElemConst& e, int g, int nl, const double* sl, const double* wd) {
+    double mvb, mvs;
+    const double lg = G ? lamS[g] : 0.0;
+    const double tr = buy_amt(e, al + lg, mvb) - sell_amt<LOTS>(e, bd + lg, sl, wd, nl, mvs);
+    const double z = e.w0 + tr;
+    if (finished) { p.w_out[row + i] = z; return; }
+    const double di = p.d[i], dinv = p.invd[i];
+    const double y = e.T + lam_b - tr * (cg * di);         // rho_old (v - z): unchanged by a rho change
+    if (rescale) p.v[rowp + i] = z + y * dinv * icgn;      // v' = z + y / rho_new
+    const double qi = p.q ? p.q[rowp + i] : -p.mu[row + i];
+    const double r = cgn * di * z - y - qi;
+    const double rt = r * dinv * igc;                      // M_i = gamma d_i (1 + c)
+    p.rt[rowp + i] = rt;
+    p.cc[rowp + i] = rt - z;
+  });
+}
+
+template <class Src> __device__ __forceinline__ long long src_nlive(const Src&) { return 0; }
+__device__ __forceinline__ long long src_nlive(const SrcSmem& s) { return s.n_live; }
+
+template <bool LOTS, class Src>
+__device__ __forceinline__ void prox_body(const ProxArgs& p, int mode, Src& src, int a, double gam, double c,
+                                          double kappa, double lam_b) {
+  __shared__ double scratch[12 * 32];
   __shared__ double gbin[16 * PRISM_MAX_GROUPS];    // per-warp group bins (deterministic accumulation)
   __shared__ double lamS[PRISM_MAX_GROUPS];
   __shared__ double gsum[PRISM_MAX_GROUPS];
@@ -216,130 +461,157 @@ __device__ __forceinline__ void prox_body(const ProxArgs& p, int mode, Src& src,
   const int tid = threadIdx.x, nt = blockDim.x;
   const int64_t N = p.N, row = (int64_t)a * N, rowp = (int64_t)a * p.ldw;
   double cg = c * gam;
-  const double kappa = p.kappa ? p.kappa[a] : 0.0;
-  const double lam_b = kappa + (p.c_buy ? p.c_buy[a] : 0.0);
+  const double Delta = lam_b + kappa;
   const double tau = p.tau ? p.tau[a] : INFINITY;
   const double b = p.ap.bsum[a];
   const int G = p.G;
   for (int g = tid; g < G; g += nt) lamS[g] = p.lamG[(int64_t)a * G + g];
   __syncthreads();
 
+  long long t0 = clock64(), t_ev = 0, t_gs = 0, t1, t2, t3;
   double alpha = p.ap.alpha[a], beta = p.ap.beta[a];
   int amode = p.ap.mode[a];
   if (!(amode == 1 && isfinite(tau))) { amode = 0; beta = alpha; }
-  double a_min, a_max, b_min, b_max;
+  const double alpha_w = alpha, beta_w = beta;       // warm start (previous iteration's thresholds)
+  const int amode_w = amode;
+  const double* lam_w = p.lamG + (int64_t)a * G;
+  src.classify(alpha_w, beta_w, lam_w, Src::kWindowed ? p.ap.win[a] : INFINITY, (int*)scratch);
+  double a_min = -INFINITY, a_max = INFINITY, b_min = -INFINITY, b_max = INFINITY;   // brackets, computed lazily
+  bool have_br = false;
   double P = 0, R = 0, sP = 0, sR = 0, Pa = 0, Ra = 0, pa = 0, ra = 0;
+  int n_eval = 0, n_win_fail = 0;
 
-  // pass 0: totals at the warm start and the range of the breakpoints (brackets)
-  {
-    double lP = 0, lR = 0, lsP = 0, lsR = 0, x4 = INFINITY, x5 = -INFINITY, x6 = INFINITY, x7 = -INFINITY;
-    src.for_each([&](int64_t, const ElemConst& e, int g, int nl, const double* sl, const double* wd) {
-      double mvb, mvs;
-      const double lg = G ? lamS[g] : 0.0;
-      lP += buy_amt(e, lam_b, alpha + lg, mvb);
-      lR += sell_amt<LOTS>(e, kappa, beta + lg, sl, wd, nl, mvs);
-      lsP += mvb; lsR += mvs;
-      const double rho = 1.0 / e.ir;
-      if (e.bh > e.bl) { x4 = fmin(x4, rho * (e.u - e.bh) - lam_b); x5 = fmax(x5, rho * (e.u - e.bl) - lam_b); }
-      double sh = e.sh, s_first = 0.0, s_last = 0.0;
-      if (LOTS && nl > 0) { double Q = 0; for (int l = 0; l < nl; ++l) Q += wd[l]; sh = fmin(sh, Q); s_first = sl[0]; s_last = sl[nl - 1]; }
-      if (sh > e.sl) { x6 = fmin(x6, rho * (e.u + e.sl) + kappa + s_first); x7 = fmax(x7, rho * (e.u + sh) + kappa + s_last); }
-    });
-    double val[8] = {lP, lR, lsP, lsR, x4, x5, x6, x7};
-    const int op[8] = {0, 0, 0, 0, 2, 1, 2, 1};
-    block_reduce<8>(val, op, scratch);
-    P = val[0]; R = val[1]; sP = val[2]; sR = val[3];
-    a_min = val[4]; a_max = val[5]; b_min = val[6]; b_max = val[7];
-  }
-  // one pass: totals at thresholds (al, be) shifted by the group multipliers; with sel >= 0 also the sums of group sel
-  int n_eval = 1;
-  auto eval = [&](double al, double be, int sel) {
-    ++n_eval;
-    double lP = 0, lR = 0, lsP = 0, lsR = 0, x4 = 0, x5 = 0, x6 = 0, x7 = 0;
-    src.for_each([&](int64_t, const ElemConst& e, int g, int nl, const double* sl, const double* wd) {
-      double mvb, mvs;
-      const double lg = G ? lamS[g] : 0.0;
-      const double pb = buy_amt(e, lam_b, al + lg, mvb);
-      const double ps = sell_amt<LOTS>(e, kappa, be + lg, sl, wd, nl, mvs);
-      lP += pb; lR += ps; lsP += mvb; lsR += mvs;
-      if (g == sel) { x4 += pb; x5 += ps; x6 += mvb; x7 += mvs; }
-    });
-    if (sel >= 0) {
-      double val[8] = {lP, lR, lsP, lsR, x4, x5, x6, x7};
-      const int op[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-      block_reduce<8>(val, op, scratch);
-      P = val[0]; R = val[1]; sP = val[2]; sR = val[3]; Pa = val[4]; Ra = val[5]; pa = val[6]; ra = val[7];
-    } else {
-      double val[4] = {lP, lR, lsP, lsR};
-      const int op[4] = {0, 0, 0, 0};
-      block_reduce<4>(val, op, scratch);
-      P = val[0]; R = val[1]; sP = val[2]; sR = val[3];
-    }
+  // range of the breakpoints in threshold space (only when a root find needs bisection)
+  auto brackets = [&]() {
+    double out[4];
+    prox_brackets<LOTS>(src, Delta, scratch, out);
+    a_min = out[0]; a_max = out[1]; b_min = out[2]; b_max = out[3];
+    const double span = fmax(fmax(fabs(a_min), fabs(a_max)), fmax(fabs(b_min), fabs(b_max)));
+    const double pad = 1e-9 * fmax(span, 1e-300) + 1e-300;
+    if (!(a_min <= a_max)) { a_min = -1.0; a_max = 1.0; }
+    if (!(b_min <= b_max)) { b_min = -1.0; b_max = 1.0; }
+    a_min -= pad; a_max += pad; b_min -= pad; b_max += pad;
+    have_br = true;
   };
-  const double span = fmax(fmax(fabs(a_min), fabs(a_max)), fmax(fabs(b_min), fabs(b_max)));
-  const double pad = 1e-9 * fmax(span, 1e-300) + 1e-300;
-  if (!(a_min <= a_max)) { a_min = -1.0; a_max = 1.0; }
-  if (!(b_min <= b_max)) { b_min = -1.0; b_max = 1.0; }
-  a_min -= pad; a_max += pad; b_min -= pad; b_max += pad;
+  double Pb = 0, Rb = 0, pb2 = 0, rb2 = 0;     // sums of a second selected group (joint Newton)
+  auto eval2 = [&](double al, double be, int s1, int s2) {
+    ++n_eval;
+    double out[12];
+    long long te = clock64();
+    prox_eval<LOTS>(src, lamS, G, al, be - Delta, s1, s2, scratch, out);
+    t_ev += clock64() - te;
+    P = out[0]; R = out[1]; sP = out[2]; sR = out[3];
+    if (s1 >= 0 || s2 >= 0) { Pa = out[4]; Ra = out[5]; pa = out[6]; ra = out[7]; Pb = out[8]; Rb = out[9]; pb2 = out[10]; rb2 = out[11]; }
+  };
+  auto eval = [&](double al, double be, int sel) { eval2(al, be, sel, -1); };
   const double tol = 2e-15 * fmax(1.0, fabs(b) + (isfinite(tau) ? tau : 0.0));
   const double Pt = 0.5 * (tau + b), Rt = 0.5 * (tau - b);
-  const double Lmax = 2.0 * (fmax(a_max, b_max) - fmin(a_min, b_min)) + 1.0;
-  bool fresh = true;     // P, R, ... correspond to (alpha, beta, lamS, sel = -1)
 
   // (alpha, beta) for the current group multipliers; leaves the sums of the final thresholds (and of group sel)
   auto solve_ab = [&](int sel) {
     double lmin = 0.0, lmax = 0.0;
     for (int g = 0; g < G; ++g) { lmin = fmin(lmin, lamS[g]); lmax = fmax(lmax, lamS[g]); }
-    const double alo = a_min - lmax, ahi = a_max - lmin, blo = b_min - lmax, bhi = b_max - lmin;
-    for (int attempt = 0; attempt < 3; ++attempt) {
+    for (int attempt = 0; attempt < 4; ++attempt) {
+      const double alo = a_min - lmax, ahi = a_max - lmin, blo = b_min - lmax, bhi = b_max - lmin;
+      bool need = false;
       if (amode == 1) {
         Root1D ra_ = {fmin(fmax(alpha, alo), ahi), alo, ahi, 0};
         Root1D rb_ = {fmin(fmax(beta, blo), bhi), blo, bhi, 0};
-        if (!fresh || sel >= 0 || ra_.x != alpha || rb_.x != beta) eval(ra_.x, rb_.x, sel);
-        fresh = false;
+        eval(ra_.x, rb_.x, sel);
         for (int it = 0; it < 80; ++it) {
-          root_step(ra_, P, sP, Pt, -1, tol);
-          root_step(rb_, R, sR, Rt, +1, tol);
-          if (ra_.done && rb_.done) break;
+          need = root_step(ra_, P, sP, Pt, -1, tol) | root_step(rb_, R, sR, Rt, +1, tol);
+          if (need || (ra_.done && rb_.done)) break;
           eval(ra_.x, rb_.x, sel);
         }
         alpha = ra_.x; beta = rb_.x;
+        if (need) { brackets(); continue; }
         if (alpha >= beta) break;
         amode = 0; alpha = beta = 0.5 * (alpha + beta);
       } else {
         const double lo_b = fmin(alo, blo), hi_b = fmax(ahi, bhi);
         Root1D rn = {fmin(fmax(alpha, lo_b), hi_b), lo_b, hi_b, 0};
-        if (!fresh || sel >= 0 || rn.x != alpha || beta != alpha) eval(rn.x, rn.x, sel);
-        fresh = false;
+        eval(rn.x, rn.x, sel);
         for (int it = 0; it < 80; ++it) {
-          root_step(rn, P - R, sP + sR, b, -1, tol);
-          if (rn.done) break;
+          need = root_step(rn, P - R, sP + sR, b, -1, tol);
+          if (need || rn.done) break;
           eval(rn.x, rn.x, sel);
         }
         alpha = beta = rn.x;
+        if (need) { brackets(); continue; }
         if (!isfinite(tau) || P + R <= tau + tol) break;
         amode = 1;
       }
     }
   };
 
+  for (int wpass = 0; wpass < 2; ++wpass) {
+  // Fast path when one or two bands were active at the previous iteration: semismooth Newton on (alpha, beta,
+  // lambda_g1[, lambda_g2]) jointly, one pass per step (the system is piecewise linear; from the warm start it lands
+  // on the final piece in a few steps).  Anything unexpected falls through to the robust nested solve below.
+  if (G > 0) {
+    int g1 = -1, g2 = -1, nact = 0;
+    for (int g = 0; g < G; ++g) if (lamS[g] != 0.0) { if (nact == 0) g1 = g; else if (nact == 1) g2 = g; ++nact; }
+    if (nact >= 1 && nact <= 2) {
+      const double bnd1 = lamS[g1] > 0.0 ? p.band_hi[(int64_t)a * G + g1] : p.band_lo[(int64_t)a * G + g1];
+      const double bnd2 = g2 >= 0 ? (lamS[g2] > 0.0 ? p.band_hi[(int64_t)a * G + g2] : p.band_lo[(int64_t)a * G + g2]) : 0.0;
+      const double gw1 = p.gw0[(int64_t)a * G + g1], gw2 = g2 >= 0 ? p.gw0[(int64_t)a * G + g2] : 0.0;
+      const double sg1 = lamS[g1] > 0.0 ? 1.0 : -1.0, sg2 = g2 >= 0 ? (lamS[g2] > 0.0 ? 1.0 : -1.0) : 1.0;
+      double al = alpha, be = beta, l1 = lamS[g1], l2 = g2 >= 0 ? lamS[g2] : 0.0;
+      bool ok = false;
+      for (int it = 0; it < 10; ++it) {
+        eval2(al, be, g1, g2);
+        const double F1 = gw1 + Pa - Ra - bnd1, F2 = g2 >= 0 ? gw2 + Pb - Rb - bnd2 : 0.0;
+        double FA, FB;                                   // residuals of the (alpha, beta) equations
+        if (amode == 1) { FA = P - Pt; FB = R - Rt; } else { FA = P - R - b; FB = 0.0; }
+        if (fabs(F1) <= tol && fabs(F2) <= tol && fabs(FA) <= tol && fabs(FB) <= tol) { ok = true; break; }
+        // reduced Newton system in (dl1, dl2)
+        double M11, M12, M22, r1, r2;
+        const double s1 = pa + ra, s2 = pb2 + rb2;
+        if (amode == 1) {
+          if (!(sP > 0.0) || !(sR > 0.0)) break;
+          M11 = -s1 + pa * pa / sP + ra * ra / sR; M22 = -s2 + pb2 * pb2 / sP + rb2 * rb2 / sR;
+          M12 = pa * pb2 / sP + ra * rb2 / sR;
+          r1 = -F1 + pa * FA / sP - ra * FB / sR; r2 = -F2 + pb2 * FA / sP - rb2 * FB / sR;
+        } else {
+          const double st = sP + sR;
+          if (!(st > 0.0)) break;
+          M11 = -s1 + s1 * s1 / st; M22 = -s2 + s2 * s2 / st; M12 = s1 * s2 / st;
+          r1 = -F1 + s1 * FA / st; r2 = -F2 + s2 * FA / st;
+        }
+        double d1, d2 = 0.0;
+        if (g2 >= 0) {
+          const double det = M11 * M22 - M12 * M12;
+          if (!(fabs(det) > 1e-300)) break;
+          d1 = (r1 * M22 - M12 * r2) / det; d2 = (M11 * r2 - M12 * r1) / det;
+        } else {
+          if (!(fabs(M11) > 1e-300)) break;
+          d1 = r1 / M11;
+        }
+        if (amode == 1) { al += (FA - pa * d1 - pb2 * d2) / sP; be += (-FB - ra * d1 - rb2 * d2) / sR; }
+        else { al += (FA - s1 * d1 - s2 * d2) / (sP + sR); be = al; }
+        l1 += d1; l2 += d2;
+        if (!(l1 == l1) || !(l2 == l2) || !(al == al) || !(be == be)) break;
+        __syncthreads();
+        if (tid == 0) { lamS[g1] = l1; if (g2 >= 0) lamS[g2] = l2; }
+        __syncthreads();
+      }
+      // accept only a consistent solution: multiplier signs kept, theta >= 0 / cap slack; otherwise restore and fall through
+      bool good = ok && l1 * sg1 > 0.0 && (g2 < 0 || l2 * sg2 > 0.0);
+      if (good) good = amode == 1 ? (al >= be) : (!isfinite(tau) || P + R <= tau + tol);
+      __syncthreads();
+      if (good) { alpha = al; beta = be; }
+      else if (tid == 0) { lamS[g1] = p.lamG[(int64_t)a * G + g1]; if (g2 >= 0) lamS[g2] = p.lamG[(int64_t)a * G + g2]; }
+      __syncthreads();
+    }
+  }
+
   for (int round = 0; round < 2 * G + 2; ++round) {
     solve_ab(-1);
     if (G == 0) break;
     // all group sums at the current solution (deterministic binned pass)
-    for (int g = tid; g < 16 * G; g += nt) gbin[g] = 0.0;
-    __syncthreads();
-    src.for_each_uniform([&](bool valid, int64_t, const ElemConst& e, int g, int nl, const double* sl, const double* wd) {
-      double t = 0.0;
-      if (valid) {
-        double mvb, mvs;
-        t = buy_amt(e, lam_b, alpha + lamS[g], mvb) - sell_amt<LOTS>(e, kappa, beta + lamS[g], sl, wd, nl, mvs);
-      }
-      warp_group_add(gbin, G, valid ? g : 0, t, valid);
-    });
-    __syncthreads();
-    for (int g = tid; g < G; g += nt) gsum[g] = p.gw0[(int64_t)a * G + g] + group_total(gbin, G, g);
-    __syncthreads();
+    { long long tg = clock64();
+    prox_group_sums<LOTS>(src, lamS, G, alpha, beta - Delta, p.gw0 + (int64_t)a * G, gbin, gsum);
+    t_gs += clock64() - tg; }
     if (tid == 0) {
       int sel = -1, sgn = 0; double worst = 8.0 * tol;
       for (int g = 0; g < G; ++g) {
@@ -357,6 +629,8 @@ __device__ __forceinline__ void prox_body(const ProxArgs& p, int mode, Src& src,
     const int sel = selS[0], sgn = selS[1];
     if (sel < 0) break;
     // scalar problem in m = sgn * lambda_sel >= 0:  h(m) = sgn * (S_sel - bound) is non-increasing, want h = 0 or m = 0
+    if (!have_br) brackets();
+    const double Lmax = 2.0 * (fmax(a_max, b_max) - fmin(a_min, b_min)) + 1.0;
     const double bound = sgn > 0 ? p.band_hi[(int64_t)a * G + sel] : p.band_lo[(int64_t)a * G + sel];
     const double gw = p.gw0[(int64_t)a * G + sel];
     double m = sgn * lamS[sel], mlo = 0.0, mhi = Lmax;
@@ -380,32 +654,29 @@ __device__ __forceinline__ void prox_body(const ProxArgs& p, int mode, Src& src,
       if (mn == m) break;
       m = mn;
     }
-    fresh = false;
+  }
+  __syncthreads();
+    if (src.window_ok(alpha, beta, lamS)) break;
+    // the solution left the window the live list was built for: rebuild it with every asset and solve again
+    alpha = alpha_w; beta = beta_w; amode = amode_w;
+    __syncthreads();
+    for (int g = tid; g < G; g += nt) lamS[g] = lam_w[g];
+    __syncthreads();
+    src.classify(alpha_w, beta_w, lam_w, INFINITY, (int*)scratch);
+    have_br = false; a_min = b_min = -INFINITY; a_max = b_max = INFINITY;
+    ++n_win_fail;
   }
   __syncthreads();
 
+  t1 = clock64();
   // ---------------------------------------------------------------- check: residuals, mask, rho adaptation
-  double rescale = 1.0;
+  double c_new = c;
   int finished = 0;
+  const double bdf = beta - Delta;
   if (mode & PROX_CHECK) {
-    double nx = 0, nz = 0, nrp = 0, nrd = 0, nPx = 0, ny = 0, nq = 0;
-    src.for_each([&](int64_t i, const ElemConst& e, int g, int nl, const double* sl, const double* wd) {
-      double mvb, mvs;
-      const double lg = G ? lamS[g] : 0.0;
-      const double tr = buy_amt(e, lam_b, alpha + lg, mvb) - sell_amt<LOTS>(e, kappa, beta + lg, sl, wd, nl, mvs);
-      const double z = e.w0 + tr;
-      const double y = (e.u - tr) / e.ir;                 // rho (v - z)
-      const double x = p.xs[rowp + i], pq = p.pxq[rowp + i];
-      const double qi = p.q ? p.q[rowp + i] : -p.mu[row + i];
-      nx = fmax(nx, fabs(x)); nz = fmax(nz, fabs(z)); nrp = fmax(nrp, fabs(x - z));
-      nrd = fmax(nrd, fabs(pq + y)); nPx = fmax(nPx, fabs(pq - qi)); ny = fmax(ny, fabs(y)); nq = fmax(nq, fabs(qi));
-      if (!(z == z) || !(x == x) || !(e.u == e.u)) nrp = INFINITY;     // fmax drops NaN: poison explicitly
-    });
-    double val[7] = {nx, nz, nrp, nrd, nPx, ny, nq};
-    const int op[7] = {1, 1, 1, 1, 1, 1, 1};
-    block_reduce<7>(val, op, scratch);
-    const double rp = val[2] / fmax(fmax(val[0], val[1]), 1e-300);
-    const double rd = val[3] / fmax(fmax(val[4], fmax(val[5], val[6])), 1e-300);
+    double rr[2];
+    prox_check<LOTS>(p, src, lamS, a, alpha, bdf, lam_b, cg, scratch, rr);
+    const double rp = rr[0], rd = rr[1];
     const bool bad = !(rp < INFINITY) || !(rd < INFINITY);
     const bool conv = !bad && rp <= p.eps && rd <= p.eps;
     if (tid == 0) {
@@ -420,38 +691,31 @@ __device__ __forceinline__ void prox_body(const ProxArgs& p, int mode, Src& src,
       // rho <- rho sqrt(r_p / r_d), clipped, applied when the two scaled residuals are out of balance
       const double ratio = sqrt(rp / fmax(rd, 1e-300));
       if (ratio > 3.0 || ratio < 1.0 / 3.0) {
-        const double cn = c * fmin(fmax(ratio, 0.2), 5.0);
-        rescale = c / cn;          // v' = z + (rho/rho') (v - z) keeps y = rho (v - z) unchanged
-        c = cn; cg = c * gam;
-        if (tid == 0) { p.ap.c[a] = c; p.ap.refactor[a] = 1; }
+        c_new = c * fmin(fmax(ratio, 0.2), 5.0);
+        if (tid == 0) { p.ap.c[a] = c_new; p.ap.refactor[a] = 1; }
       }
       if (tid == 0) p.ap.nadapt[a] = p.iter;
     }
   }
   if (mode & PROX_FINAL) finished = 1;
 
-  // ---------------------------------------------------------------- output pass (e.ir still refers to the old rho)
-  const double igc = 1.0 / (gam * (1.0 + c));
-  src.for_each([&](int64_t i, const ElemConst& e, int g, int nl, const double* sl, const double* wd) {
-    double mvb, mvs;
-    const double lg = G ? lamS[g] : 0.0;
-    const double tr = buy_amt(e, lam_b, alpha + lg, mvb) - sell_amt<LOTS>(e, kappa, beta + lg, sl, wd, nl, mvs);
-    const double z = e.w0 + tr;
-    if (finished) { p.w_out[row + i] = z; return; }
-    const double y = (e.u - tr) / e.ir;                    // rho_old (v - z)
-    if (rescale != 1.0) src.store_v(i, z + rescale * (e.u - tr));
-    const double dinv = p.invd[i];
-    const double rho = cg / dinv;                          // new rho_i
-    const double qi = p.q ? p.q[rowp + i] : -p.mu[row + i];
-    const double r = rho * z - y - qi;
-    const double rt = r * dinv * igc;                      // M_i = gamma d_i (1 + c)
-    p.rt[rowp + i] = rt;
-    p.cc[rowp + i] = rt - z;
-  });
+  // ---------------------------------------------------------------- output pass (e.T, e.ir refer to the old rho)
+  t2 = clock64();
+  prox_output<LOTS>(p, src, lamS, a, alpha, bdf, lam_b, gam, c, c_new, finished);
+  t3 = clock64();
+  if (p.dbg && tid == 0) { long long* d = p.dbg + (int64_t)a * 12; d[8] += src_nlive(src); d[9] += n_win_fail; d[0] += t1 - t0; d[1] += t_ev; d[2] += t_gs; d[3] += t2 - t1; d[4] += t3 - t2; d[5] += n_eval; d[6] += 1; }
+  (void)n_win_fail;
+  double mv_l = 0.0;
+  for (int g = 0; g < G; ++g) mv_l = fmax(mv_l, fabs(lamS[g] - lam_w[g]));
+  __syncthreads();
   for (int g = tid; g < G; g += nt) p.lamG[(int64_t)a * G + g] = lamS[g];
   if (tid == 0) {
     p.resid[(int64_t)a * PRISM_NRES + PRISM_R_RESERVED] += (double)n_eval;   // trial evaluations (passes) so far
     p.ap.alpha[a] = alpha; p.ap.beta[a] = beta; p.ap.mode[a] = amode;
+    if (Src::kWindowed) {                      // next window: a multiple of how far the thresholds moved in this launch
+      const double mv = fmax(fmax(fabs(alpha - alpha_w), fabs(beta - beta_w)), mv_l);
+      p.ap.win[a] = fmax(32.0 * mv, 1e-9 + 1e-7 * (fabs(alpha) + fabs(beta)));
+    }
     if (finished) {
       p.ap.done[a] = 1;
       p.ap.iters[a] = p.iter;
@@ -460,7 +724,7 @@ __device__ __forceinline__ void prox_body(const ProxArgs& p, int mode, Src& src,
       du[0] = 0.5 * (alpha + beta);
       du[1] = 0.5 * (alpha - beta);
       for (int g = 0; g < G; ++g) { du[2 + g] = fmax(lamS[g], 0.0); du[2 + G + g] = fmax(-lamS[g], 0.0); }
-      p.resid[(int64_t)a * PRISM_NRES + PRISM_R_RHO] = c;
+      p.resid[(int64_t)a * PRISM_NRES + PRISM_R_RHO] = c_new;
     }
   }
 }
@@ -471,16 +735,22 @@ __global__ void __launch_bounds__(512) k_prox(ProxArgs p, int mode) {
   const int a = blockIdx.x;
   if (p.ap.done[a]) return;
   const double gam = p.gamma[a], c = p.ap.c[a];
-  SrcGlobal<LOTS> src(p, a, c * gam, p.lo[a], p.hi[a]);
-  prox_body<LOTS>(p, mode, src, a, gam, c);
+  const double kappa = p.kappa ? p.kappa[a] : 0.0;
+  const double lam_b = kappa + (p.c_buy ? p.c_buy[a] : 0.0);
+  SrcGlobal<LOTS> src(p, a, c * gam, p.lo[a], p.hi[a], lam_b);
+  prox_body<LOTS>(p, mode, src, a, gam, c, kappa, lam_b);
 }
 
-// shared-memory-resident kernel: 16 N bytes of dynamic shared memory, no lots, no per-asset caps
+// shared-memory-resident kernel: 18 N bytes of dynamic shared memory, no lots, no per-asset caps
 __global__ void __launch_bounds__(512, 1) k_prox_smem(ProxArgs p, int mode) {
   extern __shared__ __align__(16) double prox_smem[];
   const int a = blockIdx.x;
   if (p.ap.done[a]) return;
   const double gam = p.gamma[a], c = p.ap.c[a];
-  SrcSmem src(p, a, c * gam, p.lo[a], p.hi[a], prox_smem);
-  prox_body<false>(p, mode, src, a, gam, c);
+  const double kappa = p.kappa ? p.kappa[a] : 0.0;
+  const double lam_b = kappa + (p.c_buy ? p.c_buy[a] : 0.0);
+  long long tc = clock64();
+  SrcSmem src(p, a, c * gam, p.lo[a], p.hi[a], lam_b, lam_b + kappa, prox_smem);
+  if (p.dbg && threadIdx.x == 0) p.dbg[(int64_t)a * 12 + 7] += clock64() - tc;
+  prox_body<false>(p, mode, src, a, gam, c, kappa, lam_b);
 }

@@ -32,8 +32,7 @@ __global__ void k_gram(const double* Bt, int64_t ldn, const uint8_t* gid, const 
     s = fma(ur * uc, invd[i], s);
   }
   double val[1] = {s};
-  const int op[1] = {0};
-  block_reduce<1>(val, op, scratch);
+  block_reduce<1, 0>(val, scratch);
   if (threadIdx.x == 0) { gram[(int64_t)r * Kp + c] = val[0]; gram[(int64_t)c * Kp + r] = val[0]; }
 }
 
@@ -65,8 +64,7 @@ __global__ void k_init_accounts(InitArgs p) {
     if (p.G) warp_group_add(gs, p.G, valid ? p.group_id[i] : 0, w, valid);
   }
   double val[1] = {s};
-  const int op[1] = {0};
-  block_reduce<1>(val, op, scratch);
+  block_reduce<1, 0>(val, scratch);
   for (int g = tid; g < p.G; g += blockDim.x) {
     const int64_t e = (int64_t)a * p.G + g;
     p.gw0[e] = group_total(gs, p.G, g);     // group sums of w0: S_g = gw0_g + sum of the group's trades
@@ -75,7 +73,7 @@ __global__ void k_init_accounts(InitArgs p) {
   if (tid == 0) {
     p.ap.bsum[a] = 1.0 - val[0];
     p.ap.c[a] = p.rho_scale;
-    p.ap.alpha[a] = 0.0; p.ap.beta[a] = 0.0; p.ap.mode[a] = 0;
+    p.ap.alpha[a] = 0.0; p.ap.beta[a] = 0.0; p.ap.mode[a] = 0; p.ap.win[a] = INFINITY;
     p.ap.done[a] = 0; p.ap.conv[a] = 0; p.ap.iters[a] = 0; p.ap.refactor[a] = 1; p.ap.nadapt[a] = 0;
   }
 }
@@ -131,17 +129,20 @@ __global__ void __launch_bounds__(128) k_solve(SolveArgs p) {
   const int Kp = p.kp;
   for (int j = tid; j < Kp; j += blockDim.x) {
     double s = 0.0;
+#pragma unroll 8
     for (int ch = 0; ch < p.nchunk; ++ch) s += p.Tpart[((int64_t)ch * p.A + a) * p.ldv + j];   // fixed order => deterministic
     T[j] = s;
   }
   __syncthreads();
+  // S^-1 is symmetric: thread r walks column r (coalesced across threads, independent loads, no shuffles)
   const double* Si = p.Sinv + (int64_t)a * Kp * Kp;
-  for (int r = warp; r < Kp; r += 4) {
+  for (int r = tid; r < Kp; r += blockDim.x) {
     double s = 0.0;
-    for (int c = lane; c < Kp; c += 32) s = fma(Si[(int64_t)r * Kp + c], T[c], s);
-    s = warp_sum(s);
-    if (lane == 0) p.V[(int64_t)a * p.ldv + r] = s;
+#pragma unroll 8
+    for (int c = 0; c < Kp; ++c) s = fma(Si[(int64_t)c * Kp + r], T[c], s);
+    p.V[(int64_t)a * p.ldv + r] = s;
   }
+  (void)lane; (void)warp;
 }
 
 // V[a][j] = gamma_a f_j * sum_ch Tpart[ch][a][j]   (Sigma-apply: B (F (B'x)) via GEMM-1 then GEMM-2)
