@@ -66,6 +66,7 @@ enum { PROX_CHECK = 1, PROX_FINAL = 2, PROX_INIT = 4 };
 // (with lots: sum over lots of clamp((b - Delta - s_l - T)/rho - Q_{l-1}, 0, q_l), clipped to [sl, min(sl + wS, Q_L)]).
 struct ElemConst {
   double T, ir, bl, wB, sl, wS, w0;      // ir = 1 / rho_i; buy range [bl, bl + wB]; sell range [sl, sl + wS]
+  double d, qv;                          // d_i and q_ai: filled by for_each_all only (check / output passes)
 };
 
 __device__ __forceinline__ void elem_ranges(ElemConst& e, double lo, double hi) {
@@ -173,7 +174,15 @@ struct SrcGlobal {
     }
   }
   template <class F>
-  __device__ __forceinline__ void for_each_all(F f) const { for_each(f); }
+  __device__ __forceinline__ void for_each_all(F f) const {
+    for (int64_t i = threadIdx.x; i < p.N; i += blockDim.x) {
+      ElemConst e; int g, nl; const double *sl, *wd;
+      load(i, e, g, nl, sl, wd);
+      e.d = p.d[i];
+      e.qv = p.q ? p.q[rowp + i] : -p.mu[row + i];
+      f(i, e, g, nl, sl, wd);
+    }
+  }
   __device__ __forceinline__ void classify(double, double, const double*, double, int*) {}
   __device__ __forceinline__ bool window_ok(double, double, const double*) const { return true; }
   static constexpr bool kWindowed = false;
@@ -300,24 +309,27 @@ struct SrcSmem {
       f(valid, i, e, g, 0, (const double*)nullptr, (const double*)nullptr);
     }
   }
-  // every asset (check and output passes), loads batched
+  // every asset (check and output passes), loads batched (shared memory, 1/d, d and q of PB slots together)
   template <class F>
   __device__ __forceinline__ void for_each_all(F f) const {
-    constexpr int PB = 4;
+    constexpr int PB = 6;
     const int64_t nt = blockDim.x;
     for (int64_t i0 = threadIdx.x; i0 < p.N; i0 += PB * nt) {
-      double T4[PB], w4[PB], iv4[PB]; int c4[PB], g4[PB];
+      double T4[PB], w4[PB], iv4[PB], d4[PB], q4[PB]; int c4[PB], g4[PB];
 #pragma unroll
       for (int u = 0; u < PB; ++u) {
         const int64_t i = i0 + u * nt;
-        if (i < p.N) { T4[u] = Ts[i]; w4[u] = ws[i]; iv4[u] = p.invd[i]; c4[u] = cls[i]; g4[u] = gid[i]; }
+        if (i < p.N) {
+          T4[u] = Ts[i]; w4[u] = ws[i]; iv4[u] = p.invd[i]; d4[u] = p.d[i]; c4[u] = cls[i]; g4[u] = gid[i];
+          q4[u] = p.q ? p.q[rowp + i] : -p.mu[row + i];
+        }
       }
 #pragma unroll
       for (int u = 0; u < PB; ++u) {
         const int64_t i = i0 + u * nt;
         if (i < p.N) {
           ElemConst e;
-          e.w0 = w4[u]; e.T = T4[u]; e.ir = iv4[u] * icg;
+          e.w0 = w4[u]; e.T = T4[u]; e.ir = iv4[u] * icg; e.d = d4[u]; e.qv = q4[u];
           if (c4[u] == 0) { e.bl = 0.0; e.sl = 0.0; e.wB = hi_a - e.w0; e.wS = e.w0 - lo_a; }
           else elem_ranges(e, c4[u] == 1 ? 0.0 : lo_a, c4[u] == 1 ? 0.0 : hi_a);
           f(i, e, g4[u], 0, (const double*)nullptr, (const double*)nullptr);
@@ -408,9 +420,9 @@ __device__ __noinline__ void prox_check(const ProxArgs& p, const Src& src, const
     const double lg = G ? lamS[g] : 0.0;
     const double tr = buy_amt(e, al + lg, mvb) - sell_amt<LOTS>(e, bd + lg, sl, wd, nl, mvs);
     const double z = e.w0 + tr;
-    const double y = e.T + lam_b - tr * (cg * p.d[i]);  // rho (v - z) = rho u - rho t
+    const double y = e.T + lam_b - tr * (cg * e.d);     // rho (v - z) = rho u - rho t
     const double x = p.xs[rowp + i], pq = p.pxq[rowp + i];
-    const double qi = p.q ? p.q[rowp + i] : -p.mu[row + i];
+    const double qi = e.qv;
     nx = fmax(nx, fabs(x)); nz = fmax(nz, fabs(z)); nrp = fmax(nrp, fabs(x - z));
     nrd = fmax(nrd, fabs(pq + y)); nPx = fmax(nPx, fabs(pq - qi)); ny = fmax(ny, fabs(y)); nq = fmax(nq, fabs(qi));
     if (!(z == z) || !(x == x) || !(e.T == e.T)) nrp = INFINITY;     // fmax drops NaN: poison explicitly
@@ -436,10 +448,10 @@ __device__ __noinline__ void prox_output(const ProxArgs& p, const Src& src, cons
     const double tr = buy_amt(e, al + lg, mvb) - sell_amt<LOTS>(e, bd + lg, sl, wd, nl, mvs);
     const double z = e.w0 + tr;
     if (finished) { p.w_out[row + i] = z; return; }
-    const double di = p.d[i], dinv = p.invd[i];
+    const double di = e.d, dinv = e.ir * cg;               // e.ir = 1 / (c_old gamma d_i)
     const double y = e.T + lam_b - tr * (cg * di);         // rho_old (v - z): unchanged by a rho change
     if (rescale) p.v[rowp + i] = z + y * dinv * icgn;      // v' = z + y / rho_new
-    const double qi = p.q ? p.q[rowp + i] : -p.mu[row + i];
+    const double qi = e.qv;
     const double r = cgn * di * z - y - qi;
     const double rt = r * dinv * igc;                      // M_i = gamma d_i (1 + c)
     p.rt[rowp + i] = rt;
