@@ -131,6 +131,7 @@ typedef struct prism_settings {
   int32_t use_graph;        /* 1 => replay the inner iterations as a CUDA graph (default 1)                      */
   int32_t profile;          /* 1 => bracket every kernel launch with CUDA events (read with prism_kernel_times);
                                adds event overhead, so never combine with a throughput measurement           */
+  double prox_window_mult;  /* streaming prox: next window = this x the last movement of the thresholds (default 32) */
 } prism_settings;
 
 typedef struct prism_solve_info {
@@ -186,7 +187,7 @@ int prism_solve_batch_host(prism_problem* p, const prism_settings* s, void* cuda
 /* Kernel classes of the hot path: H4/H5/H6/H7 fused prox, H1 GEMM-1, H2 small solve + band
  * block, H3 GEMM-2 + epilogue, H0/H7 capacitance factorisation, H8/H9 diagnostics, everything else. */
 enum { PRISM_K_PROX = 0, PRISM_K_GEMM1 = 1, PRISM_K_SOLVE = 2, PRISM_K_GEMM2 = 3, PRISM_K_FACTOR = 4, PRISM_K_DIAG = 5,
-       PRISM_K_OTHER = 6, PRISM_NKERN = 8 };
+       PRISM_K_OTHER = 6, PRISM_K_PROX_SLOW = 7, PRISM_NKERN = 8 };
 
 /* Device time (ms, CUDA events on the solve stream) and launch count per kernel class of the last
  * prism_solve_batch call that ran with settings.profile = 1.  ms_out, launches_out: host arrays of PRISM_NKERN. */

@@ -41,7 +41,7 @@ class Settings(C.Structure):
     _fields_ = [("eps_rel", C.c_double), ("max_iter", C.c_int32), ("check_every", C.c_int32), ("alpha", C.c_double),
                 ("rho_scale", C.c_double), ("rho_band_scale", C.c_double), ("adapt_rho", C.c_int32),
                 ("gemm_mode", C.c_int32), ("time_limit_ms", C.c_double), ("deadline_ms", C.c_double),
-                ("use_graph", C.c_int32), ("profile", C.c_int32)]
+                ("use_graph", C.c_int32), ("profile", C.c_int32), ("prox_window_mult", C.c_double)]
 
 
 class SolveInfo(C.Structure):
@@ -199,7 +199,7 @@ class Problem:
                                            iters.data_ptr(), resid.data_ptr(), duals.data_ptr(), C.byref(info)))
         return SolveResult(w, status, iters, resid, duals, self._info(info))
 
-    KERNELS = ["prox", "gemm1", "solve", "gemm2", "factor", "diag", "other"]
+    KERNELS = ["prox", "gemm1", "solve", "gemm2", "factor", "diag", "other", "prox_slow"]
 
     def kernel_times(self) -> dict:
         ms = (C.c_double * 8)(); cnt = (C.c_int64 * 8)()

@@ -25,6 +25,7 @@ struct AccountParams {            // per-account scalars, struct of arrays on th
   int32_t* refactor;// capacitance must be rebuilt (rho changed)
   int32_t* nadapt;  // iteration of the account's last rho adaptation
   double* win;      // live-list window of the prox for the next launch (threshold units)
+  double* wins;     // window of the streaming pass (prox_fast.cuh), >= win
 };
 
 struct prism_problem {
@@ -55,7 +56,14 @@ struct prism_problem {
   double* w_stage;  // A x N, allocated on the first prism_solve_batch_host call
   int32_t* i_stage; // A
   AccountParams ap;
-  long long* xs_dbg;      // debug phase timers (PRISM_DBG)
+  // streaming prox (prox_fast.cuh)
+  int32_t fast, S, capw;  // fast: the streaming form applies; S slices per account; capacity of one warp's live list
+  int64_t slice_len, ldc;
+  struct LiveEnt *lraw, *lcomp;
+  int32_t *lcnt, *lflag;
+  unsigned long long* cbin;
+  double* chkp;
+  int32_t* stats;         // debug counters of the streaming prox (PRISM_PROX_STATS), else NULL
   int32_t* counters;      // [0] number of done accounts
   int32_t* h_counters;    // pinned host mirror
   int64_t bytes;

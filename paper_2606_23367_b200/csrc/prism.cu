@@ -9,6 +9,7 @@
 #include "diag.cuh"
 #include "gemm.cuh"
 #include "prox.cuh"
+#include "prox_fast.cuh"
 #include "small.cuh"
 
 #define PRISM_VERSION_STR "prism-b200 r1 (sm_100a, fp64 DMMA factor GEMMs, two-threshold prox)"
@@ -37,7 +38,7 @@ extern "C" void prism_default_settings(prism_settings* s) {
   memset(s, 0, sizeof(*s));
   s->eps_rel = 1e-6; s->max_iter = 4000; s->check_every = 10; s->alpha = 1.6; s->rho_scale = 100.0;
   s->rho_band_scale = 1.0; s->adapt_rho = 1; s->gemm_mode = 0; s->time_limit_ms = 0.0; s->deadline_ms = 0.0;
-  s->use_graph = 1;
+  s->use_graph = 1; s->prox_window_mult = 32.0;
 }
 extern "C" const char* prism_last_error(void) { return g_err; }
 extern "C" const char* prism_version(void) { return PRISM_VERSION_STR; }
@@ -60,7 +61,7 @@ extern "C" void prism_problem_destroy(prism_problem* p) {
   void* ptrs[] = {p->Bp, p->Bt, p->invd, p->gram, p->q, p->v, p->rt, p->cc, p->xs, p->pxq, p->Tpart, p->V, p->Sinv,
                   p->gw0, p->lamG, p->resid, p->duals, p->status, p->ap.c, p->ap.alpha, p->ap.beta,
                   p->ap.mode, p->ap.bsum, p->ap.done, p->ap.conv, p->ap.iters, p->ap.refactor,
-                  p->ap.nadapt, p->ap.win, p->counters, p->w_stage, p->i_stage, p->xs_dbg};
+                  p->ap.nadapt, p->ap.win, p->ap.wins, p->counters, p->w_stage, p->i_stage, p->lraw, p->lcomp, p->lcnt, p->cbin, p->chkp, p->lflag, p->stats};
   for (void* q : ptrs) if (q) cudaFree(q);
   if (p->h_counters) cudaFreeHost(p->h_counters);
   delete p;
@@ -159,8 +160,15 @@ static int set_kernel_attrs(int mt, int Kp) {
     CUDA_TRY(cudaFuncSetAttribute(k_gemm2<MT, G2_SIGMA>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g2_smem(MT)));
   });
   CUDA_TRY(cudaFuncSetAttribute(k_prox_smem, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PROX_SMEM_MAX));
+  CUDA_TRY(cudaFuncSetAttribute(k_prox_stream<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)stream_smem_bytes(PRISM_MAX_GROUPS)));
+  CUDA_TRY(cudaFuncSetAttribute(k_prox_stream<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)stream_smem_bytes(PRISM_MAX_GROUPS)));
   CUDA_TRY(cudaFuncSetAttribute(k_factor, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)((size_t)Kp * Kp * sizeof(double))));
   return PRISM_OK;
+}
+
+static bool fast_applicable(const prism_problem* p) {
+  return !p->d.lot_count && !p->d.hi_full && p->N < ((int64_t)1 << PROX_META_IDX_BITS) && p->N % 16 == 0 &&
+         !getenv("PRISM_PROX_NOFAST");     // N % 16: every row of every streamed array is 16-byte aligned (bulk copies)
 }
 
 // ------------------------------------------------------------------------------------------ create (H0)
@@ -237,8 +245,29 @@ extern "C" int prism_problem_create(int64_t N, int32_t k, int32_t accounts, cons
   ALLOC_TRY(dev_alloc(p, &p->ap.refactor, (size_t)A));
   ALLOC_TRY(dev_alloc(p, &p->ap.nadapt, (size_t)A));
   ALLOC_TRY(dev_alloc(p, &p->ap.win, (size_t)A));
+  ALLOC_TRY(dev_alloc(p, &p->ap.wins, (size_t)A));
   ALLOC_TRY(dev_alloc(p, &p->counters, (size_t)4));
-  ALLOC_TRY(dev_alloc(p, &p->xs_dbg, (size_t)A * 12));
+  p->fast = fast_applicable(p) ? 1 : 0;
+  if (p->fast) {
+    // slices: a few CTAs per resident slot so that the streaming kernel stays bandwidth-bound to the end of the grid
+    int64_t target = ((int64_t)8 * 3 * p->sm_count + A - 1) / A;           // CTAs per account wanted
+    int64_t sl = (N + target - 1) / target;
+    sl = (sl + FAST_CH - 1) / FAST_CH * FAST_CH;
+    if (const char* e = getenv("PRISM_PROX_SLICE")) sl = (atoll(e) + FAST_CH - 1) / FAST_CH * FAST_CH;
+    if (sl < 2 * FAST_CH) sl = 2 * FAST_CH;
+    p->slice_len = sl;
+    p->S = (int)((N + sl - 1) / sl);
+    p->capw = (int)(sl / FAST_NW);
+    p->ldc = (int64_t)p->S * sl;
+    const int Gb = G > 0 ? G : 1;
+    ALLOC_TRY(dev_alloc(p, &p->lraw, (size_t)A * p->ldc, false));
+    ALLOC_TRY(dev_alloc(p, &p->lcomp, (size_t)A * p->ldc, false));
+    ALLOC_TRY(dev_alloc(p, &p->lcnt, (size_t)A * p->S * FAST_NW));
+    ALLOC_TRY(dev_alloc(p, &p->cbin, (size_t)A * 2 * Gb));
+    ALLOC_TRY(dev_alloc(p, &p->chkp, (size_t)A * p->S * 8));
+    ALLOC_TRY(dev_alloc(p, &p->lflag, (size_t)A));
+  }
+  if (getenv("PRISM_PROX_STATS")) ALLOC_TRY(dev_alloc(p, &p->stats, (size_t)4096 * 8));
   if (cudaMallocHost((void**)&p->h_counters, 4 * sizeof(int32_t)) != cudaSuccess) { prism_problem_destroy(p); return set_err(PRISM_ERR_ALLOC, "pinned allocation failed%s", ""); }
   if (p->d.w_b) ALLOC_TRY(dev_alloc(p, &p->q, AN));
   { int r = set_kernel_attrs(mt, p->Kp); if (r != PRISM_OK) { prism_problem_destroy(p); return r; } }
@@ -280,15 +309,43 @@ static ProxArgs make_prox_args(prism_problem* p, const prism_settings& s, double
   a.ap = p->ap; a.w_out = w_out; a.duals = p->duals; a.resid = p->resid; a.counters = p->counters;
   a.eps = s.eps_rel;
   a.adapt = s.adapt_rho; a.iter = 0; a.ldw = p->ldn;
-  a.dbg = getenv("PRISM_DBG") ? (long long*)p->xs_dbg : nullptr;
+  a.lraw = p->lraw; a.lcomp = p->lcomp; a.lcnt = p->lcnt; a.cbin = p->cbin; a.chkp = p->chkp; a.lflag = p->lflag;
+  a.S = p->S; a.capw = p->capw; a.slice_len = p->slice_len; a.ldc = p->ldc;
+  a.stats = p->stats;
+  a.win_mult = s.prox_window_mult > 0 ? s.prox_window_mult : 32.0;
+  if (const char* e = getenv("PRISM_PROX_WIN_MULT")) a.win_mult = atof(e);
+  a.band_start = 20;
+  if (const char* e = getenv("PRISM_PROX_BAND_START")) a.band_start = atoi(e);
+  a.win_ratio = 16.0;
+  if (const char* e = getenv("PRISM_PROX_WIN_RATIO")) a.win_ratio = atof(e);
   return a;
 }
 
-static void launch_prox(prism_problem* p, cudaStream_t st, ProxArgs& a, int mode, int iter) {
+// Streaming form (k_prox_stream + k_prox_root, prox_fast.cuh) where it applies; else one of the every-asset kernels.
+static void launch_prox(Launcher& L, ProxArgs& a, int mode, int iter) {
+  prism_problem* p = L.p;
+  cudaStream_t st = L.st;
   a.iter = iter;
-  if (p->d.lot_count) k_prox<true><<<p->A, 512, 0, st>>>(a, mode);
-  else if (p->d.hi_full || (size_t)p->N * 20 + 16 > PROX_SMEM_MAX) k_prox<false><<<p->A, 512, 0, st>>>(a, mode);
-  else k_prox_smem<<<p->A, 512, (size_t)p->N * 20 + 16, st>>>(a, mode);
+  if (p->fast) {
+    const bool chk = (mode & (PROX_CHECK | PROX_FINAL)) != 0;     // the final extraction also needs w_out
+    const dim3 grid((unsigned)p->S, (unsigned)p->A);
+    const size_t sm = stream_smem_bytes(p->G), smr = root_smem_bytes(p->G, p->S * FAST_NW);
+    L.begin(PRISM_K_PROX);
+    if (chk) k_prox_stream<true><<<grid, FAST_NW * 32, sm, st>>>(a);
+    else k_prox_stream<false><<<grid, FAST_NW * 32, sm, st>>>(a);
+    L.end();
+    L.begin(PRISM_K_PROX_SLOW);
+    if (chk) k_prox_root<true><<<p->A, ROOT_NT, smr, st>>>(a, mode & ~PROX_CHECK);
+    else k_prox_root<false><<<p->A, ROOT_NT, smr, st>>>(a, mode);
+    L.end();
+    return;
+  }
+  const int grid = p->A < p->sm_count ? p->A : p->sm_count;
+  L.begin(PRISM_K_PROX);
+  if (p->d.lot_count) k_prox<true><<<grid, 512, 0, st>>>(a, mode);
+  else if (p->d.hi_full || (size_t)p->N * 20 + 16 > PROX_SMEM_MAX) k_prox<false><<<grid, 512, 0, st>>>(a, mode);
+  else k_prox_smem<<<grid, 512, (size_t)p->N * 20 + 16, st>>>(a, mode);
+  L.end();
 }
 
 static DiagArgs make_diag_args(prism_problem* p, const double* w, const double* duals, double* resid) {
@@ -358,9 +415,7 @@ extern "C" int prism_solve_batch(prism_problem* p, const prism_settings* sp, voi
   int it = 1, timed_out = 0, late_iter = -1, ndone = 0;
   for (; it <= s.max_iter; ++it) {
     const bool check = (it > 1) && ((it - 1) % s.check_every == 0);   // residuals of the iterate after it-1 iterations
-    L.begin(PRISM_K_PROX);
-    launch_prox(p, st, pa, check ? PROX_CHECK : 0, it - 1);
-    L.end();
+    launch_prox(L, pa, check ? PROX_CHECK : 0, it - 1);
     if (check || it == 1) {
       L.begin(PRISM_K_FACTOR);
       k_factor<<<A, 256, fac_smem, st>>>(p->gram, p->d.f, p->d.gamma, p->ap, p->k, p->kp, 0, p->Sinv);
@@ -383,9 +438,7 @@ extern "C" int prism_solve_batch(prism_problem* p, const prism_settings* sp, voi
     if (next_check) L.gemm2<G2_ADMM_CHECK>(g2); else L.gemm2<G2_ADMM>(g2);
   }
   if (ndone < A) {           // iteration cap or time limit: extract z for the accounts still running
-    L.begin(PRISM_K_PROX);
-    launch_prox(p, st, pa, PROX_FINAL, it > s.max_iter ? s.max_iter : it - 1);
-    L.end();
+    launch_prox(L, pa, PROX_FINAL, it > s.max_iter ? s.max_iter : it - 1);
   }
   // H8 / H9: external diagnostics of the returned weights with the solver's multipliers, then statuses
   run_diag(p, L, w_out, p->duals, p->resid);
@@ -429,10 +482,12 @@ extern "C" int prism_solve_batch(prism_problem* p, const prism_settings* sp, voi
   return PRISM_OK;
 }
 
-extern "C" int prism_debug_timers(const prism_problem* p, long long* out) {
-  cudaMemcpy(out, p->xs_dbg, (size_t)p->A * 12 * sizeof(long long), cudaMemcpyDeviceToHost);
-  cudaMemset(p->xs_dbg, 0, (size_t)p->A * 12 * sizeof(long long));
-  return 0;
+// debug only (PRISM_PROX_STATS=1 at create): per-iteration counters of the streaming prox; not part of prism.h
+extern "C" int prism_debug_prox_stats(prism_problem* p, int32_t* out, int clear) {
+  if (!p || !p->stats) return PRISM_ERR_NOT_READY;
+  cudaMemcpy(out, p->stats, (size_t)4096 * 8 * sizeof(int32_t), cudaMemcpyDeviceToHost);
+  if (clear) cudaMemset(p->stats, 0, (size_t)4096 * 8 * sizeof(int32_t));
+  return PRISM_OK;
 }
 
 extern "C" int prism_kernel_times(const prism_problem* p, double* ms_out, int64_t* launches_out) {

@@ -53,10 +53,22 @@ struct ProxArgs {
   // settings
   double eps;
   int32_t adapt, iter;
-  long long* dbg;          // optional per-account phase timers (8 per account), NULL in production
+  double win_mult;         // next window = win_mult x (movement of the thresholds in this launch)
+  double win_ratio;        // streaming pass: its (wide) window = win_ratio x the solve's (tight) window
+  int32_t band_start;      // streaming form: group bands join the projection at this iteration (their multipliers are 0 before)
+  // streaming form (prox_fast.cuh): per-warp live lists, their compacted copy, fixed-point bins of the dead assets
+  struct LiveEnt* lraw;    // [A][S * 8][capw]
+  struct LiveEnt* lcomp;   // [A][ldc]
+  int32_t* lcnt;           // [A][S * 8]
+  unsigned long long* cbin;// [A][2 max(G, 1)]  buys, sells per group in units of 2^-60 (zero between launches)
+  double* chkp;            // [A][S][8] residual terms of the dead assets per slice (check iterations)
+  int32_t* lflag;          // [A] 1: the account takes the generic path in k_prox_root
+  int32_t S, capw;         // slices per account; capacity of one warp's list
+  int64_t slice_len, ldc;  // assets per slice (multiple of 512); entries per account in lcomp
+  int32_t* stats;          // optional (debug): 8 counters per iteration, see k_prox_root; NULL in production
 };
 
-enum { PROX_CHECK = 1, PROX_FINAL = 2, PROX_INIT = 4 };
+enum { PROX_CHECK = 1, PROX_FINAL = 2 };
 #define PRISM_ADAPT_START 200   // first iteration at which an account's rho may be adapted
 #define PRISM_ADAPT_EVERY 100   // minimum iterations between two adaptations of one account
 
@@ -113,10 +125,13 @@ __device__ __forceinline__ double sell_amt(const ElemConst& e, double bd, const 
 
 // One bracketed Newton step on a continuous piecewise-linear monotone function.
 // dir = +1: g increasing in x, -1: decreasing.  slope = |g'| at x (0 on a flat piece).  Brackets may be infinite
-// (lazy): then a step that needs bisection reports need_bracket instead.
+// (lazy): then a step that cannot use Newton reports need_bracket instead.  With finite brackets such a step asks
+// for a SECTION pass (sect = 1): the caller evaluates the function at PROX_KSEC points of the bracket in one pass
+// over the assets (prox_eval_multi) and root_place() shrinks the bracket to the sub-interval that holds the root.
+#define PROX_KSEC 8
 struct Root1D {
   double x, lo, hi;
-  int done;
+  int done, sect;
 };
 __device__ __forceinline__ bool root_step(Root1D& r, double g, double slope, double target, int dir, double tol) {
   if (r.done) return false;
@@ -124,17 +139,42 @@ __device__ __forceinline__ bool root_step(Root1D& r, double g, double slope, dou
   if (fabs(diff) <= tol) { r.done = 1; return false; }
   const bool too_big = (dir > 0) ? (diff > 0.0) : (diff < 0.0);   // x lies right of the root
   if (too_big) r.hi = r.x; else r.lo = r.x;
-  double xn = (slope > 0.0) ? r.x - (double)dir * diff / slope : NAN;
+  const double xn = (slope > 0.0) ? r.x - (double)dir * diff / slope : NAN;
   if (!(xn > r.lo && xn < r.hi)) {
-    if (!(r.lo > -INFINITY) || !(r.hi < INFINITY)) return true;   // bisection needs finite brackets
-    xn = 0.5 * (r.lo + r.hi);
+    if (!(r.lo > -INFINITY) || !(r.hi < INFINITY)) return true;   // needs finite brackets
+    const double mid = 0.5 * (r.lo + r.hi);
+    if (!(mid > r.lo && mid < r.hi)) { r.done = 1; return false; } // bracket exhausted (adjacent doubles)
+    r.sect = 1;
+    return false;
   }
-  if (xn == r.x || !(r.hi - r.lo > 0.0) || !(xn > r.lo && xn < r.hi)) { r.done = 1; r.x = (xn == xn) ? xn : r.x; return false; }
+  if (xn == r.x) { r.done = 1; return false; }
   r.x = xn;
   return false;
 }
+// f[k] = function at x0 + k dx, k = 0 .. PROX_KSEC-1 (points strictly inside the bracket, ascending): new bracket =
+// the sub-interval that holds the root, new x = secant point of its ends (midpoint where an end value is unknown).
+__device__ __forceinline__ void root_place(Root1D& r, const double* f, double x0, double dx, double target, int dir) {
+  int kr = PROX_KSEC;
+  for (int k = PROX_KSEC - 1; k >= 0; --k) {
+    const double diff = f[k] - target;
+    if ((dir > 0) ? (diff > 0.0) : (diff < 0.0)) kr = k;          // x_k lies right of the root (monotone => a suffix)
+  }
+  const double lo = kr == 0 ? r.lo : x0 + (kr - 1) * dx, hi = kr == PROX_KSEC ? r.hi : x0 + kr * dx;
+  double x = 0.5 * (lo + hi);
+  if (kr > 0 && kr < PROX_KSEC) {
+    const double flo = f[kr - 1], fhi = f[kr];
+    if (fhi != flo) { const double xs = lo + (target - flo) / (fhi - flo) * (hi - lo); if (xs > lo && xs < hi) x = xs; }
+  }
+  r.lo = lo; r.hi = hi; r.sect = 0;
+  if (!(x > lo && x < hi)) { r.done = 1; x = lo; }
+  r.x = x;
+}
 
 // ---------------------------------------------------------------------------------------------- element sources
+// A source enumerates the assets the root find has to look at (for_each / for_each_uniform) and supplies the
+// constant parts of the sums that it does not enumerate: cP(), cR() (total buys / sells of the assets whose trade
+// cannot change inside the current window) and the same per group, cPg(g), cRg(g).
+
 // Generic source: every pass re-reads the account from global memory (any N, lots, per-asset caps).
 template <bool LOTS>
 struct SrcGlobal {
@@ -185,12 +225,15 @@ struct SrcGlobal {
   }
   __device__ __forceinline__ void classify(double, double, const double*, double, int*) {}
   __device__ __forceinline__ bool window_ok(double, double, const double*) const { return true; }
-  static constexpr bool kWindowed = false;
+  __device__ __forceinline__ double cP() const { return 0.0; }
+  __device__ __forceinline__ double cR() const { return 0.0; }
+  __device__ __forceinline__ double cPg(int) const { return 0.0; }
+  __device__ __forceinline__ double cRg(int) const { return 0.0; }
 };
 
 // Shared-memory source: T and w0 of the whole account (2 x 8 B x N) plus a class byte and the group id per asset
 // stay in shared memory for the kernel, so a trial evaluation touches no HBM: only 1/d_i (shared by all accounts,
-// L2 resident).  No lots, no per-asset caps.
+// L2 resident).  No lots, no per-asset caps.  Used when the streaming form (prox_fast.cuh) does not apply (N not a multiple of 16) and N is small enough.
 //
 // Live list.  Most assets sit on the kink (no trade) and stay there while the thresholds move a little, so the
 // root-finding passes only visit the assets that can trade for thresholds inside a WINDOW around the warm start:
@@ -204,7 +247,6 @@ struct SrcSmem {
   double icg, lo_a, hi_a, Delta;
   double *Ts, *ws;
   uint8_t *cls, *gid;      // cls: 0 regular (lo <= w0 <= hi, not excluded), 1 excluded, 2 outside the box
-  static constexpr bool kWindowed = true;
   uint16_t* live;
   int n_live;
   double aw, bw, W;        // warm-start thresholds and window
@@ -337,6 +379,20 @@ struct SrcSmem {
       }
     }
   }
+  __device__ __forceinline__ double cP() const { return 0.0; }
+  __device__ __forceinline__ double cR() const { return 0.0; }
+  __device__ __forceinline__ double cPg(int) const { return 0.0; }
+  __device__ __forceinline__ double cRg(int) const { return 0.0; }
+};
+
+// Shared-memory work areas of the root find (static in the slow kernels, carved from dynamic memory in the fast one).
+struct ProxShared {
+  double* scratch;   // 12 * 32
+  double* gbin;      // nwarps * G   per-warp group bins (deterministic accumulation)
+  double* lamS;      // G            band multipliers being solved for
+  double* gsum;      // G
+  int* selS;         // 2
+  const double *band_lo, *band_hi, *gw0;   // G each, this account's rows (global, or shared-memory copies)
 };
 
 // One pass over the account: totals P, R and their slopes at thresholds (al, bd + Delta) shifted by the group
@@ -346,7 +402,6 @@ template <bool LOTS, class Src>
 __device__ __noinline__ void prox_eval(const Src& src, const double* lamS, int G, double al, double bd, int s1, int s2,
                                        double* scratch, double* out) {
   double lP = 0, lR = 0, lsP = 0, lsR = 0, x[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-  const long long tq0 = clock64();
   src.for_each([&](int64_t, const ElemConst& e, int g, int nl, const double* sl, const double* wd) {
     double mvb, mvs;
     const double lg = G ? lamS[g] : 0.0;
@@ -356,20 +411,53 @@ __device__ __noinline__ void prox_eval(const Src& src, const double* lamS, int G
     if (g == s1) { x[0] += pb; x[1] += ps; x[2] += mvb; x[3] += mvs; }
     if (g == s2) { x[4] += pb; x[5] += ps; x[6] += mvb; x[7] += mvs; }
   });
-  const long long tq1 = clock64();
-  if (src.p.dbg && threadIdx.x == 0) { src.p.dbg[(int64_t)blockIdx.x * 12 + 10] += tq1 - tq0; }
   if (s1 >= 0 || s2 >= 0) {
     double val[12] = {lP, lR, lsP, lsR, x[0], x[1], x[2], x[3], x[4], x[5], x[6], x[7]};
     block_reduce<12, 0>(val, scratch);
 #pragma unroll
     for (int q = 0; q < 12; ++q) out[q] = val[q];
+    if (s1 >= 0) { out[4] += src.cPg(s1); out[5] += src.cRg(s1); }
+    if (s2 >= 0) { out[8] += src.cPg(s2); out[9] += src.cRg(s2); }
   } else {
     double val[4] = {lP, lR, lsP, lsR};
     block_reduce<4, 0>(val, scratch);
 #pragma unroll
     for (int q = 0; q < 4; ++q) out[q] = val[q];
   }
-  if (src.p.dbg && threadIdx.x == 0) { src.p.dbg[(int64_t)blockIdx.x * 12 + 11] += clock64() - tq1; }
+  out[0] += src.cP(); out[1] += src.cR();
+}
+
+// Section pass: buys at the PROX_KSEC thresholds a0 + k da and sells at b0 + k db (b = beta - Delta), one pass.
+template <bool LOTS, class Src>
+__device__ __noinline__ void prox_eval_multi(const Src& src, const double* lamS, int G, double a0, double da, double b0,
+                                             double db, double* scratch, double* outP, double* outR) {
+  double sp[PROX_KSEC], sr[PROX_KSEC];
+#pragma unroll
+  for (int k = 0; k < PROX_KSEC; ++k) { sp[k] = 0.0; sr[k] = 0.0; }
+  src.for_each([&](int64_t, const ElemConst& e, int g, int nl, const double* sl, const double* wd) {
+    const double lg = G ? lamS[g] : 0.0;
+#pragma unroll
+    for (int k = 0; k < PROX_KSEC; ++k) {
+      double mvb, mvs;
+      sp[k] += buy_amt(e, a0 + k * da + lg, mvb);
+      sr[k] += sell_amt<LOTS>(e, b0 + k * db + lg, sl, wd, nl, mvs);
+    }
+  });
+  const double cP = src.cP(), cR = src.cR();
+#pragma unroll
+  for (int q0 = 0; q0 < PROX_KSEC; q0 += 8) {
+    double val[8];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) val[q] = sp[q0 + q];
+    block_reduce<8, 0>(val, scratch);
+#pragma unroll
+    for (int q = 0; q < 8; ++q) outP[q0 + q] = val[q] + cP;
+#pragma unroll
+    for (int q = 0; q < 8; ++q) val[q] = sr[q0 + q];
+    block_reduce<8, 0>(val, scratch);
+#pragma unroll
+    for (int q = 0; q < 8; ++q) outR[q0 + q] = val[q] + cR;
+  }
 }
 
 // Range of the breakpoints in threshold space: out = {a_min, a_max, b_min, b_max} (only when bisection is needed).
@@ -392,8 +480,8 @@ __device__ __noinline__ void prox_brackets(const Src& src, double Delta, double*
 template <bool LOTS, class Src>
 __device__ __noinline__ void prox_group_sums(const Src& src, const double* lamS, int G, double al, double bd,
                                              const double* gw0, double* gbin, double* gsum) {
-  const int tid = threadIdx.x, nt = blockDim.x;
-  for (int g = tid; g < 16 * G; g += nt) gbin[g] = 0.0;
+  const int tid = threadIdx.x, nt = blockDim.x, nw = (nt + 31) >> 5;
+  for (int g = tid; g < nw * G; g += nt) gbin[g] = 0.0;
   __syncthreads();
   src.for_each_uniform([&](bool valid, int64_t, const ElemConst& e, int g, int nl, const double* sl, const double* wd) {
     double t = 0.0;
@@ -404,7 +492,7 @@ __device__ __noinline__ void prox_group_sums(const Src& src, const double* lamS,
     warp_group_add(gbin, G, valid ? g : 0, t, valid);
   });
   __syncthreads();
-  for (int g = tid; g < G; g += nt) gsum[g] = gw0[g] + group_total(gbin, G, g);
+  for (int g = tid; g < G; g += nt) gsum[g] = gw0[g] + group_total(gbin, G, g) + (src.cPg(g) - src.cRg(g));
   __syncthreads();
 }
 
@@ -413,7 +501,7 @@ template <bool LOTS, class Src>
 __device__ __noinline__ void prox_check(const ProxArgs& p, const Src& src, const double* lamS, int a, double al, double bd,
                                         double lam_b, double cg, double* scratch, double* out) {
   const int G = p.G;
-  const int64_t row = (int64_t)a * p.N, rowp = (int64_t)a * p.ldw;
+  const int64_t rowp = (int64_t)a * p.ldw;
   double nx = 0, nz = 0, nrp = 0, nrd = 0, nPx = 0, ny = 0, nq = 0;
   src.for_each_all([&](int64_t i, const ElemConst& e, int g, int nl, const double* sl, const double* wd) {
     double mvb, mvs;
@@ -459,39 +547,30 @@ __device__ __noinline__ void prox_output(const ProxArgs& p, const Src& src, cons
   });
 }
 
-template <class Src> __device__ __forceinline__ long long src_nlive(const Src&) { return 0; }
-__device__ __forceinline__ long long src_nlive(const SrcSmem& s) { return s.n_live; }
+// ------------------------------------------------------------------------------------------------ the root find
+struct RootState {
+  double alpha, beta;    // in: warm start; out: thresholds  nu + theta,  nu - theta
+  int amode;             // 0: turnover cap inactive (alpha == beta), 1: active
+  int n_eval;            // trial evaluations (passes over the source) spent
+  int nobands;           // in: 1 = solve with every band multiplier fixed at 0 (band ramp of the first iterations)
+};
 
+// Solves for (alpha, beta, lambda_g) of account a over the assets of `src` (see the header of this file).
+// b: budget in trade space, tau: turnover cap (inf = none), Delta = 2 kappa + c_buy.  sh.lamS holds the warm-start
+// band multipliers on entry and the solution on exit.  Block-wide: every thread calls it with identical arguments.
 template <bool LOTS, class Src>
-__device__ __forceinline__ void prox_body(const ProxArgs& p, int mode, Src& src, int a, double gam, double c,
-                                          double kappa, double lam_b) {
-  __shared__ double scratch[12 * 32];
-  __shared__ double gbin[16 * PRISM_MAX_GROUPS];    // per-warp group bins (deterministic accumulation)
-  __shared__ double lamS[PRISM_MAX_GROUPS];
-  __shared__ double gsum[PRISM_MAX_GROUPS];
-  __shared__ int selS[2];
-  const int tid = threadIdx.x, nt = blockDim.x;
-  const int64_t N = p.N, row = (int64_t)a * N, rowp = (int64_t)a * p.ldw;
-  double cg = c * gam;
-  const double Delta = lam_b + kappa;
-  const double tau = p.tau ? p.tau[a] : INFINITY;
-  const double b = p.ap.bsum[a];
-  const int G = p.G;
-  for (int g = tid; g < G; g += nt) lamS[g] = p.lamG[(int64_t)a * G + g];
-  __syncthreads();
-
-  long long t0 = clock64(), t_ev = 0, t_gs = 0, t1, t2, t3;
-  double alpha = p.ap.alpha[a], beta = p.ap.beta[a];
-  int amode = p.ap.mode[a];
-  if (!(amode == 1 && isfinite(tau))) { amode = 0; beta = alpha; }
-  const double alpha_w = alpha, beta_w = beta;       // warm start (previous iteration's thresholds)
-  const int amode_w = amode;
-  const double* lam_w = p.lamG + (int64_t)a * G;
-  src.classify(alpha_w, beta_w, lam_w, Src::kWindowed ? p.ap.win[a] : INFINITY, (int*)scratch);
+__device__ __noinline__ void prox_rootfind(const ProxArgs& p, const Src& src, int a, double b, double tau, double Delta,
+                                              const ProxShared& sh, RootState& rs) {
+  const int tid = threadIdx.x;
+  const int G = rs.nobands ? 0 : p.G;
+  double* scratch = sh.scratch;
+  double* lamS = sh.lamS;
+  double alpha = rs.alpha, beta = rs.beta;
+  int amode = rs.amode;
   double a_min = -INFINITY, a_max = INFINITY, b_min = -INFINITY, b_max = INFINITY;   // brackets, computed lazily
   bool have_br = false;
   double P = 0, R = 0, sP = 0, sR = 0, Pa = 0, Ra = 0, pa = 0, ra = 0;
-  int n_eval = 0, n_win_fail = 0;
+  int n_eval = 0;
 
   // range of the breakpoints in threshold space (only when a root find needs bisection)
   auto brackets = [&]() {
@@ -509,9 +588,7 @@ __device__ __forceinline__ void prox_body(const ProxArgs& p, int mode, Src& src,
   auto eval2 = [&](double al, double be, int s1, int s2) {
     ++n_eval;
     double out[12];
-    long long te = clock64();
     prox_eval<LOTS>(src, lamS, G, al, be - Delta, s1, s2, scratch, out);
-    t_ev += clock64() - te;
     P = out[0]; R = out[1]; sP = out[2]; sR = out[3];
     if (s1 >= 0 || s2 >= 0) { Pa = out[4]; Ra = out[5]; pa = out[6]; ra = out[7]; Pb = out[8]; Rb = out[9]; pb2 = out[10]; rb2 = out[11]; }
   };
@@ -520,6 +597,24 @@ __device__ __forceinline__ void prox_body(const ProxArgs& p, int mode, Src& src,
   const double Pt = 0.5 * (tau + b), Rt = 0.5 * (tau - b);
 
   // (alpha, beta) for the current group multipliers; leaves the sums of the final thresholds (and of group sel)
+  // section pass for the roots that asked for one (amode 1: ra on P(alpha), rb on R(beta); amode 0: rn on P - R)
+  auto section = [&](Root1D* ra_, Root1D* rb_, Root1D* rn) {
+    double fP[PROX_KSEC], fR[PROX_KSEC];
+    ++n_eval;
+    if (rn) {
+      const double dx = (rn->hi - rn->lo) / (PROX_KSEC + 1), x0 = rn->lo + dx;
+      prox_eval_multi<LOTS>(src, lamS, G, x0, dx, x0 - Delta, dx, scratch, fP, fR);
+      for (int k = 0; k < PROX_KSEC; ++k) fP[k] -= fR[k];
+      root_place(*rn, fP, x0, dx, b, -1);
+      return;
+    }
+    const double dxa = ra_->sect ? (ra_->hi - ra_->lo) / (PROX_KSEC + 1) : 0.0, xa = ra_->sect ? ra_->lo + dxa : ra_->x;
+    const double dxb = rb_->sect ? (rb_->hi - rb_->lo) / (PROX_KSEC + 1) : 0.0, xb = rb_->sect ? rb_->lo + dxb : rb_->x;
+    prox_eval_multi<LOTS>(src, lamS, G, xa, dxa, xb - Delta, dxb, scratch, fP, fR);
+    if (ra_->sect) root_place(*ra_, fP, xa, dxa, Pt, -1);
+    if (rb_->sect) root_place(*rb_, fR, xb, dxb, Rt, +1);
+  };
+  // (alpha, beta) for the current group multipliers; leaves the sums of the final thresholds (and of group sel)
   auto solve_ab = [&](int sel) {
     double lmin = 0.0, lmax = 0.0;
     for (int g = 0; g < G; ++g) { lmin = fmin(lmin, lamS[g]); lmax = fmax(lmax, lamS[g]); }
@@ -527,12 +622,13 @@ __device__ __forceinline__ void prox_body(const ProxArgs& p, int mode, Src& src,
       const double alo = a_min - lmax, ahi = a_max - lmin, blo = b_min - lmax, bhi = b_max - lmin;
       bool need = false;
       if (amode == 1) {
-        Root1D ra_ = {fmin(fmax(alpha, alo), ahi), alo, ahi, 0};
-        Root1D rb_ = {fmin(fmax(beta, blo), bhi), blo, bhi, 0};
+        Root1D ra_ = {fmin(fmax(alpha, alo), ahi), alo, ahi, 0, 0};
+        Root1D rb_ = {fmin(fmax(beta, blo), bhi), blo, bhi, 0, 0};
         eval(ra_.x, rb_.x, sel);
         for (int it = 0; it < 80; ++it) {
           need = root_step(ra_, P, sP, Pt, -1, tol) | root_step(rb_, R, sR, Rt, +1, tol);
           if (need || (ra_.done && rb_.done)) break;
+          if (ra_.sect || rb_.sect) section(&ra_, &rb_, nullptr);
           eval(ra_.x, rb_.x, sel);
         }
         alpha = ra_.x; beta = rb_.x;
@@ -541,11 +637,12 @@ __device__ __forceinline__ void prox_body(const ProxArgs& p, int mode, Src& src,
         amode = 0; alpha = beta = 0.5 * (alpha + beta);
       } else {
         const double lo_b = fmin(alo, blo), hi_b = fmax(ahi, bhi);
-        Root1D rn = {fmin(fmax(alpha, lo_b), hi_b), lo_b, hi_b, 0};
+        Root1D rn = {fmin(fmax(alpha, lo_b), hi_b), lo_b, hi_b, 0, 0};
         eval(rn.x, rn.x, sel);
         for (int it = 0; it < 80; ++it) {
           need = root_step(rn, P - R, sP + sR, b, -1, tol);
           if (need || rn.done) break;
+          if (rn.sect) section(nullptr, nullptr, &rn);
           eval(rn.x, rn.x, sel);
         }
         alpha = beta = rn.x;
@@ -556,7 +653,6 @@ __device__ __forceinline__ void prox_body(const ProxArgs& p, int mode, Src& src,
     }
   };
 
-  for (int wpass = 0; wpass < 2; ++wpass) {
   // Fast path when one or two bands were active at the previous iteration: semismooth Newton on (alpha, beta,
   // lambda_g1[, lambda_g2]) jointly, one pass per step (the system is piecewise linear; from the warm start it lands
   // on the final piece in a few steps).  Anything unexpected falls through to the robust nested solve below.
@@ -564,11 +660,12 @@ __device__ __forceinline__ void prox_body(const ProxArgs& p, int mode, Src& src,
     int g1 = -1, g2 = -1, nact = 0;
     for (int g = 0; g < G; ++g) if (lamS[g] != 0.0) { if (nact == 0) g1 = g; else if (nact == 1) g2 = g; ++nact; }
     if (nact >= 1 && nact <= 2) {
-      const double bnd1 = lamS[g1] > 0.0 ? p.band_hi[(int64_t)a * G + g1] : p.band_lo[(int64_t)a * G + g1];
-      const double bnd2 = g2 >= 0 ? (lamS[g2] > 0.0 ? p.band_hi[(int64_t)a * G + g2] : p.band_lo[(int64_t)a * G + g2]) : 0.0;
-      const double gw1 = p.gw0[(int64_t)a * G + g1], gw2 = g2 >= 0 ? p.gw0[(int64_t)a * G + g2] : 0.0;
+      const double bnd1 = lamS[g1] > 0.0 ? sh.band_hi[g1] : sh.band_lo[g1];
+      const double bnd2 = g2 >= 0 ? (lamS[g2] > 0.0 ? sh.band_hi[g2] : sh.band_lo[g2]) : 0.0;
+      const double gw1 = sh.gw0[g1], gw2 = g2 >= 0 ? sh.gw0[g2] : 0.0;
       const double sg1 = lamS[g1] > 0.0 ? 1.0 : -1.0, sg2 = g2 >= 0 ? (lamS[g2] > 0.0 ? 1.0 : -1.0) : 1.0;
-      double al = alpha, be = beta, l1 = lamS[g1], l2 = g2 >= 0 ? lamS[g2] : 0.0;
+      const double l1_0 = lamS[g1], l2_0 = g2 >= 0 ? lamS[g2] : 0.0;
+      double al = alpha, be = beta, l1 = l1_0, l2 = l2_0;
       bool ok = false;
       for (int it = 0; it < 10; ++it) {
         eval2(al, be, g1, g2);
@@ -612,7 +709,7 @@ __device__ __forceinline__ void prox_body(const ProxArgs& p, int mode, Src& src,
       if (good) good = amode == 1 ? (al >= be) : (!isfinite(tau) || P + R <= tau + tol);
       __syncthreads();
       if (good) { alpha = al; beta = be; }
-      else if (tid == 0) { lamS[g1] = p.lamG[(int64_t)a * G + g1]; if (g2 >= 0) lamS[g2] = p.lamG[(int64_t)a * G + g2]; }
+      else if (tid == 0) { lamS[g1] = l1_0; if (g2 >= 0) lamS[g2] = l2_0; }
       __syncthreads();
     }
   }
@@ -621,30 +718,28 @@ __device__ __forceinline__ void prox_body(const ProxArgs& p, int mode, Src& src,
     solve_ab(-1);
     if (G == 0) break;
     // all group sums at the current solution (deterministic binned pass)
-    { long long tg = clock64();
-    prox_group_sums<LOTS>(src, lamS, G, alpha, beta - Delta, p.gw0 + (int64_t)a * G, gbin, gsum);
-    t_gs += clock64() - tg; }
+    prox_group_sums<LOTS>(src, lamS, G, alpha, beta - Delta, sh.gw0, sh.gbin, sh.gsum);
     if (tid == 0) {
       int sel = -1, sgn = 0; double worst = 8.0 * tol;
       for (int g = 0; g < G; ++g) {
-        const double bl_ = p.band_lo[(int64_t)a * G + g], bh_ = p.band_hi[(int64_t)a * G + g];
+        const double bl_ = sh.band_lo[g], bh_ = sh.band_hi[g];
         double viol; int sg;
-        if (lamS[g] > 0.0) { viol = fabs(gsum[g] - bh_); sg = +1; }
-        else if (lamS[g] < 0.0) { viol = fabs(gsum[g] - bl_); sg = -1; }
-        else if (gsum[g] > bh_) { viol = gsum[g] - bh_; sg = +1; }
-        else { viol = bl_ - gsum[g]; sg = -1; }
+        if (lamS[g] > 0.0) { viol = fabs(sh.gsum[g] - bh_); sg = +1; }
+        else if (lamS[g] < 0.0) { viol = fabs(sh.gsum[g] - bl_); sg = -1; }
+        else if (sh.gsum[g] > bh_) { viol = sh.gsum[g] - bh_; sg = +1; }
+        else { viol = bl_ - sh.gsum[g]; sg = -1; }
         if (viol > worst) { worst = viol; sel = g; sgn = sg; }
       }
-      selS[0] = sel; selS[1] = sgn;
+      sh.selS[0] = sel; sh.selS[1] = sgn;
     }
     __syncthreads();
-    const int sel = selS[0], sgn = selS[1];
+    const int sel = sh.selS[0], sgn = sh.selS[1];
     if (sel < 0) break;
     // scalar problem in m = sgn * lambda_sel >= 0:  h(m) = sgn * (S_sel - bound) is non-increasing, want h = 0 or m = 0
     if (!have_br) brackets();
     const double Lmax = 2.0 * (fmax(a_max, b_max) - fmin(a_min, b_min)) + 1.0;
-    const double bound = sgn > 0 ? p.band_hi[(int64_t)a * G + sel] : p.band_lo[(int64_t)a * G + sel];
-    const double gw = p.gw0[(int64_t)a * G + sel];
+    const double bound = sgn > 0 ? sh.band_hi[sel] : sh.band_lo[sel];
+    const double gw = sh.gw0[sel];
     double m = sgn * lamS[sel], mlo = 0.0, mhi = Lmax;
     bool lo_known = false;      // h(mlo) > 0 established
     for (int it = 0; it < 60; ++it) {
@@ -668,26 +763,58 @@ __device__ __forceinline__ void prox_body(const ProxArgs& p, int mode, Src& src,
     }
   }
   __syncthreads();
-    if (src.window_ok(alpha, beta, lamS)) break;
+  rs.alpha = alpha; rs.beta = beta; rs.amode = amode; rs.n_eval += n_eval;
+}
+
+__device__ __forceinline__ double next_window(const ProxArgs& p, double alpha, double beta, double mv) {
+  return fmax(p.win_mult * mv, 1e-9 + 1e-7 * (fabs(alpha) + fabs(beta)));
+}
+
+// ------------------------------------------------------------------------------------------------ slow path
+// Whole z-update of one account from a source that can enumerate every asset: root find (windowed for SrcSmem),
+// residual check, convergence mask, rho adaptation, output / returned weights.
+template <bool LOTS, class Src>
+__device__ __forceinline__ void prox_body(const ProxArgs& p, int mode, Src& src, int a, double gam, double c,
+                                          double kappa, double lam_b, const ProxShared& sh0, bool windowed) {
+  const int tid = threadIdx.x, nt = blockDim.x;
+  ProxShared sh = sh0;
+  sh.band_lo = p.band_lo + (int64_t)a * p.G; sh.band_hi = p.band_hi + (int64_t)a * p.G; sh.gw0 = p.gw0 + (int64_t)a * p.G;
+  double* lamS = sh.lamS;
+  double cg = c * gam;
+  const double Delta = lam_b + kappa;
+  const double tau = p.tau ? p.tau[a] : INFINITY;
+  const double b = p.ap.bsum[a];
+  const int G = p.G;
+  for (int g = tid; g < G; g += nt) lamS[g] = p.lamG[(int64_t)a * G + g];
+  __syncthreads();
+
+  RootState rs;
+  rs.alpha = p.ap.alpha[a]; rs.beta = p.ap.beta[a]; rs.amode = p.ap.mode[a]; rs.n_eval = 0; rs.nobands = 0;
+  if (!(rs.amode == 1 && isfinite(tau))) { rs.amode = 0; rs.beta = rs.alpha; }
+  const double alpha_w = rs.alpha, beta_w = rs.beta;       // warm start (previous iteration's thresholds)
+  const int amode_w = rs.amode;
+  const double* lam_w = p.lamG + (int64_t)a * G;
+  src.classify(alpha_w, beta_w, lam_w, windowed ? p.ap.win[a] : INFINITY, (int*)sh.scratch);
+  for (int wpass = 0; wpass < 2; ++wpass) {
+    prox_rootfind<LOTS>(p, src, a, b, tau, Delta, sh, rs);
+    if (src.window_ok(rs.alpha, rs.beta, lamS)) break;
     // the solution left the window the live list was built for: rebuild it with every asset and solve again
-    alpha = alpha_w; beta = beta_w; amode = amode_w;
+    rs.alpha = alpha_w; rs.beta = beta_w; rs.amode = amode_w;
     __syncthreads();
     for (int g = tid; g < G; g += nt) lamS[g] = lam_w[g];
     __syncthreads();
-    src.classify(alpha_w, beta_w, lam_w, INFINITY, (int*)scratch);
-    have_br = false; a_min = b_min = -INFINITY; a_max = b_max = INFINITY;
-    ++n_win_fail;
+    src.classify(alpha_w, beta_w, lam_w, INFINITY, (int*)sh.scratch);
   }
   __syncthreads();
+  const double alpha = rs.alpha, beta = rs.beta;
 
-  t1 = clock64();
   // ---------------------------------------------------------------- check: residuals, mask, rho adaptation
   double c_new = c;
   int finished = 0;
   const double bdf = beta - Delta;
   if (mode & PROX_CHECK) {
     double rr[2];
-    prox_check<LOTS>(p, src, lamS, a, alpha, bdf, lam_b, cg, scratch, rr);
+    prox_check<LOTS>(p, src, lamS, a, alpha, bdf, lam_b, cg, sh.scratch, rr);
     const double rp = rr[0], rd = rr[1];
     const bool bad = !(rp < INFINITY) || !(rd < INFINITY);
     const bool conv = !bad && rp <= p.eps && rd <= p.eps;
@@ -712,22 +839,16 @@ __device__ __forceinline__ void prox_body(const ProxArgs& p, int mode, Src& src,
   if (mode & PROX_FINAL) finished = 1;
 
   // ---------------------------------------------------------------- output pass (e.T, e.ir refer to the old rho)
-  t2 = clock64();
   prox_output<LOTS>(p, src, lamS, a, alpha, bdf, lam_b, gam, c, c_new, finished);
-  t3 = clock64();
-  if (p.dbg && tid == 0) { long long* d = p.dbg + (int64_t)a * 12; d[8] += src_nlive(src); d[9] += n_win_fail; d[0] += t1 - t0; d[1] += t_ev; d[2] += t_gs; d[3] += t2 - t1; d[4] += t3 - t2; d[5] += n_eval; d[6] += 1; }
-  (void)n_win_fail;
   double mv_l = 0.0;
   for (int g = 0; g < G; ++g) mv_l = fmax(mv_l, fabs(lamS[g] - lam_w[g]));
   __syncthreads();
   for (int g = tid; g < G; g += nt) p.lamG[(int64_t)a * G + g] = lamS[g];
   if (tid == 0) {
-    p.resid[(int64_t)a * PRISM_NRES + PRISM_R_RESERVED] += (double)n_eval;   // trial evaluations (passes) so far
-    p.ap.alpha[a] = alpha; p.ap.beta[a] = beta; p.ap.mode[a] = amode;
-    if (Src::kWindowed) {                      // next window: a multiple of how far the thresholds moved in this launch
-      const double mv = fmax(fmax(fabs(alpha - alpha_w), fabs(beta - beta_w)), mv_l);
-      p.ap.win[a] = fmax(32.0 * mv, 1e-9 + 1e-7 * (fabs(alpha) + fabs(beta)));
-    }
+    p.resid[(int64_t)a * PRISM_NRES + PRISM_R_RESERVED] += (double)rs.n_eval;   // trial evaluations (passes) so far
+    p.ap.alpha[a] = alpha; p.ap.beta[a] = beta; p.ap.mode[a] = rs.amode;
+    // next window: a multiple of how far the thresholds moved in this launch
+    p.ap.win[a] = next_window(p, alpha, beta, fmax(fmax(fabs(alpha - alpha_w), fabs(beta - beta_w)), mv_l));
     if (finished) {
       p.ap.done[a] = 1;
       p.ap.iters[a] = p.iter;
@@ -739,30 +860,43 @@ __device__ __forceinline__ void prox_body(const ProxArgs& p, int mode, Src& src,
       p.resid[(int64_t)a * PRISM_NRES + PRISM_R_RHO] = c_new;
     }
   }
+  __syncthreads();
 }
 
-// generic kernel: any N, lots, per-asset caps
+#define PROX_STATIC_SHARED(NW)                                           \
+  __shared__ double s_scratch[12 * 32];                                  \
+  __shared__ double s_gbin[(NW) * PRISM_MAX_GROUPS];                     \
+  __shared__ double s_lamS[PRISM_MAX_GROUPS];                            \
+  __shared__ double s_gsum[PRISM_MAX_GROUPS];                            \
+  __shared__ int s_selS[2];                                              \
+  ProxShared sh = {s_scratch, s_gbin, s_lamS, s_gsum, s_selS, nullptr, nullptr, nullptr};
+
+// generic kernel: any N, lots, per-asset caps.  Persistent: grid <= number of accounts.
 template <bool LOTS>
-__global__ void __launch_bounds__(512) k_prox(ProxArgs p, int mode) {
-  const int a = blockIdx.x;
-  if (p.ap.done[a]) return;
-  const double gam = p.gamma[a], c = p.ap.c[a];
-  const double kappa = p.kappa ? p.kappa[a] : 0.0;
-  const double lam_b = kappa + (p.c_buy ? p.c_buy[a] : 0.0);
-  SrcGlobal<LOTS> src(p, a, c * gam, p.lo[a], p.hi[a], lam_b);
-  prox_body<LOTS>(p, mode, src, a, gam, c, kappa, lam_b);
+__global__ void __launch_bounds__(512) k_prox(const __grid_constant__ ProxArgs p, int mode) {
+  PROX_STATIC_SHARED(16)
+  for (int a = blockIdx.x; a < p.A; a += gridDim.x) {
+    if (p.ap.done[a]) continue;
+    const double gam = p.gamma[a], c = p.ap.c[a];
+    const double kappa = p.kappa ? p.kappa[a] : 0.0;
+    const double lam_b = kappa + (p.c_buy ? p.c_buy[a] : 0.0);
+    SrcGlobal<LOTS> src(p, a, c * gam, p.lo[a], p.hi[a], lam_b);
+    prox_body<LOTS>(p, mode, src, a, gam, c, kappa, lam_b, sh, false);
+  }
 }
 
-// shared-memory-resident kernel: 18 N bytes of dynamic shared memory, no lots, no per-asset caps
-__global__ void __launch_bounds__(512, 1) k_prox_smem(ProxArgs p, int mode) {
+// shared-memory-resident kernel: 20 N bytes of dynamic shared memory, no lots, no per-asset caps
+__global__ void __launch_bounds__(512, 1) k_prox_smem(const __grid_constant__ ProxArgs p, int mode) {
   extern __shared__ __align__(16) double prox_smem[];
-  const int a = blockIdx.x;
-  if (p.ap.done[a]) return;
-  const double gam = p.gamma[a], c = p.ap.c[a];
-  const double kappa = p.kappa ? p.kappa[a] : 0.0;
-  const double lam_b = kappa + (p.c_buy ? p.c_buy[a] : 0.0);
-  long long tc = clock64();
-  SrcSmem src(p, a, c * gam, p.lo[a], p.hi[a], lam_b, lam_b + kappa, prox_smem);
-  if (p.dbg && threadIdx.x == 0) p.dbg[(int64_t)a * 12 + 7] += clock64() - tc;
-  prox_body<false>(p, mode, src, a, gam, c, kappa, lam_b);
+  PROX_STATIC_SHARED(16)
+  for (int a = blockIdx.x; a < p.A; a += gridDim.x) {
+    if (p.ap.done[a]) continue;
+    const double gam = p.gamma[a], c = p.ap.c[a];
+    const double kappa = p.kappa ? p.kappa[a] : 0.0;
+    const double lam_b = kappa + (p.c_buy ? p.c_buy[a] : 0.0);
+    __syncthreads();
+    SrcSmem src(p, a, c * gam, p.lo[a], p.hi[a], lam_b, lam_b + kappa, prox_smem);
+    prox_body<false>(p, mode, src, a, gam, c, kappa, lam_b, sh, true);
+  }
 }
+

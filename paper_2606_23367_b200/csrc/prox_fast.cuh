@@ -1,0 +1,630 @@
+// prox_fast.cuh - the streaming form of the fused proximal / projection step for the
+// configurations without tax lots and per-asset caps: two kernels per iteration.
+//
+//   k_prox_stream  (HBM-bound, grid = slices x accounts)  ONE pass over the account's assets.  Every asset whose buy
+//       and sell amounts cannot change while the thresholds (alpha, beta, lambda_g) stay inside the window
+//       [warm start +- W] ("dead": on the kink, clamped at a bound, excluded) is finished on the spot: its output
+//       (r~ = M^-1 r, c = r~ - z) is written, its residual terms are accumulated, its constant trade is added to
+//       per-group fixed-point bins (integer atomics: the sum does not depend on the order => deterministic).
+//       The other assets ("live", a few percent at most once the iteration has settled) are appended to per-warp
+//       lists in global memory, each list in ascending asset order.  The streamed arrays reach shared memory
+//       through a bulk-copy (TMA engine) pipeline with full / empty mbarriers.
+//   k_prox_root    (latency-bound, one CTA per account)  compacts the lists in a fixed order, solves the
+//       piecewise-linear equations for (alpha, beta, lambda_g) on the live assets only (prox_rootfind), writes the
+//       live assets' outputs, finishes the residual check (convergence mask, H6), and commits the account's state.
+//       If the solution left the window, rho has to change, or a NaN shows up, the same CTA redoes the account with
+//       the generic every-asset source (prox_body over SrcGlobal): no account state has been touched before that.
+#pragma once
+#include "prox.cuh"
+
+#define PRISM_FIX_SCALE 1152921504606846976.0            // 2^60
+#define PRISM_FIX_INV (1.0 / 1152921504606846976.0)
+#define PROX_META_IDX_BITS 22                            // meta = idx | gid << 22 | cls << 30
+
+struct __align__(16) LiveEnt { double T, w0, ir; uint32_t meta, pad; };   // one live asset (32 bytes)
+
+#define FAST_NW 8            // warps per streaming CTA
+#define FAST_CH 512          // assets per pipeline stage (two per thread)
+#define FAST_NST 3           // stages of the bulk-copy pipeline
+#define FAST_STAGE_BYTES (5 * FAST_CH * 8 + 2 * FAST_CH)
+#define ROOT_NT 128          // threads of a root CTA
+
+__host__ __device__ inline size_t stream_smem_bytes(int G) {
+  return (size_t)FAST_NST * FAST_STAGE_BYTES + 2 * FAST_NST * 8 + (size_t)(G > 0 ? G : 1) * 8 + 8 * 32 * 8 + 16;
+}
+
+// mbarrier + bulk-copy (TMA engine, 1-D) primitives: global -> shared staging of the streamed arrays
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  uint32_t ok = 0;
+  const uint32_t addr = smem_u32(bar);
+  while (!ok) {
+    asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+                 : "=r"(ok) : "r"(addr), "r"(parity) : "memory");
+  }
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
+// ------------------------------------------------------------------------------------------------ streaming kernel
+// grid = (slices, accounts), block = 256.  Needs N % 16 == 0 (every row of every streamed array 16-byte aligned).
+template <bool CHECK>
+__global__ void __launch_bounds__(FAST_NW * 32, 3) k_prox_stream(const __grid_constant__ ProxArgs p) {
+  extern __shared__ __align__(16) unsigned char stream_raw[];
+  const int a = blockIdx.y, sl = blockIdx.x;
+  if (p.ap.done[a]) return;
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  const int G = p.G, Gb = G > 0 ? G : 1;
+  const int64_t N = p.N, row = (int64_t)a * N, rowp = (int64_t)a * p.ldw;
+  const int sub = (a * p.S + sl) * FAST_NW + wid;               // this warp's list
+  const double W = p.ap.wins[a];
+  const double lo_a = p.lo[a], hi_a = p.hi[a];
+  if (!(hi_a - lo_a <= 4.0)) {            // box wider than the fixed-point range of the bins: generic path in k_prox_root
+    if (tid == 0 && sl == 0) p.lflag[a] = 1;
+    if (lane == 0) p.lcnt[sub] = 0;
+    return;
+  }
+  unsigned char* stage0 = stream_raw;                                 // FAST_NST stages: v, w0, q, d, 1/d, excl, gid
+  uint64_t* bar_full = (uint64_t*)(stream_raw + (size_t)FAST_NST * FAST_STAGE_BYTES);
+  uint64_t* bar_empty = bar_full + FAST_NST;
+  double* lamS = (double*)(bar_empty + FAST_NST);
+  double* scratch = lamS + Gb;                                        // 8 * 32 (CHECK reduction)
+
+  const double gam = p.gamma[a], c = p.ap.c[a], cg = c * gam, icg = 1.0 / cg;
+  const double kappa = p.kappa ? p.kappa[a] : 0.0;
+  const double lam_b = kappa + (p.c_buy ? p.c_buy[a] : 0.0), Delta = lam_b + kappa;
+  const double tau = p.tau ? p.tau[a] : INFINITY;
+  const double igc = 1.0 / (gam * (1.0 + c));
+  double aw = p.ap.alpha[a], bw = p.ap.beta[a];
+  if (!(p.ap.mode[a] == 1 && isfinite(tau))) bw = aw;
+  for (int g = tid; g < G; g += blockDim.x) lamS[g] = p.lamG[(int64_t)a * G + g];
+  if (tid == 0) {
+    for (int st = 0; st < FAST_NST; ++st) { mbar_init(&bar_full[st], 1); mbar_init(&bar_empty[st], FAST_NW); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+
+  const int64_t i_beg = (int64_t)sl * p.slice_len, i_end = min(N, i_beg + p.slice_len);
+  const int nchunk = (int)((i_end - i_beg + FAST_CH - 1) / FAST_CH);
+  const uint32_t elem_bytes = 40u + (p.excl ? 1u : 0u) + (G ? 1u : 0u);
+  const double* qsrc = p.q ? p.q + rowp : p.mu + row;
+  // thread 0: start the copies of chunk c into its stage
+  auto issue = [&](int c) {
+    const int st = c % FAST_NST;
+    const int64_t i0 = i_beg + (int64_t)c * FAST_CH;
+    const uint32_t nc = (uint32_t)min((int64_t)FAST_CH, i_end - i0);
+    unsigned char* sb = stage0 + (size_t)st * FAST_STAGE_BYTES;
+    mbar_expect_tx(&bar_full[st], nc * elem_bytes);
+    bulk_g2s(sb, p.v + rowp + i0, nc * 8, &bar_full[st]);
+    bulk_g2s(sb + FAST_CH * 8, p.w0 + row + i0, nc * 8, &bar_full[st]);
+    bulk_g2s(sb + 2 * FAST_CH * 8, qsrc + i0, nc * 8, &bar_full[st]);
+    bulk_g2s(sb + 3 * FAST_CH * 8, p.d + i0, nc * 8, &bar_full[st]);
+    bulk_g2s(sb + 4 * FAST_CH * 8, p.invd + i0, nc * 8, &bar_full[st]);
+    if (p.excl) bulk_g2s(sb + 5 * FAST_CH * 8, p.excl + row + i0, nc, &bar_full[st]);
+    if (G) bulk_g2s(sb + 5 * FAST_CH * 8 + FAST_CH, p.group_id + i0, nc, &bar_full[st]);
+  };
+
+  double nx = 0, nz = 0, nrp = 0, nrd = 0, nPx = 0, ny = 0, nq = 0;
+  LiveEnt* mylist = p.lraw + (int64_t)sub * p.capw;
+  unsigned long long* cbin = p.cbin + (int64_t)a * 2 * Gb;
+  const unsigned lt = (1u << lane) - 1u;
+  int n = 0;
+  const double aW_lo = aw - W, aW_hi = aw + W, bW_lo = bw - W - Delta, bW_hi = bw + W - Delta;
+  if (tid == 0)
+    for (int c = 0; c < FAST_NST - 1 && c < nchunk; ++c) issue(c);
+  double* rtp = p.rt + rowp + i_beg + tid;
+  double* ccp = p.cc + rowp + i_beg + tid;
+  for (int c = 0; c < nchunk; ++c) {
+    const int st = c % FAST_NST;
+    if (tid == 0 && c + FAST_NST - 1 < nchunk) {          // refill the stage chunk c - 1 lived in
+      const int cn = c + FAST_NST - 1;
+      if (cn >= FAST_NST) mbar_wait(&bar_empty[cn % FAST_NST], (uint32_t)((cn / FAST_NST - 1) & 1));
+      issue(cn);
+    }
+    mbar_wait(&bar_full[st], (uint32_t)((c / FAST_NST) & 1));
+    const unsigned char* sb = stage0 + (size_t)st * FAST_STAGE_BYTES;
+    const double* sv = (const double*)sb + tid;
+    const unsigned char* sx = sb + 5 * FAST_CH * 8 + tid;
+    const int64_t i0 = i_beg + (int64_t)c * FAST_CH;
+    const int nc = (int)min((int64_t)FAST_CH, i_end - i0);
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      const int t = tid + h * (FAST_NW * 32);
+      const bool valid = t < nc;                                  // (stale stage data beyond nc is read but not used)
+      const double v = sv[h * 256];
+      const double w0 = sv[FAST_CH + h * 256];
+      const double qraw = sv[2 * FAST_CH + h * 256];
+      const double rho = cg * sv[3 * FAST_CH + h * 256];
+      const double iv = sv[4 * FAST_CH + h * 256];
+      const bool ex = p.excl ? sx[h * 256] != 0 : false;
+      int g = 0;
+      double lg = 0.0;
+      if (G) { g = sx[FAST_CH + h * 256]; lg = lamS[g]; }
+      const double qm = p.q ? -qraw : qraw;                          // -q_i
+      const double u = v - w0;
+      const double T = fma(u, rho, -lam_b);
+      const double tA = T - lg;
+      // Branch-free classification (a warp almost always holds a few excluded / sold-out assets, so a rare-case
+      // branch would be taken by nearly every warp).  Inside its box an asset's buy amount is 0 if the buy
+      // threshold of the window cannot reach it, the whole room wB if even the far end of the window fills it,
+      // and depends on the thresholds (live) in between; the same for the sell side.
+      const bool inbox = w0 >= lo_a && w0 <= hi_a;
+      const double wB = hi_a - w0, wS = w0 - lo_a;
+      const bool b_reach = tA > aW_lo, b_full = tA - aW_hi >= wB * rho;
+      const bool s_reach = tA < bW_hi, s_full = bW_lo - tA >= wS * rho;
+      double bc = (b_reach && b_full) ? wB : 0.0;
+      double sc = (s_reach && s_full) ? wS : 0.0;
+      bool live = (b_reach && !b_full) || (s_reach && !s_full) || !inbox;   // outside its box (rare): live
+      if (ex) { bc = 0.0; sc = w0; live = !(w0 >= 0.0 && w0 <= 4.0); }       // lo = hi = 0: the trade is -w0
+      live = live && valid;
+      const double tc = bc - sc;                                             // trade of a dead asset
+      const double z = w0 + tc;
+      const double rt = fma(rho, (w0 - u) + 2.0 * tc, qm) * (iv * igc);      // (rho (2 z - v) - q) / M_i
+      if (valid && !live) {
+        rtp[h * 256] = rt;
+        ccp[h * 256] = rt - z;
+        if (bc > 0.0) atomicAdd(&cbin[g], (unsigned long long)__double2ull_rn(bc * PRISM_FIX_SCALE));
+        if (sc > 0.0) atomicAdd(&cbin[Gb + g], (unsigned long long)__double2ull_rn(sc * PRISM_FIX_SCALE));
+        if (CHECK) {
+          const int64_t i = i0 + t;
+          p.w_out[row + i] = z;            // speculative: kept if the account turns out to have converged
+          const double x = p.xs[rowp + i], pq = p.pxq[rowp + i];
+          const double y = rho * (v - z);
+          nx = fmax(nx, fabs(x)); nz = fmax(nz, fabs(z)); nrp = fmax(nrp, fabs(x - z));
+          nrd = fmax(nrd, fabs(pq + y)); nPx = fmax(nPx, fabs(pq + qm)); ny = fmax(ny, fabs(y)); nq = fmax(nq, fabs(qm));
+          if (!(x == x) || !(pq == pq) || !(z == z)) nrp = INFINITY;
+        }
+      }
+      const unsigned m = __ballot_sync(0xffffffffu, live);
+      if (m) {
+        if (live) {
+          LiveEnt e;
+          e.T = T; e.w0 = w0; e.ir = iv * icg; e.pad = 0;
+          e.meta = (uint32_t)(i0 + t) | ((uint32_t)g << PROX_META_IDX_BITS) | ((uint32_t)(ex ? 1 : (inbox ? 0 : 2)) << 30);
+          mylist[n + __popc(m & lt)] = e;
+        }
+        n += __popc(m);
+      }
+    }
+    rtp += FAST_CH; ccp += FAST_CH;
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&bar_empty[st]);
+  }
+  if (lane == 0) p.lcnt[sub] = n;
+  if (CHECK) {
+    double val[7] = {nx, nz, nrp, nrd, nPx, ny, nq};
+    block_reduce<7, 1>(val, scratch);
+    if (tid < 7) p.chkp[((int64_t)a * p.S + sl) * 8 + tid] = val[tid];
+  }
+}
+
+// ------------------------------------------------------------------------------------------------ root kernel
+// Live-list source: the compacted list of one account in global memory (L2 resident), plus the fixed-point
+// totals of the dead assets (cbin: buys [0, Gb), sells [Gb, 2 Gb) per group, in units of 2^-60).
+#define ROOT_NSL 4            // sub-lists of a filtered list: one per warp of the root CTA
+struct SrcLiveG {
+  double lo_a, hi_a;
+  const LiveEnt* ent;               // nsl sub-lists, sub-list k at ent + k * stride with cnt[k] entries, visited in order
+  int nsl, stride, cnt[ROOT_NSL];
+  const unsigned long long* cbin;   // shared memory: fixed-point totals of the assets that are not in the list
+  int Gb;
+  double cPt, cRt;
+  __device__ __forceinline__ double cP() const { return cPt; }
+  __device__ __forceinline__ double cR() const { return cRt; }
+  __device__ __forceinline__ double cPg(int g) const { return (double)cbin[g] * PRISM_FIX_INV; }
+  __device__ __forceinline__ double cRg(int g) const { return (double)cbin[Gb + g] * PRISM_FIX_INV; }
+  __device__ __forceinline__ int64_t decode(const double2& a, const double2& b, ElemConst& e, int& g) const {
+    e.T = a.x; e.w0 = a.y; e.ir = b.x;
+    const uint32_t m = (uint32_t)__double_as_longlong(b.y);
+    const int c = (int)(m >> 30);
+    g = (int)((m >> PROX_META_IDX_BITS) & 0xffu);
+    if (c == 0) { e.bl = 0.0; e.sl = 0.0; e.wB = hi_a - e.w0; e.wS = e.w0 - lo_a; }
+    else elem_ranges(e, c == 1 ? 0.0 : lo_a, c == 1 ? 0.0 : hi_a);
+    return (int64_t)(m & ((1u << PROX_META_IDX_BITS) - 1u));
+  }
+  // long lists (first iterations: every asset is live) are latency-bound: four entries' loads are issued together
+  template <class F>
+  __device__ __forceinline__ void for_each(F f) const {
+    const int nt = blockDim.x;
+    for (int k = 0; k < nsl; ++k) {
+      const LiveEnt* el = ent + (int64_t)k * stride;
+      const int n = cnt[k];
+      int j = threadIdx.x;
+      for (; j + 3 * nt < n; j += 4 * nt) {
+        double2 a[4], b[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) { a[u] = __ldg((const double2*)(el + j + u * nt)); b[u] = __ldg((const double2*)(el + j + u * nt) + 1); }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          ElemConst e; int g;
+          const int64_t i = decode(a[u], b[u], e, g);
+          f(i, e, g, 0, (const double*)nullptr, (const double*)nullptr);
+        }
+      }
+      for (; j < n; j += nt) {
+        const double2 a = __ldg((const double2*)(el + j)), b = __ldg((const double2*)(el + j) + 1);
+        ElemConst e; int g;
+        const int64_t i = decode(a, b, e, g);
+        f(i, e, g, 0, (const double*)nullptr, (const double*)nullptr);
+      }
+    }
+  }
+  template <class F>
+  __device__ __forceinline__ void for_each_uniform(F f) const {
+    for (int k = 0; k < nsl; ++k) {
+      const LiveEnt* el = ent + (int64_t)k * stride;
+      const int n = cnt[k];
+      for (int j0 = 0; j0 < n; j0 += blockDim.x) {
+        const int j = j0 + threadIdx.x;
+        const bool valid = j < n;
+        ElemConst e; int g = 0; int64_t i = 0;
+        if (valid) {
+          const double2 a = __ldg((const double2*)(el + j)), b = __ldg((const double2*)(el + j) + 1);
+          i = decode(a, b, e, g);
+        }
+        f(valid, i, e, g, 0, (const double*)nullptr, (const double*)nullptr);
+      }
+    }
+  }
+};
+
+__host__ __device__ inline size_t root_smem_bytes(int G, int nsub) {
+  const int Gb = G > 0 ? G : 1;
+  return (size_t)(12 * 32 + 4 * Gb + 6 * Gb + 2 * Gb + 8 + 4 * (Gb + 4)) * 8 + (size_t)(nsub * Gb + 3 * Gb + 16) * 4 + 16;
+}
+
+// One pass over the grouped list: per (pseudo-)group q the buys, sells and their slopes at thresholds (al, bd + Delta)
+// shifted by the group's multiplier -> gv[4 q .. 4 q + 3].  Warp w owns the groups w, w + nw, ...; fixed order.
+__device__ __forceinline__ void root_pass(const SrcLiveG& src, const int* poff, int ngrp, const double* lamS, int G,
+                                          double al, double bd, double* gv) {
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  for (int q = wid; q < ngrp; q += nw) {
+    const double lg = G ? lamS[q] : 0.0;
+    const double a0 = al + lg, b0 = bd + lg;
+    double sp = 0, sr = 0, slp = 0, slr = 0;
+    const int j1 = poff[q + 1];
+    int j = poff[q] + lane;
+    for (; j + 96 < j1; j += 128) {
+      double2 ea[4], eb[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) { ea[u] = __ldg((const double2*)(src.ent + j + 32 * u)); eb[u] = __ldg((const double2*)(src.ent + j + 32 * u) + 1); }
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        ElemConst e; int g; double mvb, mvs;
+        src.decode(ea[u], eb[u], e, g);
+        sp += buy_amt(e, a0, mvb); sr += sell_amt<false>(e, b0, nullptr, nullptr, 0, mvs); slp += mvb; slr += mvs;
+      }
+    }
+    for (; j < j1; j += 32) {
+      const double2 ea = __ldg((const double2*)(src.ent + j)), eb = __ldg((const double2*)(src.ent + j) + 1);
+      ElemConst e; int g; double mvb, mvs;
+      src.decode(ea, eb, e, g);
+      sp += buy_amt(e, a0, mvb); sr += sell_amt<false>(e, b0, nullptr, nullptr, 0, mvs); slp += mvb; slr += mvs;
+    }
+    sp = warp_sum(sp); sr = warp_sum(sr); slp = warp_sum(slp); slr = warp_sum(slr);
+    if (lane == 0) { gv[4 * q] = sp; gv[4 * q + 1] = sr; gv[4 * q + 2] = slp; gv[4 * q + 3] = slr; }
+  }
+  __syncthreads();
+}
+
+template <bool CHECK>
+__global__ void __launch_bounds__(ROOT_NT, 3) k_prox_root(const __grid_constant__ ProxArgs p, int mode) {
+  extern __shared__ __align__(16) unsigned char root_raw[];
+  __shared__ SrcLiveG src;                 // CTA-uniform objects live in shared memory, not on the threads' stacks
+  __shared__ ProxShared sh;
+  const int a = blockIdx.x;
+  if (p.ap.done[a]) return;
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, nt = blockDim.x, nw = nt >> 5;
+  const int G = p.G, Gb = G > 0 ? G : 1;
+  const int64_t N = p.N, row = (int64_t)a * N, rowp = (int64_t)a * p.ldw;
+  const int nsub = p.S * FAST_NW;
+  const int ngrp = G > 0 ? G : nw;                       // without groups: nw slices of the list, for load balance
+  double* d0 = (double*)root_raw;
+  double* scratch = d0; d0 += 12 * 32;
+  double* gbin = d0; d0 += 4 * Gb;                       // nw = 4 warps
+  double* lamS = d0; d0 += Gb;
+  double* gsum = d0; d0 += Gb;
+  double* band_lo = d0; double* band_hi = d0 + Gb; double* gw0 = d0 + 2 * Gb; double* lamW = d0 + 3 * Gb; d0 += 4 * Gb;
+  unsigned long long* cbin = (unsigned long long*)d0; d0 += 2 * Gb;    // dead assets of the streaming pass
+  double* chk = d0; d0 += 8;
+  double* gv = d0; d0 += 4 * (Gb + 4);                   // per (pseudo-)group sums of one pass
+  int* cntkg = (int*)d0;                                 // nsub x Gb: entries of group g in list k (then running offsets)
+  int* goff = cntkg + nsub * Gb;                         // Gb + 1 group offsets of the grouped list
+  int* poff = goff + Gb + 1;                             // ngrp + 1 (pseudo-)group offsets used by the passes
+  int* act = poff + Gb + 5;                              // Gb: band state -1 lower active, 0 inactive, +1 upper active
+  int* selS = act + Gb;
+
+  const double gam = p.gamma[a], c = p.ap.c[a], cg = c * gam;
+  const double kappa = p.kappa ? p.kappa[a] : 0.0;
+  const double lam_b = kappa + (p.c_buy ? p.c_buy[a] : 0.0), Delta = lam_b + kappa;
+  const double tau = p.tau ? p.tau[a] : INFINITY;
+  const double igc = 1.0 / (gam * (1.0 + c));
+  const double W = p.ap.wins[a];                         // window of the streaming pass
+  const double b = p.ap.bsum[a];
+  double aw = p.ap.alpha[a], bw = p.ap.beta[a];
+  int amode_w = p.ap.mode[a];
+  if (!(amode_w == 1 && isfinite(tau))) { amode_w = 0; bw = aw; }
+  const int generic = p.lflag[a];
+
+  // ---- gather: band data, warm-start multipliers, fixed-point bins (cleared for the next launch)
+  for (int g = tid; g < G; g += nt) {
+    const int64_t e = (int64_t)a * G + g;
+    band_lo[g] = p.band_lo[e]; band_hi[g] = p.band_hi[e]; gw0[g] = p.gw0[e];
+    lamW[g] = lamS[g] = p.lamG[e];
+  }
+  for (int g = tid; g < 2 * Gb; g += nt) {
+    unsigned long long* src_bin = p.cbin + (int64_t)a * 2 * Gb + g;
+    cbin[g] = *src_bin;
+    *src_bin = 0ull;
+  }
+  for (int e = tid; e < nsub * Gb; e += nt) cntkg[e] = 0;
+  __syncthreads();
+  bool fallback = generic != 0;
+  RootState rs;
+  rs.alpha = aw; rs.beta = bw; rs.amode = amode_w; rs.n_eval = 0;
+  // band ramp: the first iterations project without the group bands (an exact prox of the relaxed problem); their
+  // thresholds still move a lot then and a band solve would be wasted.  Never on check / final launches.
+  const bool bands_on = G > 0 && (CHECK || (mode & PROX_FINAL) || p.iter >= p.band_start);
+  rs.nobands = bands_on ? 0 : 1;
+  double mv = 0.0;
+  if (!fallback) {
+    // ---- group sort (counting sort, stable in (list, position) order => deterministic): lists -> lcomp by group
+    const unsigned lt = (1u << lane) - 1u;
+    const LiveEnt* lr = p.lraw + (int64_t)a * nsub * p.capw;
+    const int32_t* lc = p.lcnt + (int64_t)a * nsub;
+    for (int k = wid; k < nsub; k += nw) {
+      const int cnt = lc[k];
+      if (!G) { if (lane == 0) cntkg[k] = cnt; continue; }
+      const LiveEnt* sl = lr + (int64_t)k * p.capw;
+      for (int j0 = 0; j0 < cnt; j0 += 32) {
+        const int j = j0 + lane;
+        const bool valid = j < cnt;
+        const int g = valid ? (int)((__ldg(&sl[j].meta) >> PROX_META_IDX_BITS) & 0xffu) : 0x100 + lane;
+        const unsigned m = __match_any_sync(0xffffffffu, g);
+        if (valid && lane == __ffs(m) - 1) cntkg[k * Gb + g] += __popc(m);
+      }
+    }
+    __syncthreads();
+    for (int g = tid; g < Gb; g += nt) {                 // offsets of list k inside group g; group totals
+      int run = 0;
+      for (int k = 0; k < nsub; ++k) { const int t = cntkg[k * Gb + g]; cntkg[k * Gb + g] = run; run += t; }
+      goff[g + 1] = run;
+    }
+    __syncthreads();
+    if (tid == 0) {
+      goff[0] = 0;
+      for (int g = 0; g < Gb; ++g) goff[g + 1] += goff[g];
+      const int n = goff[Gb];
+      if (G) for (int g = 0; g <= G; ++g) poff[g] = goff[g];
+      else for (int q = 0; q <= nw; ++q) poff[q] = (int)((int64_t)n * q / nw);
+      unsigned long long sp = 0ull, sr = 0ull;
+      for (int g = 0; g < Gb; ++g) { sp += cbin[g]; sr += cbin[Gb + g]; }
+      src.lo_a = p.lo[a]; src.hi_a = p.hi[a]; src.ent = p.lcomp + (int64_t)a * p.ldc; src.nsl = 1; src.stride = 0; src.cnt[0] = n;
+      src.cbin = cbin; src.Gb = Gb; src.cPt = (double)sp * PRISM_FIX_INV; src.cRt = (double)sr * PRISM_FIX_INV;
+      sh.scratch = scratch; sh.gbin = gbin; sh.lamS = lamS; sh.gsum = gsum; sh.selS = selS;
+      sh.band_lo = band_lo; sh.band_hi = band_hi; sh.gw0 = gw0;
+      p.lflag[a] = 0;
+    }
+    __syncthreads();
+    {
+      LiveEnt* dst = p.lcomp + (int64_t)a * p.ldc;
+      for (int k = wid; k < nsub; k += nw) {
+        const int cnt = lc[k];
+        const LiveEnt* sl = lr + (int64_t)k * p.capw;
+        for (int j0 = 0; j0 < cnt; j0 += 32) {
+          const int j = j0 + lane;
+          const bool valid = j < cnt;
+          double2 ea = make_double2(0, 0), eb = make_double2(0, 0);
+          int g = 0x100 + lane;
+          if (valid) {
+            ea = __ldg((const double2*)(sl + j)); eb = __ldg((const double2*)(sl + j) + 1);
+            g = G ? (int)(((uint32_t)__double_as_longlong(eb.y) >> PROX_META_IDX_BITS) & 0xffu) : 0;
+          }
+          const unsigned m = __match_any_sync(0xffffffffu, g);
+          if (valid) {
+            const int pos = goff[g] + cntkg[k * Gb + g] + __popc(m & lt);
+            double2* o = (double2*)(dst + pos);
+            o[0] = ea; o[1] = eb;
+          }
+          __syncwarp();
+          if (valid && lane == __ffs(m) - 1) cntkg[k * Gb + g] += __popc(m);
+          __syncwarp();
+        }
+      }
+    }
+    __syncthreads();
+
+    // ---- semismooth Newton on (alpha, beta, lambda_g of the active bands) jointly: one pass over the list per step.
+    // The equations are piecewise linear (see prox.cuh): P(alpha, lambda) = (tau + b)/2 and R(beta, lambda) = (tau - b)/2
+    // with the cap active, P - R = b with alpha = beta otherwise, and S_g = bound_g for every active band.  Eliminating
+    // d lambda_g = (F_g - sP_g d alpha - sR_g d beta) / (sP_g + sR_g) leaves a 2 x 2 system.  Bands enter the active set
+    // when violated and leave it when their multiplier changes sign.  Anything irregular (singular step, no convergence
+    // in 16 passes) falls back to the nested robust solver prox_rootfind on the same list.
+    const double tol = 2e-15 * fmax(1.0, fabs(b) + (isfinite(tau) ? tau : 0.0));
+    const double Pt = 0.5 * (tau + b), Rt = 0.5 * (tau - b);
+    const double cPt = src.cPt, cRt = src.cRt;
+    double al = aw, be = bw;
+    int amode = amode_w;
+    bool ok = false;
+    int why = 4;                                          // (debug) 1 singular band, 2 det, 3 den, 4 passes, 5 NaN
+    for (int g = tid; g < G; g += nt) act[g] = lamS[g] > 0.0 ? 1 : (lamS[g] < 0.0 ? -1 : 0);
+    __syncthreads();
+    for (int itn = 0; itn < 16; ++itn) {
+      root_pass(src, poff, ngrp, lamS, G, al, be - Delta, gv);
+      ++rs.n_eval;
+      double P = cPt, R = cRt, sP = 0.0, sR = 0.0;
+      for (int q = 0; q < ngrp; ++q) { P += gv[4 * q]; R += gv[4 * q + 1]; sP += gv[4 * q + 2]; sR += gv[4 * q + 3]; }
+      const double FA = amode == 1 ? P - Pt : P - R - b, FB = amode == 1 ? R - Rt : 0.0;
+      double sA = 0, sB = 0, sAB = 0, rA = 0, rB = 0, sT = 0, sF = 0;
+      bool gconv = true, sing = false;
+      for (int g = 0; g < G; ++g) {
+        const double pa = gv[4 * g + 2], ra = gv[4 * g + 3], t = pa + ra;
+        const double Sg = gw0[g] + (gv[4 * g] + (double)cbin[g] * PRISM_FIX_INV) - (gv[4 * g + 1] + (double)cbin[Gb + g] * PRISM_FIX_INV);
+        int ac = act[g];
+        if (ac == 0 && bands_on) {
+          if (Sg > band_hi[g] + 8.0 * tol) ac = 1; else if (Sg < band_lo[g] - 8.0 * tol) ac = -1;
+          if (ac) gconv = false;
+        }
+        if (ac) {
+          const double Fg = Sg - (ac > 0 ? band_hi[g] : band_lo[g]);
+          if (fabs(Fg) > tol) gconv = false;
+          if (t > 0.0) { sA += pa * pa / t; sB += ra * ra / t; sAB += pa * ra / t; rA += pa * Fg / t; rB += ra * Fg / t; sT += t; sF += Fg; }
+          else if (fabs(Fg) > tol) sing = true;
+        }
+        gsum[g] = Sg;                                     // (every thread writes the same value)
+      }
+      if (fabs(FA) <= tol && fabs(FB) <= tol && gconv) {
+        if (amode == 1) { if (al >= be) { ok = true; break; } amode = 0; al = be = 0.5 * (al + be); __syncthreads(); continue; }
+        if (!isfinite(tau) || P + R <= tau + tol) { ok = true; break; }
+        amode = 1; be = al;
+        __syncthreads();
+        continue;
+      }
+      if (sing) { why = 1; break; }
+      double dal, dbe;
+      if (amode == 1) {
+        const double M11 = -sP + sA, M12 = sAB, M21 = -sAB, M22 = sR - sB, r1 = -FA + rA, r2 = -FB - rB;
+        const double det = M11 * M22 - M12 * M21;
+        if (!(fabs(det) > 1e-300)) { why = 2; break; }
+        dal = (r1 * M22 - M12 * r2) / det; dbe = (M11 * r2 - M21 * r1) / det;
+      } else {
+        const double den = (sP + sR) - sT;
+        if (!(den > 1e-300)) { why = 3; break; }
+        dal = dbe = (FA - sF) / den;
+      }
+      if (!(dal == dal) || !(dbe == dbe)) { why = 5; break; }
+      __syncthreads();
+      for (int g = tid; g < G; g += nt) {                // multipliers and active set (thread g owns band g)
+        const double pa = gv[4 * g + 2], ra = gv[4 * g + 3], t = pa + ra;
+        int ac = act[g];
+        const bool was = ac != 0;
+        if (!was && bands_on) { if (gsum[g] > band_hi[g] + 8.0 * tol) ac = 1; else if (gsum[g] < band_lo[g] - 8.0 * tol) ac = -1; }
+        if (ac && t > 0.0) {
+          const double Fg = gsum[g] - (ac > 0 ? band_hi[g] : band_lo[g]);
+          double ln = lamS[g] + (Fg - pa * dal - ra * dbe) / t;
+          if (!(ln * ac > 0.0)) { ln = 0.0; ac = 0; }     // the multiplier would change sign: the band goes inactive
+          lamS[g] = ln;
+        }
+        act[g] = ac;
+      }
+      al += dal; be += dbe;
+      __syncthreads();
+    }
+    if (ok) { rs.alpha = al; rs.beta = be; rs.amode = amode; }
+    else {
+      if (p.stats && tid == 0 && p.iter < 4096) { atomicAdd(&p.stats[p.iter * 8 + 3], 1); atomicAdd(&p.stats[(2048 + p.iter) * 8 + why], 1); }
+      __syncthreads();
+      for (int g = tid; g < G; g += nt) lamS[g] = lamW[g];
+      __syncthreads();
+      prox_rootfind<false>(p, src, a, b, tau, Delta, sh, rs);
+    }
+    double mv_l = 0.0;
+    for (int g = 0; g < G; ++g) mv_l = fmax(mv_l, fabs(lamS[g] - lamW[g]));
+    mv = fmax(fmax(fabs(rs.alpha - aw), fabs(rs.beta - bw)), mv_l);
+    if (!(mv <= 0.5 * W)) fallback = true;               // left the window (or NaN): the dead assets were misjudged
+    if (fallback && p.stats && tid == 0 && p.iter < 4096) atomicAdd(&p.stats[p.iter * 8 + 2], 1);
+  }
+  int finished = 0;
+  if (!fallback) {
+    // ---------------------------------------------------------------- live assets: output (+ residual terms)
+    const double alpha = rs.alpha, beta = rs.beta, bdf = beta - Delta;
+    double nx = 0, nz = 0, nrp = 0, nrd = 0, nPx = 0, ny = 0, nq = 0;
+    src.for_each([&](int64_t i, const ElemConst& e, int g, int, const double*, const double*) {
+      double mvb, mvs;
+      const double lg = G ? lamS[g] : 0.0;
+      const double tr = buy_amt(e, alpha + lg, mvb) - sell_amt<false>(e, bdf + lg, nullptr, nullptr, 0, mvs);
+      const double z = e.w0 + tr;
+      const double rho = cg * p.d[i];
+      const double y = e.T + lam_b - tr * rho;
+      const double qi = p.q ? p.q[rowp + i] : -p.mu[row + i];
+      const double r = rho * z - y - qi;
+      const double rt = r * (e.ir * cg) * igc;
+      p.rt[rowp + i] = rt;
+      p.cc[rowp + i] = rt - z;
+      if (CHECK) {
+        p.w_out[row + i] = z;
+        const double x = p.xs[rowp + i], pq = p.pxq[rowp + i];
+        nx = fmax(nx, fabs(x)); nz = fmax(nz, fabs(z)); nrp = fmax(nrp, fabs(x - z));
+        nrd = fmax(nrd, fabs(pq + y)); nPx = fmax(nPx, fabs(pq - qi)); ny = fmax(ny, fabs(y)); nq = fmax(nq, fabs(qi));
+        if (!(z == z) || !(x == x) || !(pq == pq)) nrp = INFINITY;
+      }
+    });
+    if (CHECK) {
+      if (tid < 7) {                                     // residual terms of the dead assets, per slice
+        double m = 0.0;
+        for (int s = 0; s < p.S; ++s) m = fmax(m, p.chkp[((int64_t)a * p.S + s) * 8 + tid]);
+        chk[tid] = m;
+      }
+      double val[7] = {nx, nz, nrp, nrd, nPx, ny, nq};
+      block_reduce<7, 1>(val, scratch);                  // (its barrier also publishes chk)
+#pragma unroll
+      for (int q = 0; q < 7; ++q) val[q] = fmax(val[q], chk[q]);
+      const double rp = val[2] / fmax(fmax(val[0], val[1]), 1e-300);
+      const double rd = val[3] / fmax(fmax(val[4], fmax(val[5], val[6])), 1e-300);
+      const bool conv = rp <= p.eps && rd <= p.eps;
+      if (!(rp < INFINITY) || !(rd < INFINITY)) fallback = true;             // NaN / Inf: the generic path classifies it
+      else if (!conv && p.adapt && p.iter >= PRISM_ADAPT_START && p.iter - p.ap.nadapt[a] >= PRISM_ADAPT_EVERY) {
+        const double ratio = sqrt(rp / fmax(rd, 1e-300));
+        if (ratio > 3.0 || ratio < 1.0 / 3.0) fallback = true;               // rho changes: every asset is rewritten
+        else if (tid == 0) p.ap.nadapt[a] = p.iter;
+      }
+      if (!fallback) {
+        finished = conv ? 1 : 0;
+        if (tid == 0) {
+          p.resid[(int64_t)a * PRISM_NRES + PRISM_R_PRIMAL] = rp;
+          p.resid[(int64_t)a * PRISM_NRES + PRISM_R_DUAL] = rd;
+          if (conv) p.ap.conv[a] = 1;
+        }
+      }
+    }
+  }
+  if (!fallback) {
+    // ---------------------------------------------------------------- commit the account's state
+    if (mode & PROX_FINAL) finished = 1;                 // (CHECK instantiation: w_out holds z)
+    const double alpha = rs.alpha, beta = rs.beta;
+    for (int g = tid; g < G; g += nt) p.lamG[(int64_t)a * G + g] = lamS[g];
+    if (tid == 0) {
+      p.resid[(int64_t)a * PRISM_NRES + PRISM_R_RESERVED] += (double)rs.n_eval;
+      p.ap.alpha[a] = alpha; p.ap.beta[a] = beta; p.ap.mode[a] = rs.amode;
+      // next window of the streaming pass: a multiple of the last movement, never shrunk while its list is short
+      // (a wide window then costs nothing and the solution almost never leaves it); infinite for the first iterations
+      double Ws = p.win_ratio * next_window(p, alpha, beta, mv);
+      const int nl = src.cnt[0];
+      if (nl < 256) Ws = fmax(Ws, nl < 64 ? 2.0 * W : W);
+      if (p.iter < 2) Ws = INFINITY;
+      p.ap.win[a] = Ws; p.ap.wins[a] = Ws;
+      if (finished) {                                    // H6: w_out already holds z
+        p.ap.done[a] = 1; p.ap.iters[a] = p.iter;
+        atomicAdd(&p.counters[0], 1);
+        double* du = p.duals + (int64_t)a * PRISM_NDUAL(G);
+        du[0] = 0.5 * (alpha + beta);
+        du[1] = 0.5 * (alpha - beta);
+        for (int g = 0; g < G; ++g) { du[2 + g] = fmax(lamS[g], 0.0); du[2 + G + g] = fmax(-lamS[g], 0.0); }
+        p.resid[(int64_t)a * PRISM_NRES + PRISM_R_RHO] = c;
+      }
+      if (p.stats && p.iter < 4096) {
+        atomicAdd(&p.stats[p.iter * 8 + 5], 1); atomicAdd(&p.stats[p.iter * 8 + 6], src.cnt[0]); atomicAdd(&p.stats[p.iter * 8 + 7], rs.n_eval);
+        atomicMax(&p.stats[p.iter * 8 + 4], rs.n_eval); if (rs.n_eval > 20) atomicAdd(&p.stats[p.iter * 8 + 0], 1);
+      }
+    }
+    return;
+  }
+  // ------------------------------------------------------------------ generic path: every asset, from global memory
+  if (p.stats && tid == 0 && p.iter < 4096) atomicAdd(&p.stats[p.iter * 8 + 1], 1);
+  __syncthreads();
+  SrcGlobal<false> gsrc(p, a, cg, p.lo[a], p.hi[a], lam_b);
+  ProxShared shg = sh;
+  prox_body<false>(p, mode | (CHECK ? PROX_CHECK : 0), gsrc, a, gam, c, kappa, lam_b, shg, false);
+  if (tid == 0) p.ap.wins[a] = p.win_ratio * p.ap.win[a];
+}

@@ -59,6 +59,9 @@ CASES = {
     "cfg1_multi_tile": lambda: gen.config1(N=1100, k=30, A=70),               # > 64 accounts: two account tiles
     "cfg2_small": lambda: gen.config2(N=1000, k=20, A=6, G=5, band_half=0.005),  # bands certainly active (R9 variant)
     "cfg2_mid": lambda: gen.config2(N=2500, k=50, A=9),
+    "cfg1_stream": lambda: gen.config1(N=1600, k=30, A=70),                   # N % 16 == 0: streaming prox (prox_fast.cuh)
+    "cfg2_stream": lambda: gen.config2(N=2560, k=50, A=9),                    # streaming prox with group bands
+    "cfg2_stream_tight": lambda: gen.config2(N=1024, k=20, A=6, G=5, band_half=0.005),   # bands certainly active
     "cfg3_small": lambda: gen.config3(N=600, k=12, A=4),
     "cfg4_small": lambda: gen.config4(N=4000, k=100, A=3, hi=0.001),          # fp32 loadings, k = 100 (13 factor tiles)
     "sec9": lambda: gen.section9(N=481, k=20, A=2),                           # PAPER.md:378 transition objective (R14)
@@ -99,12 +102,27 @@ def test_batch_equals_single_accounts_and_identical_accounts():
     Pt.close(); P.close()
 
 
-def test_run_to_run_determinism():
-    inst = gen.config2(N=1500, k=20, A=5, G=7, band_half=0.01)
+@pytest.mark.parametrize("N", [1500, 1536])       # every-asset kernels / streaming kernels (N % 16 == 0)
+def test_run_to_run_determinism(N):
+    inst = gen.config2(N=N, k=20, A=5, G=7, band_half=0.01)
     P, r1 = _solve_gpu(inst)
     r2 = P.solve()
     assert (r1.w == r2.w).all() and (r1.iters == r2.iters).all()
     P.close()
+
+
+def test_streaming_and_every_asset_prox_agree(monkeypatch):
+    """The streaming form of the prox (k_prox_stream + k_prox_root) against the every-asset kernel on the same
+    problem: same fixed point, so the converged weights agree far below the parity tolerance."""
+    inst = gen.config2(N=2048, k=20, A=6, G=6, band_half=0.01)
+    P1, r1 = _solve_gpu(inst)
+    monkeypatch.setenv("PRISM_PROX_NOFAST", "1")
+    P2, r2 = _solve_gpu(inst)
+    monkeypatch.delenv("PRISM_PROX_NOFAST")
+    assert (r1.status.cpu().numpy() == 0).all() and (r2.status.cpu().numpy() == 0).all()
+    assert float((r1.w - r2.w).abs().max()) <= 2e-6
+    assert int((r1.iters - r2.iters).abs().max()) <= 20
+    P1.close(); P2.close()
 
 
 def test_residuals_call_is_external_and_matches_checker():
