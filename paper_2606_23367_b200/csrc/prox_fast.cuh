@@ -281,11 +281,29 @@ struct SrcLiveG {
 
 __host__ __device__ inline size_t root_smem_bytes(int G, int nsub) {
   const int Gb = G > 0 ? G : 1;
-  return (size_t)(12 * 32 + 4 * Gb + 6 * Gb + 2 * Gb + 8 + 4 * (Gb + 4)) * 8 + (size_t)(nsub * Gb + 3 * Gb + 16) * 4 + 16;
+  return (size_t)(16 * 32 + 4 * Gb + 6 * Gb + 2 * Gb + 8 + 4 * (Gb + 4)) * 8 + (size_t)(nsub + 1 + 4 * Gb + 3 * Gb + 16 + ROOT_NSL) * 4 + 16;
 }
 
 // One pass over the grouped list: per (pseudo-)group q the buys, sells and their slopes at thresholds (al, bd + Delta)
 // shifted by the group's multiplier -> gv[4 q .. 4 q + 3].  Warp w owns the groups w, w + nw, ...; fixed order.
+// buys, sells and slopes of one list entry at thresholds (a0, b0); the common class (inside its box) without branches
+__device__ __forceinline__ void root_entry(const SrcLiveG& src, const double2& ea, const double2& eb, double a0, double b0,
+                                           double& sp, double& sr, double& slp, double& slr) {
+  const uint32_t m = (uint32_t)__double_as_longlong(eb.y);
+  const double T = ea.x, w0 = ea.y, ir = eb.x;
+  if ((m >> 30) == 0) {
+    const double wB = src.hi_a - w0, wS = w0 - src.lo_a;
+    const double tb = (T - a0) * ir, ts = (b0 - T) * ir;
+    sp += tb <= 0.0 ? 0.0 : (tb >= wB ? wB : tb);
+    sr += ts <= 0.0 ? 0.0 : (ts >= wS ? wS : ts);
+    slp += (tb > 0.0 && tb < wB) ? ir : 0.0;
+    slr += (ts > 0.0 && ts < wS) ? ir : 0.0;
+  } else {
+    ElemConst e; int g; double mvb, mvs;
+    src.decode(ea, eb, e, g);
+    sp += buy_amt(e, a0, mvb); sr += sell_amt<false>(e, b0, nullptr, nullptr, 0, mvs); slp += mvb; slr += mvs;
+  }
+}
 __device__ __forceinline__ void root_pass(const SrcLiveG& src, const int* poff, int ngrp, const double* lamS, int G,
                                           double al, double bd, double* gv) {
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
@@ -300,17 +318,11 @@ __device__ __forceinline__ void root_pass(const SrcLiveG& src, const int* poff, 
 #pragma unroll
       for (int u = 0; u < 4; ++u) { ea[u] = __ldg((const double2*)(src.ent + j + 32 * u)); eb[u] = __ldg((const double2*)(src.ent + j + 32 * u) + 1); }
 #pragma unroll
-      for (int u = 0; u < 4; ++u) {
-        ElemConst e; int g; double mvb, mvs;
-        src.decode(ea[u], eb[u], e, g);
-        sp += buy_amt(e, a0, mvb); sr += sell_amt<false>(e, b0, nullptr, nullptr, 0, mvs); slp += mvb; slr += mvs;
-      }
+      for (int u = 0; u < 4; ++u) root_entry(src, ea[u], eb[u], a0, b0, sp, sr, slp, slr);
     }
     for (; j < j1; j += 32) {
       const double2 ea = __ldg((const double2*)(src.ent + j)), eb = __ldg((const double2*)(src.ent + j) + 1);
-      ElemConst e; int g; double mvb, mvs;
-      src.decode(ea, eb, e, g);
-      sp += buy_amt(e, a0, mvb); sr += sell_amt<false>(e, b0, nullptr, nullptr, 0, mvs); slp += mvb; slr += mvs;
+      root_entry(src, ea, eb, a0, b0, sp, sr, slp, slr);
     }
     sp = warp_sum(sp); sr = warp_sum(sr); slp = warp_sum(slp); slr = warp_sum(slr);
     if (lane == 0) { gv[4 * q] = sp; gv[4 * q + 1] = sr; gv[4 * q + 2] = slp; gv[4 * q + 3] = slr; }
@@ -318,10 +330,89 @@ __device__ __forceinline__ void root_pass(const SrcLiveG& src, const int* poff, 
   __syncthreads();
 }
 
+// The grouped list as a source of the nested robust solver prox_rootfind: its evaluation routines are overloaded
+// here so that every trial evaluation is one lean root_pass (the per-group sums it leaves in gv also serve the
+// selected-group sums and the all-groups pass of the solver).
+struct SrcGrouped {
+  const SrcLiveG* L;
+  const int* poff;
+  int ngrp;
+  double* gv;
+  __device__ __forceinline__ double cP() const { return L->cPt; }
+  __device__ __forceinline__ double cR() const { return L->cRt; }
+};
+template <bool LOTS>
+__device__ __noinline__ void prox_eval(const SrcGrouped& s, const double* lamS, int G, double al, double bd, int s1, int s2,
+                                       double* scratch, double* out) {
+  root_pass(*s.L, s.poff, s.ngrp, lamS, G, al, bd, s.gv);
+  double val[4] = {0.0, 0.0, 0.0, 0.0};
+  if ((int)threadIdx.x < s.ngrp) {
+#pragma unroll
+    for (int q = 0; q < 4; ++q) val[q] = s.gv[4 * threadIdx.x + q];
+  }
+  block_reduce<4, 0>(val, scratch);
+  out[0] = val[0] + s.L->cPt; out[1] = val[1] + s.L->cRt; out[2] = val[2]; out[3] = val[3];
+#pragma unroll
+  for (int q = 4; q < 12; ++q) out[q] = 0.0;
+  if (s1 >= 0) { out[4] = s.gv[4 * s1] + s.L->cPg(s1); out[5] = s.gv[4 * s1 + 1] + s.L->cRg(s1); out[6] = s.gv[4 * s1 + 2]; out[7] = s.gv[4 * s1 + 3]; }
+  if (s2 >= 0) { out[8] = s.gv[4 * s2] + s.L->cPg(s2); out[9] = s.gv[4 * s2 + 1] + s.L->cRg(s2); out[10] = s.gv[4 * s2 + 2]; out[11] = s.gv[4 * s2 + 3]; }
+  __syncthreads();                                       // gv is rewritten by the next pass
+}
+template <bool LOTS>
+__device__ __noinline__ void prox_group_sums(const SrcGrouped& s, const double* lamS, int G, double al, double bd,
+                                             const double* gw0, double* gbin, double* gsum) {
+  root_pass(*s.L, s.poff, s.ngrp, lamS, G, al, bd, s.gv);
+  for (int g = threadIdx.x; g < G; g += blockDim.x)
+    gsum[g] = gw0[g] + (s.gv[4 * g] + s.L->cPg(g)) - (s.gv[4 * g + 1] + s.L->cRg(g));
+  __syncthreads();
+}
+template <bool LOTS>
+__device__ __noinline__ void prox_brackets(const SrcGrouped& s, double Delta, double* scratch, double* out) {
+  prox_brackets<LOTS>(*s.L, Delta, scratch, out);
+}
+template <bool LOTS>
+__device__ __noinline__ void prox_eval_multi(const SrcGrouped& s, const double* lamS, int G, double a0, double da, double b0,
+                                             double db, double* scratch, double* outP, double* outR) {
+  const SrcLiveG& L = *s.L;
+  double sp[PROX_KSEC], sr[PROX_KSEC];
+#pragma unroll
+  for (int k = 0; k < PROX_KSEC; ++k) { sp[k] = 0.0; sr[k] = 0.0; }
+  const int n = L.cnt[0];
+  for (int j = threadIdx.x; j < n; j += blockDim.x) {
+    const double2 ea = __ldg((const double2*)(L.ent + j)), eb = __ldg((const double2*)(L.ent + j) + 1);
+    const uint32_t m = (uint32_t)__double_as_longlong(eb.y);
+    const double lg = G ? lamS[(m >> PROX_META_IDX_BITS) & 0xffu] : 0.0;
+    if ((m >> 30) == 0) {
+      const double T = ea.x, w0 = ea.y, ir = eb.x, wB = L.hi_a - w0, wS = w0 - L.lo_a;
+      const double tb0 = (T - a0 - lg) * ir, ts0 = (b0 + lg - T) * ir, dtb = da * ir, dts = db * ir;
+#pragma unroll
+      for (int k = 0; k < PROX_KSEC; ++k) {
+        const double tb = tb0 - k * dtb, ts = ts0 + k * dts;
+        sp[k] += tb <= 0.0 ? 0.0 : (tb >= wB ? wB : tb);
+        sr[k] += ts <= 0.0 ? 0.0 : (ts >= wS ? wS : ts);
+      }
+    } else {
+      ElemConst e; int g;
+      L.decode(ea, eb, e, g);
+#pragma unroll
+      for (int k = 0; k < PROX_KSEC; ++k) {
+        double mvb, mvs;
+        sp[k] += buy_amt(e, a0 + k * da + lg, mvb);
+        sr[k] += sell_amt<false>(e, b0 + k * db + lg, nullptr, nullptr, 0, mvs);
+      }
+    }
+  }
+  block_reduce<PROX_KSEC, 0>(sp, scratch);
+  block_reduce<PROX_KSEC, 0>(sr, scratch);
+#pragma unroll
+  for (int k = 0; k < PROX_KSEC; ++k) { outP[k] = sp[k] + L.cPt; outR[k] = sr[k] + L.cRt; }
+}
+
 template <bool CHECK>
-__global__ void __launch_bounds__(ROOT_NT, 3) k_prox_root(const __grid_constant__ ProxArgs p, int mode) {
+__global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant__ ProxArgs p, int mode) {
   extern __shared__ __align__(16) unsigned char root_raw[];
   __shared__ SrcLiveG src;                 // CTA-uniform objects live in shared memory, not on the threads' stacks
+  __shared__ SrcGrouped sgrp;
   __shared__ ProxShared sh;
   const int a = blockIdx.x;
   if (p.ap.done[a]) return;
@@ -331,7 +422,7 @@ __global__ void __launch_bounds__(ROOT_NT, 3) k_prox_root(const __grid_constant_
   const int nsub = p.S * FAST_NW;
   const int ngrp = G > 0 ? G : nw;                       // without groups: nw slices of the list, for load balance
   double* d0 = (double*)root_raw;
-  double* scratch = d0; d0 += 12 * 32;
+  double* scratch = d0; d0 += 16 * 32;
   double* gbin = d0; d0 += 4 * Gb;                       // nw = 4 warps
   double* lamS = d0; d0 += Gb;
   double* gsum = d0; d0 += Gb;
@@ -339,8 +430,9 @@ __global__ void __launch_bounds__(ROOT_NT, 3) k_prox_root(const __grid_constant_
   unsigned long long* cbin = (unsigned long long*)d0; d0 += 2 * Gb;    // dead assets of the streaming pass
   double* chk = d0; d0 += 8;
   double* gv = d0; d0 += 4 * (Gb + 4);                   // per (pseudo-)group sums of one pass
-  int* cntkg = (int*)d0;                                 // nsub x Gb: entries of group g in list k (then running offsets)
-  int* goff = cntkg + nsub * Gb;                         // Gb + 1 group offsets of the grouped list
+  int* offs = (int*)d0;                                  // nsub + 1: start of raw list k in the sequence of all lists
+  int* wcnt = offs + nsub + 1;                           // nw x Gb: entries of group g in warp w's part (then running offsets)
+  int* goff = wcnt + 4 * Gb;                             // Gb + 1 group offsets of the grouped list
   int* poff = goff + Gb + 1;                             // ngrp + 1 (pseudo-)group offsets used by the passes
   int* act = poff + Gb + 5;                              // Gb: band state -1 lower active, 0 inactive, +1 upper active
   int* selS = act + Gb;
@@ -368,7 +460,8 @@ __global__ void __launch_bounds__(ROOT_NT, 3) k_prox_root(const __grid_constant_
     cbin[g] = *src_bin;
     *src_bin = 0ull;
   }
-  for (int e = tid; e < nsub * Gb; e += nt) cntkg[e] = 0;
+  for (int e = tid; e < 4 * Gb; e += nt) wcnt[e] = 0;
+  for (int k = tid; k < nsub; k += nt) offs[k + 1] = p.lcnt[(int64_t)a * nsub + k];
   __syncthreads();
   bool fallback = generic != 0;
   RootState rs;
@@ -379,33 +472,50 @@ __global__ void __launch_bounds__(ROOT_NT, 3) k_prox_root(const __grid_constant_
   rs.nobands = bands_on ? 0 : 1;
   double mv = 0.0;
   if (!fallback) {
-    // ---- group sort (counting sort, stable in (list, position) order => deterministic): lists -> lcomp by group
+    // ---- group sort (counting sort, stable in (list, position) order => deterministic): lists -> lcomp by group.
+    // The lists are taken as one sequence (offs = their start offsets); warp w handles a contiguous quarter of it.
     const unsigned lt = (1u << lane) - 1u;
     const LiveEnt* lr = p.lraw + (int64_t)a * nsub * p.capw;
-    const int32_t* lc = p.lcnt + (int64_t)a * nsub;
-    for (int k = wid; k < nsub; k += nw) {
-      const int cnt = lc[k];
-      if (!G) { if (lane == 0) cntkg[k] = cnt; continue; }
-      const LiveEnt* sl = lr + (int64_t)k * p.capw;
-      for (int j0 = 0; j0 < cnt; j0 += 32) {
-        const int j = j0 + lane;
-        const bool valid = j < cnt;
-        const int g = valid ? (int)((__ldg(&sl[j].meta) >> PROX_META_IDX_BITS) & 0xffu) : 0x100 + lane;
-        const unsigned m = __match_any_sync(0xffffffffu, g);
-        if (valid && lane == __ffs(m) - 1) cntkg[k * Gb + g] += __popc(m);
+    if (wid == 0) {                                      // inclusive scan of the list lengths
+      int carry = 0;
+      for (int k0 = 0; k0 < nsub; k0 += 32) {
+        int v = k0 + lane < nsub ? offs[k0 + lane + 1] : 0;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, v, o); if (lane >= o) v += t; }
+        if (k0 + lane < nsub) offs[k0 + lane + 1] = v + carry;
+        carry += __shfl_sync(0xffffffffu, v, 31);
       }
+      if (lane == 0) offs[0] = 0;
     }
     __syncthreads();
-    for (int g = tid; g < Gb; g += nt) {                 // offsets of list k inside group g; group totals
+    const int n = offs[nsub];
+    const int segw = (((n + nw - 1) / nw) + 31) & ~31;
+    const int j_beg = min(n, wid * segw), j_end = min(n, (wid + 1) * segw);
+    auto locate = [&](int j) -> const LiveEnt* {         // entry j of the sequence
+      int lo = 0, hi = nsub;
+      while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (offs[mid] <= j) lo = mid; else hi = mid; }
+      return lr + (int64_t)lo * p.capw + (j - offs[lo]);
+    };
+    if (!G) { if (lane == 0) wcnt[wid] = j_end - j_beg; }
+    else
+      for (int j0 = j_beg; j0 < j_end; j0 += 32) {
+        const int j = j0 + lane;
+        const bool valid = j < j_end;
+        const int g = valid ? (int)((__ldg(&locate(j)->meta) >> PROX_META_IDX_BITS) & 0xffu) : 0x100 + lane;
+        const unsigned m = __match_any_sync(0xffffffffu, g);
+        if (valid && lane == __ffs(m) - 1) wcnt[wid * Gb + g] += __popc(m);
+        __syncwarp();
+      }
+    __syncthreads();
+    for (int g = tid; g < Gb; g += nt) {                 // start of warp w's entries inside group g; group totals
       int run = 0;
-      for (int k = 0; k < nsub; ++k) { const int t = cntkg[k * Gb + g]; cntkg[k * Gb + g] = run; run += t; }
+      for (int w = 0; w < nw; ++w) { const int t = wcnt[w * Gb + g]; wcnt[w * Gb + g] = run; run += t; }
       goff[g + 1] = run;
     }
     __syncthreads();
     if (tid == 0) {
       goff[0] = 0;
       for (int g = 0; g < Gb; ++g) goff[g + 1] += goff[g];
-      const int n = goff[Gb];
       if (G) for (int g = 0; g <= G; ++g) poff[g] = goff[g];
       else for (int q = 0; q <= nw; ++q) poff[q] = (int)((int64_t)n * q / nw);
       unsigned long long sp = 0ull, sr = 0ull;
@@ -419,28 +529,24 @@ __global__ void __launch_bounds__(ROOT_NT, 3) k_prox_root(const __grid_constant_
     __syncthreads();
     {
       LiveEnt* dst = p.lcomp + (int64_t)a * p.ldc;
-      for (int k = wid; k < nsub; k += nw) {
-        const int cnt = lc[k];
-        const LiveEnt* sl = lr + (int64_t)k * p.capw;
-        for (int j0 = 0; j0 < cnt; j0 += 32) {
-          const int j = j0 + lane;
-          const bool valid = j < cnt;
-          double2 ea = make_double2(0, 0), eb = make_double2(0, 0);
-          int g = 0x100 + lane;
-          if (valid) {
-            ea = __ldg((const double2*)(sl + j)); eb = __ldg((const double2*)(sl + j) + 1);
-            g = G ? (int)(((uint32_t)__double_as_longlong(eb.y) >> PROX_META_IDX_BITS) & 0xffu) : 0;
-          }
-          const unsigned m = __match_any_sync(0xffffffffu, g);
-          if (valid) {
-            const int pos = goff[g] + cntkg[k * Gb + g] + __popc(m & lt);
-            double2* o = (double2*)(dst + pos);
-            o[0] = ea; o[1] = eb;
-          }
-          __syncwarp();
-          if (valid && lane == __ffs(m) - 1) cntkg[k * Gb + g] += __popc(m);
-          __syncwarp();
+      for (int j0 = j_beg; j0 < j_end; j0 += 32) {
+        const int j = j0 + lane;
+        const bool valid = j < j_end;
+        double2 ea = make_double2(0, 0), eb = make_double2(0, 0);
+        int g = 0x100 + lane;
+        if (valid) {
+          const LiveEnt* e = locate(j);
+          ea = __ldg((const double2*)e); eb = __ldg((const double2*)e + 1);
+          g = G ? (int)(((uint32_t)__double_as_longlong(eb.y) >> PROX_META_IDX_BITS) & 0xffu) : 0;
         }
+        const unsigned m = __match_any_sync(0xffffffffu, g);
+        if (valid) {
+          double2* o = (double2*)(dst + goff[g] + wcnt[wid * Gb + g] + __popc(m & lt));
+          o[0] = ea; o[1] = eb;
+        }
+        __syncwarp();
+        if (valid && lane == __ffs(m) - 1) wcnt[wid * Gb + g] += __popc(m);
+        __syncwarp();
       }
     }
     __syncthreads();
@@ -463,27 +569,37 @@ __global__ void __launch_bounds__(ROOT_NT, 3) k_prox_root(const __grid_constant_
     for (int itn = 0; itn < 16; ++itn) {
       root_pass(src, poff, ngrp, lamS, G, al, be - Delta, gv);
       ++rs.n_eval;
-      double P = cPt, R = cRt, sP = 0.0, sR = 0.0;
-      for (int q = 0; q < ngrp; ++q) { P += gv[4 * q]; R += gv[4 * q + 1]; sP += gv[4 * q + 2]; sR += gv[4 * q + 3]; }
-      const double FA = amode == 1 ? P - Pt : P - R - b, FB = amode == 1 ? R - Rt : 0.0;
-      double sA = 0, sB = 0, sAB = 0, rA = 0, rB = 0, sT = 0, sF = 0;
-      bool gconv = true, sing = false;
-      for (int g = 0; g < G; ++g) {
-        const double pa = gv[4 * g + 2], ra = gv[4 * g + 3], t = pa + ra;
-        const double Sg = gw0[g] + (gv[4 * g] + (double)cbin[g] * PRISM_FIX_INV) - (gv[4 * g + 1] + (double)cbin[Gb + g] * PRISM_FIX_INV);
-        int ac = act[g];
-        if (ac == 0 && bands_on) {
-          if (Sg > band_hi[g] + 8.0 * tol) ac = 1; else if (Sg < band_lo[g] - 8.0 * tol) ac = -1;
-          if (ac) gconv = false;
+      // thread q: the terms of (pseudo-)group q; fixed-order block reduction (deterministic)
+      double P, R, sP, sR, sA, sB, sAB, rA, rB, sT, sF;
+      bool gconv, sing;
+      {
+        double v16[16];
+#pragma unroll
+        for (int q = 0; q < 16; ++q) v16[q] = 0.0;
+        if (tid < ngrp) { v16[0] = gv[4 * tid]; v16[1] = gv[4 * tid + 1]; v16[2] = gv[4 * tid + 2]; v16[3] = gv[4 * tid + 3]; }
+        if (tid < G) {
+          const int g = tid;
+          const double pa = v16[2], ra = v16[3], t = pa + ra;
+          const double Sg = gw0[g] + (v16[0] + (double)cbin[g] * PRISM_FIX_INV) - (v16[1] + (double)cbin[Gb + g] * PRISM_FIX_INV);
+          int ac = act[g];
+          if (ac == 0 && bands_on) {
+            if (Sg > band_hi[g] + 8.0 * tol) ac = 1; else if (Sg < band_lo[g] - 8.0 * tol) ac = -1;
+            if (ac) v16[11] = 1.0;
+          }
+          if (ac) {
+            const double Fg = Sg - (ac > 0 ? band_hi[g] : band_lo[g]);
+            if (fabs(Fg) > tol) v16[11] = 1.0;
+            if (t > 0.0) { v16[4] = pa * pa / t; v16[5] = ra * ra / t; v16[6] = pa * ra / t; v16[7] = pa * Fg / t; v16[8] = ra * Fg / t; v16[9] = t; v16[10] = Fg; }
+            else if (fabs(Fg) > tol) v16[12] = 1.0;
+          }
+          gsum[g] = Sg;
         }
-        if (ac) {
-          const double Fg = Sg - (ac > 0 ? band_hi[g] : band_lo[g]);
-          if (fabs(Fg) > tol) gconv = false;
-          if (t > 0.0) { sA += pa * pa / t; sB += ra * ra / t; sAB += pa * ra / t; rA += pa * Fg / t; rB += ra * Fg / t; sT += t; sF += Fg; }
-          else if (fabs(Fg) > tol) sing = true;
-        }
-        gsum[g] = Sg;                                     // (every thread writes the same value)
+        block_reduce<16, 0>(v16, scratch);
+        P = cPt + v16[0]; R = cRt + v16[1]; sP = v16[2]; sR = v16[3];
+        sA = v16[4]; sB = v16[5]; sAB = v16[6]; rA = v16[7]; rB = v16[8]; sT = v16[9]; sF = v16[10];
+        gconv = !(v16[11] > 0.0); sing = v16[12] > 0.0;
       }
+      const double FA = amode == 1 ? P - Pt : P - R - b, FB = amode == 1 ? R - Rt : 0.0;
       if (fabs(FA) <= tol && fabs(FB) <= tol && gconv) {
         if (amode == 1) { if (al >= be) { ok = true; break; } amode = 0; al = be = 0.5 * (al + be); __syncthreads(); continue; }
         if (!isfinite(tau) || P + R <= tau + tol) { ok = true; break; }
@@ -524,10 +640,13 @@ __global__ void __launch_bounds__(ROOT_NT, 3) k_prox_root(const __grid_constant_
     if (ok) { rs.alpha = al; rs.beta = be; rs.amode = amode; }
     else {
       if (p.stats && tid == 0 && p.iter < 4096) { atomicAdd(&p.stats[p.iter * 8 + 3], 1); atomicAdd(&p.stats[(2048 + p.iter) * 8 + why], 1); }
+      // nested robust solver on the same grouped list (lean passes through the SrcGrouped overloads)
       __syncthreads();
       for (int g = tid; g < G; g += nt) lamS[g] = lamW[g];
+      if (tid == 0) { sgrp.L = &src; sgrp.poff = poff; sgrp.ngrp = ngrp; sgrp.gv = gv; }
       __syncthreads();
-      prox_rootfind<false>(p, src, a, b, tau, Delta, sh, rs);
+      rs.alpha = aw; rs.beta = bw; rs.amode = amode_w;
+      prox_rootfind<false>(p, sgrp, a, b, tau, Delta, sh, rs);
     }
     double mv_l = 0.0;
     for (int g = 0; g < G; ++g) mv_l = fmax(mv_l, fabs(lamS[g] - lamW[g]));
@@ -603,7 +722,7 @@ __global__ void __launch_bounds__(ROOT_NT, 3) k_prox_root(const __grid_constant_
       const int nl = src.cnt[0];
       if (nl < 256) Ws = fmax(Ws, nl < 64 ? 2.0 * W : W);
       if (p.iter < 2) Ws = INFINITY;
-      p.ap.win[a] = Ws; p.ap.wins[a] = Ws;
+      p.ap.win[a] = p.iter < 2 ? INFINITY : next_window(p, alpha, beta, mv); p.ap.wins[a] = Ws;
       if (finished) {                                    // H6: w_out already holds z
         p.ap.done[a] = 1; p.ap.iters[a] = p.iter;
         atomicAdd(&p.counters[0], 1);
