@@ -238,7 +238,8 @@ def main():
     prox_bytes_per_launch = PROX_BYTES_PER_ELEM * elem_iters / max(prox["launches"], 1)
     prox_ms_per_launch = prox["ms"] / max(prox["launches"], 1)
     achieved = prox_bytes_per_launch / (prox_ms_per_launch * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "kernel": "k_prox (H4 fused prox/projection + rhs assembly)", "achieved": achieved, "peak": peak,
+    roofline = {"bound": "hbm", "kernel": "k_prox_stream (H4/H5 fused projection + rhs assembly + residual terms, streaming pass)",
+                "achieved": achieved, "peak": peak,
                 "unit": "GB/s", "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
                 "bytes_per_launch": prox_bytes_per_launch, "ms_per_launch": prox_ms_per_launch,
                 "dominant_by_time": dom,

@@ -184,10 +184,12 @@ int prism_solve_batch_host(prism_problem* p, const prism_settings* s, void* cuda
                            const double* w0_host, double* w_host, int32_t* status_host, int32_t* iters_host,
                            double* resid_host, prism_solve_info* info);
 
-/* Kernel classes of the hot path: H4/H5/H6/H7 fused prox, H1 GEMM-1, H2 small solve + band
- * block, H3 GEMM-2 + epilogue, H0/H7 capacitance factorisation, H8/H9 diagnostics, everything else. */
+/* Kernel classes of the hot path: H4/H5 fused prox (the streaming pass k_prox_stream where it
+ * applies, else the every-asset kernel), H1 GEMM-1, H2 small solve, H3 GEMM-2 + epilogue, H0/H7 capacitance
+ * factorisation, H8/H9 diagnostics, everything else, and H4/H6/H7 per-account root find / convergence mask /
+ * rho adaptation of the streaming form (k_prox_root). */
 enum { PRISM_K_PROX = 0, PRISM_K_GEMM1 = 1, PRISM_K_SOLVE = 2, PRISM_K_GEMM2 = 3, PRISM_K_FACTOR = 4, PRISM_K_DIAG = 5,
-       PRISM_K_OTHER = 6, PRISM_K_PROX_SLOW = 7, PRISM_NKERN = 8 };
+       PRISM_K_OTHER = 6, PRISM_K_PROX_ROOT = 7, PRISM_NKERN = 8 };
 
 /* Device time (ms, CUDA events on the solve stream) and launch count per kernel class of the last
  * prism_solve_batch call that ran with settings.profile = 1.  ms_out, launches_out: host arrays of PRISM_NKERN. */

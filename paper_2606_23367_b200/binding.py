@@ -199,7 +199,7 @@ class Problem:
                                            iters.data_ptr(), resid.data_ptr(), duals.data_ptr(), C.byref(info)))
         return SolveResult(w, status, iters, resid, duals, self._info(info))
 
-    KERNELS = ["prox", "gemm1", "solve", "gemm2", "factor", "diag", "other", "prox_slow"]
+    KERNELS = ["prox", "gemm1", "solve", "gemm2", "factor", "diag", "other", "prox_root"]
 
     def kernel_times(self) -> dict:
         ms = (C.c_double * 8)(); cnt = (C.c_int64 * 8)()

@@ -116,7 +116,7 @@ __global__ void k_gemm1_ref(Gemm1Args p, int kp) {
 // ------------------------------------------------------------------------------------------------ GEMM-2
 enum { G2_ADMM = 0, G2_ADMM_CHECK = 1, G2_SIGMA = 2 };
 #define G2_TM 64     // accounts per CTA
-#define G2_TN 128    // assets per CTA
+#define G2_TN 64     // assets per CTA
 
 struct Gemm2Args {
   const double* Bp; int32_t kp;
@@ -153,8 +153,12 @@ __device__ __forceinline__ void g2_epilogue(const Gemm2Args& p, int a, int64_t i
   }
 }
 
+// Tile: 64 accounts x 64 assets per CTA, K = kp.  Warp w owns accounts a0 + 8 w .. + 7 and walks the 64 assets in two
+// column groups of 32; the epilogue operands of a group (v, c pairs) are requested BEFORE the group's DMMA loop so
+// that their latency overlaps the tensor work, and every access is a 16-byte pair.  61 KB of shared memory and
+// <= 85 registers: three CTAs per SM.
 template <int MT, int MODE>
-__global__ void __launch_bounds__(256) k_gemm2(Gemm2Args p) {
+__global__ void __launch_bounds__(256, 3) k_gemm2(Gemm2Args p) {
   extern __shared__ __align__(16) double smem[];
   constexpr int KP = 8 * MT, LD = KP + 4;
   double* Vs = smem;                       // [TM][LD]
@@ -178,29 +182,77 @@ __global__ void __launch_bounds__(256) k_gemm2(Gemm2Args p) {
     cp_async16(Bs + r * LD + cc, p.Bp + i * KP + cc);
   }
   cp_async_commit();
+  const int fr = lane >> 2, fc = lane & 3;
+  const int a = a0 + warp * 8 + fr;
+  const bool arow = a < p.A && !(p.done && p.done[a]);
+  const bool fastep = MODE != G2_SIGMA && !p.G;          // pair-wise epilogue (the rows are padded to 32: always in range)
+  double gsc = 0.0, gam = 0.0;
+  if (arow && MODE != G2_SIGMA) { gam = p.gamma[a]; gsc = 1.0 / (gam * (1.0 + p.c[a])); }
+  const int64_t rowp = (int64_t)a * p.ldw;
   cp_async_wait<0>();
   __syncthreads();
-  constexpr int NT = G2_TN / 8;
-  double acc[NT][2];
-#pragma unroll
-  for (int n = 0; n < NT; ++n) acc[n][0] = acc[n][1] = 0.0;
-  const int fr = lane >> 2, fc = lane & 3;
   const double* vs = Vs + (warp * 8 + fr) * LD;
+#pragma unroll 1
+  for (int cg = 0; cg < G2_TN / 32; ++cg) {
+    // D[a][i = ib + 8 n + 2 fc + {0,1}], n = 0..3
+    const int64_t ib = i0 + cg * 32 + fc * 2;
+    double2 v2[4], c2[4];
+    if (fastep && arow) {
+#pragma unroll
+      for (int n = 0; n < 4; ++n) {
+        if (ib + n * 8 < p.ldw) {
+          v2[n] = *(const double2*)(p.v + rowp + ib + n * 8);
+          c2[n] = *(const double2*)(p.cc + rowp + ib + n * 8);
+        }
+      }
+    }
+    double acc[4][2];
+#pragma unroll
+    for (int n = 0; n < 4; ++n) acc[n][0] = acc[n][1] = 0.0;
+    const double* bs = Bs + (cg * 32 + fr) * LD + fc;
 #pragma unroll 2
-  for (int k0 = 0; k0 < KP; k0 += 4) {
-    const double av = vs[k0 + fc];
+    for (int k0 = 0; k0 < KP; k0 += 4) {
+      const double av = vs[k0 + fc];
 #pragma unroll
-    for (int n = 0; n < NT; ++n) dmma884(acc[n][0], acc[n][1], av, Bs[(n * 8 + fr) * LD + k0 + fc]);
-  }
-  // D[a = a0 + 8 warp + lane/4][i = i0 + 8 n + 2 (lane%4) + {0,1}]
-  const int a = a0 + warp * 8 + fr;
-  if (a >= p.A || (p.done && p.done[a])) return;
+      for (int n = 0; n < 4; ++n) dmma884(acc[n][0], acc[n][1], av, bs[n * 8 * LD + k0]);
+    }
+    if (!arow) continue;
+    if (fastep) {
 #pragma unroll
-  for (int n = 0; n < NT; ++n) {
+      for (int n = 0; n < 4; ++n) {
+        const int64_t i = ib + n * 8;
+        if (i >= p.ldw) continue;
+        const double2 iv = *(const double2*)(p.invd + i);                   // (invd is padded with zeros to ldw)
+        const double s0 = acc[n][0] * iv.x * gsc, s1 = acc[n][1] * iv.y * gsc;
+        double2 vn;
+        vn.x = v2[n].x + p.relax * (c2[n].x - s0);
+        vn.y = v2[n].y + p.relax * (c2[n].y - s1);
+        const bool in0 = i < p.N, in1 = i + 1 < p.N;
+        if (in1) *(double2*)(p.v + rowp + i) = vn; else if (in0) p.v[rowp + i] = vn.x;
+        if (MODE == G2_ADMM_CHECK) {
+          const double2 rt2 = *(const double2*)(p.rt + rowp + i);
+          const double x0 = rt2.x - s0, x1 = rt2.y - s1;
+          if (in0) {
+            const double q0 = p.q ? p.q[rowp + i] : -p.mu[(int64_t)a * p.N + i];
+            p.xs[rowp + i] = x0;
+            p.pxq[rowp + i] = acc[n][0] + gam * p.d[i] * x0 + q0;
+          }
+          if (in1) {
+            const double q1 = p.q ? p.q[rowp + i + 1] : -p.mu[(int64_t)a * p.N + i + 1];
+            p.xs[rowp + i + 1] = x1;
+            p.pxq[rowp + i + 1] = acc[n][1] + gam * p.d[i + 1] * x1 + q1;
+          }
+        }
+      }
+    } else {
 #pragma unroll
-    for (int h = 0; h < 2; ++h) {
-      const int64_t i = i0 + n * 8 + fc * 2 + h;
-      if (i < p.N) g2_epilogue<MODE>(p, a, i, acc[n][h]);
+      for (int n = 0; n < 4; ++n) {
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+          const int64_t i = ib + n * 8 + h;
+          if (i < p.N) g2_epilogue<MODE>(p, a, i, acc[n][h]);
+        }
+      }
     }
   }
 }

@@ -12,7 +12,7 @@
 #include "prox_fast.cuh"
 #include "small.cuh"
 
-#define PRISM_VERSION_STR "prism-b200 r1 (sm_100a, fp64 DMMA factor GEMMs, two-threshold prox)"
+#define PRISM_VERSION_STR "prism-b200 r1 (sm_100a, fp64 DMMA factor GEMMs, streaming two-threshold prox with TMA bulk-copy pipeline)"
 
 static const int kMT[] = {2, 4, 7, 8, 13, 16};
 static int pick_mt(int k) {
@@ -219,7 +219,7 @@ extern "C" int prism_problem_create(int64_t N, int32_t k, int32_t accounts, cons
   const size_t AN = (size_t)A * p->ldn;
   ALLOC_TRY(dev_alloc(p, &p->Bp, (size_t)N * p->kp));
   ALLOC_TRY(dev_alloc(p, &p->Bt, (size_t)p->kp * p->ldn));
-  ALLOC_TRY(dev_alloc(p, &p->invd, (size_t)N));
+  ALLOC_TRY(dev_alloc(p, &p->invd, (size_t)p->ldn));       // padded with zeros (pair-wise GEMM-2 epilogue)
   ALLOC_TRY(dev_alloc(p, &p->gram, (size_t)p->Kp * p->Kp));
   ALLOC_TRY(dev_alloc(p, &p->v, AN));
   ALLOC_TRY(dev_alloc(p, &p->rt, AN));
@@ -334,7 +334,7 @@ static void launch_prox(Launcher& L, ProxArgs& a, int mode, int iter) {
     if (chk) k_prox_stream<true><<<grid, FAST_NW * 32, sm, st>>>(a);
     else k_prox_stream<false><<<grid, FAST_NW * 32, sm, st>>>(a);
     L.end();
-    L.begin(PRISM_K_PROX_SLOW);
+    L.begin(PRISM_K_PROX_ROOT);
     if (chk) k_prox_root<true><<<p->A, ROOT_NT, smr, st>>>(a, mode & ~PROX_CHECK);
     else k_prox_root<false><<<p->A, ROOT_NT, smr, st>>>(a, mode);
     L.end();
@@ -432,7 +432,7 @@ extern "C" int prism_solve_batch(prism_problem* p, const prism_settings* sp, voi
     }
     L.gemm1(p->rt, p->ap.done);
     L.begin(PRISM_K_SOLVE);
-    k_solve<<<A, 128, 0, st>>>(sa);
+    k_solve<<<A, 256, 0, st>>>(sa);
     L.end();
     const bool next_check = (it % s.check_every == 0);
     if (next_check) L.gemm2<G2_ADMM_CHECK>(g2); else L.gemm2<G2_ADMM>(g2);

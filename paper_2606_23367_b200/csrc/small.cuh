@@ -122,27 +122,44 @@ struct SolveArgs {
   double *V;
   AccountParams ap;
 };
-__global__ void __launch_bounds__(128) k_solve(SolveArgs p) {
+// 256 threads.  (1) T = sum of the split-K partials: four threads per entry, each over a quarter of the chunks with all
+// its loads in flight, combined in a fixed order (deterministic).  (2) V = S^-1 T: one warp per row group, a row of
+// the (symmetric) inverse read coalesced by the lanes, warp-shuffle reduction: one round of global-load latency.
+__global__ void __launch_bounds__(256) k_solve(SolveArgs p) {
   __shared__ double T[PRISM_MAX_KPRIME];
+  __shared__ double Tq[4][PRISM_MAX_KPRIME];
   const int a = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   if (p.ap.done[a]) return;
   const int Kp = p.kp;
-  for (int j = tid; j < Kp; j += blockDim.x) {
-    double s = 0.0;
-#pragma unroll 8
-    for (int ch = 0; ch < p.nchunk; ++ch) s += p.Tpart[((int64_t)ch * p.A + a) * p.ldv + j];   // fixed order => deterministic
-    T[j] = s;
+  {
+    const int part = tid >> 6, nper = (p.nchunk + 3) >> 2;
+    const int c0 = part * nper, c1 = min(p.nchunk, c0 + nper);
+    for (int j = tid & 63; j < Kp; j += 64) {
+      double s = 0.0;
+#pragma unroll 4
+      for (int ch = c0; ch < c1; ++ch) s += p.Tpart[((int64_t)ch * p.A + a) * p.ldv + j];
+      Tq[part][j] = s;
+    }
   }
   __syncthreads();
-  // S^-1 is symmetric: thread r walks column r (coalesced across threads, independent loads, no shuffles)
+  for (int j = tid; j < Kp; j += 256) T[j] = ((Tq[0][j] + Tq[1][j]) + Tq[2][j]) + Tq[3][j];
+  __syncthreads();
   const double* Si = p.Sinv + (int64_t)a * Kp * Kp;
-  for (int r = tid; r < Kp; r += blockDim.x) {
-    double s = 0.0;
-#pragma unroll 8
-    for (int c = 0; c < Kp; ++c) s = fma(Si[(int64_t)c * Kp + r], T[c], s);
-    p.V[(int64_t)a * p.ldv + r] = s;
+  for (int r0 = warp; r0 < Kp; r0 += 32) {               // rows r0, r0 + 8, r0 + 16, r0 + 24 of this warp together
+    double acc[4] = {0.0, 0.0, 0.0, 0.0};
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int r = r0 + 8 * u;
+      if (r < Kp)
+        for (int c = lane; c < Kp; c += 32) acc[u] = fma(Si[(int64_t)r * Kp + c], T[c], acc[u]);
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const double v = warp_sum(acc[u]);
+      const int r = r0 + 8 * u;
+      if (lane == 0 && r < Kp) p.V[(int64_t)a * p.ldv + r] = v;
+    }
   }
-  (void)lane; (void)warp;
 }
 
 // V[a][j] = gamma_a f_j * sum_ch Tpart[ch][a][j]   (Sigma-apply: B (F (B'x)) via GEMM-1 then GEMM-2)
