@@ -612,8 +612,10 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
       if (amode == 1) {
         const double M11 = -sP + sA, M12 = sAB, M21 = -sAB, M22 = sR - sB, r1 = -FA + rA, r2 = -FB - rB;
         const double det = M11 * M22 - M12 * M21;
-        if (!(fabs(det) > 1e-300)) { why = 2; break; }
-        dal = (r1 * M22 - M12 * r2) / det; dbe = (M11 * r2 - M21 * r1) / det;
+        if (fabs(det) > 1e-300) { dal = (r1 * M22 - M12 * r2) / det; dbe = (M11 * r2 - M21 * r1) / det; }
+        else if (fabs(r1) <= tol && fabs(M11) <= 1e-300 && fabs(M22) > 1e-300) { dal = 0.0; dbe = r2 / M22; }   // buy side flat and satisfied
+        else if (fabs(r2) <= tol && fabs(M22) <= 1e-300 && fabs(M11) > 1e-300) { dbe = 0.0; dal = r1 / M11; }   // sell side flat and satisfied
+        else { why = 2; break; }
       } else {
         const double den = (sP + sR) - sT;
         if (!(den > 1e-300)) { why = 3; break; }
@@ -641,11 +643,13 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
     else {
       if (p.stats && tid == 0 && p.iter < 4096) { atomicAdd(&p.stats[p.iter * 8 + 3], 1); atomicAdd(&p.stats[(2048 + p.iter) * 8 + why], 1); }
       // nested robust solver on the same grouped list (lean passes through the SrcGrouped overloads)
+      // (it continues from where the Newton iteration stopped when that state is usable)
+      const bool keep = al == al && be == be && fabs(al - aw) <= 0.5 * W && fabs(be - bw) <= 0.5 * W;
       __syncthreads();
-      for (int g = tid; g < G; g += nt) lamS[g] = lamW[g];
+      if (!keep) for (int g = tid; g < G; g += nt) lamS[g] = lamW[g];
       if (tid == 0) { sgrp.L = &src; sgrp.poff = poff; sgrp.ngrp = ngrp; sgrp.gv = gv; }
       __syncthreads();
-      rs.alpha = aw; rs.beta = bw; rs.amode = amode_w;
+      rs.alpha = keep ? al : aw; rs.beta = keep ? be : bw; rs.amode = keep ? amode : amode_w;
       prox_rootfind<false>(p, sgrp, a, b, tau, Delta, sh, rs);
     }
     double mv_l = 0.0;
