@@ -26,6 +26,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 PROX_BYTES_PER_ELEM = 41.0      # v 8 + w0 8 + mu 8 + exclusion mask 1 read; r~ 8 + c 8 written (kernel table)
+PROX_CHECK_EXTRA_BYTES = 24.0   # check iterations: x 8 + (P x + q) 8 read, w_out 8 written (kernel table)
 
 
 def load_peaks():
@@ -235,7 +236,10 @@ def main():
     peak, peak_src = load_peaks()
     prox = kt["prox"]
     elem_iters = float(N) * float(rp.info["iters_total"])          # account-iterations x N: elements the prox launches processed
-    prox_bytes_per_launch = PROX_BYTES_PER_ELEM * elem_iters / max(prox["launches"], 1)
+    # check launches (every check_every-th iteration of an account) also read x and P x + q and write w_out: + 24 B
+    it_prof = rp.iters.cpu().numpy().astype(np.int64)
+    check_elems = float(N) * float((it_prof // int(prof.check_every)).sum())
+    prox_bytes_per_launch = (PROX_BYTES_PER_ELEM * elem_iters + PROX_CHECK_EXTRA_BYTES * check_elems) / max(prox["launches"], 1)
     prox_ms_per_launch = prox["ms"] / max(prox["launches"], 1)
     achieved = prox_bytes_per_launch / (prox_ms_per_launch * 1e-3) / 1e9
     roofline = {"bound": "hbm", "kernel": "k_prox_stream (H4/H5 fused projection + rhs assembly + residual terms, streaming pass)",

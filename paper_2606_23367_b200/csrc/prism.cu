@@ -250,7 +250,7 @@ extern "C" int prism_problem_create(int64_t N, int32_t k, int32_t accounts, cons
   p->fast = fast_applicable(p) ? 1 : 0;
   if (p->fast) {
     // slices: a few CTAs per resident slot so that the streaming kernel stays bandwidth-bound to the end of the grid
-    int64_t target = ((int64_t)8 * 3 * p->sm_count + A - 1) / A;           // CTAs per account wanted
+    int64_t target = ((int64_t)4 * 3 * p->sm_count + A - 1) / A;           // CTAs per account wanted
     int64_t sl = (N + target - 1) / target;
     sl = (sl + FAST_CH - 1) / FAST_CH * FAST_CH;
     if (const char* e = getenv("PRISM_PROX_SLICE")) sl = (atoll(e) + FAST_CH - 1) / FAST_CH * FAST_CH;

@@ -28,6 +28,7 @@ struct __align__(16) LiveEnt { double T, w0, ir; uint32_t meta, pad; };   // one
 #define FAST_NST 3           // stages of the bulk-copy pipeline
 #define FAST_STAGE_BYTES (5 * FAST_CH * 8 + 2 * FAST_CH)
 #define ROOT_NT 128          // threads of a root CTA
+#define ROOT_SCAP 512         // a sorted list up to this length is kept in shared memory (no global-load latency per pass)
 
 __host__ __device__ inline size_t stream_smem_bytes(int G) {
   return (size_t)FAST_NST * FAST_STAGE_BYTES + 2 * FAST_NST * 8 + (size_t)(G > 0 ? G : 1) * 8 + 8 * 32 * 8 + 16;
@@ -68,7 +69,6 @@ __global__ void __launch_bounds__(FAST_NW * 32, 3) k_prox_stream(const __grid_co
   const int G = p.G, Gb = G > 0 ? G : 1;
   const int64_t N = p.N, row = (int64_t)a * N, rowp = (int64_t)a * p.ldw;
   const int sub = (a * p.S + sl) * FAST_NW + wid;               // this warp's list
-  const double W = p.ap.wins[a];
   const double lo_a = p.lo[a], hi_a = p.hi[a];
   if (!(hi_a - lo_a <= 4.0)) {            // box wider than the fixed-point range of the bins: generic path in k_prox_root
     if (tid == 0 && sl == 0) p.lflag[a] = 1;
@@ -80,20 +80,6 @@ __global__ void __launch_bounds__(FAST_NW * 32, 3) k_prox_stream(const __grid_co
   uint64_t* bar_empty = bar_full + FAST_NST;
   double* lamS = (double*)(bar_empty + FAST_NST);
   double* scratch = lamS + Gb;                                        // 8 * 32 (CHECK reduction)
-
-  const double gam = p.gamma[a], c = p.ap.c[a], cg = c * gam, icg = 1.0 / cg;
-  const double kappa = p.kappa ? p.kappa[a] : 0.0;
-  const double lam_b = kappa + (p.c_buy ? p.c_buy[a] : 0.0), Delta = lam_b + kappa;
-  const double tau = p.tau ? p.tau[a] : INFINITY;
-  const double igc = 1.0 / (gam * (1.0 + c));
-  double aw = p.ap.alpha[a], bw = p.ap.beta[a];
-  if (!(p.ap.mode[a] == 1 && isfinite(tau))) bw = aw;
-  for (int g = tid; g < G; g += blockDim.x) lamS[g] = p.lamG[(int64_t)a * G + g];
-  if (tid == 0) {
-    for (int st = 0; st < FAST_NST; ++st) { mbar_init(&bar_full[st], 1); mbar_init(&bar_empty[st], FAST_NW); }
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-  }
-  __syncthreads();
 
   const int64_t i_beg = (int64_t)sl * p.slice_len, i_end = min(N, i_beg + p.slice_len);
   const int nchunk = (int)((i_end - i_beg + FAST_CH - 1) / FAST_CH);
@@ -114,6 +100,22 @@ __global__ void __launch_bounds__(FAST_NW * 32, 3) k_prox_stream(const __grid_co
     if (p.excl) bulk_g2s(sb + 5 * FAST_CH * 8, p.excl + row + i0, nc, &bar_full[st]);
     if (G) bulk_g2s(sb + 5 * FAST_CH * 8 + FAST_CH, p.group_id + i0, nc, &bar_full[st]);
   };
+  // the first copies start before anything else is read: the account's constants load while they are in flight
+  if (tid == 0) {
+    for (int st = 0; st < FAST_NST; ++st) { mbar_init(&bar_full[st], 1); mbar_init(&bar_empty[st], FAST_NW); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    for (int c = 0; c < FAST_NST - 1 && c < nchunk; ++c) issue(c);
+  }
+  const double W = p.ap.wins[a];
+  const double gam = p.gamma[a], c = p.ap.c[a], cg = c * gam, icg = 1.0 / cg;
+  const double kappa = p.kappa ? p.kappa[a] : 0.0;
+  const double lam_b = kappa + (p.c_buy ? p.c_buy[a] : 0.0), Delta = lam_b + kappa;
+  const double tau = p.tau ? p.tau[a] : INFINITY;
+  const double igc = 1.0 / (gam * (1.0 + c));
+  double aw = p.ap.alpha[a], bw = p.ap.beta[a];
+  if (!(p.ap.mode[a] == 1 && isfinite(tau))) bw = aw;
+  for (int g = tid; g < G; g += blockDim.x) lamS[g] = p.lamG[(int64_t)a * G + g];
+  __syncthreads();
 
   double nx = 0, nz = 0, nrp = 0, nrd = 0, nPx = 0, ny = 0, nq = 0;
   LiveEnt* mylist = p.lraw + (int64_t)sub * p.capw;
@@ -121,8 +123,6 @@ __global__ void __launch_bounds__(FAST_NW * 32, 3) k_prox_stream(const __grid_co
   const unsigned lt = (1u << lane) - 1u;
   int n = 0;
   const double aW_lo = aw - W, aW_hi = aw + W, bW_lo = bw - W - Delta, bW_hi = bw + W - Delta;
-  if (tid == 0)
-    for (int c = 0; c < FAST_NST - 1 && c < nchunk; ++c) issue(c);
   double* rtp = p.rt + rowp + i_beg + tid;
   double* ccp = p.cc + rowp + i_beg + tid;
   for (int c = 0; c < nchunk; ++c) {
@@ -244,7 +244,7 @@ struct SrcLiveG {
       for (; j + 3 * nt < n; j += 4 * nt) {
         double2 a[4], b[4];
 #pragma unroll
-        for (int u = 0; u < 4; ++u) { a[u] = __ldg((const double2*)(el + j + u * nt)); b[u] = __ldg((const double2*)(el + j + u * nt) + 1); }
+        for (int u = 0; u < 4; ++u) { a[u] = *((const double2*)(el + j + u * nt)); b[u] = *((const double2*)(el + j + u * nt) + 1); }
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
           ElemConst e; int g;
@@ -253,7 +253,7 @@ struct SrcLiveG {
         }
       }
       for (; j < n; j += nt) {
-        const double2 a = __ldg((const double2*)(el + j)), b = __ldg((const double2*)(el + j) + 1);
+        const double2 a = *((const double2*)(el + j)), b = *((const double2*)(el + j) + 1);
         ElemConst e; int g;
         const int64_t i = decode(a, b, e, g);
         f(i, e, g, 0, (const double*)nullptr, (const double*)nullptr);
@@ -270,7 +270,7 @@ struct SrcLiveG {
         const bool valid = j < n;
         ElemConst e; int g = 0; int64_t i = 0;
         if (valid) {
-          const double2 a = __ldg((const double2*)(el + j)), b = __ldg((const double2*)(el + j) + 1);
+          const double2 a = *((const double2*)(el + j)), b = *((const double2*)(el + j) + 1);
           i = decode(a, b, e, g);
         }
         f(valid, i, e, g, 0, (const double*)nullptr, (const double*)nullptr);
@@ -281,7 +281,7 @@ struct SrcLiveG {
 
 __host__ __device__ inline size_t root_smem_bytes(int G, int nsub) {
   const int Gb = G > 0 ? G : 1;
-  return (size_t)(16 * 32 + 4 * Gb + 6 * Gb + 2 * Gb + 8 + 4 * (Gb + 4)) * 8 + (size_t)(nsub + 1 + 4 * Gb + 3 * Gb + 16 + ROOT_NSL) * 4 + 16;
+  return (size_t)(16 * 32 + 4 * Gb + 6 * Gb + 6 * Gb + 8 + 4 * (Gb + 4)) * 8 + (size_t)(nsub + 1 + 4 * Gb + 3 * Gb + 16 + ROOT_NSL) * 4 + 32 + (size_t)ROOT_SCAP * 32;
 }
 
 // One pass over the grouped list: per (pseudo-)group q the buys, sells and their slopes at thresholds (al, bd + Delta)
@@ -316,12 +316,12 @@ __device__ __forceinline__ void root_pass(const SrcLiveG& src, const int* poff, 
     for (; j + 96 < j1; j += 128) {
       double2 ea[4], eb[4];
 #pragma unroll
-      for (int u = 0; u < 4; ++u) { ea[u] = __ldg((const double2*)(src.ent + j + 32 * u)); eb[u] = __ldg((const double2*)(src.ent + j + 32 * u) + 1); }
+      for (int u = 0; u < 4; ++u) { ea[u] = *((const double2*)(src.ent + j + 32 * u)); eb[u] = *((const double2*)(src.ent + j + 32 * u) + 1); }
 #pragma unroll
       for (int u = 0; u < 4; ++u) root_entry(src, ea[u], eb[u], a0, b0, sp, sr, slp, slr);
     }
     for (; j < j1; j += 32) {
-      const double2 ea = __ldg((const double2*)(src.ent + j)), eb = __ldg((const double2*)(src.ent + j) + 1);
+      const double2 ea = *((const double2*)(src.ent + j)), eb = *((const double2*)(src.ent + j) + 1);
       root_entry(src, ea, eb, a0, b0, sp, sr, slp, slr);
     }
     sp = warp_sum(sp); sr = warp_sum(sr); slp = warp_sum(slp); slr = warp_sum(slr);
@@ -379,7 +379,7 @@ __device__ __noinline__ void prox_eval_multi(const SrcGrouped& s, const double* 
   for (int k = 0; k < PROX_KSEC; ++k) { sp[k] = 0.0; sr[k] = 0.0; }
   const int n = L.cnt[0];
   for (int j = threadIdx.x; j < n; j += blockDim.x) {
-    const double2 ea = __ldg((const double2*)(L.ent + j)), eb = __ldg((const double2*)(L.ent + j) + 1);
+    const double2 ea = *((const double2*)(L.ent + j)), eb = *((const double2*)(L.ent + j) + 1);
     const uint32_t m = (uint32_t)__double_as_longlong(eb.y);
     const double lg = G ? lamS[(m >> PROX_META_IDX_BITS) & 0xffu] : 0.0;
     if ((m >> 30) == 0) {
@@ -428,6 +428,8 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
   double* gsum = d0; d0 += Gb;
   double* band_lo = d0; double* band_hi = d0 + Gb; double* gw0 = d0 + 2 * Gb; double* lamW = d0 + 3 * Gb; d0 += 4 * Gb;
   unsigned long long* cbin = (unsigned long long*)d0; d0 += 2 * Gb;    // dead assets of the streaming pass
+  unsigned long long* fbin = (unsigned long long*)d0; d0 += 2 * Gb;    // + list entries outside the tight window
+  unsigned long long* ubin = (unsigned long long*)d0; d0 += 2 * Gb;    // their sum: what the solve uses
   double* chk = d0; d0 += 8;
   double* gv = d0; d0 += 4 * (Gb + 4);                   // per (pseudo-)group sums of one pass
   int* offs = (int*)d0;                                  // nsub + 1: start of raw list k in the sequence of all lists
@@ -436,13 +438,15 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
   int* poff = goff + Gb + 1;                             // ngrp + 1 (pseudo-)group offsets used by the passes
   int* act = poff + Gb + 5;                              // Gb: band state -1 lower active, 0 inactive, +1 upper active
   int* selS = act + Gb;
+  LiveEnt* ents = (LiveEnt*)(((uintptr_t)(selS + 4) + 15) & ~(uintptr_t)15);   // ROOT_SCAP entries
 
   const double gam = p.gamma[a], c = p.ap.c[a], cg = c * gam;
   const double kappa = p.kappa ? p.kappa[a] : 0.0;
   const double lam_b = kappa + (p.c_buy ? p.c_buy[a] : 0.0), Delta = lam_b + kappa;
   const double tau = p.tau ? p.tau[a] : INFINITY;
   const double igc = 1.0 / (gam * (1.0 + c));
-  const double W = p.ap.wins[a];                         // window of the streaming pass
+  const double W = p.ap.wins[a], Wt = p.ap.win[a];       // window of the streaming pass; tight window (32 x last movement)
+  const double src_lo = p.lo[a], src_hi = p.hi[a];
   const double b = p.ap.bsum[a];
   double aw = p.ap.alpha[a], bw = p.ap.beta[a];
   int amode_w = p.ap.mode[a];
@@ -472,8 +476,7 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
   rs.nobands = bands_on ? 0 : 1;
   double mv = 0.0;
   if (!fallback) {
-    // ---- group sort (counting sort, stable in (list, position) order => deterministic): lists -> lcomp by group.
-    // The lists are taken as one sequence (offs = their start offsets); warp w handles a contiguous quarter of it.
+    // ---- the raw lists as one sequence (offs = their start offsets); warp w handles a contiguous quarter of it
     const unsigned lt = (1u << lane) - 1u;
     const LiveEnt* lr = p.lraw + (int64_t)a * nsub * p.capw;
     if (wid == 0) {                                      // inclusive scan of the list lengths
@@ -488,47 +491,84 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
       if (lane == 0) offs[0] = 0;
     }
     __syncthreads();
-    const int n = offs[nsub];
-    const int segw = (((n + nw - 1) / nw) + 31) & ~31;
-    const int j_beg = min(n, wid * segw), j_end = min(n, (wid + 1) * segw);
+    const int nraw = offs[nsub];
+    const int segw = (((nraw + nw - 1) / nw) + 31) & ~31;
+    const int j_beg = min(nraw, wid * segw), j_end = min(nraw, (wid + 1) * segw);
     auto locate = [&](int j) -> const LiveEnt* {         // entry j of the sequence
       int lo = 0, hi = nsub;
       while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (offs[mid] <= j) lo = mid; else hi = mid; }
       return lr + (int64_t)lo * p.capw + (j - offs[lo]);
     };
-    if (!G) { if (lane == 0) wcnt[wid] = j_end - j_beg; }
-    else
-      for (int j0 = j_beg; j0 < j_end; j0 += 32) {
-        const int j = j0 + lane;
-        const bool valid = j < j_end;
-        const int g = valid ? (int)((__ldg(&locate(j)->meta) >> PROX_META_IDX_BITS) & 0xffu) : 0x100 + lane;
-        const unsigned m = __match_any_sync(0xffffffffu, g);
-        if (valid && lane == __ffs(m) - 1) wcnt[wid * Gb + g] += __popc(m);
-        __syncwarp();
+    // Is this entry dead for every threshold within Wf of the warm start?  (Then bc / sc are its constant amounts.)
+    auto tight_dead = [&](const double2& ea, const double2& eb, double Wf, double& bc, double& sc) -> bool {
+      const uint32_t m = (uint32_t)__double_as_longlong(eb.y);
+      if ((m >> 30) != 0) return false;                  // excluded with an odd w0 / outside its box: always kept
+      const double T = ea.x, w0 = ea.y, ir = eb.x, wB = src_hi - w0, wS = w0 - src_lo;
+      const double lg = (bands_on && G) ? lamW[(m >> PROX_META_IDX_BITS) & 0xffu] : 0.0;
+      bc = 0.0; sc = 0.0;
+      if (wB > 0.0) {
+        if ((T - (aw + lg - Wf)) * ir <= 0.0) bc = 0.0;
+        else if ((T - (aw + lg + Wf)) * ir >= wB) bc = wB;
+        else return false;
       }
-    __syncthreads();
-    for (int g = tid; g < Gb; g += nt) {                 // start of warp w's entries inside group g; group totals
-      int run = 0;
-      for (int w = 0; w < nw; ++w) { const int t = wcnt[w * Gb + g]; wcnt[w * Gb + g] = run; run += t; }
-      goff[g + 1] = run;
-    }
-    __syncthreads();
-    if (tid == 0) {
-      goff[0] = 0;
-      for (int g = 0; g < Gb; ++g) goff[g + 1] += goff[g];
-      if (G) for (int g = 0; g <= G; ++g) poff[g] = goff[g];
-      else for (int q = 0; q <= nw; ++q) poff[q] = (int)((int64_t)n * q / nw);
-      unsigned long long sp = 0ull, sr = 0ull;
-      for (int g = 0; g < Gb; ++g) { sp += cbin[g]; sr += cbin[Gb + g]; }
-      src.lo_a = p.lo[a]; src.hi_a = p.hi[a]; src.ent = p.lcomp + (int64_t)a * p.ldc; src.nsl = 1; src.stride = 0; src.cnt[0] = n;
-      src.cbin = cbin; src.Gb = Gb; src.cPt = (double)sp * PRISM_FIX_INV; src.cRt = (double)sr * PRISM_FIX_INV;
-      sh.scratch = scratch; sh.gbin = gbin; sh.lamS = lamS; sh.gsum = gsum; sh.selS = selS;
-      sh.band_lo = band_lo; sh.band_hi = band_hi; sh.gw0 = gw0;
-      p.lflag[a] = 0;
-    }
-    __syncthreads();
-    {
-      LiveEnt* dst = p.lcomp + (int64_t)a * p.ldc;
+      if (wS > 0.0) {
+        if (((bw + lg + Wf - Delta) - T) * ir <= 0.0) sc = 0.0;
+        else if (((bw + lg - Wf - Delta) - T) * ir >= wS) sc = wS;
+        else return false;
+      }
+      return true;
+    };
+    // ---- group sort (counting sort, stable in sequence order => deterministic): kept entries -> lcomp by group.
+    // With a finite Wf only the entries a TIGHT window around the warm start can reach are kept; the constant trades
+    // of the others go to fixed-point bins, exactly as in the streaming pass.
+    auto sort_lists = [&](double Wf) {
+      const bool filt = Wf < INFINITY;
+      for (int e = tid; e < 4 * Gb; e += nt) wcnt[e] = 0;
+      for (int g = tid; g < 2 * Gb; g += nt) fbin[g] = 0ull;
+      __syncthreads();
+      if (!G && !filt) { if (lane == 0) wcnt[wid] = j_end - j_beg; }
+      else
+        for (int j0 = j_beg; j0 < j_end; j0 += 32) {
+          const int j = j0 + lane;
+          const bool valid = j < j_end;
+          int g = 0x100 + lane;
+          if (valid) {
+            const LiveEnt* e = locate(j);
+            if (filt) {
+              const double2 ea = __ldg((const double2*)e), eb = __ldg((const double2*)e + 1);
+              const int ge = G ? (int)(((uint32_t)__double_as_longlong(eb.y) >> PROX_META_IDX_BITS) & 0xffu) : 0;
+              double bc, sc;
+              if (tight_dead(ea, eb, Wf, bc, sc)) {
+                if (bc > 0.0) atomicAdd(&fbin[ge], (unsigned long long)__double2ull_rn(bc * PRISM_FIX_SCALE));
+                if (sc > 0.0) atomicAdd(&fbin[Gb + ge], (unsigned long long)__double2ull_rn(sc * PRISM_FIX_SCALE));
+              } else g = ge;
+            } else g = (int)((__ldg(&e->meta) >> PROX_META_IDX_BITS) & 0xffu);
+          }
+          const unsigned m = __match_any_sync(0xffffffffu, g);
+          if (g < 0x100 && lane == __ffs(m) - 1) wcnt[wid * Gb + g] += __popc(m);
+          __syncwarp();
+        }
+      __syncthreads();
+      for (int g = tid; g < Gb; g += nt) {               // start of warp w's entries inside group g; group totals
+        int run = 0;
+        for (int w = 0; w < nw; ++w) { const int t = wcnt[w * Gb + g]; wcnt[w * Gb + g] = run; run += t; }
+        goff[g + 1] = run;
+      }
+      for (int g = tid; g < 2 * Gb; g += nt) ubin[g] = cbin[g] + fbin[g];
+      __syncthreads();
+      if (tid == 0) {
+        goff[0] = 0;
+        for (int g = 0; g < Gb; ++g) goff[g + 1] += goff[g];
+        const int n = goff[Gb];
+        if (G) for (int g = 0; g <= G; ++g) poff[g] = goff[g];
+        else for (int q = 0; q <= nw; ++q) poff[q] = (int)((int64_t)n * q / nw);
+        unsigned long long sp = 0ull, sr = 0ull;
+        for (int g = 0; g < Gb; ++g) { sp += ubin[g]; sr += ubin[Gb + g]; }
+        src.lo_a = src_lo; src.hi_a = src_hi; src.ent = n <= ROOT_SCAP ? ents : p.lcomp + (int64_t)a * p.ldc; src.nsl = 1; src.stride = 0; src.cnt[0] = n;
+        src.cbin = ubin; src.Gb = Gb; src.cPt = (double)sp * PRISM_FIX_INV; src.cRt = (double)sr * PRISM_FIX_INV;
+      }
+      __syncthreads();
+      LiveEnt* dst = const_cast<LiveEnt*>(src.ent);
       for (int j0 = j_beg; j0 < j_end; j0 += 32) {
         const int j = j0 + lane;
         const bool valid = j < j_end;
@@ -537,134 +577,159 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
         if (valid) {
           const LiveEnt* e = locate(j);
           ea = __ldg((const double2*)e); eb = __ldg((const double2*)e + 1);
-          g = G ? (int)(((uint32_t)__double_as_longlong(eb.y) >> PROX_META_IDX_BITS) & 0xffu) : 0;
+          double bc, sc;
+          if (!(filt && tight_dead(ea, eb, Wf, bc, sc)))
+            g = G ? (int)(((uint32_t)__double_as_longlong(eb.y) >> PROX_META_IDX_BITS) & 0xffu) : 0;
         }
         const unsigned m = __match_any_sync(0xffffffffu, g);
-        if (valid) {
+        if (g < 0x100) {
           double2* o = (double2*)(dst + goff[g] + wcnt[wid * Gb + g] + __popc(m & lt));
           o[0] = ea; o[1] = eb;
         }
         __syncwarp();
-        if (valid && lane == __ffs(m) - 1) wcnt[wid * Gb + g] += __popc(m);
+        if (g < 0x100 && lane == __ffs(m) - 1) wcnt[wid * Gb + g] += __popc(m);
         __syncwarp();
       }
+      __syncthreads();
+    };
+    if (tid == 0) {
+      sh.scratch = scratch; sh.gbin = gbin; sh.lamS = lamS; sh.gsum = gsum; sh.selS = selS;
+      sh.band_lo = band_lo; sh.band_hi = band_hi; sh.gw0 = gw0;
+      p.lflag[a] = 0;
     }
-    __syncthreads();
-
-    // ---- semismooth Newton on (alpha, beta, lambda_g of the active bands) jointly: one pass over the list per step.
-    // The equations are piecewise linear (see prox.cuh): P(alpha, lambda) = (tau + b)/2 and R(beta, lambda) = (tau - b)/2
-    // with the cap active, P - R = b with alpha = beta otherwise, and S_g = bound_g for every active band.  Eliminating
-    // d lambda_g = (F_g - sP_g d alpha - sR_g d beta) / (sP_g + sR_g) leaves a 2 x 2 system.  Bands enter the active set
-    // when violated and leave it when their multiplier changes sign.  Anything irregular (singular step, no convergence
-    // in 16 passes) falls back to the nested robust solver prox_rootfind on the same list.
-    const double tol = 2e-15 * fmax(1.0, fabs(b) + (isfinite(tau) ? tau : 0.0));
-    const double Pt = 0.5 * (tau + b), Rt = 0.5 * (tau - b);
-    const double cPt = src.cPt, cRt = src.cRt;
-    double al = aw, be = bw;
-    int amode = amode_w;
-    bool ok = false;
-    int why = 4;                                          // (debug) 1 singular band, 2 det, 3 den, 4 passes, 5 NaN
-    for (int g = tid; g < G; g += nt) act[g] = lamS[g] > 0.0 ? 1 : (lamS[g] < 0.0 ? -1 : 0);
-    __syncthreads();
-    for (int itn = 0; itn < 16; ++itn) {
-      root_pass(src, poff, ngrp, lamS, G, al, be - Delta, gv);
-      ++rs.n_eval;
-      // thread q: the terms of (pseudo-)group q; fixed-order block reduction (deterministic)
-      double P, R, sP, sR, sA, sB, sAB, rA, rB, sT, sF;
-      bool gconv, sing;
-      {
-        double v16[16];
-#pragma unroll
-        for (int q = 0; q < 16; ++q) v16[q] = 0.0;
-        if (tid < ngrp) { v16[0] = gv[4 * tid]; v16[1] = gv[4 * tid + 1]; v16[2] = gv[4 * tid + 2]; v16[3] = gv[4 * tid + 3]; }
-        if (tid < G) {
-          const int g = tid;
-          const double pa = v16[2], ra = v16[3], t = pa + ra;
-          const double Sg = gw0[g] + (v16[0] + (double)cbin[g] * PRISM_FIX_INV) - (v16[1] + (double)cbin[Gb + g] * PRISM_FIX_INV);
-          int ac = act[g];
-          if (ac == 0 && bands_on) {
-            if (Sg > band_hi[g] + 8.0 * tol) ac = 1; else if (Sg < band_lo[g] - 8.0 * tol) ac = -1;
-            if (ac) v16[11] = 1.0;
+    // A long list is first solved on its tight part; a solution that leaves the tight window repeats the solve on the
+    // whole list, and one that leaves the streaming pass's window sends the account to the generic path.
+    double Wf = (nraw > 512 && Wt < 0.125 * W) ? Wt : INFINITY;
+    for (int att = 0; att < 2; ++att) {
+      sort_lists(Wf);
+      rs.alpha = aw; rs.beta = bw; rs.amode = amode_w;
+      for (int g = tid; g < G; g += nt) lamS[g] = lamW[g];
+      __syncthreads();
+      // ---- semismooth Newton on (alpha, beta, lambda_g of the active bands) jointly: one pass over the list per step.
+      // The equations are piecewise linear (see prox.cuh): P(alpha, lambda) = (tau + b)/2 and R(beta, lambda) = (tau - b)/2
+      // with the cap active, P - R = b with alpha = beta otherwise, and S_g = bound_g for every active band.  Eliminating
+      // d lambda_g = (F_g - sP_g d alpha - sR_g d beta) / (sP_g + sR_g) leaves a 2 x 2 system.  Bands enter the active set
+      // when violated and leave it when their multiplier changes sign.  Anything irregular (singular step, no convergence
+      // in 16 passes) falls back to the nested robust solver prox_rootfind on the same list.
+      const double tol = 2e-15 * fmax(1.0, fabs(b) + (isfinite(tau) ? tau : 0.0));
+      const double Pt = 0.5 * (tau + b), Rt = 0.5 * (tau - b);
+      const double cPt = src.cPt, cRt = src.cRt;
+      double al = aw, be = bw;
+      int amode = amode_w;
+      bool ok = false;
+      int why = 4;                                          // (debug) 1 singular band, 2 det, 3 den, 4 passes, 5 NaN
+      for (int g = tid; g < G; g += nt) act[g] = lamS[g] > 0.0 ? 1 : (lamS[g] < 0.0 ? -1 : 0);
+      __syncthreads();
+      for (int itn = 0; itn < 16; ++itn) {
+        root_pass(src, poff, ngrp, lamS, G, al, be - Delta, gv);
+        ++rs.n_eval;
+        // thread q: the terms of (pseudo-)group q; fixed-order block reduction (deterministic)
+        double P, R, sP, sR, sA, sB, sAB, rA, rB, sT, sF;
+        bool gconv, sing;
+        {
+          double v16[16];
+  #pragma unroll
+          for (int q = 0; q < 16; ++q) v16[q] = 0.0;
+          if (tid < ngrp) { v16[0] = gv[4 * tid]; v16[1] = gv[4 * tid + 1]; v16[2] = gv[4 * tid + 2]; v16[3] = gv[4 * tid + 3]; }
+          if (tid < G) {
+            const int g = tid;
+            const double pa = v16[2], ra = v16[3], t = pa + ra;
+            const double Sg = gw0[g] + (v16[0] + (double)ubin[g] * PRISM_FIX_INV) - (v16[1] + (double)ubin[Gb + g] * PRISM_FIX_INV);
+            int ac = act[g];
+            if (ac == 0 && bands_on) {
+              if (Sg > band_hi[g] + 8.0 * tol) ac = 1; else if (Sg < band_lo[g] - 8.0 * tol) ac = -1;
+              if (ac) v16[11] = 1.0;
+            }
+            if (ac) {
+              const double Fg = Sg - (ac > 0 ? band_hi[g] : band_lo[g]);
+              if (fabs(Fg) > tol) v16[11] = 1.0;
+              if (t > 0.0) { v16[4] = pa * pa / t; v16[5] = ra * ra / t; v16[6] = pa * ra / t; v16[7] = pa * Fg / t; v16[8] = ra * Fg / t; v16[9] = t; v16[10] = Fg; }
+              else if (fabs(Fg) > tol) v16[12] = 1.0;
+            }
+            gsum[g] = Sg;
           }
-          if (ac) {
-            const double Fg = Sg - (ac > 0 ? band_hi[g] : band_lo[g]);
-            if (fabs(Fg) > tol) v16[11] = 1.0;
-            if (t > 0.0) { v16[4] = pa * pa / t; v16[5] = ra * ra / t; v16[6] = pa * ra / t; v16[7] = pa * Fg / t; v16[8] = ra * Fg / t; v16[9] = t; v16[10] = Fg; }
-            else if (fabs(Fg) > tol) v16[12] = 1.0;
-          }
-          gsum[g] = Sg;
+          block_reduce<16, 0>(v16, scratch);
+          P = cPt + v16[0]; R = cRt + v16[1]; sP = v16[2]; sR = v16[3];
+          sA = v16[4]; sB = v16[5]; sAB = v16[6]; rA = v16[7]; rB = v16[8]; sT = v16[9]; sF = v16[10];
+          gconv = !(v16[11] > 0.0); sing = v16[12] > 0.0;
         }
-        block_reduce<16, 0>(v16, scratch);
-        P = cPt + v16[0]; R = cRt + v16[1]; sP = v16[2]; sR = v16[3];
-        sA = v16[4]; sB = v16[5]; sAB = v16[6]; rA = v16[7]; rB = v16[8]; sT = v16[9]; sF = v16[10];
-        gconv = !(v16[11] > 0.0); sing = v16[12] > 0.0;
-      }
-      const double FA = amode == 1 ? P - Pt : P - R - b, FB = amode == 1 ? R - Rt : 0.0;
-      if (fabs(FA) <= tol && fabs(FB) <= tol && gconv) {
-        if (amode == 1) { if (al >= be) { ok = true; break; } amode = 0; al = be = 0.5 * (al + be); __syncthreads(); continue; }
-        if (!isfinite(tau) || P + R <= tau + tol) { ok = true; break; }
-        amode = 1; be = al;
+        const double FA = amode == 1 ? P - Pt : P - R - b, FB = amode == 1 ? R - Rt : 0.0;
+        if (fabs(FA) <= tol && fabs(FB) <= tol && gconv) {
+          if (amode == 1) { if (al >= be) { ok = true; break; } amode = 0; al = be = 0.5 * (al + be); __syncthreads(); continue; }
+          if (!isfinite(tau) || P + R <= tau + tol) { ok = true; break; }
+          amode = 1; be = al;
+          __syncthreads();
+          continue;
+        }
+        if (sing) { why = 1; break; }
+        double dal, dbe;
+        if (amode == 1) {
+          const double M11 = -sP + sA, M12 = sAB, M21 = -sAB, M22 = sR - sB, r1 = -FA + rA, r2 = -FB - rB;
+          const double det = M11 * M22 - M12 * M21;
+          if (fabs(det) > 1e-300) { dal = (r1 * M22 - M12 * r2) / det; dbe = (M11 * r2 - M21 * r1) / det; }
+          else if (fabs(r1) <= tol && fabs(M11) <= 1e-300 && fabs(M22) > 1e-300) { dal = 0.0; dbe = r2 / M22; }   // buy side flat and satisfied
+          else if (fabs(r2) <= tol && fabs(M22) <= 1e-300 && fabs(M11) > 1e-300) { dbe = 0.0; dal = r1 / M11; }   // sell side flat and satisfied
+          else { why = 2; break; }
+        } else {
+          const double den = (sP + sR) - sT;
+          if (!(den > 1e-300)) { why = 3; break; }
+          dal = dbe = (FA - sF) / den;
+        }
+        if (!(dal == dal) || !(dbe == dbe)) { why = 5; break; }
         __syncthreads();
-        continue;
-      }
-      if (sing) { why = 1; break; }
-      double dal, dbe;
-      if (amode == 1) {
-        const double M11 = -sP + sA, M12 = sAB, M21 = -sAB, M22 = sR - sB, r1 = -FA + rA, r2 = -FB - rB;
-        const double det = M11 * M22 - M12 * M21;
-        if (fabs(det) > 1e-300) { dal = (r1 * M22 - M12 * r2) / det; dbe = (M11 * r2 - M21 * r1) / det; }
-        else if (fabs(r1) <= tol && fabs(M11) <= 1e-300 && fabs(M22) > 1e-300) { dal = 0.0; dbe = r2 / M22; }   // buy side flat and satisfied
-        else if (fabs(r2) <= tol && fabs(M22) <= 1e-300 && fabs(M11) > 1e-300) { dbe = 0.0; dal = r1 / M11; }   // sell side flat and satisfied
-        else { why = 2; break; }
-      } else {
-        const double den = (sP + sR) - sT;
-        if (!(den > 1e-300)) { why = 3; break; }
-        dal = dbe = (FA - sF) / den;
-      }
-      if (!(dal == dal) || !(dbe == dbe)) { why = 5; break; }
-      __syncthreads();
-      for (int g = tid; g < G; g += nt) {                // multipliers and active set (thread g owns band g)
-        const double pa = gv[4 * g + 2], ra = gv[4 * g + 3], t = pa + ra;
-        int ac = act[g];
-        const bool was = ac != 0;
-        if (!was && bands_on) { if (gsum[g] > band_hi[g] + 8.0 * tol) ac = 1; else if (gsum[g] < band_lo[g] - 8.0 * tol) ac = -1; }
-        if (ac && t > 0.0) {
-          const double Fg = gsum[g] - (ac > 0 ? band_hi[g] : band_lo[g]);
-          double ln = lamS[g] + (Fg - pa * dal - ra * dbe) / t;
-          if (!(ln * ac > 0.0)) { ln = 0.0; ac = 0; }     // the multiplier would change sign: the band goes inactive
-          lamS[g] = ln;
+        for (int g = tid; g < G; g += nt) {                // multipliers and active set (thread g owns band g)
+          const double pa = gv[4 * g + 2], ra = gv[4 * g + 3], t = pa + ra;
+          int ac = act[g];
+          const bool was = ac != 0;
+          if (!was && bands_on) { if (gsum[g] > band_hi[g] + 8.0 * tol) ac = 1; else if (gsum[g] < band_lo[g] - 8.0 * tol) ac = -1; }
+          if (ac && t > 0.0) {
+            const double Fg = gsum[g] - (ac > 0 ? band_hi[g] : band_lo[g]);
+            double ln = lamS[g] + (Fg - pa * dal - ra * dbe) / t;
+            if (!(ln * ac > 0.0)) { ln = 0.0; ac = 0; }     // the multiplier would change sign: the band goes inactive
+            lamS[g] = ln;
+          }
+          act[g] = ac;
         }
-        act[g] = ac;
+        al += dal; be += dbe;
+        __syncthreads();
       }
-      al += dal; be += dbe;
+      if (ok) { rs.alpha = al; rs.beta = be; rs.amode = amode; }
+      else {
+        if (p.stats && tid == 0 && p.iter < 4096) { atomicAdd(&p.stats[p.iter * 8 + 3], 1); atomicAdd(&p.stats[(2048 + p.iter) * 8 + why], 1); }
+        // nested robust solver on the same grouped list (lean passes through the SrcGrouped overloads)
+        // (it continues from where the Newton iteration stopped when that state is usable)
+        const bool keep = al == al && be == be && fabs(al - aw) <= 0.5 * W && fabs(be - bw) <= 0.5 * W;
+        __syncthreads();
+        if (!keep) for (int g = tid; g < G; g += nt) lamS[g] = lamW[g];
+        if (tid == 0) { sgrp.L = &src; sgrp.poff = poff; sgrp.ngrp = ngrp; sgrp.gv = gv; }
+        __syncthreads();
+        rs.alpha = keep ? al : aw; rs.beta = keep ? be : bw; rs.amode = keep ? amode : amode_w;
+        prox_rootfind<false>(p, sgrp, a, b, tau, Delta, sh, rs);
+      }
+      double mv_l = 0.0;
+      for (int g = 0; g < G; ++g) mv_l = fmax(mv_l, fabs(lamS[g] - lamW[g]));
+      mv = fmax(fmax(fabs(rs.alpha - aw), fabs(rs.beta - bw)), mv_l);
+      if (mv <= 0.5 * fmin(Wf, W)) break;
+      if (!(Wf < INFINITY)) { fallback = true; break; }   // left the streaming window (or NaN): the dead assets were misjudged
+      if (p.stats && tid == 0 && p.iter < 4096) atomicAdd(&p.stats[p.iter * 8 + 0], 1);
+      Wf = INFINITY;
       __syncthreads();
     }
-    if (ok) { rs.alpha = al; rs.beta = be; rs.amode = amode; }
-    else {
-      if (p.stats && tid == 0 && p.iter < 4096) { atomicAdd(&p.stats[p.iter * 8 + 3], 1); atomicAdd(&p.stats[(2048 + p.iter) * 8 + why], 1); }
-      // nested robust solver on the same grouped list (lean passes through the SrcGrouped overloads)
-      // (it continues from where the Newton iteration stopped when that state is usable)
-      const bool keep = al == al && be == be && fabs(al - aw) <= 0.5 * W && fabs(be - bw) <= 0.5 * W;
-      __syncthreads();
-      if (!keep) for (int g = tid; g < G; g += nt) lamS[g] = lamW[g];
-      if (tid == 0) { sgrp.L = &src; sgrp.poff = poff; sgrp.ngrp = ngrp; sgrp.gv = gv; }
-      __syncthreads();
-      rs.alpha = keep ? al : aw; rs.beta = keep ? be : bw; rs.amode = keep ? amode : amode_w;
-      prox_rootfind<false>(p, sgrp, a, b, tau, Delta, sh, rs);
-    }
-    double mv_l = 0.0;
-    for (int g = 0; g < G; ++g) mv_l = fmax(mv_l, fabs(lamS[g] - lamW[g]));
-    mv = fmax(fmax(fabs(rs.alpha - aw), fabs(rs.beta - bw)), mv_l);
-    if (!(mv <= 0.5 * W)) fallback = true;               // left the window (or NaN): the dead assets were misjudged
     if (fallback && p.stats && tid == 0 && p.iter < 4096) atomicAdd(&p.stats[p.iter * 8 + 2], 1);
   }
   int finished = 0;
   if (!fallback) {
     // ---------------------------------------------------------------- live assets: output (+ residual terms)
     const double alpha = rs.alpha, beta = rs.beta, bdf = beta - Delta;
+    const int nraw_all = offs[nsub];
     double nx = 0, nz = 0, nrp = 0, nrd = 0, nPx = 0, ny = 0, nq = 0;
-    src.for_each([&](int64_t i, const ElemConst& e, int g, int, const double*, const double*) {
-      double mvb, mvs;
+    for (int j = tid; j < nraw_all; j += nt) {           // every entry of the raw lists (the solve may have used a part)
+      int lo = 0, hi = nsub;
+      while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (offs[mid] <= j) lo = mid; else hi = mid; }
+      const LiveEnt* ep = p.lraw + ((int64_t)a * nsub + lo) * p.capw + (j - offs[lo]);
+      const double2 ea = __ldg((const double2*)ep), eb = __ldg((const double2*)ep + 1);
+      ElemConst e; int g; double mvb, mvs;
+      const int64_t i = src.decode(ea, eb, e, g);
       const double lg = G ? lamS[g] : 0.0;
       const double tr = buy_amt(e, alpha + lg, mvb) - sell_amt<false>(e, bdf + lg, nullptr, nullptr, 0, mvs);
       const double z = e.w0 + tr;
@@ -682,7 +747,7 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
         nrd = fmax(nrd, fabs(pq + y)); nPx = fmax(nPx, fabs(pq - qi)); ny = fmax(ny, fabs(y)); nq = fmax(nq, fabs(qi));
         if (!(z == z) || !(x == x) || !(pq == pq)) nrp = INFINITY;
       }
-    });
+    }
     if (CHECK) {
       if (tid < 7) {                                     // residual terms of the dead assets, per slice
         double m = 0.0;
@@ -723,7 +788,7 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
       // next window of the streaming pass: a multiple of the last movement, never shrunk while its list is short
       // (a wide window then costs nothing and the solution almost never leaves it); infinite for the first iterations
       double Ws = p.win_ratio * next_window(p, alpha, beta, mv);
-      const int nl = src.cnt[0];
+      const int nl = offs[nsub];
       if (nl < 256) Ws = fmax(Ws, nl < 64 ? 2.0 * W : W);
       if (p.iter < 2) Ws = INFINITY;
       p.ap.win[a] = p.iter < 2 ? INFINITY : next_window(p, alpha, beta, mv); p.ap.wins[a] = Ws;
