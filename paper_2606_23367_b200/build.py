@@ -8,7 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(HERE, "csrc", "prism.cu")
 LIB = os.path.join(HERE, "libprism.so")
-DEPS = [os.path.join(HERE, "csrc", f) for f in ("prism.cu", "common.cuh", "prox.cuh", "gemm.cuh", "small.cuh", "diag.cuh")] + [
+DEPS = [os.path.join(HERE, "csrc", f) for f in ("prism.cu", "common.cuh", "prox.cuh", "prox_fast.cuh", "gemm.cuh", "small.cuh", "diag.cuh")] + [
     os.path.join(os.path.dirname(HERE), "include", "prism.h")]
 
 
