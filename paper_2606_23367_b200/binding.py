@@ -41,7 +41,8 @@ class Settings(C.Structure):
     _fields_ = [("eps_rel", C.c_double), ("max_iter", C.c_int32), ("check_every", C.c_int32), ("alpha", C.c_double),
                 ("rho_scale", C.c_double), ("rho_band_scale", C.c_double), ("adapt_rho", C.c_int32),
                 ("gemm_mode", C.c_int32), ("time_limit_ms", C.c_double), ("deadline_ms", C.c_double),
-                ("use_graph", C.c_int32), ("profile", C.c_int32), ("prox_window_mult", C.c_double)]
+                ("use_graph", C.c_int32), ("profile", C.c_int32), ("prox_window_mult", C.c_double),
+                ("first_check", C.c_int32), ("reserved0", C.c_int32)]
 
 
 class SolveInfo(C.Structure):

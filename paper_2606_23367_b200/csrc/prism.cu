@@ -38,7 +38,7 @@ extern "C" void prism_default_settings(prism_settings* s) {
   memset(s, 0, sizeof(*s));
   s->eps_rel = 1e-6; s->max_iter = 4000; s->check_every = 10; s->alpha = 1.6; s->rho_scale = 100.0;
   s->rho_band_scale = 1.0; s->adapt_rho = 1; s->gemm_mode = 0; s->time_limit_ms = 0.0; s->deadline_ms = 0.0;
-  s->use_graph = 1; s->prox_window_mult = 32.0;
+  s->use_graph = 1; s->prox_window_mult = 32.0; s->first_check = 30; s->reserved0 = 0;
 }
 extern "C" const char* prism_last_error(void) { return g_err; }
 extern "C" const char* prism_version(void) { return PRISM_VERSION_STR; }
@@ -262,8 +262,8 @@ extern "C" int prism_problem_create(int64_t N, int32_t k, int32_t accounts, cons
     const int Gb = G > 0 ? G : 1;
     ALLOC_TRY(dev_alloc(p, &p->lraw, (size_t)A * p->ldc, false));
     ALLOC_TRY(dev_alloc(p, &p->lcomp, (size_t)A * p->ldc, false));
-    ALLOC_TRY(dev_alloc(p, &p->lcnt, (size_t)A * p->S * FAST_NW));
-    ALLOC_TRY(dev_alloc(p, &p->cbin, (size_t)A * 2 * Gb));
+    ALLOC_TRY(dev_alloc(p, &p->lcnt, (size_t)2 * A * p->S * FAST_NW));     // fronts, then backs of the two-level lists
+    ALLOC_TRY(dev_alloc(p, &p->cbin, (size_t)2 * A * 2 * Gb));             // bins of the dead assets, then speculative bins
     ALLOC_TRY(dev_alloc(p, &p->chkp, (size_t)A * p->S * 8));
     ALLOC_TRY(dev_alloc(p, &p->lflag, (size_t)A));
   }
@@ -329,7 +329,7 @@ static void launch_prox(Launcher& L, ProxArgs& a, int mode, int iter) {
   if (p->fast) {
     const bool chk = (mode & (PROX_CHECK | PROX_FINAL)) != 0;     // the final extraction also needs w_out
     const dim3 grid((unsigned)p->S, (unsigned)p->A);
-    const size_t sm = stream_smem_bytes(p->G), smr = root_smem_bytes(p->G, p->S * FAST_NW);
+    const size_t sm = stream_smem_bytes(p->G), smr = root_smem_bytes(p->G, 2 * p->S * FAST_NW);
     L.begin(PRISM_K_PROX);
     if (chk) k_prox_stream<true><<<grid, FAST_NW * 32, sm, st>>>(a);
     else k_prox_stream<false><<<grid, FAST_NW * 32, sm, st>>>(a);
@@ -414,7 +414,7 @@ extern "C" int prism_solve_batch(prism_problem* p, const prism_settings* sp, voi
 
   int it = 1, timed_out = 0, late_iter = -1, ndone = 0;
   for (; it <= s.max_iter; ++it) {
-    const bool check = (it > 1) && ((it - 1) % s.check_every == 0);   // residuals of the iterate after it-1 iterations
+    const bool check = (it > 1) && ((it - 1) % s.check_every == 0) && (it - 1 >= s.first_check);   // residuals of the iterate after it-1 iterations
     launch_prox(L, pa, check ? PROX_CHECK : 0, it - 1);
     if (check || it == 1) {
       L.begin(PRISM_K_FACTOR);
@@ -434,7 +434,7 @@ extern "C" int prism_solve_batch(prism_problem* p, const prism_settings* sp, voi
     L.begin(PRISM_K_SOLVE);
     k_solve<<<A, 256, 0, st>>>(sa);
     L.end();
-    const bool next_check = (it % s.check_every == 0);
+    const bool next_check = (it % s.check_every == 0) && (it >= s.first_check);
     if (next_check) L.gemm2<G2_ADMM_CHECK>(g2); else L.gemm2<G2_ADMM>(g2);
   }
   if (ndone < A) {           // iteration cap or time limit: extract z for the accounts still running

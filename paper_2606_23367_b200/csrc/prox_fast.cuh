@@ -72,7 +72,7 @@ __global__ void __launch_bounds__(FAST_NW * 32, 3) k_prox_stream(const __grid_co
   const double lo_a = p.lo[a], hi_a = p.hi[a];
   if (!(hi_a - lo_a <= 4.0)) {            // box wider than the fixed-point range of the bins: generic path in k_prox_root
     if (tid == 0 && sl == 0) p.lflag[a] = 1;
-    if (lane == 0) p.lcnt[sub] = 0;
+    if (lane == 0) { p.lcnt[sub] = 0; p.lcnt[p.A * p.S * FAST_NW + sub] = 0; }
     return;
   }
   unsigned char* stage0 = stream_raw;                                 // FAST_NST stages: v, w0, q, d, 1/d, excl, gid
@@ -106,7 +106,13 @@ __global__ void __launch_bounds__(FAST_NW * 32, 3) k_prox_stream(const __grid_co
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     for (int c = 0; c < FAST_NST - 1 && c < nchunk; ++c) issue(c);
   }
-  const double W = p.ap.wins[a];
+  const double W = p.ap.wins[a], Wt = p.ap.win[a];
+  // Two-level lists: an asset that only the WIDE window (W) can reach but the TIGHT one (Wt, what the thresholds are
+  // expected to move by) cannot is finished speculatively as dead - outputs written, trade added to the second set of
+  // bins - and parked at the back of the warp's list; k_prox_root looks at those entries only when its solution
+  // leaves the tight window.  Check / final launches keep one level (their residual terms must not be speculative).
+  const bool split = !CHECK && Wt < 0.125 * W;
+  const double Wn = split ? Wt : W;
   const double gam = p.gamma[a], c = p.ap.c[a], cg = c * gam, icg = 1.0 / cg;
   const double kappa = p.kappa ? p.kappa[a] : 0.0;
   const double lam_b = kappa + (p.c_buy ? p.c_buy[a] : 0.0), Delta = lam_b + kappa;
@@ -120,8 +126,10 @@ __global__ void __launch_bounds__(FAST_NW * 32, 3) k_prox_stream(const __grid_co
   double nx = 0, nz = 0, nrp = 0, nrd = 0, nPx = 0, ny = 0, nq = 0;
   LiveEnt* mylist = p.lraw + (int64_t)sub * p.capw;
   unsigned long long* cbin = p.cbin + (int64_t)a * 2 * Gb;
+  const int64_t fbin_off = (int64_t)p.A * 2 * Gb;                       // second set of bins: speculative trades
   const unsigned lt = (1u << lane) - 1u;
-  int n = 0;
+  int n = 0, nw_ = 0;
+  const double aN_lo = aw - Wn, aN_hi = aw + Wn, bN_lo = bw - Wn - Delta, bN_hi = bw + Wn - Delta;
   const double aW_lo = aw - W, aW_hi = aw + W, bW_lo = bw - W - Delta, bW_hi = bw + W - Delta;
   double* rtp = p.rt + rowp + i_beg + tid;
   double* ccp = p.cc + rowp + i_beg + tid;
@@ -161,21 +169,26 @@ __global__ void __launch_bounds__(FAST_NW * 32, 3) k_prox_stream(const __grid_co
       // and depends on the thresholds (live) in between; the same for the sell side.
       const bool inbox = w0 >= lo_a && w0 <= hi_a;
       const double wB = hi_a - w0, wS = w0 - lo_a;
-      const bool b_reach = tA > aW_lo, b_full = tA - aW_hi >= wB * rho;
-      const bool s_reach = tA < bW_hi, s_full = bW_lo - tA >= wS * rho;
+      const double wBr = wB * rho, wSr = wS * rho;
+      const bool b_reach = tA > aN_lo, b_full = tA - aN_hi >= wBr;
+      const bool s_reach = tA < bN_hi, s_full = bN_lo - tA >= wSr;
       double bc = (b_reach && b_full) ? wB : 0.0;
       double sc = (s_reach && s_full) ? wS : 0.0;
       bool live = (b_reach && !b_full) || (s_reach && !s_full) || !inbox;   // outside its box (rare): live
-      if (ex) { bc = 0.0; sc = w0; live = !(w0 >= 0.0 && w0 <= 4.0); }       // lo = hi = 0: the trade is -w0
+      bool spec = false;                                                     // dead in the tight window, live in the wide one
+      if (split) spec = !live && ((tA > aW_lo && !(tA - aW_hi >= wBr)) || (tA < bW_hi && !(bW_lo - tA >= wSr)));
+      if (ex) { bc = 0.0; sc = w0; live = !(w0 >= 0.0 && w0 <= 4.0); spec = false; }   // lo = hi = 0: the trade is -w0
       live = live && valid;
+      spec = spec && valid;
       const double tc = bc - sc;                                             // trade of a dead asset
       const double z = w0 + tc;
       const double rt = fma(rho, (w0 - u) + 2.0 * tc, qm) * (iv * igc);      // (rho (2 z - v) - q) / M_i
       if (valid && !live) {
         rtp[h * 256] = rt;
         ccp[h * 256] = rt - z;
-        if (bc > 0.0) atomicAdd(&cbin[g], (unsigned long long)__double2ull_rn(bc * PRISM_FIX_SCALE));
-        if (sc > 0.0) atomicAdd(&cbin[Gb + g], (unsigned long long)__double2ull_rn(sc * PRISM_FIX_SCALE));
+        unsigned long long* bin = spec ? cbin + fbin_off : cbin;
+        if (bc > 0.0) atomicAdd(&bin[g], (unsigned long long)__double2ull_rn(bc * PRISM_FIX_SCALE));
+        if (sc > 0.0) atomicAdd(&bin[Gb + g], (unsigned long long)__double2ull_rn(sc * PRISM_FIX_SCALE));
         if (CHECK) {
           const int64_t i = i0 + t;
           p.w_out[row + i] = z;            // speculative: kept if the account turns out to have converged
@@ -187,21 +200,24 @@ __global__ void __launch_bounds__(FAST_NW * 32, 3) k_prox_stream(const __grid_co
         }
       }
       const unsigned m = __ballot_sync(0xffffffffu, live);
-      if (m) {
-        if (live) {
+      const unsigned ms = split ? __ballot_sync(0xffffffffu, spec) : 0u;
+      if (m | ms) {
+        if (live || spec) {
           LiveEnt e;
           e.T = T; e.w0 = w0; e.ir = iv * icg; e.pad = 0;
           e.meta = (uint32_t)(i0 + t) | ((uint32_t)g << PROX_META_IDX_BITS) | ((uint32_t)(ex ? 1 : (inbox ? 0 : 2)) << 30);
-          mylist[n + __popc(m & lt)] = e;
+          // tight list from the front, speculative entries from the back of the same buffer (n + nw_ <= capw always)
+          mylist[live ? n + __popc(m & lt) : p.capw - 1 - (nw_ + __popc(ms & lt))] = e;
         }
         n += __popc(m);
+        nw_ += __popc(ms);
       }
     }
     rtp += FAST_CH; ccp += FAST_CH;
     __syncwarp();
     if (lane == 0) mbar_arrive(&bar_empty[st]);
   }
-  if (lane == 0) p.lcnt[sub] = n;
+  if (lane == 0) { p.lcnt[sub] = n; p.lcnt[p.A * p.S * FAST_NW + sub] = nw_; }
   if (CHECK) {
     double val[7] = {nx, nz, nrp, nrd, nPx, ny, nq};
     block_reduce<7, 1>(val, scratch);
@@ -414,9 +430,11 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
   __shared__ SrcLiveG src;                 // CTA-uniform objects live in shared memory, not on the threads' stacks
   __shared__ SrcGrouped sgrp;
   __shared__ ProxShared sh;
+  __shared__ int nback_s;                  // entries at the backs of the lists (speculatively finished by the streaming pass)
   const int a = blockIdx.x;
   if (p.ap.done[a]) return;
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, nt = blockDim.x, nw = nt >> 5;
+  if (tid == 0) nback_s = 0;
   const int G = p.G, Gb = G > 0 ? G : 1;
   const int64_t N = p.N, row = (int64_t)a * N, rowp = (int64_t)a * p.ldw;
   const int nsub = p.S * FAST_NW;
@@ -432,8 +450,8 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
   unsigned long long* ubin = (unsigned long long*)d0; d0 += 2 * Gb;    // their sum: what the solve uses
   double* chk = d0; d0 += 8;
   double* gv = d0; d0 += 4 * (Gb + 4);                   // per (pseudo-)group sums of one pass
-  int* offs = (int*)d0;                                  // nsub + 1: start of raw list k in the sequence of all lists
-  int* wcnt = offs + nsub + 1;                           // nw x Gb: entries of group g in warp w's part (then running offsets)
+  int* offs = (int*)d0;                                  // 2 nsub + 1: start of raw list k in the sequence of lists in use
+  int* wcnt = offs + 2 * nsub + 1;                       // nw x Gb: entries of group g in warp w's part (then running offsets)
   int* goff = wcnt + 4 * Gb;                             // Gb + 1 group offsets of the grouped list
   int* poff = goff + Gb + 1;                             // ngrp + 1 (pseudo-)group offsets used by the passes
   int* act = poff + Gb + 5;                              // Gb: band state -1 lower active, 0 inactive, +1 upper active
@@ -446,6 +464,7 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
   const double tau = p.tau ? p.tau[a] : INFINITY;
   const double igc = 1.0 / (gam * (1.0 + c));
   const double W = p.ap.wins[a], Wt = p.ap.win[a];       // window of the streaming pass; tight window (32 x last movement)
+  const bool split = !CHECK && Wt < 0.125 * W;           // the streaming pass made two-level lists (same test there)
   const double src_lo = p.lo[a], src_hi = p.hi[a];
   const double b = p.ap.bsum[a];
   double aw = p.ap.alpha[a], bw = p.ap.beta[a];
@@ -463,11 +482,15 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
     unsigned long long* src_bin = p.cbin + (int64_t)a * 2 * Gb + g;
     cbin[g] = *src_bin;
     *src_bin = 0ull;
+    src_bin += (int64_t)p.A * 2 * Gb;                    // speculative trades (entries at the back of the lists)
+    fbin[g] = *src_bin;
+    *src_bin = 0ull;
   }
   for (int e = tid; e < 4 * Gb; e += nt) wcnt[e] = 0;
   for (int k = tid; k < nsub; k += nt) offs[k + 1] = p.lcnt[(int64_t)a * nsub + k];
   __syncthreads();
   bool fallback = generic != 0;
+  int nlist_used = nsub;
   RootState rs;
   rs.alpha = aw; rs.beta = bw; rs.amode = amode_w; rs.n_eval = 0;
   // band ramp: the first iterations project without the group bands (an exact prox of the relaxed problem); their
@@ -476,77 +499,62 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
   rs.nobands = bands_on ? 0 : 1;
   double mv = 0.0;
   if (!fallback) {
-    // ---- the raw lists as one sequence (offs = their start offsets); warp w handles a contiguous quarter of it
+    // ---- the raw lists as one sequence (offs = their start offsets); warp w handles a contiguous quarter of it.
+    // Level 0: the tight parts (fronts) of the nsub lists.  Level 1 (only after a solution left the tight window):
+    // fronts and backs together, 2 nsub lists; entry m of a back sits at position capw - 1 - m of its buffer.
     const unsigned lt = (1u << lane) - 1u;
     const LiveEnt* lr = p.lraw + (int64_t)a * nsub * p.capw;
-    if (wid == 0) {                                      // inclusive scan of the list lengths
-      int carry = 0;
-      for (int k0 = 0; k0 < nsub; k0 += 32) {
-        int v = k0 + lane < nsub ? offs[k0 + lane + 1] : 0;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, v, o); if (lane >= o) v += t; }
-        if (k0 + lane < nsub) offs[k0 + lane + 1] = v + carry;
-        carry += __shfl_sync(0xffffffffu, v, 31);
-      }
-      if (lane == 0) offs[0] = 0;
-    }
-    __syncthreads();
-    const int nraw = offs[nsub];
-    const int segw = (((nraw + nw - 1) / nw) + 31) & ~31;
-    const int j_beg = min(nraw, wid * segw), j_end = min(nraw, (wid + 1) * segw);
-    auto locate = [&](int j) -> const LiveEnt* {         // entry j of the sequence
-      int lo = 0, hi = nsub;
-      while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (offs[mid] <= j) lo = mid; else hi = mid; }
-      return lr + (int64_t)lo * p.capw + (j - offs[lo]);
-    };
-    // Is this entry dead for every threshold within Wf of the warm start?  (Then bc / sc are its constant amounts.)
-    auto tight_dead = [&](const double2& ea, const double2& eb, double Wf, double& bc, double& sc) -> bool {
-      const uint32_t m = (uint32_t)__double_as_longlong(eb.y);
-      if ((m >> 30) != 0) return false;                  // excluded with an odd w0 / outside its box: always kept
-      const double T = ea.x, w0 = ea.y, ir = eb.x, wB = src_hi - w0, wS = w0 - src_lo;
-      const double lg = (bands_on && G) ? lamW[(m >> PROX_META_IDX_BITS) & 0xffu] : 0.0;
-      bc = 0.0; sc = 0.0;
-      if (wB > 0.0) {
-        if ((T - (aw + lg - Wf)) * ir <= 0.0) bc = 0.0;
-        else if ((T - (aw + lg + Wf)) * ir >= wB) bc = wB;
-        else return false;
-      }
-      if (wS > 0.0) {
-        if (((bw + lg + Wf - Delta) - T) * ir <= 0.0) sc = 0.0;
-        else if (((bw + lg - Wf - Delta) - T) * ir >= wS) sc = wS;
-        else return false;
-      }
-      return true;
-    };
-    // ---- group sort (counting sort, stable in sequence order => deterministic): kept entries -> lcomp by group.
-    // With a finite Wf only the entries a TIGHT window around the warm start can reach are kept; the constant trades
-    // of the others go to fixed-point bins, exactly as in the streaming pass.
-    auto sort_lists = [&](double Wf) {
-      const bool filt = Wf < INFINITY;
-      for (int e = tid; e < 4 * Gb; e += nt) wcnt[e] = 0;
-      for (int g = tid; g < 2 * Gb; g += nt) fbin[g] = 0ull;
+    const int32_t* lcw = p.lcnt + (int64_t)p.A * nsub + (int64_t)a * nsub;   // lengths of the backs
+    int nlist = nsub, nraw = 0, j_beg = 0, j_end = 0;
+    auto scan_lists = [&](int level) {
+      nlist = level ? 2 * nsub : nsub;
       __syncthreads();
-      if (!G && !filt) { if (lane == 0) wcnt[wid] = j_end - j_beg; }
+      for (int k = tid; k < nlist; k += nt) offs[k + 1] = k < nsub ? p.lcnt[(int64_t)a * nsub + k] : lcw[k - nsub];
+      __syncthreads();
+      if (wid == 0) {                                      // inclusive scan of the list lengths
+        int carry = 0;
+        for (int k0 = 0; k0 < nlist; k0 += 32) {
+          int v = k0 + lane < nlist ? offs[k0 + lane + 1] : 0;
+#pragma unroll
+          for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, v, o); if (lane >= o) v += t; }
+          if (k0 + lane < nlist) offs[k0 + lane + 1] = v + carry;
+          carry += __shfl_sync(0xffffffffu, v, 31);
+        }
+        if (lane == 0) offs[0] = 0;
+      }
+      __syncthreads();
+      nraw = offs[nlist];
+      const int segw = (((nraw + nw - 1) / nw) + 31) & ~31;
+      j_beg = min(nraw, wid * segw); j_end = min(nraw, (wid + 1) * segw);
+    };
+    auto locate = [&](int j) -> const LiveEnt* {         // entry j of the sequence
+      int lo = 0, hi = nlist;
+      while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (offs[mid] <= j) lo = mid; else hi = mid; }
+      const int pos = j - offs[lo];
+      return lo < nsub ? lr + (int64_t)lo * p.capw + pos : lr + (int64_t)(lo - nsub) * p.capw + (p.capw - 1 - pos);
+    };
+    // ---- group sort (counting sort, stable in sequence order => deterministic): entries -> lcomp (or shared memory) by
+    // group.  use_f: the speculative trades of the backs (fbin) count as constants (level 0 of a two-level list).
+    auto sort_lists = [&](bool use_f) {
+      for (int e = tid; e < 4 * Gb; e += nt) wcnt[e] = 0;
+      __syncthreads();
+      if (!G) { if (lane == 0) wcnt[wid] = j_end - j_beg; }
       else
-        for (int j0 = j_beg; j0 < j_end; j0 += 32) {
-          const int j = j0 + lane;
-          const bool valid = j < j_end;
-          int g = 0x100 + lane;
-          if (valid) {
-            const LiveEnt* e = locate(j);
-            if (filt) {
-              const double2 ea = __ldg((const double2*)e), eb = __ldg((const double2*)e + 1);
-              const int ge = G ? (int)(((uint32_t)__double_as_longlong(eb.y) >> PROX_META_IDX_BITS) & 0xffu) : 0;
-              double bc, sc;
-              if (tight_dead(ea, eb, Wf, bc, sc)) {
-                if (bc > 0.0) atomicAdd(&fbin[ge], (unsigned long long)__double2ull_rn(bc * PRISM_FIX_SCALE));
-                if (sc > 0.0) atomicAdd(&fbin[Gb + ge], (unsigned long long)__double2ull_rn(sc * PRISM_FIX_SCALE));
-              } else g = ge;
-            } else g = (int)((__ldg(&e->meta) >> PROX_META_IDX_BITS) & 0xffu);
+        for (int j0 = j_beg; j0 < j_end; j0 += 128) {     // four groups of 32 entries: their loads are issued together
+          int g4[4];
+#pragma unroll
+          for (int u = 0; u < 4; ++u) {
+            const int j = j0 + 32 * u + lane;
+            g4[u] = 0x100 + lane;
+            if (j < j_end) g4[u] = (int)((__ldg(&locate(j)->meta) >> PROX_META_IDX_BITS) & 0xffu);
           }
-          const unsigned m = __match_any_sync(0xffffffffu, g);
-          if (g < 0x100 && lane == __ffs(m) - 1) wcnt[wid * Gb + g] += __popc(m);
-          __syncwarp();
+#pragma unroll
+          for (int u = 0; u < 4; ++u) {
+            const int g = g4[u];
+            const unsigned m = __match_any_sync(0xffffffffu, g);
+            if (g < 0x100 && lane == __ffs(m) - 1) wcnt[wid * Gb + g] += __popc(m);
+            __syncwarp();
+          }
         }
       __syncthreads();
       for (int g = tid; g < Gb; g += nt) {               // start of warp w's entries inside group g; group totals
@@ -554,7 +562,7 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
         for (int w = 0; w < nw; ++w) { const int t = wcnt[w * Gb + g]; wcnt[w * Gb + g] = run; run += t; }
         goff[g + 1] = run;
       }
-      for (int g = tid; g < 2 * Gb; g += nt) ubin[g] = cbin[g] + fbin[g];
+      for (int g = tid; g < 2 * Gb; g += nt) ubin[g] = cbin[g] + (use_f ? fbin[g] : 0ull);
       __syncthreads();
       if (tid == 0) {
         goff[0] = 0;
@@ -569,26 +577,28 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
       }
       __syncthreads();
       LiveEnt* dst = const_cast<LiveEnt*>(src.ent);
-      for (int j0 = j_beg; j0 < j_end; j0 += 32) {
-        const int j = j0 + lane;
-        const bool valid = j < j_end;
-        double2 ea = make_double2(0, 0), eb = make_double2(0, 0);
-        int g = 0x100 + lane;
-        if (valid) {
-          const LiveEnt* e = locate(j);
-          ea = __ldg((const double2*)e); eb = __ldg((const double2*)e + 1);
-          double bc, sc;
-          if (!(filt && tight_dead(ea, eb, Wf, bc, sc)))
-            g = G ? (int)(((uint32_t)__double_as_longlong(eb.y) >> PROX_META_IDX_BITS) & 0xffu) : 0;
+      for (int j0 = j_beg; j0 < j_end; j0 += 128) {
+        double2 ea[4], eb[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          const int j = j0 + 32 * u + lane;
+          ea[u] = make_double2(0, 0); eb[u] = make_double2(0, 0);
+          if (j < j_end) { const LiveEnt* e = locate(j); ea[u] = __ldg((const double2*)e); eb[u] = __ldg((const double2*)e + 1); }
         }
-        const unsigned m = __match_any_sync(0xffffffffu, g);
-        if (g < 0x100) {
-          double2* o = (double2*)(dst + goff[g] + wcnt[wid * Gb + g] + __popc(m & lt));
-          o[0] = ea; o[1] = eb;
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          const int j = j0 + 32 * u + lane;
+          int g = 0x100 + lane;
+          if (j < j_end) g = G ? (int)(((uint32_t)__double_as_longlong(eb[u].y) >> PROX_META_IDX_BITS) & 0xffu) : 0;
+          const unsigned m = __match_any_sync(0xffffffffu, g);
+          if (g < 0x100) {
+            double2* o = (double2*)(dst + goff[g] + wcnt[wid * Gb + g] + __popc(m & lt));
+            o[0] = ea[u]; o[1] = eb[u];
+          }
+          __syncwarp();
+          if (g < 0x100 && lane == __ffs(m) - 1) wcnt[wid * Gb + g] += __popc(m);
+          __syncwarp();
         }
-        __syncwarp();
-        if (g < 0x100 && lane == __ffs(m) - 1) wcnt[wid * Gb + g] += __popc(m);
-        __syncwarp();
       }
       __syncthreads();
     };
@@ -599,9 +609,16 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
     }
     // A long list is first solved on its tight part; a solution that leaves the tight window repeats the solve on the
     // whole list, and one that leaves the streaming pass's window sends the account to the generic path.
-    double Wf = (nraw > 512 && Wt < 0.125 * W) ? Wt : INFINITY;
+    double Wf = split ? Wt : INFINITY;
+    {
+      int nb = 0;
+      for (int k = tid; k < nsub; k += nt) nb += lcw[k];
+      if (nb) atomicAdd(&nback_s, nb);
+    }
     for (int att = 0; att < 2; ++att) {
-      sort_lists(Wf);
+      scan_lists(att);                                   // level 0: the fronts; level 1: fronts and backs
+      nlist_used = nlist;
+      sort_lists(split && att == 0);
       rs.alpha = aw; rs.beta = bw; rs.amode = amode_w;
       for (int g = tid; g < G; g += nt) lamS[g] = lamW[g];
       __syncthreads();
@@ -721,12 +738,14 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
   if (!fallback) {
     // ---------------------------------------------------------------- live assets: output (+ residual terms)
     const double alpha = rs.alpha, beta = rs.beta, bdf = beta - Delta;
-    const int nraw_all = offs[nsub];
+    const int nlist_o = nlist_used, nraw_all = offs[nlist_o];
     double nx = 0, nz = 0, nrp = 0, nrd = 0, nPx = 0, ny = 0, nq = 0;
-    for (int j = tid; j < nraw_all; j += nt) {           // every entry of the raw lists (the solve may have used a part)
-      int lo = 0, hi = nsub;
+    for (int j = tid; j < nraw_all; j += nt) {           // every entry of the lists the solve used (the others are finished)
+      int lo = 0, hi = nlist_o;
       while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (offs[mid] <= j) lo = mid; else hi = mid; }
-      const LiveEnt* ep = p.lraw + ((int64_t)a * nsub + lo) * p.capw + (j - offs[lo]);
+      const int pos = j - offs[lo];
+      const LiveEnt* ep = p.lraw + (int64_t)a * nsub * p.capw +
+                          (lo < nsub ? (int64_t)lo * p.capw + pos : (int64_t)(lo - nsub) * p.capw + (p.capw - 1 - pos));
       const double2 ea = __ldg((const double2*)ep), eb = __ldg((const double2*)ep + 1);
       ElemConst e; int g; double mvb, mvs;
       const int64_t i = src.decode(ea, eb, e, g);
@@ -788,7 +807,7 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
       // next window of the streaming pass: a multiple of the last movement, never shrunk while its list is short
       // (a wide window then costs nothing and the solution almost never leaves it); infinite for the first iterations
       double Ws = p.win_ratio * next_window(p, alpha, beta, mv);
-      const int nl = offs[nsub];
+      const int nl = offs[nlist_used] + (nlist_used == nsub ? nback_s : 0);   // live assets of the streaming window
       if (nl < 256) Ws = fmax(Ws, nl < 64 ? 2.0 * W : W);
       if (p.iter < 2) Ws = INFINITY;
       p.ap.win[a] = p.iter < 2 ? INFINITY : next_window(p, alpha, beta, mv); p.ap.wins[a] = Ws;
@@ -803,6 +822,7 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
       }
       if (p.stats && p.iter < 4096) {
         atomicAdd(&p.stats[p.iter * 8 + 5], 1); atomicAdd(&p.stats[p.iter * 8 + 6], src.cnt[0]); atomicAdd(&p.stats[p.iter * 8 + 7], rs.n_eval);
+        atomicAdd(&p.stats[(2048 + p.iter) * 8 + 6], nl);
         atomicMax(&p.stats[p.iter * 8 + 4], rs.n_eval); if (rs.n_eval > 20) atomicAdd(&p.stats[p.iter * 8 + 0], 1);
       }
     }
