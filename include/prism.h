@@ -132,7 +132,7 @@ typedef struct prism_settings {
   int32_t profile;          /* 1 => bracket every kernel launch with CUDA events (read with prism_kernel_times);
                                adds event overhead, so never combine with a throughput measurement           */
   double prox_window_mult;  /* streaming prox: next window = this x the last movement of the thresholds (default 32) */
-  int32_t first_check;      /* no residual check before this many iterations (default 30): the first checks of a
+  int32_t first_check;      /* no residual check before this many iterations (default 40): the first checks of a
                                cold start never pass and a check launch costs several plain ones             */
   int32_t reserved0;        /* keep 0 */
 } prism_settings;

@@ -26,8 +26,10 @@ struct AccountParams {            // per-account scalars, struct of arrays on th
   int32_t* nadapt;  // iteration of the account's last rho adaptation
   double* win;      // live-list window of the prox for the next launch (threshold units)
   double* wins;     // window of the streaming pass (prox_fast.cuh), >= win
+  double* slack;    // band ramp (prox_fast.cuh): largest band violation of the band-free projection at band_start
 };
 
+#define PRISM_MAX_PARTS 8
 struct prism_problem {
   int64_t N;
   int32_t k, kp, A, G, Kp;       // kp: k padded to 8 * MT; Kp = kp: rows of T and V per account (U = Bp)
@@ -71,6 +73,14 @@ struct prism_problem {
   double dbar;            // mean of d (host copy at create)
   double prof_ms[PRISM_NKERN];   // per-kernel-class device time of the last profiled solve
   int64_t prof_cnt[PRISM_NKERN];
+  // account groups (prism.cu, "parts"): a large batch is split into contiguous account ranges, each a complete
+  // problem object of its own, solved concurrently on its own stream by its own host thread.  The parent holds
+  // no iterate; parts[i] covers accounts [part_a0[i], part_a0[i + 1]).
+  int32_t nparts;
+  prism_problem* parts[PRISM_MAX_PARTS];
+  int32_t part_a0[PRISM_MAX_PARTS + 1];
+  cudaStream_t part_stream[PRISM_MAX_PARTS];
+  cudaEvent_t part_done[PRISM_MAX_PARTS];
 };
 
 static thread_local char g_err[512] = "";

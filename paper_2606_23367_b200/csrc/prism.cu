@@ -2,6 +2,8 @@
 // Single translation unit: the kernels live in the .cuh files included here.  No torch types, no CPU fallback.
 #include <chrono>
 #include <new>
+#include <string>
+#include <thread>
 #include <vector>
 #include <cstdlib>
 
@@ -38,7 +40,7 @@ extern "C" void prism_default_settings(prism_settings* s) {
   memset(s, 0, sizeof(*s));
   s->eps_rel = 1e-6; s->max_iter = 4000; s->check_every = 10; s->alpha = 1.6; s->rho_scale = 100.0;
   s->rho_band_scale = 1.0; s->adapt_rho = 1; s->gemm_mode = 0; s->time_limit_ms = 0.0; s->deadline_ms = 0.0;
-  s->use_graph = 1; s->prox_window_mult = 32.0; s->first_check = 30; s->reserved0 = 0;
+  s->use_graph = 1; s->prox_window_mult = 32.0; s->first_check = 40; s->reserved0 = 0;
 }
 extern "C" const char* prism_last_error(void) { return g_err; }
 extern "C" const char* prism_version(void) { return PRISM_VERSION_STR; }
@@ -58,10 +60,15 @@ static int dev_alloc(prism_problem* p, T** ptr, size_t count, bool zero = true) 
 
 extern "C" void prism_problem_destroy(prism_problem* p) {
   if (!p) return;
+  for (int i = 0; i < p->nparts; ++i) {
+    prism_problem_destroy(p->parts[i]);
+    if (p->part_stream[i]) cudaStreamDestroy(p->part_stream[i]);
+    if (p->part_done[i]) cudaEventDestroy(p->part_done[i]);
+  }
   void* ptrs[] = {p->Bp, p->Bt, p->invd, p->gram, p->q, p->v, p->rt, p->cc, p->xs, p->pxq, p->Tpart, p->V, p->Sinv,
                   p->gw0, p->lamG, p->resid, p->duals, p->status, p->ap.c, p->ap.alpha, p->ap.beta,
                   p->ap.mode, p->ap.bsum, p->ap.done, p->ap.conv, p->ap.iters, p->ap.refactor,
-                  p->ap.nadapt, p->ap.win, p->ap.wins, p->counters, p->w_stage, p->i_stage, p->lraw, p->lcomp, p->lcnt, p->cbin, p->chkp, p->lflag, p->stats};
+                  p->ap.nadapt, p->ap.win, p->ap.wins, p->ap.slack, p->counters, p->w_stage, p->i_stage, p->lraw, p->lcomp, p->lcnt, p->cbin, p->chkp, p->lflag, p->stats};
   for (void* q : ptrs) if (q) cudaFree(q);
   if (p->h_counters) cudaFreeHost(p->h_counters);
   delete p;
@@ -172,8 +179,8 @@ static bool fast_applicable(const prism_problem* p) {
 }
 
 // ------------------------------------------------------------------------------------------ create (H0)
-extern "C" int prism_problem_create(int64_t N, int32_t k, int32_t accounts, const prism_constraint_set* cs,
-                                    const prism_data* data, void* cuda_stream, prism_problem** out) {
+static int create_one(int64_t N, int32_t k, int32_t accounts, const prism_constraint_set* cs,
+                      const prism_data* data, void* cuda_stream, prism_problem** out) {
   if (out) *out = nullptr;
   if (!out || !cs || !data) return set_err(PRISM_ERR_INVALID_ARG, "null argument%s", "");
   const int A = accounts, G = (cs->flags & PRISM_GROUP_BANDS) ? cs->G : 0;
@@ -246,6 +253,7 @@ extern "C" int prism_problem_create(int64_t N, int32_t k, int32_t accounts, cons
   ALLOC_TRY(dev_alloc(p, &p->ap.nadapt, (size_t)A));
   ALLOC_TRY(dev_alloc(p, &p->ap.win, (size_t)A));
   ALLOC_TRY(dev_alloc(p, &p->ap.wins, (size_t)A));
+  ALLOC_TRY(dev_alloc(p, &p->ap.slack, (size_t)A));
   ALLOC_TRY(dev_alloc(p, &p->counters, (size_t)4));
   p->fast = fast_applicable(p) ? 1 : 0;
   if (p->fast) {
@@ -316,6 +324,8 @@ static ProxArgs make_prox_args(prism_problem* p, const prism_settings& s, double
   if (const char* e = getenv("PRISM_PROX_WIN_MULT")) a.win_mult = atof(e);
   a.band_start = 20;
   if (const char* e = getenv("PRISM_PROX_BAND_START")) a.band_start = atoi(e);
+  a.band_ramp = 0;         // measured on configs[2]: a 10 / 20-iteration slack ramp costs 6% / 23% (the thresholds keep moving)
+  if (const char* e = getenv("PRISM_PROX_BAND_RAMP")) a.band_ramp = atoi(e);
   a.win_ratio = 16.0;
   if (const char* e = getenv("PRISM_PROX_WIN_RATIO")) a.win_ratio = atof(e);
   return a;
@@ -372,9 +382,9 @@ static void run_diag(prism_problem* p, Launcher& L, const double* w, const doubl
   L.end();
 }
 
-extern "C" int prism_solve_batch(prism_problem* p, const prism_settings* sp, void* cuda_stream, double* w_out,
-                                 int32_t* status_out, int32_t* iters_out, double* resid_out, double* duals_out,
-                                 prism_solve_info* info) {
+static int solve_one(prism_problem* p, const prism_settings* sp, void* cuda_stream, double* w_out,
+                     int32_t* status_out, int32_t* iters_out, double* resid_out, double* duals_out,
+                     prism_solve_info* info) {
   if (!p) return set_err(PRISM_ERR_NOT_READY, "problem object is NULL%s", "");
   if (!w_out || !status_out || !iters_out) return set_err(PRISM_ERR_INVALID_ARG, "w_out, status_out, iters_out are mandatory%s", "");
   prism_settings s;
@@ -484,6 +494,16 @@ extern "C" int prism_solve_batch(prism_problem* p, const prism_settings* sp, voi
 
 // debug only (PRISM_PROX_STATS=1 at create): per-iteration counters of the streaming prox; not part of prism.h
 extern "C" int prism_debug_prox_stats(prism_problem* p, int32_t* out, int clear) {
+  if (p && p->nparts) {                       // sum over the account groups
+    std::vector<int32_t> t((size_t)4096 * 8);
+    for (size_t j = 0; j < t.size(); ++j) out[j] = 0;
+    for (int i = 0; i < p->nparts; ++i) {
+      const int r = prism_debug_prox_stats(p->parts[i], t.data(), clear);
+      if (r != PRISM_OK) return r;
+      for (size_t j = 0; j < t.size(); ++j) out[j] += t[j];
+    }
+    return PRISM_OK;
+  }
   if (!p || !p->stats) return PRISM_ERR_NOT_READY;
   cudaMemcpy(out, p->stats, (size_t)4096 * 8 * sizeof(int32_t), cudaMemcpyDeviceToHost);
   if (clear) cudaMemset(p->stats, 0, (size_t)4096 * 8 * sizeof(int32_t));
@@ -493,12 +513,12 @@ extern "C" int prism_debug_prox_stats(prism_problem* p, int32_t* out, int clear)
 extern "C" int prism_kernel_times(const prism_problem* p, double* ms_out, int64_t* launches_out) {
   if (!p || !ms_out || !launches_out) return set_err(PRISM_ERR_INVALID_ARG, "null argument%s", "");
   for (int i = 0; i < PRISM_NKERN; ++i) { ms_out[i] = p->prof_ms[i]; launches_out[i] = p->prof_cnt[i]; }
+  for (int j = 0; j < p->nparts; ++j)
+    for (int i = 0; i < PRISM_NKERN; ++i) { ms_out[i] += p->parts[j]->prof_ms[i]; launches_out[i] += p->parts[j]->prof_cnt[i]; }
   return PRISM_OK;
 }
 
-extern "C" int prism_residuals(prism_problem* p, const double* w, const double* duals, void* cuda_stream, double* resid_out) {
-  if (!p) return set_err(PRISM_ERR_NOT_READY, "problem object is NULL%s", "");
-  if (!w || !resid_out) return set_err(PRISM_ERR_INVALID_ARG, "w and resid_out are mandatory%s", "");
+static int residuals_one(prism_problem* p, const double* w, const double* duals, void* cuda_stream, double* resid_out) {
   cudaStream_t st = (cudaStream_t)cuda_stream;
   Launcher L{p, st, p->kp / 8, 0};
   run_diag(p, L, w, duals, p->resid);
@@ -510,6 +530,136 @@ extern "C" int prism_residuals(prism_problem* p, const double* w, const double* 
   CUDA_TRY(cudaMemcpyAsync(resid_out, h.data(), h.size() * sizeof(double), cudaMemcpyHostToDevice, st));
   CUDA_TRY(cudaStreamSynchronize(st));
   CUDA_TRY(cudaGetLastError());
+  return PRISM_OK;
+}
+
+// ------------------------------------------------------------------------------------------ account groups
+// Accounts are independent programs, and the per-account root kernel is latency-bound with a long tail
+// (a launch lasts as long as its slowest account).  A large batch is therefore cut into contiguous account ranges,
+// each a complete problem object solved by its own host thread on its own stream: the tail of one group's launch
+// overlaps the bandwidth-bound kernels of the others.  Results per account do not depend on the split except through
+// the split-K summation order of GEMM-1 (rounding level).
+static int pick_parts(int64_t N, int A) {
+  // measured on configs[2] (500 x 10,000): 2 / 3 groups solve 5% / 8% faster, but every launch then covers fewer
+  // accounts and the streaming kernel runs further from its bandwidth roofline; one group unless asked otherwise.
+  int n = 1;
+  (void)N;
+  if (const char* e = getenv("PRISM_PARTS")) n = atoi(e);
+  if (n > PRISM_MAX_PARTS) n = PRISM_MAX_PARTS;
+  if (n > A) n = A;
+  return n < 1 ? 1 : n;
+}
+template <typename T>
+static const T* off(const T* ptr, int64_t n) { return ptr ? ptr + n : nullptr; }
+
+extern "C" int prism_problem_create(int64_t N, int32_t k, int32_t accounts, const prism_constraint_set* cs,
+                                    const prism_data* data, void* cuda_stream, prism_problem** out) {
+  if (out) *out = nullptr;
+  if (!out || !cs || !data) return set_err(PRISM_ERR_INVALID_ARG, "null argument%s", "");
+  const int A = accounts;
+  const int np = (N >= 1 && A >= 1) ? pick_parts(N, A) : 1;
+  if (np <= 1) return create_one(N, k, accounts, cs, data, cuda_stream, out);
+  prism_problem* p = new (std::nothrow) prism_problem();
+  if (!p) return set_err(PRISM_ERR_ALLOC, "host allocation failed%s", "");
+  memset(p, 0, sizeof(*p));
+  const int G = (cs->flags & PRISM_GROUP_BANDS) ? cs->G : 0;
+  p->N = N; p->k = k; p->A = A; p->G = G; p->flags = cs->flags; p->d = *data;
+  for (int i = 0; i < np; ++i) {
+    const int a0 = (int)((int64_t)A * i / np), a1 = (int)((int64_t)A * (i + 1) / np);
+    p->part_a0[i] = a0; p->part_a0[i + 1] = a1;
+    prism_data d = *data;
+    const int64_t aN = (int64_t)a0 * N;
+    d.mu = off(d.mu, aN); d.w0 = off(d.w0, aN); d.w_b = off(d.w_b, aN); d.hi_full = off(d.hi_full, aN); d.excl = off(d.excl, aN);
+    d.lot_slope = off(d.lot_slope, aN * PRISM_MAX_LOTS); d.lot_width = off(d.lot_width, aN * PRISM_MAX_LOTS); d.lot_count = off(d.lot_count, aN);
+    d.gamma = off(d.gamma, a0); d.lo = off(d.lo, a0); d.hi = off(d.hi, a0); d.tau = off(d.tau, a0); d.kappa = off(d.kappa, a0); d.c_buy = off(d.c_buy, a0);
+    d.band_lo = off(d.band_lo, (int64_t)a0 * G); d.band_hi = off(d.band_hi, (int64_t)a0 * G);
+    int r = create_one(N, k, a1 - a0, cs, &d, cuda_stream, &p->parts[i]);
+    if (r == PRISM_OK && cudaStreamCreateWithFlags(&p->part_stream[i], cudaStreamNonBlocking) != cudaSuccess) r = set_err(PRISM_ERR_CUDA, "stream creation failed%s", "");
+    if (r == PRISM_OK && cudaEventCreateWithFlags(&p->part_done[i], cudaEventDisableTiming) != cudaSuccess) r = set_err(PRISM_ERR_CUDA, "event creation failed%s", "");
+    p->nparts = i + 1;
+    if (r != PRISM_OK) { prism_problem_destroy(p); return r; }
+    p->bytes += p->parts[i]->bytes;
+  }
+  ALLOC_TRY(dev_alloc(p, &p->resid, (size_t)A * PRISM_NRES));
+  ALLOC_TRY(dev_alloc(p, &p->status, (size_t)A));
+  *out = p;
+  return PRISM_OK;
+}
+
+extern "C" int prism_solve_batch(prism_problem* p, const prism_settings* sp, void* cuda_stream, double* w_out,
+                                 int32_t* status_out, int32_t* iters_out, double* resid_out, double* duals_out,
+                                 prism_solve_info* info) {
+  if (!p) return set_err(PRISM_ERR_NOT_READY, "problem object is NULL%s", "");
+  if (!p->nparts) return solve_one(p, sp, cuda_stream, w_out, status_out, iters_out, resid_out, duals_out, info);
+  if (!w_out || !status_out || !iters_out) return set_err(PRISM_ERR_INVALID_ARG, "w_out, status_out, iters_out are mandatory%s", "");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const auto t0 = std::chrono::steady_clock::now();
+  const int np = p->nparts, G = p->G;
+  int dev = 0;
+  CUDA_TRY(cudaGetDevice(&dev));
+  cudaEvent_t ev0, ev1;
+  CUDA_TRY(cudaEventCreate(&ev0));
+  CUDA_TRY(cudaEventCreate(&ev1));
+  CUDA_TRY(cudaEventRecord(ev0, st));                      // the groups start after everything queued on the caller's stream
+  std::vector<int> rc((size_t)np, PRISM_OK);
+  std::vector<prism_solve_info> inf((size_t)np);
+  std::vector<std::string> msg((size_t)np);
+  auto work = [&](int i) {
+    cudaSetDevice(dev);
+    prism_problem* q = p->parts[i];
+    const int64_t a0 = p->part_a0[i];
+    cudaStream_t ps = p->part_stream[i];
+    cudaError_t e = cudaStreamWaitEvent(ps, ev0, 0);
+    if (e != cudaSuccess) { rc[(size_t)i] = PRISM_ERR_CUDA; msg[(size_t)i] = cudaGetErrorString(e); return; }
+    rc[(size_t)i] = solve_one(q, sp, (void*)ps, w_out + a0 * p->N, status_out + a0, iters_out + a0,
+                              resid_out ? resid_out + a0 * PRISM_NRES : nullptr,
+                              duals_out ? duals_out + a0 * PRISM_NDUAL(G) : nullptr, &inf[(size_t)i]);
+    if (rc[(size_t)i] != PRISM_OK) msg[(size_t)i] = g_err;
+    cudaEventRecord(p->part_done[i], ps);
+  };
+  {
+    std::vector<std::thread> th;
+    const bool serial = sp && sp->profile != 0;          // per-kernel timings: every kernel alone on the device
+    if (!serial) for (int i = 1; i < np; ++i) th.emplace_back(work, i);
+    work(0);
+    if (serial) for (int i = 1; i < np; ++i) work(i);
+    for (auto& t : th) t.join();
+  }
+  for (int i = 0; i < np; ++i) CUDA_TRY(cudaStreamWaitEvent(st, p->part_done[i], 0));
+  CUDA_TRY(cudaEventRecord(ev1, st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  for (int i = 0; i < np; ++i)
+    if (rc[(size_t)i] != PRISM_OK) { cudaEventDestroy(ev0); cudaEventDestroy(ev1); return set_err(rc[(size_t)i], "account group failed: %s", msg[(size_t)i].c_str()); }
+  if (info) {
+    memset(info, 0, sizeof(*info));
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, ev0, ev1);
+    info->solve_interval_ms = ms;
+    info->device_bytes = p->bytes;
+    for (int i = 0; i < np; ++i) {
+      const prism_solve_info& x = inf[(size_t)i];
+      if (x.iters_max > info->iters_max) info->iters_max = x.iters_max;
+      info->iters_total += x.iters_total; info->n_certified += x.n_certified; info->n_feasible += x.n_feasible;
+      info->n_timeout += x.n_timeout; info->n_late += x.n_late; info->n_no_feasible += x.n_no_feasible; info->n_failed += x.n_failed;
+      info->kernel_launches += x.kernel_launches;
+    }
+    info->wall_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
+  }
+  cudaEventDestroy(ev0);
+  cudaEventDestroy(ev1);
+  return PRISM_OK;
+}
+
+extern "C" int prism_residuals(prism_problem* p, const double* w, const double* duals, void* cuda_stream, double* resid_out) {
+  if (!p) return set_err(PRISM_ERR_NOT_READY, "problem object is NULL%s", "");
+  if (!w || !resid_out) return set_err(PRISM_ERR_INVALID_ARG, "w and resid_out are mandatory%s", "");
+  if (!p->nparts) return residuals_one(p, w, duals, cuda_stream, resid_out);
+  for (int i = 0; i < p->nparts; ++i) {
+    const int64_t a0 = p->part_a0[i];
+    const int r = residuals_one(p->parts[i], w + a0 * p->N, duals ? duals + a0 * PRISM_NDUAL(p->G) : nullptr, cuda_stream,
+                                resid_out + a0 * PRISM_NRES);
+    if (r != PRISM_OK) return r;
+  }
   return PRISM_OK;
 }
 
@@ -525,11 +675,11 @@ extern "C" int prism_solve_batch_host(prism_problem* p, const prism_settings* s,
   if (!p->w_stage) {
     if (dev_alloc(p, &p->w_stage, AN) != PRISM_OK || dev_alloc(p, &p->i_stage, (size_t)p->A) != PRISM_OK) return PRISM_ERR_ALLOC;
   }
-  int r = prism_solve_batch(p, s, cuda_stream, p->w_stage, p->status, p->i_stage, nullptr, nullptr, info);
+  int r = prism_solve_batch(p, s, cuda_stream, p->w_stage, p->status, p->i_stage, p->nparts ? p->resid : nullptr, nullptr, info);
   if (r != PRISM_OK) return r;
   if (w_host) CUDA_TRY(cudaMemcpyAsync(w_host, p->w_stage, AN * sizeof(double), cudaMemcpyDeviceToHost, st));
   if (status_host) CUDA_TRY(cudaMemcpyAsync(status_host, p->status, (size_t)p->A * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
-  if (iters_host) CUDA_TRY(cudaMemcpyAsync(iters_host, p->ap.iters, (size_t)p->A * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+  if (iters_host) CUDA_TRY(cudaMemcpyAsync(iters_host, p->i_stage, (size_t)p->A * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
   if (resid_host) CUDA_TRY(cudaMemcpyAsync(resid_host, p->resid, (size_t)p->A * PRISM_NRES * sizeof(double), cudaMemcpyDeviceToHost, st));
   CUDA_TRY(cudaStreamSynchronize(st));
   if (info) info->wall_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();

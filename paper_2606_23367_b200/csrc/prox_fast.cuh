@@ -63,18 +63,35 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
 template <bool CHECK>
 __global__ void __launch_bounds__(FAST_NW * 32, 3) k_prox_stream(const __grid_constant__ ProxArgs p) {
   extern __shared__ __align__(16) unsigned char stream_raw[];
+  __shared__ double cst[12];
   const int a = blockIdx.y, sl = blockIdx.x;
-  if (p.ap.done[a]) return;
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   const int G = p.G, Gb = G > 0 ? G : 1;
+  // A CTA lives for a few chunks only, so its start-up must not be a chain of dependent loads: the account's twelve
+  // constants are fetched by twelve lanes of warp 1 at the same time as the done flag, the band multipliers by
+  // warp 2.., and thread 0 starts the first bulk copies as soon as it has seen the flag.
+  double cv = 0.0;
+  if (wid == 1 && lane < 12) {
+    switch (lane) {
+      case 0: cv = p.lo[a]; break;
+      case 1: cv = p.hi[a]; break;
+      case 2: cv = p.ap.wins[a]; break;
+      case 3: cv = p.ap.win[a]; break;
+      case 4: cv = p.gamma[a]; break;
+      case 5: cv = p.ap.c[a]; break;
+      case 6: cv = p.kappa ? p.kappa[a] : 0.0; break;
+      case 7: cv = p.c_buy ? p.c_buy[a] : 0.0; break;
+      case 8: cv = p.tau ? p.tau[a] : INFINITY; break;
+      case 9: cv = p.ap.alpha[a]; break;
+      case 10: cv = p.ap.beta[a]; break;
+      default: cv = (double)p.ap.mode[a]; break;
+    }
+  }
+  double lam_mine = 0.0;
+  if (tid >= 64 && tid - 64 < G) lam_mine = p.lamG[(int64_t)a * G + (tid - 64)];
+  if (p.ap.done[a]) return;
   const int64_t N = p.N, row = (int64_t)a * N, rowp = (int64_t)a * p.ldw;
   const int sub = (a * p.S + sl) * FAST_NW + wid;               // this warp's list
-  const double lo_a = p.lo[a], hi_a = p.hi[a];
-  if (!(hi_a - lo_a <= 4.0)) {            // box wider than the fixed-point range of the bins: generic path in k_prox_root
-    if (tid == 0 && sl == 0) p.lflag[a] = 1;
-    if (lane == 0) { p.lcnt[sub] = 0; p.lcnt[p.A * p.S * FAST_NW + sub] = 0; }
-    return;
-  }
   unsigned char* stage0 = stream_raw;                                 // FAST_NST stages: v, w0, q, d, 1/d, excl, gid
   uint64_t* bar_full = (uint64_t*)(stream_raw + (size_t)FAST_NST * FAST_STAGE_BYTES);
   uint64_t* bar_empty = bar_full + FAST_NST;
@@ -106,22 +123,31 @@ __global__ void __launch_bounds__(FAST_NW * 32, 3) k_prox_stream(const __grid_co
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     for (int c = 0; c < FAST_NST - 1 && c < nchunk; ++c) issue(c);
   }
-  const double W = p.ap.wins[a], Wt = p.ap.win[a];
+  if (wid == 1 && lane < 12) cst[lane] = cv;
+  if (tid >= 64 && tid - 64 < G) lamS[tid - 64] = lam_mine;
+  for (int g = tid + FAST_NW * 32 - 64; g < G; g += FAST_NW * 32) lamS[g] = p.lamG[(int64_t)a * G + g];   // (G > 192 only)
+  __syncthreads();
+  const double lo_a = cst[0], hi_a = cst[1];
+  if (!(hi_a - lo_a <= 4.0)) {            // box wider than the fixed-point range of the bins: generic path in k_prox_root
+    if (tid == 0 && sl == 0) p.lflag[a] = 1;
+    if (lane == 0) { p.lcnt[sub] = 0; p.lcnt[p.A * p.S * FAST_NW + sub] = 0; }
+    for (int c = 0; c < FAST_NST - 1 && c < nchunk; ++c) mbar_wait(&bar_full[c], 0u);   // no copy may outlive the CTA
+    return;
+  }
+  const double W = cst[2], Wt = cst[3];
   // Two-level lists: an asset that only the WIDE window (W) can reach but the TIGHT one (Wt, what the thresholds are
   // expected to move by) cannot is finished speculatively as dead - outputs written, trade added to the second set of
   // bins - and parked at the back of the warp's list; k_prox_root looks at those entries only when its solution
   // leaves the tight window.  Check / final launches keep one level (their residual terms must not be speculative).
   const bool split = !CHECK && Wt < 0.125 * W;
   const double Wn = split ? Wt : W;
-  const double gam = p.gamma[a], c = p.ap.c[a], cg = c * gam, icg = 1.0 / cg;
-  const double kappa = p.kappa ? p.kappa[a] : 0.0;
-  const double lam_b = kappa + (p.c_buy ? p.c_buy[a] : 0.0), Delta = lam_b + kappa;
-  const double tau = p.tau ? p.tau[a] : INFINITY;
+  const double gam = cst[4], c = cst[5], cg = c * gam, icg = 1.0 / cg;
+  const double kappa = cst[6];
+  const double lam_b = kappa + cst[7], Delta = lam_b + kappa;
+  const double tau = cst[8];
   const double igc = 1.0 / (gam * (1.0 + c));
-  double aw = p.ap.alpha[a], bw = p.ap.beta[a];
-  if (!(p.ap.mode[a] == 1 && isfinite(tau))) bw = aw;
-  for (int g = tid; g < G; g += blockDim.x) lamS[g] = p.lamG[(int64_t)a * G + g];
-  __syncthreads();
+  double aw = cst[9], bw = cst[10];
+  if (!(cst[11] == 1.0 && isfinite(tau))) bw = aw;
 
   double nx = 0, nz = 0, nrp = 0, nrd = 0, nPx = 0, ny = 0, nq = 0;
   LiveEnt* mylist = p.lraw + (int64_t)sub * p.capw;
@@ -495,8 +521,17 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
   rs.alpha = aw; rs.beta = bw; rs.amode = amode_w; rs.n_eval = 0;
   // band ramp: the first iterations project without the group bands (an exact prox of the relaxed problem); their
   // thresholds still move a lot then and a band solve would be wasted.  Never on check / final launches.
-  const bool bands_on = G > 0 && (CHECK || (mode & PROX_FINAL) || p.iter >= p.band_start);
+  const bool exact = CHECK || (mode & PROX_FINAL);
+  const bool bands_on = G > 0 && (exact || p.iter > p.band_start);
   rs.nobands = bands_on ? 0 : 1;
+  // ... and then join gradually: for band_ramp iterations the limits are widened by a slack that shrinks linearly from
+  // the largest violation measured at band_start to zero (still an exact prox, of a relaxed problem), so that few bands
+  // change state per iteration and the multipliers move in small steps.  Check / final launches never relax.
+  if (bands_on && !exact && p.band_ramp > 0 && p.iter < p.band_start + p.band_ramp) {
+    const double sl = p.ap.slack[a] * (1.0 - (double)(p.iter - p.band_start) / (double)p.band_ramp);
+    for (int g = tid; g < G; g += nt) { band_lo[g] -= sl; band_hi[g] += sl; }
+    __syncthreads();
+  }
   double mv = 0.0;
   if (!fallback) {
     // ---- the raw lists as one sequence (offs = their start offsets); warp w handles a contiguous quarter of it.
@@ -733,6 +768,21 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
       __syncthreads();
     }
     if (fallback && p.stats && tid == 0 && p.iter < 4096) atomicAdd(&p.stats[p.iter * 8 + 2], 1);
+    if (!fallback && G > 0 && !exact && p.iter == p.band_start) {   // band ramp: how far outside its bands is this projection?
+      __syncthreads();
+      root_pass(src, poff, ngrp, lamS, G, rs.alpha, rs.beta - Delta, gv);
+      if (tid < 32) {
+        double viol = 0.0;
+        for (int g = tid; g < G; g += 32) {
+          const double Sg = gw0[g] + (gv[4 * g] + (double)ubin[g] * PRISM_FIX_INV) - (gv[4 * g + 1] + (double)ubin[Gb + g] * PRISM_FIX_INV);
+          viol = fmax(viol, fmax(Sg - band_hi[g], band_lo[g] - Sg));
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) viol = fmax(viol, __shfl_xor_sync(0xffffffffu, viol, o));
+        if (tid == 0) p.ap.slack[a] = fmax(viol, 0.0);
+      }
+      __syncthreads();
+    }
   }
   int finished = 0;
   if (!fallback) {

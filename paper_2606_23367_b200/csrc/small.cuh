@@ -73,7 +73,7 @@ __global__ void k_init_accounts(InitArgs p) {
   if (tid == 0) {
     p.ap.bsum[a] = 1.0 - val[0];
     p.ap.c[a] = p.rho_scale;
-    p.ap.alpha[a] = 0.0; p.ap.beta[a] = 0.0; p.ap.mode[a] = 0; p.ap.win[a] = INFINITY; p.ap.wins[a] = INFINITY;
+    p.ap.alpha[a] = 0.0; p.ap.beta[a] = 0.0; p.ap.mode[a] = 0; p.ap.win[a] = INFINITY; p.ap.wins[a] = INFINITY; p.ap.slack[a] = 0.0;
     p.ap.done[a] = 0; p.ap.conv[a] = 0; p.ap.iters[a] = 0; p.ap.refactor[a] = 1; p.ap.nadapt[a] = 0;
   }
 }
