@@ -324,6 +324,8 @@ static ProxArgs make_prox_args(prism_problem* p, const prism_settings& s, double
   if (const char* e = getenv("PRISM_PROX_WIN_MULT")) a.win_mult = atof(e);
   a.band_start = 20;
   if (const char* e = getenv("PRISM_PROX_BAND_START")) a.band_start = atoi(e);
+  a.band_wide = 1;
+  if (const char* e = getenv("PRISM_PROX_BAND_WIDE")) a.band_wide = atoi(e);
   a.band_ramp = 0;         // measured on configs[2]: a 10 / 20-iteration slack ramp costs 6% / 23% (the thresholds keep moving)
   if (const char* e = getenv("PRISM_PROX_BAND_RAMP")) a.band_ramp = atoi(e);
   a.win_ratio = 16.0;

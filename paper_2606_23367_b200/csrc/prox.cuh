@@ -56,6 +56,7 @@ struct ProxArgs {
   double win_mult;         // next window = win_mult x (movement of the thresholds in this launch)
   double win_ratio;        // streaming pass: its (wide) window = win_ratio x the solve's (tight) window
   int32_t band_start;      // streaming form: group bands join the projection after this iteration (their multipliers are 0 before)
+  int32_t band_wide;       // 1: the launch in which the bands join runs with an infinite window
   int32_t band_ramp;       // ... with limits widened by slack_a (1 - (iter - band_start) / band_ramp) for band_ramp iterations
   // streaming form (prox_fast.cuh): per-warp live lists, their compacted copy, fixed-point bins of the dead assets
   struct LiveEnt* lraw;    // [A][S * 8][capw]

@@ -859,8 +859,11 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
       double Ws = p.win_ratio * next_window(p, alpha, beta, mv);
       const int nl = offs[nlist_used] + (nlist_used == nsub ? nback_s : 0);   // live assets of the streaming window
       if (nl < 256) Ws = fmax(Ws, nl < 64 ? 2.0 * W : W);
-      if (p.iter < 2) Ws = INFINITY;
-      p.ap.win[a] = p.iter < 2 ? INFINITY : next_window(p, alpha, beta, mv); p.ap.wins[a] = Ws;
+      // ... and for the launch in which the group bands join (band ramp): the thresholds jump then, a finite window
+      // would send the accounts whose bands bind through the every-asset path
+      const bool wide_next = p.iter < 2 || (G > 0 && p.iter == p.band_start && p.band_wide);
+      if (wide_next) Ws = INFINITY;
+      p.ap.win[a] = wide_next ? INFINITY : next_window(p, alpha, beta, mv); p.ap.wins[a] = Ws;
       if (finished) {                                    // H6: w_out already holds z
         p.ap.done[a] = 1; p.ap.iters[a] = p.iter;
         atomicAdd(&p.counters[0], 1);

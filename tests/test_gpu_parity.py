@@ -190,7 +190,7 @@ def test_edge_cases():
         P.close()
 
 
-@pytest.mark.parametrize("cfg,n_sample", [("cfg2", 3), ("cfg3", 2)])
+@pytest.mark.parametrize("cfg,n_sample", [("cfg1", 4), ("cfg2", 3), ("cfg3", 2)])
 def test_full_size_sampled_accounts(cfg, n_sample):
     """BASELINE.json full sizes in the launch configuration bench.py times; the oracle solves a sample of accounts
     one by one, the rest are certified through properties that hold at any size (gates, KKT residuals, statuses)."""
@@ -204,4 +204,31 @@ def test_full_size_sampled_accounts(cfg, n_sample):
     sample = sorted(rng.choice(inst.A, size=n_sample, replace=False).tolist())
     W, res = _oracle(inst, accounts=sample)
     _check_against_oracle(inst, r, W, res, accounts=sample)
+    P.close()
+
+
+def test_full_size_cfg4_properties():
+    """configs[4] at full width (32 x 384,800, k = 100, fp32 loadings).  The oracle cannot finish one such account in
+    minutes (structured interior point: > 15 min), so every account is certified through properties that hold at
+    any size: statuses, scaled residuals, the library's gates, and - for sampled accounts - the independent checker's
+    gates and the KKT certificate of the returned weights with the returned multipliers.
+    Element-wise parity of this family with the oracle is the scaled-down case cfg4_small above."""
+    from oracle import kkt_check, problem
+    inst = gen.by_name("cfg4")
+    P, r = _solve_gpu(inst)
+    st = r.status.cpu().numpy(); rs = r.resid.cpu().numpy(); w = r.w.cpu().numpy(); du = r.duals.cpu().numpy()
+    assert (st == 0).all(), np.bincount(st)
+    assert rs[:, 0:4].max() <= TOL_GATE and rs[:, 7].max() <= TOL_RES and rs[:, 8].max() <= TOL_RES
+    assert rs[:, 4].max() <= 1e-5 and rs[:, 5].max() <= 1e-9
+    for a in (0, 17, 31):
+        acc = problem.account_from_instance(inst, a)
+        feas = kkt_check.feasibility(acc, w[a])
+        assert max(feas.values()) <= TOL_GATE, feas
+        assert abs(rs[a, 0] - feas["r_budget"]) <= 1e-12 and abs(rs[a, 3] - feas["r_turnover"]) <= 1e-12
+        fg = problem.objective(acc, w[a])
+        assert abs(rs[a, 6] - fg) <= 1e-12 * max(1.0, abs(fg))
+        k = kkt_check.kkt(acc, w[a], dict(nu=du[a, 0], theta=du[a, 1], lam_hi=du[a, 2:2], lam_lo=du[a, 2:2]), delta=1e-9)
+        scale = max(np.max(np.abs(acc.mu)), 1e-12)
+        assert k["r_stat"] <= 1e-4 * scale and k["r_comp"] <= 1e-9 and k["min_multiplier"] >= -1e-15, k
+        assert abs(rs[a, 4] - k["r_stat"]) <= 1e-10
     P.close()
