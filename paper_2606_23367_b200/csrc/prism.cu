@@ -341,7 +341,8 @@ static void launch_prox(Launcher& L, ProxArgs& a, int mode, int iter) {
   if (p->fast) {
     const bool chk = (mode & (PROX_CHECK | PROX_FINAL)) != 0;     // the final extraction also needs w_out
     const dim3 grid((unsigned)p->S, (unsigned)p->A);
-    const size_t sm = stream_smem_bytes(p->G), smr = root_smem_bytes(p->G, 2 * p->S * FAST_NW);
+    const size_t sm = stream_smem_bytes(p->G);
+    const size_t smr = root_smem_bytes(p->G, 2 * p->S * FAST_NW);
     L.begin(PRISM_K_PROX);
     if (chk) k_prox_stream<true><<<grid, FAST_NW * 32, sm, st>>>(a);
     else k_prox_stream<false><<<grid, FAST_NW * 32, sm, st>>>(a);

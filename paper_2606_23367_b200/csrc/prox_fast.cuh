@@ -461,6 +461,10 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
   if (p.ap.done[a]) return;
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, nt = blockDim.x, nw = nt >> 5;
   if (tid == 0) nback_s = 0;
+  long long tk0 = clock64();
+  auto tick = [&](int k) {                 // (debug) phase timers: thread 0, units of 64 cycles
+    if (p.stats && tid == 0 && p.iter < 1024) { const long long t = clock64(); atomicAdd(&p.stats[(3072 + p.iter) * 8 + k], (int)((t - tk0) >> 6)); tk0 = t; }
+  };
   const int G = p.G, Gb = G > 0 ? G : 1;
   const int64_t N = p.N, row = (int64_t)a * N, rowp = (int64_t)a * p.ldw;
   const int nsub = p.S * FAST_NW;
@@ -651,9 +655,11 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
       if (nb) atomicAdd(&nback_s, nb);
     }
     for (int att = 0; att < 2; ++att) {
+      tick(0);
       scan_lists(att);                                   // level 0: the fronts; level 1: fronts and backs
       nlist_used = nlist;
       sort_lists(split && att == 0);
+      tick(1);
       rs.alpha = aw; rs.beta = bw; rs.amode = amode_w;
       for (int g = tid; g < G; g += nt) lamS[g] = lamW[g];
       __syncthreads();
@@ -668,6 +674,7 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
       const double cPt = src.cPt, cRt = src.cRt;
       double al = aw, be = bw;
       int amode = amode_w;
+      tick(2);
       bool ok = false;
       int why = 4;                                          // (debug) 1 singular band, 2 det, 3 den, 4 passes, 5 NaN
       for (int g = tid; g < G; g += nt) act[g] = lamS[g] > 0.0 ? 1 : (lamS[g] < 0.0 ? -1 : 0);
@@ -745,6 +752,7 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
         al += dal; be += dbe;
         __syncthreads();
       }
+      tick(3);
       if (ok) { rs.alpha = al; rs.beta = be; rs.amode = amode; }
       else {
         if (p.stats && tid == 0 && p.iter < 4096) { atomicAdd(&p.stats[p.iter * 8 + 3], 1); atomicAdd(&p.stats[(2048 + p.iter) * 8 + why], 1); }
@@ -758,6 +766,7 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
         rs.alpha = keep ? al : aw; rs.beta = keep ? be : bw; rs.amode = keep ? amode : amode_w;
         prox_rootfind<false>(p, sgrp, a, b, tau, Delta, sh, rs);
       }
+      tick(4);
       double mv_l = 0.0;
       for (int g = 0; g < G; ++g) mv_l = fmax(mv_l, fabs(lamS[g] - lamW[g]));
       mv = fmax(fmax(fabs(rs.alpha - aw), fabs(rs.beta - bw)), mv_l);
@@ -790,31 +799,52 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
     const double alpha = rs.alpha, beta = rs.beta, bdf = beta - Delta;
     const int nlist_o = nlist_used, nraw_all = offs[nlist_o];
     double nx = 0, nz = 0, nrp = 0, nrd = 0, nPx = 0, ny = 0, nq = 0;
-    for (int j = tid; j < nraw_all; j += nt) {           // every entry of the lists the solve used (the others are finished)
-      int lo = 0, hi = nlist_o;
-      while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (offs[mid] <= j) lo = mid; else hi = mid; }
-      const int pos = j - offs[lo];
-      const LiveEnt* ep = p.lraw + (int64_t)a * nsub * p.capw +
-                          (lo < nsub ? (int64_t)lo * p.capw + pos : (int64_t)(lo - nsub) * p.capw + (p.capw - 1 - pos));
-      const double2 ea = __ldg((const double2*)ep), eb = __ldg((const double2*)ep + 1);
-      ElemConst e; int g; double mvb, mvs;
-      const int64_t i = src.decode(ea, eb, e, g);
-      const double lg = G ? lamS[g] : 0.0;
-      const double tr = buy_amt(e, alpha + lg, mvb) - sell_amt<false>(e, bdf + lg, nullptr, nullptr, 0, mvs);
-      const double z = e.w0 + tr;
-      const double rho = cg * p.d[i];
-      const double y = e.T + lam_b - tr * rho;
-      const double qi = p.q ? p.q[rowp + i] : -p.mu[row + i];
-      const double r = rho * z - y - qi;
-      const double rt = r * (e.ir * cg) * igc;
-      p.rt[rowp + i] = rt;
-      p.cc[rowp + i] = rt - z;
-      if (CHECK) {
-        p.w_out[row + i] = z;
-        const double x = p.xs[rowp + i], pq = p.pxq[rowp + i];
-        nx = fmax(nx, fabs(x)); nz = fmax(nz, fabs(z)); nrp = fmax(nrp, fabs(x - z));
-        nrd = fmax(nrd, fabs(pq + y)); nPx = fmax(nPx, fabs(pq - qi)); ny = fmax(ny, fabs(y)); nq = fmax(nq, fabs(qi));
-        if (!(z == z) || !(x == x) || !(pq == pq)) nrp = INFINITY;
+    // every entry of the lists the solve used (the others are finished).  Latency-bound (entry -> asset index -> d, q):
+    // the loads of four entries, then of their four (d, q) pairs, are issued together.
+    for (int j0 = tid; j0 < nraw_all; j0 += 4 * nt) {
+      double2 ea4[4], eb4[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int j = j0 + u * nt;
+        ea4[u] = make_double2(0.0, 0.0); eb4[u] = make_double2(0.0, 0.0);
+        if (j < nraw_all) {
+          int lo = 0, hi = nlist_o;
+          while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (offs[mid] <= j) lo = mid; else hi = mid; }
+          const int pos = j - offs[lo];
+          const LiveEnt* ep = p.lraw + (int64_t)a * nsub * p.capw +
+                              (lo < nsub ? (int64_t)lo * p.capw + pos : (int64_t)(lo - nsub) * p.capw + (p.capw - 1 - pos));
+          ea4[u] = __ldg((const double2*)ep); eb4[u] = __ldg((const double2*)ep + 1);
+        }
+      }
+      double d4[4], q4[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int64_t i = (int64_t)((uint32_t)__double_as_longlong(eb4[u].y) & ((1u << PROX_META_IDX_BITS) - 1u));
+        d4[u] = 0.0; q4[u] = 0.0;
+        if (j0 + u * nt < nraw_all) { d4[u] = p.d[i]; q4[u] = p.q ? p.q[rowp + i] : -p.mu[row + i]; }
+      }
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        if (j0 + u * nt >= nraw_all) continue;
+        ElemConst e; int g; double mvb, mvs;
+        const int64_t i = src.decode(ea4[u], eb4[u], e, g);
+        const double lg = G ? lamS[g] : 0.0;
+        const double tr = buy_amt(e, alpha + lg, mvb) - sell_amt<false>(e, bdf + lg, nullptr, nullptr, 0, mvs);
+        const double z = e.w0 + tr;
+        const double rho = cg * d4[u];
+        const double y = e.T + lam_b - tr * rho;
+        const double qi = q4[u];
+        const double r = rho * z - y - qi;
+        const double rt = r * (e.ir * cg) * igc;
+        p.rt[rowp + i] = rt;
+        p.cc[rowp + i] = rt - z;
+        if (CHECK) {
+          p.w_out[row + i] = z;
+          const double x = p.xs[rowp + i], pq = p.pxq[rowp + i];
+          nx = fmax(nx, fabs(x)); nz = fmax(nz, fabs(z)); nrp = fmax(nrp, fabs(x - z));
+          nrd = fmax(nrd, fabs(pq + y)); nPx = fmax(nPx, fabs(pq - qi)); ny = fmax(ny, fabs(y)); nq = fmax(nq, fabs(qi));
+          if (!(z == z) || !(x == x) || !(pq == pq)) nrp = INFINITY;
+        }
       }
     }
     if (CHECK) {
@@ -846,6 +876,7 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
       }
     }
   }
+  tick(5);
   if (!fallback) {
     // ---------------------------------------------------------------- commit the account's state
     if (mode & PROX_FINAL) finished = 1;                 // (CHECK instantiation: w_out holds z)
