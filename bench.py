@@ -26,6 +26,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 PROX_BYTES_PER_ELEM = 41.0      # v 8 + w0 8 + mu 8 + exclusion mask 1 read; r~ 8 + c 8 written (kernel table)
+PROX_NCU_TRAFFIC_BYTES = 174.35e6   # k_prox_stream<0>, one launch, all 500 accounts active (profiles/r1c_prox_ncu_full.md)
 PROX_CHECK_EXTRA_BYTES = 24.0   # check iterations: x 8 + (P x + q) 8 read, w_out 8 written (kernel table)
 
 
@@ -238,13 +239,22 @@ def main():
     elem_iters = float(N) * float(rp.info["iters_total"])          # account-iterations x N: elements the prox launches processed
     # check launches (every check_every-th iteration of an account) also read x and P x + q and write w_out: + 24 B
     it_prof = rp.iters.cpu().numpy().astype(np.int64)
-    check_elems = float(N) * float((it_prof // int(prof.check_every)).sum())
+    ce, fc = int(prof.check_every), int(prof.first_check)
+    n_checks = np.maximum(it_prof // ce - (fc + ce - 1) // ce + 1, 0)         # checks at iterations ceil(fc/ce) ce, ... <= iters
+    check_elems = float(N) * float(n_checks.sum())
     prox_bytes_per_launch = (PROX_BYTES_PER_ELEM * elem_iters + PROX_CHECK_EXTRA_BYTES * check_elems) / max(prox["launches"], 1)
     prox_ms_per_launch = prox["ms"] / max(prox["launches"], 1)
     achieved = prox_bytes_per_launch / (prox_ms_per_launch * 1e-3) / 1e9
     roofline = {"bound": "hbm", "kernel": "k_prox_stream (H4/H5 fused projection + rhs assembly + residual terms, streaming pass)",
                 "achieved": achieved, "peak": peak,
-                "unit": "GB/s", "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                "unit": "GB/s", "frac": achieved / peak,
+                # dram__bytes_read.sum + dram__bytes_write.sum of one full-batch launch (500 accounts x 10,000), from the
+                # ncu --set full capture summarised in profiles/r1c_prox_ncu_full.md; only meaningful for the cfg2 batch
+                "traffic": PROX_NCU_TRAFFIC_BYTES if (args.config == "cfg2" and not args.accounts) else None,
+                "traffic_source": "profiles/r1c_prox_ncu_full.md (ncu --set full, one launch with all accounts active: 205 MB algorithmic)",
+                "peak_source": peak_src,
+                "factor_gemm_tensor_pipe": {"gemm1_dmma_pct_of_peak": 67.4, "gemm2_dmma_pct_of_peak": 43.0,
+                                            "source": "profiles/r1c_gemm_ncu_full.md (sm__inst_executed_pipe_tensor_subpipe_dmma, fp64 mma.sync)"},
                 "bytes_per_launch": prox_bytes_per_launch, "ms_per_launch": prox_ms_per_launch,
                 "dominant_by_time": dom,
                 "kernel_share": {n: round(v["ms"] / tot_k, 4) for n, v in kt.items()},

@@ -54,8 +54,25 @@ def test_header_constants_match_binding():
     assert int(flags["PRISM_BENCHMARK_SHIFT"]) == gen.F_BENCHMARK_SHIFT and int(flags["PRISM_EXCLUSION"]) == gen.F_EXCLUSION
     assert len(binding.STATUS_NAMES) == 6                                               # Table 14
     # struct sizes (natural alignment) as the C compiler lays them out
-    assert C.sizeof(binding.Settings) == 80 and C.sizeof(binding.ConstraintSet) == 12
+    assert C.sizeof(binding.Settings) == 88 and C.sizeof(binding.ConstraintSet) == 12
     assert C.sizeof(binding.Data) == 22 * 8
+
+
+def test_struct_sizes_match_the_c_compiler(tmp_path):
+    """The ctypes mirrors in binding.py against sizeof() of include/prism.h as gcc lays the structs out."""
+    import shutil
+    import subprocess
+    from paper_2606_23367_b200 import binding
+    if shutil.which("gcc") is None:
+        pytest.skip("gcc not available")
+    src = tmp_path / "sz.c"
+    src.write_text('#include <stdio.h>\n#include "prism.h"\nint main(void) { printf("%zu %zu %zu %zu\\n", sizeof(prism_settings), '
+                   'sizeof(prism_constraint_set), sizeof(prism_data), sizeof(prism_solve_info)); return 0; }\n')
+    exe = tmp_path / "sz"
+    inc = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "include")
+    subprocess.run(["gcc", "-I", inc, str(src), "-o", str(exe)], check=True)
+    sizes = [int(x) for x in subprocess.run([str(exe)], check=True, capture_output=True, text=True).stdout.split()]
+    assert sizes == [C.sizeof(binding.Settings), C.sizeof(binding.ConstraintSet), C.sizeof(binding.Data), C.sizeof(binding.SolveInfo)]
 
 
 def test_invalid_arguments_are_errors_not_crashes(lib):
