@@ -758,7 +758,10 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
         if (p.stats && tid == 0 && p.iter < 4096) { atomicAdd(&p.stats[p.iter * 8 + 3], 1); atomicAdd(&p.stats[(2048 + p.iter) * 8 + why], 1); }
         // nested robust solver on the same grouped list (lean passes through the SrcGrouped overloads)
         // (it continues from where the Newton iteration stopped when that state is usable)
-        const bool keep = al == al && be == be && fabs(al - aw) <= 0.5 * W && fabs(be - bw) <= 0.5 * W;
+        // (not with an infinite window while bands are in play - the launch in which they join: the multipliers a failed
+        // Newton iteration leaves there can be far off, and the Gauss-Seidel rounds of the robust solver then crawl:
+        // 12,000 passes for one account of configs[2] seed 1, minutes for seed 3)
+        const bool keep = al == al && be == be && fabs(al - aw) <= 0.5 * W && fabs(be - bw) <= 0.5 * W && (W < INFINITY || !bands_on);
         __syncthreads();
         if (!keep) for (int g = tid; g < G; g += nt) lamS[g] = lamW[g];
         if (tid == 0) { sgrp.L = &src; sgrp.poff = poff; sgrp.ngrp = ngrp; sgrp.gv = gv; }
