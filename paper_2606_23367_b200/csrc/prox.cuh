@@ -555,7 +555,16 @@ struct RootState {
   int amode;             // 0: turnover cap inactive (alpha == beta), 1: active
   int n_eval;            // trial evaluations (passes over the source) spent
   int nobands;           // in: 1 = solve with every band multiplier fixed at 0 (band ramp of the first iterations)
+  int capped;            // out: 1 = the evaluation budget ran out (PROX_EVAL_CAP): the thresholds are the last iterate, NOT a
+                         // solution.  The caller may use them for a plain iteration (an inexact prox) but must not
+                         // certify convergence with them.
 };
+// Budget of trial evaluations of one nested robust solve: its worst case (Gauss-Seidel rounds x bracketed steps x inner
+// root finds) is ~1e5 passes, and one account that wanders there holds its whole launch.  Regular solves need <= ~300;
+// the budget only bounds the damage of a pathological one (readings: robust root find).
+#ifndef PROX_EVAL_CAP
+#define PROX_EVAL_CAP 2000
+#endif
 
 // Solves for (alpha, beta, lambda_g) of account a over the assets of `src` (see the header of this file).
 // b: budget in trade space, tau: turnover cap (inf = none), Delta = 2 kappa + c_buy.  sh.lamS holds the warm-start
@@ -620,7 +629,7 @@ __device__ __noinline__ void prox_rootfind(const ProxArgs& p, const Src& src, in
   auto solve_ab = [&](int sel) {
     double lmin = 0.0, lmax = 0.0;
     for (int g = 0; g < G; ++g) { lmin = fmin(lmin, lamS[g]); lmax = fmax(lmax, lamS[g]); }
-    for (int attempt = 0; attempt < 4; ++attempt) {
+    for (int attempt = 0; attempt < 4 && n_eval <= PROX_EVAL_CAP; ++attempt) {
       const double alo = a_min - lmax, ahi = a_max - lmin, blo = b_min - lmax, bhi = b_max - lmin;
       bool need = false;
       if (amode == 1) {
@@ -630,6 +639,7 @@ __device__ __noinline__ void prox_rootfind(const ProxArgs& p, const Src& src, in
         for (int it = 0; it < 80; ++it) {
           need = root_step(ra_, P, sP, Pt, -1, tol) | root_step(rb_, R, sR, Rt, +1, tol);
           if (need || (ra_.done && rb_.done)) break;
+          if (n_eval > PROX_EVAL_CAP) break;
           if (ra_.sect || rb_.sect) section(&ra_, &rb_, nullptr);
           eval(ra_.x, rb_.x, sel);
         }
@@ -644,6 +654,7 @@ __device__ __noinline__ void prox_rootfind(const ProxArgs& p, const Src& src, in
         for (int it = 0; it < 80; ++it) {
           need = root_step(rn, P - R, sP + sR, b, -1, tol);
           if (need || rn.done) break;
+          if (n_eval > PROX_EVAL_CAP) break;
           if (rn.sect) section(nullptr, nullptr, &rn);
           eval(rn.x, rn.x, sel);
         }
@@ -716,7 +727,7 @@ __device__ __noinline__ void prox_rootfind(const ProxArgs& p, const Src& src, in
     }
   }
 
-  for (int round = 0; round < 2 * G + 2; ++round) {
+  for (int round = 0; round < 2 * G + 2 && n_eval <= PROX_EVAL_CAP; ++round) {
     solve_ab(-1);
     if (G == 0) break;
     // all group sums at the current solution (deterministic binned pass)
@@ -744,7 +755,7 @@ __device__ __noinline__ void prox_rootfind(const ProxArgs& p, const Src& src, in
     const double gw = sh.gw0[sel];
     double m = sgn * lamS[sel], mlo = 0.0, mhi = Lmax;
     bool lo_known = false;      // h(mlo) > 0 established
-    for (int it = 0; it < 60; ++it) {
+    for (int it = 0; it < 60 && n_eval <= PROX_EVAL_CAP; ++it) {
       __syncthreads();
       if (tid == 0) lamS[sel] = sgn * m;
       __syncthreads();
@@ -766,6 +777,7 @@ __device__ __noinline__ void prox_rootfind(const ProxArgs& p, const Src& src, in
   }
   __syncthreads();
   rs.alpha = alpha; rs.beta = beta; rs.amode = amode; rs.n_eval += n_eval;
+  if (n_eval > PROX_EVAL_CAP) rs.capped = 1;
 }
 
 __device__ __forceinline__ double next_window(const ProxArgs& p, double alpha, double beta, double mv) {
@@ -791,7 +803,7 @@ __device__ __forceinline__ void prox_body(const ProxArgs& p, int mode, Src& src,
   __syncthreads();
 
   RootState rs;
-  rs.alpha = p.ap.alpha[a]; rs.beta = p.ap.beta[a]; rs.amode = p.ap.mode[a]; rs.n_eval = 0; rs.nobands = 0;
+  rs.alpha = p.ap.alpha[a]; rs.beta = p.ap.beta[a]; rs.amode = p.ap.mode[a]; rs.n_eval = 0; rs.nobands = 0; rs.capped = 0;
   if (!(rs.amode == 1 && isfinite(tau))) { rs.amode = 0; rs.beta = rs.alpha; }
   const double alpha_w = rs.alpha, beta_w = rs.beta;       // warm start (previous iteration's thresholds)
   const int amode_w = rs.amode;
@@ -801,7 +813,7 @@ __device__ __forceinline__ void prox_body(const ProxArgs& p, int mode, Src& src,
     prox_rootfind<LOTS>(p, src, a, b, tau, Delta, sh, rs);
     if (src.window_ok(rs.alpha, rs.beta, lamS)) break;
     // the solution left the window the live list was built for: rebuild it with every asset and solve again
-    rs.alpha = alpha_w; rs.beta = beta_w; rs.amode = amode_w;
+    rs.alpha = alpha_w; rs.beta = beta_w; rs.amode = amode_w; rs.capped = 0;
     __syncthreads();
     for (int g = tid; g < G; g += nt) lamS[g] = lam_w[g];
     __syncthreads();
@@ -819,7 +831,7 @@ __device__ __forceinline__ void prox_body(const ProxArgs& p, int mode, Src& src,
     prox_check<LOTS>(p, src, lamS, a, alpha, bdf, lam_b, cg, sh.scratch, rr);
     const double rp = rr[0], rd = rr[1];
     const bool bad = !(rp < INFINITY) || !(rd < INFINITY);
-    const bool conv = !bad && rp <= p.eps && rd <= p.eps;
+    const bool conv = !bad && rp <= p.eps && rd <= p.eps && !rs.capped;      // never certify on an unfinished root find
     if (tid == 0) {
       p.resid[(int64_t)a * PRISM_NRES + PRISM_R_PRIMAL] = rp;
       p.resid[(int64_t)a * PRISM_NRES + PRISM_R_DUAL] = rd;

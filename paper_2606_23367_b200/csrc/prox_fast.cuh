@@ -522,7 +522,7 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
   bool fallback = generic != 0;
   int nlist_used = nsub;
   RootState rs;
-  rs.alpha = aw; rs.beta = bw; rs.amode = amode_w; rs.n_eval = 0;
+  rs.alpha = aw; rs.beta = bw; rs.amode = amode_w; rs.n_eval = 0; rs.capped = 0;
   // band ramp: the first iterations project without the group bands (an exact prox of the relaxed problem); their
   // thresholds still move a lot then and a band solve would be wasted.  Never on check / final launches.
   const bool exact = CHECK || (mode & PROX_FINAL);
@@ -660,7 +660,7 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
       nlist_used = nlist;
       sort_lists(split && att == 0);
       tick(1);
-      rs.alpha = aw; rs.beta = bw; rs.amode = amode_w;
+      rs.alpha = aw; rs.beta = bw; rs.amode = amode_w; rs.capped = 0;
       for (int g = tid; g < G; g += nt) lamS[g] = lamW[g];
       __syncthreads();
       // ---- semismooth Newton on (alpha, beta, lambda_g of the active bands) jointly: one pass over the list per step.
@@ -862,7 +862,7 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
       for (int q = 0; q < 7; ++q) val[q] = fmax(val[q], chk[q]);
       const double rp = val[2] / fmax(fmax(val[0], val[1]), 1e-300);
       const double rd = val[3] / fmax(fmax(val[4], fmax(val[5], val[6])), 1e-300);
-      const bool conv = rp <= p.eps && rd <= p.eps;
+      const bool conv = rp <= p.eps && rd <= p.eps && !rs.capped;             // never certify on an unfinished root find
       if (!(rp < INFINITY) || !(rd < INFINITY)) fallback = true;             // NaN / Inf: the generic path classifies it
       else if (!conv && p.adapt && p.iter >= PRISM_ADAPT_START && p.iter - p.ap.nadapt[a] >= PRISM_ADAPT_EVERY) {
         const double ratio = sqrt(rp / fmax(rd, 1e-300));
