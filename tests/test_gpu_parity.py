@@ -248,3 +248,36 @@ def test_full_size_cfg2_other_seeds_no_root_find_stall(seed):
     assert rs[:, 0:4].max() <= TOL_GATE and rs[:, 7].max() <= TOL_RES and rs[:, 8].max() <= TOL_RES
     assert r.info["solve_interval_ms"] < 1000.0, r.info
     P.close()
+
+
+@pytest.mark.parametrize("kw", [dict(alpha=1.8, rho_scale=50.0), dict(alpha=1.3, check_every=7, first_check=0),
+                                dict(rho_scale=300.0, first_check=10), dict(alpha=1.9, adapt_rho=0)])
+@pytest.mark.parametrize("case", ["cfg2_stream_tight", "cfg1_stream", "cfg3_small"])
+def test_solver_settings_do_not_change_the_answer(case, kw):
+    """The method is an iteration towards the unique minimiser: relaxation, rho scale, check cadence (including checks
+    inside the band ramp, first_check = 0) and rho adaptation change the path, not the answer.  Same parity bar."""
+    inst = CASES[case]()
+    W, res = _oracle(inst)
+    P, r = _solve_gpu(inst, **kw)
+    _check_against_oracle(inst, r, W, res)
+    P.close()
+
+
+def test_account_groups_match_single_group(monkeypatch):
+    """PRISM_PARTS: account groups solved concurrently on their own streams and host threads return, per account, the
+    result of the single-group solve up to the split-K summation order of GEMM-1 (rounding level), and the same
+    statuses; prism_residuals and the host-buffer lane work on the grouped object too."""
+    import torch
+    import paper_2606_23367_b200 as pr
+    inst = gen.config2(N=2560, k=50, A=9)
+    P1, r1 = _solve_gpu(inst)
+    monkeypatch.setenv("PRISM_PARTS", "3")
+    P3 = pr.Problem(inst)
+    r3 = P3.solve()
+    assert (r1.status.cpu().numpy() == 0).all() and (r3.status.cpu().numpy() == 0).all()
+    assert float((r1.w - r3.w).abs().max()) <= 1e-6
+    assert r3.info["n_certified"] == inst.A and r3.info["iters_total"] == int(r3.iters.sum())
+    rs = P3.residuals(r3.w, r3.duals).cpu().numpy()
+    assert np.nanmax(np.abs(rs[:, 0:4])) <= TOL_GATE
+    assert np.allclose(rs[:, 6], r3.resid.cpu().numpy()[:, 6], rtol=0, atol=1e-12)
+    P1.close(); P3.close()
