@@ -326,6 +326,25 @@ __host__ __device__ inline size_t root_smem_bytes(int G, int nsub) {
   return (size_t)(16 * 32 + 4 * Gb + 6 * Gb + 6 * Gb + 8 + 4 * (Gb + 4)) * 8 + (size_t)(nsub + 1 + 4 * Gb + 3 * Gb + 16 + ROOT_NSL) * 4 + 32 + (size_t)ROOT_SCAP * 32;
 }
 
+// Sum over the block of terms that only the first `nfront` threads hold (the others pass zeros): with nfront <= 32
+// warp 0 alone reduces and publishes - one butterfly and one barrier less than block_reduce on the critical path of
+// every pass, and the same bits (block_reduce would add the other warps' zeros).
+template <int NV>
+__device__ __forceinline__ void front_sum(double (&val)[NV], double* scratch, int nfront) {
+  if (nfront > 32) { block_reduce<NV, 0>(val, scratch); return; }
+  if (threadIdx.x < 32) {
+#pragma unroll
+    for (int q = 0; q < NV; ++q) {
+      const double x = warp_sum(val[q]);
+      if ((threadIdx.x & 31) == 0) scratch[q] = x;
+    }
+  }
+  __syncthreads();
+#pragma unroll
+  for (int q = 0; q < NV; ++q) val[q] = scratch[q];
+  __syncthreads();      // scratch may be reused by the next call
+}
+
 // One pass over the grouped list: per (pseudo-)group q the buys, sells and their slopes at thresholds (al, bd + Delta)
 // shifted by the group's multiplier -> gv[4 q .. 4 q + 3].  Warp w owns the groups w, w + nw, ...; fixed order.
 // buys, sells and slopes of one list entry at thresholds (a0, b0); the common class (inside its box) without branches
@@ -392,7 +411,7 @@ __device__ __noinline__ void prox_eval(const SrcGrouped& s, const double* lamS, 
 #pragma unroll
     for (int q = 0; q < 4; ++q) val[q] = s.gv[4 * threadIdx.x + q];
   }
-  block_reduce<4, 0>(val, scratch);
+  front_sum<4>(val, scratch, s.ngrp);
   out[0] = val[0] + s.L->cPt; out[1] = val[1] + s.L->cRt; out[2] = val[2]; out[3] = val[3];
 #pragma unroll
   for (int q = 4; q < 12; ++q) out[q] = 0.0;
@@ -707,7 +726,7 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
             }
             gsum[g] = Sg;
           }
-          block_reduce<16, 0>(v16, scratch);
+          front_sum<16>(v16, scratch, ngrp > G ? ngrp : G);
           P = cPt + v16[0]; R = cRt + v16[1]; sP = v16[2]; sR = v16[3];
           sA = v16[4]; sB = v16[5]; sAB = v16[6]; rA = v16[7]; rB = v16[8]; sT = v16[9]; sF = v16[10];
           gconv = !(v16[11] > 0.0); sing = v16[12] > 0.0;
