@@ -58,6 +58,9 @@ struct prism_problem {
   double* w_stage;  // A x N, allocated on the first prism_solve_batch_host call
   int32_t* i_stage; // A
   AccountParams ap;
+  // cluster-resident prox (prox_res.cuh): res != 0 when a slice of the account fits a CTA's shared memory
+  int32_t res, res_C, res_SL;
+  size_t res_smem;
   // streaming prox (prox_fast.cuh)
   int32_t fast, S, capw;  // fast: the streaming form applies; S slices per account; capacity of one warp's live list
   int64_t slice_len, ldc;

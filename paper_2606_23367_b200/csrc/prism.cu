@@ -12,6 +12,7 @@
 #include "gemm.cuh"
 #include "prox.cuh"
 #include "prox_fast.cuh"
+#include "prox_res.cuh"
 #include "small.cuh"
 
 #define PRISM_VERSION_STR "prism-b200 r1 (sm_100a, fp64 DMMA factor GEMMs, streaming two-threshold prox with TMA bulk-copy pipeline)"
@@ -173,6 +174,45 @@ static int set_kernel_attrs(int mt, int Kp) {
   return PRISM_OK;
 }
 
+// cluster-resident prox: smallest cluster size for which a slice of the account fits the shared-memory budget
+static bool res_geometry(prism_problem* p) {
+  static const int kC[] = {1, 2, 4, 8, 16};
+  for (int C : kC) {
+    int SL = 0;
+    if (res_fits(p->N, p->G, C, &SL)) {
+      p->res_C = C; p->res_SL = SL; p->res_smem = res_layout(SL, p->G, C).bytes;
+      return true;
+    }
+  }
+  return false;
+}
+template <bool LOTS, bool CHECK>
+static int res_attrs_one(const prism_problem* p) {
+  CUDA_TRY(cudaFuncSetAttribute(k_prox_res<LOTS, CHECK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->res_smem));
+  if (p->res_C > 8) CUDA_TRY(cudaFuncSetAttribute(k_prox_res<LOTS, CHECK>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+  return PRISM_OK;
+}
+static int res_attrs(const prism_problem* p) {
+  int r;
+  if (p->d.lot_count) { if ((r = res_attrs_one<true, false>(p)) != PRISM_OK) return r; return res_attrs_one<true, true>(p); }
+  if ((r = res_attrs_one<false, false>(p)) != PRISM_OK) return r;
+  return res_attrs_one<false, true>(p);
+}
+template <bool LOTS, bool CHECK>
+static cudaError_t res_launch(const prism_problem* p, cudaStream_t st, const ProxArgs& a, int mode) {
+  cudaLaunchConfig_t cfg;
+  memset(&cfg, 0, sizeof(cfg));
+  cfg.gridDim = dim3((unsigned)p->res_C, (unsigned)p->A, 1);
+  cfg.blockDim = dim3(RES_NT, 1, 1);
+  cfg.dynamicSmemBytes = p->res_smem;
+  cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeClusterDimension;
+  at[0].val.clusterDim.x = (unsigned)p->res_C; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+  cfg.attrs = at; cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, k_prox_res<LOTS, CHECK>, a, mode);
+}
+
 static bool fast_applicable(const prism_problem* p) {
   return !p->d.lot_count && !p->d.hi_full && p->N < ((int64_t)1 << PROX_META_IDX_BITS) && p->N % 16 == 0 &&
          !getenv("PRISM_PROX_NOFAST");     // N % 16: every row of every streamed array is 16-byte aligned (bulk copies)
@@ -255,7 +295,9 @@ static int create_one(int64_t N, int32_t k, int32_t accounts, const prism_constr
   ALLOC_TRY(dev_alloc(p, &p->ap.wins, (size_t)A));
   ALLOC_TRY(dev_alloc(p, &p->ap.slack, (size_t)A));
   ALLOC_TRY(dev_alloc(p, &p->counters, (size_t)4));
-  p->fast = fast_applicable(p) ? 1 : 0;
+  p->res = (res_geometry(p) && !getenv("PRISM_PROX_NORES")) ? 1 : 0;
+  if (p->res) { int r = res_attrs(p); if (r != PRISM_OK) { prism_problem_destroy(p); return r; } }
+  p->fast = (!p->res && fast_applicable(p)) ? 1 : 0;
   if (p->fast) {
     // slices: a few CTAs per resident slot so that the streaming kernel stays bandwidth-bound to the end of the grid
     int64_t target = ((int64_t)4 * 3 * p->sm_count + A - 1) / A;           // CTAs per account wanted
@@ -320,6 +362,7 @@ static ProxArgs make_prox_args(prism_problem* p, const prism_settings& s, double
   a.lraw = p->lraw; a.lcomp = p->lcomp; a.lcnt = p->lcnt; a.cbin = p->cbin; a.chkp = p->chkp; a.lflag = p->lflag;
   a.S = p->S; a.capw = p->capw; a.slice_len = p->slice_len; a.ldc = p->ldc;
   a.stats = p->stats;
+  a.res_C = p->res_C; a.res_SL = p->res_SL;
   a.win_mult = s.prox_window_mult > 0 ? s.prox_window_mult : 32.0;
   if (const char* e = getenv("PRISM_PROX_WIN_MULT")) a.win_mult = atof(e);
   a.band_start = 20;
@@ -338,6 +381,14 @@ static void launch_prox(Launcher& L, ProxArgs& a, int mode, int iter) {
   prism_problem* p = L.p;
   cudaStream_t st = L.st;
   a.iter = iter;
+  if (p->res) {
+    const bool chk = (mode & (PROX_CHECK | PROX_FINAL)) != 0;     // the final extraction also needs w_out
+    L.begin(PRISM_K_PROX);
+    if (p->d.lot_count) { if (chk) res_launch<true, true>(p, st, a, mode & ~PROX_CHECK); else res_launch<true, false>(p, st, a, mode); }
+    else { if (chk) res_launch<false, true>(p, st, a, mode & ~PROX_CHECK); else res_launch<false, false>(p, st, a, mode); }
+    L.end();
+    return;
+  }
   if (p->fast) {
     const bool chk = (mode & (PROX_CHECK | PROX_FINAL)) != 0;     // the final extraction also needs w_out
     const dim3 grid((unsigned)p->S, (unsigned)p->A);

@@ -68,6 +68,8 @@ struct ProxArgs {
   int32_t S, capw;         // slices per account; capacity of one warp's list
   int64_t slice_len, ldc;  // assets per slice (multiple of 512); entries per account in lcomp
   int32_t* stats;          // optional (debug): 8 counters per iteration, see k_prox_root; NULL in production
+  // cluster-resident form (prox_res.cuh): CTAs per account (cluster size) and assets per CTA (multiple of 256)
+  int32_t res_C, res_SL;
 };
 
 enum { PROX_CHECK = 1, PROX_FINAL = 2 };
@@ -225,6 +227,9 @@ struct SrcGlobal {
       f(i, e, g, nl, sl, wd);
     }
   }
+  // block-wide reduction used by the generic evaluation routines (a cluster-resident source reduces over its cluster)
+  template <int NV, int OP>
+  __device__ __forceinline__ void reduce(double (&val)[NV], double* scratch) const { block_reduce<NV, OP>(val, scratch); }
   __device__ __forceinline__ void classify(double, double, const double*, double, int*) {}
   __device__ __forceinline__ bool window_ok(double, double, const double*) const { return true; }
   __device__ __forceinline__ double cP() const { return 0.0; }
@@ -317,6 +322,9 @@ struct SrcSmem {
     n_live = scratch[nslot * nw];
     __syncthreads();
   }
+  // block-wide reduction used by the generic evaluation routines (a cluster-resident source reduces over its cluster)
+  template <int NV, int OP>
+  __device__ __forceinline__ void reduce(double (&val)[NV], double* scratch) const { block_reduce<NV, OP>(val, scratch); }
   __device__ __forceinline__ bool window_ok(double al, double be, const double* lamS) const {
     if (!(W < INFINITY)) return true;
     bool ok = fabs(al - aw) <= 0.5 * W && fabs(be - bw) <= 0.5 * W;
@@ -415,14 +423,14 @@ __device__ __noinline__ void prox_eval(const Src& src, const double* lamS, int G
   });
   if (s1 >= 0 || s2 >= 0) {
     double val[12] = {lP, lR, lsP, lsR, x[0], x[1], x[2], x[3], x[4], x[5], x[6], x[7]};
-    block_reduce<12, 0>(val, scratch);
+    src.template reduce<12, 0>(val, scratch);
 #pragma unroll
     for (int q = 0; q < 12; ++q) out[q] = val[q];
     if (s1 >= 0) { out[4] += src.cPg(s1); out[5] += src.cRg(s1); }
     if (s2 >= 0) { out[8] += src.cPg(s2); out[9] += src.cRg(s2); }
   } else {
     double val[4] = {lP, lR, lsP, lsR};
-    block_reduce<4, 0>(val, scratch);
+    src.template reduce<4, 0>(val, scratch);
 #pragma unroll
     for (int q = 0; q < 4; ++q) out[q] = val[q];
   }
@@ -451,12 +459,12 @@ __device__ __noinline__ void prox_eval_multi(const Src& src, const double* lamS,
     double val[8];
 #pragma unroll
     for (int q = 0; q < 8; ++q) val[q] = sp[q0 + q];
-    block_reduce<8, 0>(val, scratch);
+    src.template reduce<8, 0>(val, scratch);
 #pragma unroll
     for (int q = 0; q < 8; ++q) outP[q0 + q] = val[q] + cP;
 #pragma unroll
     for (int q = 0; q < 8; ++q) val[q] = sr[q0 + q];
-    block_reduce<8, 0>(val, scratch);
+    src.template reduce<8, 0>(val, scratch);
 #pragma unroll
     for (int q = 0; q < 8; ++q) outR[q0 + q] = val[q] + cR;
   }
@@ -474,7 +482,7 @@ __device__ __noinline__ void prox_brackets(const Src& src, double Delta, double*
     if (sh > e.sl) { x6 = fmin(x6, e.T + Delta + s_first + rho * e.sl); x7 = fmax(x7, e.T + Delta + s_last + rho * sh); }
   });
   double val[4] = {-x4, x5, -x6, x7};          // min via max of the negation: one uniform reduction
-  block_reduce<4, 1>(val, scratch);
+  src.template reduce<4, 1>(val, scratch);
   out[0] = -val[0]; out[1] = val[1]; out[2] = -val[2]; out[3] = val[3];
 }
 

@@ -262,6 +262,8 @@ struct SrcLiveG {
   const unsigned long long* cbin;   // shared memory: fixed-point totals of the assets that are not in the list
   int Gb;
   double cPt, cRt;
+  template <int NV, int OP>
+  __device__ __forceinline__ void reduce(double (&val)[NV], double* scratch) const { block_reduce<NV, OP>(val, scratch); }
   __device__ __forceinline__ double cP() const { return cPt; }
   __device__ __forceinline__ double cR() const { return cRt; }
   __device__ __forceinline__ double cPg(int g) const { return (double)cbin[g] * PRISM_FIX_INV; }
