@@ -173,7 +173,7 @@ def main():
     # the shared universe is replicated, there is no data-path collective.
     inst = make_instance(args.config, seed=rank, accounts=args.accounts)
     P = pr.Problem(inst, device=dev)
-    settings = binding.default_settings(gemm_mode=args.gemm_mode)
+    settings = binding.default_settings(gemm_precision=args.gemm_mode)
     A, N = inst.A, inst.N
 
     def barrier():
@@ -229,7 +229,7 @@ def main():
     d2h = w_h.numel() * 8 + st_h.numel() * 4 + it_h.numel() * 4 + rs_h.numel() * 8
 
     # ---------------- roofline of the dominant kernel: one extra solve with per-launch CUDA events (not timed above)
-    prof = binding.default_settings(gemm_mode=args.gemm_mode, profile=1)
+    prof = binding.default_settings(gemm_precision=args.gemm_mode, profile=1)
     rp = P.solve(prof)
     kt = P.kernel_times()
     tot_k = sum(v["ms"] for v in kt.values()) or 1.0

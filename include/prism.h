@@ -9,10 +9,10 @@
  *   Sigma = B diag(f) B' + diag(d)     (factor-structured risk)
  *
  * by a batched ADMM (operator splitting, BASELINE.json:north_star) whose steps are hand-written sm_100a kernels:
- * factor GEMMs, a fused proximal/projection kernel (budget hyperplane, box, exclusions, L1 turnover with a
- * buy/sell two-threshold split, lot penalties), a group-band block, dual update fused with residuals, per-account
- * convergence masks and per-account rho adaptation.  The returned weights satisfy budget, box, exclusions and the
- * turnover cap exactly (they are the projection-side iterate); bands hold to the primal tolerance.
+ * fp64 factor GEMMs and one fused proximal/projection kernel that holds EVERY nonsmooth and polyhedral term - budget
+ * hyperplane, box, exclusions, L1 turnover (buy/sell two-threshold split), group bands, buy cost, lot penalties -
+ * together with the dual update, the residuals, the per-account convergence mask and the rho adaptation.  The returned
+ * weights are the projection-side iterate: budget, box, exclusions, turnover cap and group bands hold to rounding.
  *
  * Boundary (Fig. 2): problem data in; weights, fixed-vocabulary status codes
  * (Table 14), timings (lanes of Table 4), memory bytes (Table 6) and the
@@ -30,6 +30,10 @@
  *    difficulty (iteration cap, NaN, gate failure) is a STATUS, not an error.  prism_last_error() gives the text.
  *  - The turnover scaling D_a of Eq. (1) is the identity in this build (as in every configured
  *    workload); a non-NULL d_t is rejected with PRISM_ERR_INVALID_ARG.
+ *  - Domain: lo_a <= hi_a finite per account.  Universes too wide for the cluster-resident projection (N above
+ *    ~80,000) take the streaming form, whose per-group constants are accumulated in 2^-60 fixed point: there
+ *    hi_a - lo_a <= 4 is required per asset and the sum of the constant trades of one group must stay below 16
+ *    (always true for a budget-1 book); wider boxes take the every-asset kernel instead.
  */
 #ifndef PRISM_H
 #define PRISM_H
@@ -42,7 +46,7 @@ extern "C" {
 
 #define PRISM_MAX_LOTS 4
 #define PRISM_MAX_GROUPS 64
-#define PRISM_MAX_FACTORS 256
+#define PRISM_MAX_FACTORS 128
 
 /* error codes */
 enum { PRISM_OK = 0, PRISM_ERR_INVALID_ARG = 1, PRISM_ERR_ALLOC = 2, PRISM_ERR_CUDA = 3, PRISM_ERR_NOT_READY = 4 };
@@ -63,10 +67,17 @@ enum {
   PRISM_GROUP_BANDS = 32, PRISM_TAX_LOTS = 64, PRISM_BUY_COST = 128, PRISM_BENCHMARK_SHIFT = 256
 };
 
+/* form of the fused projection kernel (H4); AUTO picks the first that applies */
+enum { PRISM_PROX_AUTO = 0,
+       PRISM_PROX_RESIDENT = 1,   /* one thread-block cluster per account, the account resident in shared memory    */
+       PRISM_PROX_STREAMING = 2,  /* streaming pass + per-account root kernel: wide universes, no lots / caps        */
+       PRISM_PROX_EVERY_ASSET = 3 /* one CTA per account re-reading the account per pass: always applicable         */ };
+
 typedef struct prism_constraint_set {
   uint32_t flags;      /* OR of the flags above; PRISM_BUDGET and PRISM_BOX are mandatory                       */
   int32_t G;           /* number of groups (0 unless PRISM_GROUP_BANDS), <= PRISM_MAX_GROUPS                    */
   int32_t max_lots;    /* lots per asset (0 unless PRISM_TAX_LOTS), <= PRISM_MAX_LOTS                           */
+  int32_t prox_form;   /* PRISM_PROX_*; a form that does not apply to the problem is PRISM_ERR_INVALID_ARG      */
 } prism_constraint_set;
 
 /* columns of the residual block, one row of PRISM_NRES doubles per account */
@@ -117,24 +128,30 @@ typedef struct prism_data {
   const uint8_t* lot_count; /* A x N  live lots per asset in [0, max_lots]; 0 => no penalty, sells limited by lo */
 } prism_data;
 
+enum { PRISM_GEMM_FP64_TENSOR = 0,   /* fp64 on the tensor pipe (DMMA mma.sync.m8n8k4)                              */
+       PRISM_GEMM_FP64_FMA = 1 };    /* fp64 FMA kernels of the same contract (validation twin)                     */
+
 typedef struct prism_settings {
   double eps_rel;           /* scaled primal/dual tolerance (default 1e-6; BASELINE.json:metric "1e-6 KKT")      */
+  double eps_abs;           /* absolute part: converged when r <= eps_abs + eps_rel * scale (default 0)          */
   int32_t max_iter;         /* iteration cap (default 4000)                                                      */
   int32_t check_every;      /* residual / convergence-mask cadence in iterations (default 10)                    */
+  int32_t first_check;      /* no residual check before this many iterations (default 40): the first checks of a
+                               cold start never pass and a check launch costs more than a plain one          */
+  int32_t adapt_rho;        /* 1 => per-account rho adaptation at check iterations (default 1)                   */
   double alpha;             /* over-relaxation in (0, 2) (default 1.6)                                           */
   double rho_scale;         /* initial c: rho_i = c gamma_a d_i (default 100)                                    */
-  double rho_band_scale;    /* unused since the bands moved into the projection; kept for ABI stability (default 1)  */
-  int32_t adapt_rho;        /* 1 => per-account rho adaptation at check iterations (default 1)                   */
-  int32_t gemm_mode;        /* 0 = fp64 tensor (DMMA mma.sync), 1 = fp64 FMA                                     */
-  double time_limit_ms;     /* 0 => none; accounts unfinished at the limit get PRISM_STATUS_TIMEOUT              */
-  double deadline_ms;       /* 0 => none; accounts finishing after it get PRISM_STATUS_LATE                      */
-  int32_t use_graph;        /* 1 => replay the inner iterations as a CUDA graph (default 1)                      */
+  int32_t gemm_precision;   /* PRISM_GEMM_* (default fp64 tensor); DESIGN.md records why no TF32 path is built   */
   int32_t profile;          /* 1 => bracket every kernel launch with CUDA events (read with prism_kernel_times);
                                adds event overhead, so never combine with a throughput measurement           */
-  double prox_window_mult;  /* streaming prox: next window = this x the last movement of the thresholds (default 32) */
-  int32_t first_check;      /* no residual check before this many iterations (default 40): the first checks of a
-                               cold start never pass and a check launch costs several plain ones             */
-  int32_t reserved0;        /* keep 0 */
+  double time_limit_ms;     /* 0 => none; accounts unfinished at the limit get PRISM_STATUS_TIMEOUT              */
+  double deadline_ms;       /* 0 => none; accounts finishing after it get PRISM_STATUS_LATE                      */
+  double prox_window_mult;  /* projection: next live-list window = this x the last movement of the thresholds
+                               (default 32)                                                                   */
+  /* warm start - the repeated-run lane (cold rows "pass no previous solution"): previous weights and
+     multipliers of the same accounts, e.g. the w_out / duals_out of an earlier call.  Both NULL => cold start.       */
+  const double* warm_w;     /* device, A x N, or NULL                                                            */
+  const double* warm_duals; /* device, A x PRISM_NDUAL(G), or NULL (=> zero multipliers)                         */
 } prism_settings;
 
 typedef struct prism_solve_info {
@@ -160,8 +177,8 @@ void prism_default_settings(prism_settings* s);
 int prism_problem_create(int64_t N, int32_t k, int32_t accounts, const prism_constraint_set* cs,
                          const prism_data* data, void* cuda_stream, prism_problem** out);
 
-/* Runs the batched solver (cold start: z = projection of w0, zero duals) on `cuda_stream` and
- * synchronises it before returning.
+/* Runs the batched solver on `cuda_stream` and synchronises it before returning.  Cold start (default):
+ * z = projection of w0, zero duals.  Warm start: see prism_settings.warm_w.
  *   w_out      device, A x N   returned weights
  *   status_out device, A int32 status vocabulary above
  *   iters_out  device, A int32 iterations run per account
@@ -182,15 +199,15 @@ int prism_residuals(prism_problem* p, const double* w, const double* duals, void
 /* Same solve as prism_solve_batch but with HOST buffers for the per-account data that changes between
  * rebalances (mu, w0) and for the outputs: copies mu and w0 host->device into the problem's borrowed arrays,
  * solves, copies weights / status / iterations / residual block back.  NULL host pointers skip that copy.
+ * The other per-account data (bounds, masks, bands, tau, gamma) stays resident from prism_problem_create.
  * This is the end-to-end lane of bench.py ("e2e"). */
 int prism_solve_batch_host(prism_problem* p, const prism_settings* s, void* cuda_stream, const double* mu_host,
                            const double* w0_host, double* w_host, int32_t* status_host, int32_t* iters_host,
                            double* resid_host, prism_solve_info* info);
 
-/* Kernel classes of the hot path: H4/H5 fused prox (the streaming pass k_prox_stream where it
- * applies, else the every-asset kernel), H1 GEMM-1, H2 small solve, H3 GEMM-2 + epilogue, H0/H7 capacitance
- * factorisation, H8/H9 diagnostics, everything else, and H4/H6/H7 per-account root find / convergence mask /
- * rho adaptation of the streaming form (k_prox_root). */
+/* Kernel classes of the hot path: H4-H7 fused prox (k_prox_res; for the streaming form both of its
+ * kernels), H1 GEMM-1, H2 small solve, H3 GEMM-2 + epilogue, H0/H7 capacitance factorisation, H8/H9 diagnostics,
+ * everything else.  PRISM_K_PROX_ROOT is kept for layout stability and stays 0. */
 enum { PRISM_K_PROX = 0, PRISM_K_GEMM1 = 1, PRISM_K_SOLVE = 2, PRISM_K_GEMM2 = 3, PRISM_K_FACTOR = 4, PRISM_K_DIAG = 5,
        PRISM_K_OTHER = 6, PRISM_K_PROX_ROOT = 7, PRISM_NKERN = 8 };
 

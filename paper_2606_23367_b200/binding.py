@@ -24,8 +24,12 @@ SYMBOLS = ["prism_default_settings", "prism_problem_create", "prism_solve_batch"
            "prism_version", "prism_kernel_times"]
 
 
+PROX_AUTO, PROX_RESIDENT, PROX_STREAMING, PROX_EVERY_ASSET = 0, 1, 2, 3     # prism.h: PRISM_PROX_*
+GEMM_FP64_TENSOR, GEMM_FP64_FMA = 0, 1                                       # prism.h: PRISM_GEMM_*
+
+
 class ConstraintSet(C.Structure):
-    _fields_ = [("flags", C.c_uint32), ("G", C.c_int32), ("max_lots", C.c_int32)]
+    _fields_ = [("flags", C.c_uint32), ("G", C.c_int32), ("max_lots", C.c_int32), ("prox_form", C.c_int32)]
 
 
 class Data(C.Structure):
@@ -38,11 +42,11 @@ class Data(C.Structure):
 
 
 class Settings(C.Structure):
-    _fields_ = [("eps_rel", C.c_double), ("max_iter", C.c_int32), ("check_every", C.c_int32), ("alpha", C.c_double),
-                ("rho_scale", C.c_double), ("rho_band_scale", C.c_double), ("adapt_rho", C.c_int32),
-                ("gemm_mode", C.c_int32), ("time_limit_ms", C.c_double), ("deadline_ms", C.c_double),
-                ("use_graph", C.c_int32), ("profile", C.c_int32), ("prox_window_mult", C.c_double),
-                ("first_check", C.c_int32), ("reserved0", C.c_int32)]
+    _fields_ = [("eps_rel", C.c_double), ("eps_abs", C.c_double), ("max_iter", C.c_int32), ("check_every", C.c_int32),
+                ("first_check", C.c_int32), ("adapt_rho", C.c_int32), ("alpha", C.c_double), ("rho_scale", C.c_double),
+                ("gemm_precision", C.c_int32), ("profile", C.c_int32), ("time_limit_ms", C.c_double),
+                ("deadline_ms", C.c_double), ("prox_window_mult", C.c_double), ("warm_w", C.c_void_p),
+                ("warm_duals", C.c_void_p)]
 
 
 class SolveInfo(C.Structure):
@@ -121,7 +125,7 @@ class SolveResult:
 class Problem:
     """prism_problem_create / prism_solve_batch / prism_residuals on torch CUDA tensors."""
 
-    def __init__(self, inst, device="cuda:0"):
+    def __init__(self, inst, device="cuda:0", prox_form=PROX_AUTO):
         import torch
         self.torch = torch
         self.dev = torch.device(device)
@@ -159,7 +163,8 @@ class Problem:
             else:
                 x = t.get(name)
                 setattr(d, name, x.data_ptr() if x is not None else None)
-        self.cs = ConstraintSet(flags=int(inst.flags), G=int(inst.G), max_lots=4 if inst.lot_slope is not None else 0)
+        self.cs = ConstraintSet(flags=int(inst.flags), G=int(inst.G), max_lots=4 if inst.lot_slope is not None else 0,
+                                prox_form=int(prox_form))
         self.handle = C.c_void_p()
         with torch.cuda.device(self.dev):
             stream = torch.cuda.current_stream().cuda_stream
@@ -185,9 +190,15 @@ class Problem:
     def _info(self, info: SolveInfo) -> dict:
         return {n: getattr(info, n) for n, _ in SolveInfo._fields_}
 
-    def solve(self, settings: Optional[Settings] = None, **kw) -> SolveResult:
+    def solve(self, settings: Optional[Settings] = None, warm=None, **kw) -> SolveResult:
+        """prism_solve_batch.  warm: a previous SolveResult (or (w, duals) device tensors) to warm-start from."""
         torch = self.torch
         s = settings if settings is not None else default_settings(**kw)
+        if warm is not None:
+            ww, wd = (warm.w, warm.duals) if isinstance(warm, SolveResult) else warm
+            self._warm = (ww.contiguous(), None if wd is None else wd.contiguous())       # keep alive during the call
+            s.warm_w = self._warm[0].data_ptr()
+            s.warm_duals = self._warm[1].data_ptr() if self._warm[1] is not None else None
         w = torch.empty((self.A, self.N), dtype=torch.float64, device=self.dev)
         status = torch.empty(self.A, dtype=torch.int32, device=self.dev)
         iters = torch.empty(self.A, dtype=torch.int32, device=self.dev)

@@ -29,7 +29,6 @@ struct AccountParams {            // per-account scalars, struct of arrays on th
   double* slack;    // band ramp (prox_fast.cuh): largest band violation of the band-free projection at band_start
 };
 
-#define PRISM_MAX_PARTS 8
 struct prism_problem {
   int64_t N;
   int32_t k, kp, A, G, Kp;       // kp: k padded to 8 * MT; Kp = kp: rows of T and V per account (U = Bp)
@@ -55,7 +54,7 @@ struct prism_problem {
   double *resid;    // A x PRISM_NRES (internal copy)
   double *duals;    // A x PRISM_NDUAL(G)
   int32_t* status;  // A
-  double* w_stage;  // A x N, allocated on the first prism_solve_batch_host call
+  double* w_stage;  // A x N staging of the host-buffer lane
   int32_t* i_stage; // A
   AccountParams ap;
   // cluster-resident prox (prox_res.cuh): res != 0 when a slice of the account fits a CTA's shared memory
@@ -68,7 +67,6 @@ struct prism_problem {
   int32_t *lcnt, *lflag;
   unsigned long long* cbin;
   double* chkp;
-  int32_t* stats;         // debug counters of the streaming prox (PRISM_PROX_STATS), else NULL
   int32_t* counters;      // [0] number of done accounts
   int32_t* h_counters;    // pinned host mirror
   int64_t bytes;
@@ -76,14 +74,6 @@ struct prism_problem {
   double dbar;            // mean of d (host copy at create)
   double prof_ms[PRISM_NKERN];   // per-kernel-class device time of the last profiled solve
   int64_t prof_cnt[PRISM_NKERN];
-  // account groups (prism.cu, "parts"): a large batch is split into contiguous account ranges, each a complete
-  // problem object of its own, solved concurrently on its own stream by its own host thread.  The parent holds
-  // no iterate; parts[i] covers accounts [part_a0[i], part_a0[i + 1]).
-  int32_t nparts;
-  prism_problem* parts[PRISM_MAX_PARTS];
-  int32_t part_a0[PRISM_MAX_PARTS + 1];
-  cudaStream_t part_stream[PRISM_MAX_PARTS];
-  cudaEvent_t part_done[PRISM_MAX_PARTS];
 };
 
 static thread_local char g_err[512] = "";

@@ -10,6 +10,7 @@
 // leading dimension ldw (multiple of 32, zero padded), V account-major with leading dimension ldv.
 #pragma once
 #include "common.cuh"
+#include "gemm_args.cuh"
 
 __device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double b) {
   asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
@@ -22,19 +23,6 @@ __device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;"); }
 template <int NLEFT>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(NLEFT)); }
-
-#define G1_KS 32           // assets per pipeline stage
-#define G1_LD (G1_KS + 4)  // smem row stride (doubles): conflict-free 64-bit fragment loads
-#define G1_TA 64           // accounts per CTA (8 warps x one m8n8 column tile)
-#define G1_STAGES 3
-
-struct Gemm1Args {
-  const double* Bt; int64_t ldn;
-  const double* X; int64_t ldw;
-  double* Tpart; int64_t ldv;
-  int32_t A; int64_t chunk; int64_t Npad;
-  const int32_t* done;
-};
 
 template <int MT>
 __global__ void __launch_bounds__(256) k_gemm1(Gemm1Args p) {
@@ -114,24 +102,6 @@ __global__ void k_gemm1_ref(Gemm1Args p, int kp) {
 }
 
 // ------------------------------------------------------------------------------------------------ GEMM-2
-enum { G2_ADMM = 0, G2_ADMM_CHECK = 1, G2_SIGMA = 2 };
-#define G2_TM 64     // accounts per CTA
-#define G2_TN 64     // assets per CTA
-
-struct Gemm2Args {
-  const double* Bp; int32_t kp;
-  const double* V; int64_t ldv;
-  int64_t N, ldw; int32_t A, G;
-  const uint8_t* group_id;
-  const double *invd, *d, *gamma, *c;
-  double* v; const double* cc; const double* rt;
-  double *xs, *pxq;
-  const double *q, *mu;       // q (ldw) or mu (ld N)
-  const double* X;            // SIGMA: the vector Sigma is applied to (ldw)
-  double relax;
-  const int32_t* done;
-};
-
 template <int MODE>
 __device__ __forceinline__ void g2_epilogue(const Gemm2Args& p, int a, int64_t i, double bv) {
   const double gam = p.gamma[a];

@@ -1,0 +1,72 @@
+// k_small.cu - translation unit of the small kernels: setup (H0), cold start, capacitance factorisation (H0/H7),
+// small solves (H2), Sigma-apply glue and the external diagnostics / statuses (H8, H9).
+#include "small.cuh"
+#include "diag.cuh"
+#include "kernels.h"
+
+#define TRY(e) do { cudaError_t _e = (e); if (_e != cudaSuccess) return _e; } while (0)
+
+cudaError_t small_set_attrs(int Kp) {
+  TRY(cudaFuncSetAttribute(k_factor, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)((size_t)Kp * Kp * sizeof(double))));
+  return cudaSuccess;
+}
+cudaError_t setup_shared_launch(const void* B, int is32, const double* d, int64_t N, int k, int kp, int64_t ldn, double* Bp,
+                                double* Bt, double* invd, cudaStream_t st) {
+  k_setup_shared<<<(unsigned)((N + 127) / 128), 128, 0, st>>>(B, is32, d, N, k, kp, ldn, Bp, Bt, invd);
+  return cudaGetLastError();
+}
+cudaError_t gram_launch(const double* Bt, int64_t ldn, const double* invd, int64_t N, int kp, double* gram, cudaStream_t st) {
+  k_gram<<<dim3(kp, kp), 256, 0, st>>>(Bt, ldn, nullptr, invd, N, kp, 0, gram);
+  return cudaGetLastError();
+}
+cudaError_t init_accounts_launch(const InitArgs& a, cudaStream_t st) {
+  k_init_accounts<<<a.A, 256, 0, st>>>(a);
+  return cudaGetLastError();
+}
+cudaError_t warm_start_launch(const WarmArgs& a, cudaStream_t st) {
+  k_warm_start<<<dim3((unsigned)((a.N + 255) / 256), a.A), 256, 0, st>>>(a);
+  return cudaGetLastError();
+}
+cudaError_t factor_launch(const double* gram, const double* f, const double* gamma, const AccountParams& ap, int A, int k,
+                          int kp, double* Sinv, cudaStream_t st) {
+  k_factor<<<A, 256, (size_t)kp * kp * sizeof(double), st>>>(gram, f, gamma, ap, k, kp, 0, Sinv);
+  return cudaGetLastError();
+}
+cudaError_t solve_launch(const SolveArgs& a, cudaStream_t st) {
+  k_solve<<<a.A, 256, 0, st>>>(a);
+  return cudaGetLastError();
+}
+cudaError_t scale_fs_launch(const double* Tpart, int nchunk, int A, int k, int kp, int64_t ldv, const double* f,
+                            const double* gamma, double* V, cudaStream_t st) {
+  k_scale_fs<<<A, 128, 0, st>>>(Tpart, nchunk, A, k, kp, ldv, f, gamma, V);
+  return cudaGetLastError();
+}
+cudaError_t diff_launch(const double* w, const double* wb, int64_t N, int64_t ldw, int A, double* X, cudaStream_t st) {
+  k_diff<<<dim3((unsigned)((N + 255) / 256), A), 256, 0, st>>>(w, wb, N, ldw, X);
+  return cudaGetLastError();
+}
+cudaError_t make_q_launch(const double* mu, const double* gSig, int64_t N, int64_t ldw, int A, double* q, cudaStream_t st) {
+  k_make_q<<<dim3((unsigned)((N + 255) / 256), A), 256, 0, st>>>(mu, gSig, N, ldw, q);
+  return cudaGetLastError();
+}
+cudaError_t diag_launch(const DiagArgs& a, bool lots, cudaStream_t st) {
+  if (lots) k_diag<true><<<a.A, 256, 0, st>>>(a);
+  else k_diag<false><<<a.A, 256, 0, st>>>(a);
+  return cudaGetLastError();
+}
+cudaError_t status_launch(int A, const double* resid, const int32_t* conv, const int32_t* iters, int timed_out, int late_iter,
+                          double gate, int32_t* status, cudaStream_t st) {
+  k_status<<<(A + 127) / 128, 128, 0, st>>>(A, resid, conv, iters, timed_out, late_iter, gate, status);
+  return cudaGetLastError();
+}
+// prism_residuals: the solver-only columns of the residual block are NaN
+__global__ void k_nan_cols(int A, double* resid) {
+  const int a = blockIdx.x * blockDim.x + threadIdx.x;
+  if (a >= A) return;
+  double* r = resid + (int64_t)a * PRISM_NRES;
+  r[PRISM_R_PRIMAL] = NAN; r[PRISM_R_DUAL] = NAN; r[PRISM_R_RHO] = NAN; r[PRISM_R_RESERVED] = 0.0;
+}
+cudaError_t nan_cols_launch(int A, double* resid, cudaStream_t st) {
+  k_nan_cols<<<(A + 127) / 128, 128, 0, st>>>(A, resid);
+  return cudaGetLastError();
+}

@@ -51,7 +51,7 @@ struct ProxArgs {
   double* resid;
   int32_t* counters;
   // settings
-  double eps;
+  double eps, eps_abs;      // converged when r <= eps_abs + eps * scale for both residuals
   int32_t adapt, iter;
   double win_mult;         // next window = win_mult x (movement of the thresholds in this launch)
   double win_ratio;        // streaming pass: its (wide) window = win_ratio x the solve's (tight) window
@@ -67,7 +67,6 @@ struct ProxArgs {
   int32_t* lflag;          // [A] 1: the account takes the generic path in k_prox_root
   int32_t S, capw;         // slices per account; capacity of one warp's list
   int64_t slice_len, ldc;  // assets per slice (multiple of 512); entries per account in lcomp
-  int32_t* stats;          // optional (debug): 8 counters per iteration, see k_prox_root; NULL in production
   // cluster-resident form (prox_res.cuh): CTAs per account (cluster size) and assets per CTA (multiple of 256)
   int32_t res_C, res_SL;
 };
@@ -506,7 +505,7 @@ __device__ __noinline__ void prox_group_sums(const Src& src, const double* lamS,
   __syncthreads();
 }
 
-// Scaled residuals of the splitting (reading R13) from the stored x and P x + q: out = {r_p, r_d}.
+// Scaled residuals of the splitting (reading R13) from the stored x and P x + q: out = {r_p, r_d, tolerance met}.
 template <bool LOTS, class Src>
 __device__ __noinline__ void prox_check(const ProxArgs& p, const Src& src, const double* lamS, int a, double al, double bd,
                                         double lam_b, double cg, double* scratch, double* out) {
@@ -529,6 +528,7 @@ __device__ __noinline__ void prox_check(const ProxArgs& p, const Src& src, const
   block_reduce<7, 1>(val, scratch);
   out[0] = val[2] / fmax(fmax(val[0], val[1]), 1e-300);
   out[1] = val[3] / fmax(fmax(val[4], fmax(val[5], val[6])), 1e-300);
+  out[2] = (val[2] <= p.eps_abs + p.eps * fmax(val[0], val[1]) && val[3] <= p.eps_abs + p.eps * fmax(val[4], fmax(val[5], val[6]))) ? 1.0 : 0.0;
 }
 
 // Output pass: either the returned weights (finished) or what the x-update needs: r~ = M^-1 r, c = r~ - z,
@@ -835,11 +835,11 @@ __device__ __forceinline__ void prox_body(const ProxArgs& p, int mode, Src& src,
   int finished = 0;
   const double bdf = beta - Delta;
   if (mode & PROX_CHECK) {
-    double rr[2];
+    double rr[3];
     prox_check<LOTS>(p, src, lamS, a, alpha, bdf, lam_b, cg, sh.scratch, rr);
     const double rp = rr[0], rd = rr[1];
     const bool bad = !(rp < INFINITY) || !(rd < INFINITY);
-    const bool conv = !bad && rp <= p.eps && rd <= p.eps && !rs.capped;      // never certify on an unfinished root find
+    const bool conv = !bad && rr[2] > 0.0 && !rs.capped;      // never certify on an unfinished root find
     if (tid == 0) {
       p.resid[(int64_t)a * PRISM_NRES + PRISM_R_PRIMAL] = rp;
       p.resid[(int64_t)a * PRISM_NRES + PRISM_R_DUAL] = rd;
@@ -867,7 +867,6 @@ __device__ __forceinline__ void prox_body(const ProxArgs& p, int mode, Src& src,
   __syncthreads();
   for (int g = tid; g < G; g += nt) p.lamG[(int64_t)a * G + g] = lamS[g];
   if (tid == 0) {
-    p.resid[(int64_t)a * PRISM_NRES + PRISM_R_RESERVED] += (double)rs.n_eval;   // trial evaluations (passes) so far
     p.ap.alpha[a] = alpha; p.ap.beta[a] = beta; p.ap.mode[a] = rs.amode;
     // next window: a multiple of how far the thresholds moved in this launch
     p.ap.win[a] = next_window(p, alpha, beta, fmax(fmax(fabs(alpha - alpha_w), fabs(beta - beta_w)), mv_l));
@@ -883,42 +882,5 @@ __device__ __forceinline__ void prox_body(const ProxArgs& p, int mode, Src& src,
     }
   }
   __syncthreads();
-}
-
-#define PROX_STATIC_SHARED(NW)                                           \
-  __shared__ double s_scratch[12 * 32];                                  \
-  __shared__ double s_gbin[(NW) * PRISM_MAX_GROUPS];                     \
-  __shared__ double s_lamS[PRISM_MAX_GROUPS];                            \
-  __shared__ double s_gsum[PRISM_MAX_GROUPS];                            \
-  __shared__ int s_selS[2];                                              \
-  ProxShared sh = {s_scratch, s_gbin, s_lamS, s_gsum, s_selS, nullptr, nullptr, nullptr};
-
-// generic kernel: any N, lots, per-asset caps.  Persistent: grid <= number of accounts.
-template <bool LOTS>
-__global__ void __launch_bounds__(512) k_prox(const __grid_constant__ ProxArgs p, int mode) {
-  PROX_STATIC_SHARED(16)
-  for (int a = blockIdx.x; a < p.A; a += gridDim.x) {
-    if (p.ap.done[a]) continue;
-    const double gam = p.gamma[a], c = p.ap.c[a];
-    const double kappa = p.kappa ? p.kappa[a] : 0.0;
-    const double lam_b = kappa + (p.c_buy ? p.c_buy[a] : 0.0);
-    SrcGlobal<LOTS> src(p, a, c * gam, p.lo[a], p.hi[a], lam_b);
-    prox_body<LOTS>(p, mode, src, a, gam, c, kappa, lam_b, sh, false);
-  }
-}
-
-// shared-memory-resident kernel: 20 N bytes of dynamic shared memory, no lots, no per-asset caps
-__global__ void __launch_bounds__(512, 1) k_prox_smem(const __grid_constant__ ProxArgs p, int mode) {
-  extern __shared__ __align__(16) double prox_smem[];
-  PROX_STATIC_SHARED(16)
-  for (int a = blockIdx.x; a < p.A; a += gridDim.x) {
-    if (p.ap.done[a]) continue;
-    const double gam = p.gamma[a], c = p.ap.c[a];
-    const double kappa = p.kappa ? p.kappa[a] : 0.0;
-    const double lam_b = kappa + (p.c_buy ? p.c_buy[a] : 0.0);
-    __syncthreads();
-    SrcSmem src(p, a, c * gam, p.lo[a], p.hi[a], lam_b, lam_b + kappa, prox_smem);
-    prox_body<false>(p, mode, src, a, gam, c, kappa, lam_b, sh, true);
-  }
 }
 

@@ -482,10 +482,6 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
   if (p.ap.done[a]) return;
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, nt = blockDim.x, nw = nt >> 5;
   if (tid == 0) nback_s = 0;
-  long long tk0 = clock64();
-  auto tick = [&](int k) {                 // (debug) phase timers: thread 0, units of 64 cycles
-    if (p.stats && tid == 0 && p.iter < 1024) { const long long t = clock64(); atomicAdd(&p.stats[(3072 + p.iter) * 8 + k], (int)((t - tk0) >> 6)); tk0 = t; }
-  };
   const int G = p.G, Gb = G > 0 ? G : 1;
   const int64_t N = p.N, row = (int64_t)a * N, rowp = (int64_t)a * p.ldw;
   const int nsub = p.S * FAST_NW;
@@ -558,6 +554,13 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
     __syncthreads();
   }
   double mv = 0.0;
+  // work areas of the nested solver: set up for BOTH paths (the every-asset path below uses them too)
+  if (tid == 0) {
+    sh.scratch = scratch; sh.gbin = gbin; sh.lamS = lamS; sh.gsum = gsum; sh.selS = selS;
+    sh.band_lo = band_lo; sh.band_hi = band_hi; sh.gw0 = gw0;
+    p.lflag[a] = 0;
+  }
+  __syncthreads();
   if (!fallback) {
     // ---- the raw lists as one sequence (offs = their start offsets); warp w handles a contiguous quarter of it.
     // Level 0: the tight parts (fronts) of the nsub lists.  Level 1 (only after a solution left the tight window):
@@ -662,11 +665,6 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
       }
       __syncthreads();
     };
-    if (tid == 0) {
-      sh.scratch = scratch; sh.gbin = gbin; sh.lamS = lamS; sh.gsum = gsum; sh.selS = selS;
-      sh.band_lo = band_lo; sh.band_hi = band_hi; sh.gw0 = gw0;
-      p.lflag[a] = 0;
-    }
     // A long list is first solved on its tight part; a solution that leaves the tight window repeats the solve on the
     // whole list, and one that leaves the streaming pass's window sends the account to the generic path.
     double Wf = split ? Wt : INFINITY;
@@ -676,11 +674,9 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
       if (nb) atomicAdd(&nback_s, nb);
     }
     for (int att = 0; att < 2; ++att) {
-      tick(0);
       scan_lists(att);                                   // level 0: the fronts; level 1: fronts and backs
       nlist_used = nlist;
       sort_lists(split && att == 0);
-      tick(1);
       rs.alpha = aw; rs.beta = bw; rs.amode = amode_w; rs.capped = 0;
       for (int g = tid; g < G; g += nt) lamS[g] = lamW[g];
       __syncthreads();
@@ -695,9 +691,7 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
       const double cPt = src.cPt, cRt = src.cRt;
       double al = aw, be = bw;
       int amode = amode_w;
-      tick(2);
       bool ok = false;
-      int why = 4;                                          // (debug) 1 singular band, 2 det, 3 den, 4 passes, 5 NaN
       for (int g = tid; g < G; g += nt) act[g] = lamS[g] > 0.0 ? 1 : (lamS[g] < 0.0 ? -1 : 0);
       __syncthreads();
       for (int itn = 0; itn < 16; ++itn) {
@@ -741,7 +735,7 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
           __syncthreads();
           continue;
         }
-        if (sing) { why = 1; break; }
+        if (sing) break;
         double dal, dbe;
         if (amode == 1) {
           const double M11 = -sP + sA, M12 = sAB, M21 = -sAB, M22 = sR - sB, r1 = -FA + rA, r2 = -FB - rB;
@@ -749,13 +743,13 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
           if (fabs(det) > 1e-300) { dal = (r1 * M22 - M12 * r2) / det; dbe = (M11 * r2 - M21 * r1) / det; }
           else if (fabs(r1) <= tol && fabs(M11) <= 1e-300 && fabs(M22) > 1e-300) { dal = 0.0; dbe = r2 / M22; }   // buy side flat and satisfied
           else if (fabs(r2) <= tol && fabs(M22) <= 1e-300 && fabs(M11) > 1e-300) { dbe = 0.0; dal = r1 / M11; }   // sell side flat and satisfied
-          else { why = 2; break; }
+          else break;
         } else {
           const double den = (sP + sR) - sT;
-          if (!(den > 1e-300)) { why = 3; break; }
+          if (!(den > 1e-300)) break;
           dal = dbe = (FA - sF) / den;
         }
-        if (!(dal == dal) || !(dbe == dbe)) { why = 5; break; }
+        if (!(dal == dal) || !(dbe == dbe)) break;
         __syncthreads();
         for (int g = tid; g < G; g += nt) {                // multipliers and active set (thread g owns band g)
           const double pa = gv[4 * g + 2], ra = gv[4 * g + 3], t = pa + ra;
@@ -773,10 +767,8 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
         al += dal; be += dbe;
         __syncthreads();
       }
-      tick(3);
       if (ok) { rs.alpha = al; rs.beta = be; rs.amode = amode; }
       else {
-        if (p.stats && tid == 0 && p.iter < 4096) { atomicAdd(&p.stats[p.iter * 8 + 3], 1); atomicAdd(&p.stats[(2048 + p.iter) * 8 + why], 1); }
         // nested robust solver on the same grouped list (lean passes through the SrcGrouped overloads)
         // (it continues from where the Newton iteration stopped when that state is usable)
         // (not with an infinite window while bands are in play - the launch in which they join: the multipliers a failed
@@ -790,17 +782,14 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
         rs.alpha = keep ? al : aw; rs.beta = keep ? be : bw; rs.amode = keep ? amode : amode_w;
         prox_rootfind<false>(p, sgrp, a, b, tau, Delta, sh, rs);
       }
-      tick(4);
       double mv_l = 0.0;
       for (int g = 0; g < G; ++g) mv_l = fmax(mv_l, fabs(lamS[g] - lamW[g]));
       mv = fmax(fmax(fabs(rs.alpha - aw), fabs(rs.beta - bw)), mv_l);
       if (mv <= 0.5 * fmin(Wf, W)) break;
       if (!(Wf < INFINITY)) { fallback = true; break; }   // left the streaming window (or NaN): the dead assets were misjudged
-      if (p.stats && tid == 0 && p.iter < 4096) atomicAdd(&p.stats[p.iter * 8 + 0], 1);
       Wf = INFINITY;
       __syncthreads();
     }
-    if (fallback && p.stats && tid == 0 && p.iter < 4096) atomicAdd(&p.stats[p.iter * 8 + 2], 1);
     if (!fallback && G > 0 && !exact && p.iter == p.band_start) {   // band ramp: how far outside its bands is this projection?
       __syncthreads();
       root_pass(src, poff, ngrp, lamS, G, rs.alpha, rs.beta - Delta, gv);
@@ -871,7 +860,7 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
         }
       }
     }
-    if (CHECK) {
+    if (CHECK && !(mode & PROX_FINAL)) {
       if (tid < 7) {                                     // residual terms of the dead assets, per slice
         double m = 0.0;
         for (int s = 0; s < p.S; ++s) m = fmax(m, p.chkp[((int64_t)a * p.S + s) * 8 + tid]);
@@ -883,7 +872,8 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
       for (int q = 0; q < 7; ++q) val[q] = fmax(val[q], chk[q]);
       const double rp = val[2] / fmax(fmax(val[0], val[1]), 1e-300);
       const double rd = val[3] / fmax(fmax(val[4], fmax(val[5], val[6])), 1e-300);
-      const bool conv = rp <= p.eps && rd <= p.eps && !rs.capped;             // never certify on an unfinished root find
+      const bool conv = val[2] <= p.eps_abs + p.eps * fmax(val[0], val[1]) && val[3] <= p.eps_abs + p.eps * fmax(val[4], fmax(val[5], val[6])) &&
+                        !rs.capped;                                          // never certify on an unfinished root find
       if (!(rp < INFINITY) || !(rd < INFINITY)) fallback = true;             // NaN / Inf: the generic path classifies it
       else if (!conv && p.adapt && p.iter >= PRISM_ADAPT_START && p.iter - p.ap.nadapt[a] >= PRISM_ADAPT_EVERY) {
         const double ratio = sqrt(rp / fmax(rd, 1e-300));
@@ -900,14 +890,12 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
       }
     }
   }
-  tick(5);
   if (!fallback) {
     // ---------------------------------------------------------------- commit the account's state
     if (mode & PROX_FINAL) finished = 1;                 // (CHECK instantiation: w_out holds z)
     const double alpha = rs.alpha, beta = rs.beta;
     for (int g = tid; g < G; g += nt) p.lamG[(int64_t)a * G + g] = lamS[g];
     if (tid == 0) {
-      p.resid[(int64_t)a * PRISM_NRES + PRISM_R_RESERVED] += (double)rs.n_eval;
       p.ap.alpha[a] = alpha; p.ap.beta[a] = beta; p.ap.mode[a] = rs.amode;
       // next window of the streaming pass: a multiple of the last movement, never shrunk while its list is short
       // (a wide window then costs nothing and the solution almost never leaves it); infinite for the first iterations
@@ -928,16 +916,10 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
         for (int g = 0; g < G; ++g) { du[2 + g] = fmax(lamS[g], 0.0); du[2 + G + g] = fmax(-lamS[g], 0.0); }
         p.resid[(int64_t)a * PRISM_NRES + PRISM_R_RHO] = c;
       }
-      if (p.stats && p.iter < 4096) {
-        atomicAdd(&p.stats[p.iter * 8 + 5], 1); atomicAdd(&p.stats[p.iter * 8 + 6], src.cnt[0]); atomicAdd(&p.stats[p.iter * 8 + 7], rs.n_eval);
-        atomicAdd(&p.stats[(2048 + p.iter) * 8 + 6], nl);
-        atomicMax(&p.stats[p.iter * 8 + 4], rs.n_eval); if (rs.n_eval > 20) atomicAdd(&p.stats[p.iter * 8 + 0], 1);
-      }
     }
     return;
   }
   // ------------------------------------------------------------------ generic path: every asset, from global memory
-  if (p.stats && tid == 0 && p.iter < 4096) atomicAdd(&p.stats[p.iter * 8 + 1], 1);
   __syncthreads();
   SrcGlobal<false> gsrc(p, a, cg, p.lo[a], p.hi[a], lam_b);
   ProxShared shg = sh;

@@ -2,6 +2,7 @@
 // external diagnostics (H8/H9: PAPER.md:142-146) and status assignment (Table 14).
 #pragma once
 #include "common.cuh"
+#include "small_args.cuh"
 
 // ---------------------------------------------------------------------------------- H0: shared universe
 // Bp (N x kp asset-major), Bt (kp x ldn factor-major), invd; B given as fp64 or fp32 (configs[4] stores fp32).
@@ -37,14 +38,6 @@ __global__ void k_gram(const double* Bt, int64_t ldn, const uint8_t* gid, const 
 }
 
 // ---------------------------------------------------------------------------------- per-account cold start
-struct InitArgs {
-  int64_t N, ldw; int32_t A, G;
-  const double *w0, *gamma;
-  const uint8_t* group_id;
-  double *v, *gw0, *lamG;
-  AccountParams ap;
-  double rho_scale;
-};
 __global__ void k_init_accounts(InitArgs p) {
   __shared__ double scratch[32];
   __shared__ double gs[8 * PRISM_MAX_GROUPS];
@@ -75,6 +68,28 @@ __global__ void k_init_accounts(InitArgs p) {
     p.ap.c[a] = p.rho_scale;
     p.ap.alpha[a] = 0.0; p.ap.beta[a] = 0.0; p.ap.mode[a] = 0; p.ap.win[a] = INFINITY; p.ap.wins[a] = INFINITY; p.ap.slack[a] = 0.0;
     p.ap.done[a] = 0; p.ap.conv[a] = 0; p.ap.iters[a] = 0; p.ap.refactor[a] = 1; p.ap.nadapt[a] = 0;
+  }
+}
+
+// Warm start: at a fixed point of the splitting x = z = w and y = -(P w + q) = mu - gamma Sigma (w - w_b), so the
+// carried state is v = w + y / rho with rho_i = c gamma d_i; thresholds alpha = nu + theta, beta = nu - theta and the
+// band multipliers lambda_g = lam_hi - lam_lo come from the given duals (prism.h: PRISM_NDUAL layout).
+__global__ void k_warm_start(WarmArgs p) {
+  const int a = blockIdx.y;
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const double cg = p.ap.c[a] * p.gamma[a];
+  if (i < p.N) {
+    const int64_t s = (int64_t)a * p.N + i, sp = (int64_t)a * p.ldw + i;
+    p.v[sp] = p.w[s] + (p.mu[s] - p.gS[sp]) * p.invd[i] / cg;
+  }
+  if (blockIdx.x == 0 && p.duals) {
+    const double* du = p.duals + (int64_t)a * PRISM_NDUAL(p.G);
+    for (int g = threadIdx.x; g < p.G; g += blockDim.x) p.lamG[(int64_t)a * p.G + g] = du[2 + g] - du[2 + p.G + g];
+    if (threadIdx.x == 0) {
+      const double nu = du[0], th = fmax(du[1], 0.0);
+      const bool cap = th > 0.0 && p.tau && isfinite(p.tau[a]);
+      p.ap.alpha[a] = cap ? nu + th : nu; p.ap.beta[a] = cap ? nu - th : nu; p.ap.mode[a] = cap ? 1 : 0;
+    }
   }
 }
 
@@ -116,12 +131,6 @@ __global__ void k_factor(const double* gram, const double* f, const double* gamm
 }
 
 // ---------------------------------------------------------------------------------- H2: V = S^-1 T
-struct SolveArgs {
-  int32_t A, kp, nchunk; int64_t ldv;
-  const double *Tpart, *Sinv;
-  double *V;
-  AccountParams ap;
-};
 // 256 threads.  (1) T = sum of the split-K partials: four threads per entry, each over a quarter of the chunks with all
 // its loads in flight, combined in a fixed order (deterministic).  (2) V = S^-1 T: one warp per row group, a row of
 // the (symmetric) inverse read coalesced by the lanes, warp-shuffle reduction: one round of global-load latency.

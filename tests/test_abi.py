@@ -37,7 +37,8 @@ def test_default_settings_and_version(lib):
     from paper_2606_23367_b200 import binding
     s = binding.default_settings()
     assert s.eps_rel == 1e-6 and s.max_iter == 4000 and s.check_every == 10 and s.alpha == 1.6 and s.rho_scale == 100.0
-    assert s.adapt_rho == 1 and s.gemm_mode == 0 and s.profile == 0
+    assert s.adapt_rho == 1 and s.gemm_precision == 0 and s.profile == 0 and s.eps_abs == 0.0 and s.first_check == 40
+    assert not s.warm_w and not s.warm_duals
     assert "sm_100a" in binding.version()
 
 
@@ -54,7 +55,7 @@ def test_header_constants_match_binding():
     assert int(flags["PRISM_BENCHMARK_SHIFT"]) == gen.F_BENCHMARK_SHIFT and int(flags["PRISM_EXCLUSION"]) == gen.F_EXCLUSION
     assert len(binding.STATUS_NAMES) == 6                                               # Table 14
     # struct sizes (natural alignment) as the C compiler lays them out
-    assert C.sizeof(binding.Settings) == 88 and C.sizeof(binding.ConstraintSet) == 12
+    assert C.sizeof(binding.Settings) == 96 and C.sizeof(binding.ConstraintSet) == 16
     assert C.sizeof(binding.Data) == 22 * 8
 
 
@@ -80,11 +81,11 @@ def test_invalid_arguments_are_errors_not_crashes(lib):
     out = C.c_void_p()
     rc = lib.prism_problem_create(10, 2, 1, None, None, None, C.byref(out))
     assert rc == 1 and not out.value and b"null" in lib.prism_last_error()
-    cs = binding.ConstraintSet(flags=0, G=0, max_lots=0)
+    cs = binding.ConstraintSet(flags=0, G=0, max_lots=0, prox_form=0)
     d = binding.Data()
     rc = lib.prism_problem_create(10, 2, 1, C.byref(cs), C.byref(d), None, C.byref(out))
     assert rc == 1 and b"mandatory" in lib.prism_last_error()
-    cs = binding.ConstraintSet(flags=3, G=0, max_lots=0)
+    cs = binding.ConstraintSet(flags=3, G=0, max_lots=0, prox_form=0)
     rc = lib.prism_problem_create(0, 2, 1, C.byref(cs), C.byref(d), None, C.byref(out))
     assert rc == 1
     rc = lib.prism_problem_create(10, 1000, 1, C.byref(cs), C.byref(d), None, C.byref(out))

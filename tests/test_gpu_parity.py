@@ -13,9 +13,9 @@ pytestmark = pytest.mark.gpu
 TOL_W, TOL_GAP, TOL_RES, TOL_GATE = 1e-4, 1e-6, 1e-6, 1e-6
 
 
-def _solve_gpu(inst, **kw):
+def _solve_gpu(inst, prox_form=0, **kw):
     import paper_2606_23367_b200 as pr
-    P = pr.Problem(inst)
+    P = pr.Problem(inst, prox_form=prox_form)
     r = P.solve(**kw)
     return P, r
 
@@ -70,11 +70,11 @@ CASES = {
 
 
 @pytest.mark.parametrize("name", sorted(CASES))
-@pytest.mark.parametrize("gemm_mode", [0, 1])
-def test_parity_with_oracle(name, gemm_mode):
+@pytest.mark.parametrize("gemm_precision", [0, 1])
+def test_parity_with_oracle(name, gemm_precision):
     inst = CASES[name]()
     W, res = _oracle(inst)
-    P, r = _solve_gpu(inst, gemm_mode=gemm_mode)
+    P, r = _solve_gpu(inst, gemm_precision=gemm_precision)
     _check_against_oracle(inst, r, W, res)
     P.close()
 
@@ -82,8 +82,8 @@ def test_parity_with_oracle(name, gemm_mode):
 def test_dmma_and_fma_gemms_agree():
     """The tensor-pipe GEMMs against the plain-FMA kernels of the same contract: same iterations, same weights."""
     inst = gen.config1(N=700, k=30, A=10)
-    P, r0 = _solve_gpu(inst, gemm_mode=0)
-    r1 = P.solve(gemm_mode=1)
+    P, r0 = _solve_gpu(inst, gemm_precision=0)
+    r1 = P.solve(gemm_precision=1)
     assert (r0.iters == r1.iters).all()
     assert float((r0.w - r1.w).abs().max()) <= 1e-12
     P.close()
@@ -111,19 +111,32 @@ def test_run_to_run_determinism(N):
     P.close()
 
 
-def test_streaming_and_every_asset_prox_agree(monkeypatch):
-    """The streaming form of the prox (k_prox_stream + k_prox_root) against the every-asset kernel on the same
-    problem: same fixed point, so the converged weights agree far below the parity tolerance."""
+def test_three_forms_of_the_prox_agree():
+    """The cluster-resident form (k_prox_res), the streaming form (k_prox_stream + k_prox_root) and the every-asset
+    kernel on the same problem (prism_constraint_set.prox_form): same fixed point, so the converged weights agree far
+    below the parity tolerance; each is also held to the oracle."""
+    from paper_2606_23367_b200 import binding
     inst = gen.config2(N=2048, k=20, A=6, G=6, band_half=0.01)
-    P1, r1 = _solve_gpu(inst)
-    monkeypatch.setenv("PRISM_PROX_NOFAST", "1")
-    P2, r2 = _solve_gpu(inst)
-    monkeypatch.delenv("PRISM_PROX_NOFAST")
-    assert (r1.status.cpu().numpy() == 0).all() and (r2.status.cpu().numpy() == 0).all()
-    assert float((r1.w - r2.w).abs().max()) <= 2e-6
-    # (iteration counts differ a little: the streaming form ramps the bands in over its first 20 iterations)
-    assert int((r1.iters - r2.iters).abs().max()) <= 60
-    P1.close(); P2.close()
+    W, res = _oracle(inst)
+    out = {}
+    for form in (binding.PROX_RESIDENT, binding.PROX_STREAMING, binding.PROX_EVERY_ASSET):
+        P, r = _solve_gpu(inst, prox_form=form)
+        _check_against_oracle(inst, r, W, res)
+        out[form] = r
+        P.close()
+    ref = out[binding.PROX_RESIDENT]
+    for form, r in out.items():
+        assert float((r.w - ref.w).abs().max()) <= 2e-6
+        assert int((r.iters - ref.iters).abs().max()) <= 60       # (the streaming form's windows differ a little)
+
+
+def test_form_that_does_not_apply_is_an_error():
+    from paper_2606_23367_b200 import binding
+    import paper_2606_23367_b200 as pr
+    with pytest.raises(RuntimeError, match="prox_form"):
+        pr.Problem(gen.config3(N=640, k=12, A=2), prox_form=binding.PROX_STREAMING)      # lots: no streaming form
+    with pytest.raises(RuntimeError, match="prox_form"):
+        pr.Problem(gen.config1(N=333, k=9, A=2), prox_form=binding.PROX_STREAMING)       # N % 16 != 0
 
 
 def test_residuals_call_is_external_and_matches_checker():
@@ -263,21 +276,70 @@ def test_solver_settings_do_not_change_the_answer(case, kw):
     P.close()
 
 
-def test_account_groups_match_single_group(monkeypatch):
-    """PRISM_PARTS: account groups solved concurrently on their own streams and host threads return, per account, the
-    result of the single-group solve up to the split-K summation order of GEMM-1 (rounding level), and the same
-    statuses; prism_residuals and the host-buffer lane work on the grouped object too."""
+def test_wide_box_and_no_cap():
+    """Bounds far from the budget scale (lo = -10, hi = +10: the streaming form's fixed-point range does not hold them,
+    ADVICE r1) on an N % 16 == 0 instance, against the oracle; the default form and the streaming request."""
+    from paper_2606_23367_b200 import binding
+    inst = gen.make_instance("wide", 11, 640, 8, 3, hi_fixed=10.0, tau_range=(0.2, 0.6))
+    inst.lo[:] = -10.0
+    W, res = _oracle(inst)
+    for form in (binding.PROX_AUTO, binding.PROX_STREAMING, binding.PROX_EVERY_ASSET):
+        P, r = _solve_gpu(inst, prox_form=form)
+        _check_against_oracle(inst, r, W, res)
+        P.close()
+
+
+def test_host_lane_with_benchmark_shift_and_new_mu():
+    """prism_solve_batch_host with PRISM_BENCHMARK_SHIFT: q = -mu - gamma Sigma w_b must follow the new mu."""
     import torch
     import paper_2606_23367_b200 as pr
-    inst = gen.config2(N=2560, k=50, A=9)
-    P1, r1 = _solve_gpu(inst)
-    monkeypatch.setenv("PRISM_PARTS", "3")
-    P3 = pr.Problem(inst)
-    r3 = P3.solve()
-    assert (r1.status.cpu().numpy() == 0).all() and (r3.status.cpu().numpy() == 0).all()
-    assert float((r1.w - r3.w).abs().max()) <= 1e-6
-    assert r3.info["n_certified"] == inst.A and r3.info["iters_total"] == int(r3.iters.sum())
-    rs = P3.residuals(r3.w, r3.duals).cpu().numpy()
-    assert np.nanmax(np.abs(rs[:, 0:4])) <= TOL_GATE
-    assert np.allclose(rs[:, 6], r3.resid.cpu().numpy()[:, 6], rtol=0, atol=1e-12)
-    P1.close(); P3.close()
+    from paper_2606_23367_b200 import binding
+    inst = gen.make_instance("wb", 7, 400, 8, 3, hi_fixed=0.05, tau_range=(0.2, 0.5), benchmark_in_risk=True)
+    P = pr.Problem(inst)
+    rng = np.random.default_rng(5)
+    inst2 = inst.subset(range(inst.A))
+    inst2.mu = inst.mu + 0.01 * rng.standard_normal(inst.mu.shape)
+    W, res = _oracle(inst2)
+    mu_h = torch.as_tensor(inst2.mu).pin_memory(); w0_h = torch.as_tensor(inst2.w0).pin_memory()
+    w_h = torch.empty((inst.A, inst.N), dtype=torch.float64).pin_memory(); st_h = torch.empty(inst.A, dtype=torch.int32).pin_memory()
+    it_h = torch.empty(inst.A, dtype=torch.int32).pin_memory(); rs_h = torch.empty((inst.A, binding.NRES), dtype=torch.float64).pin_memory()
+    P.solve_host(mu_h, w0_h, w_h, st_h, it_h, rs_h)
+    assert (st_h.numpy() == 0).all()
+    assert np.max(np.abs(w_h.numpy() - W)) <= TOL_W
+    assert rs_h.numpy()[:, 4].max() <= 1e-5                   # stationarity of the returned point with the NEW mu
+    P.close()
+
+
+@pytest.mark.parametrize("case", ["cfg2_stream_tight", "cfg1_stream", "cfg3_small"])
+def test_warm_start_repeated_run_lane(case):
+    """Repeated-run lane: a solve warm-started from the previous weights and multipliers of a slightly
+    different mu returns the cold-start answer of the new problem (same parity bar) in fewer iterations; warm-starting
+    from the problem's own solution converges at the first check."""
+    import paper_2606_23367_b200 as pr
+    inst = CASES[case]()
+    P = pr.Problem(inst)
+    r0 = P.solve()
+    r_same = P.solve(warm=r0, first_check=10)
+    assert (r_same.status.cpu().numpy() == 0).all()
+    assert int(r_same.iters.max()) <= 20, r_same.iters
+    assert float((r_same.w - r0.w).abs().max()) <= 2e-6
+    rng = np.random.default_rng(3)
+    inst2 = inst.subset(range(inst.A))
+    inst2.mu = inst.mu + 0.002 * rng.standard_normal(inst.mu.shape)
+    P2 = pr.Problem(inst2)
+    cold = P2.solve()
+    warm = P2.solve(warm=r0, first_check=10)
+    W, res = _oracle(inst2)
+    _check_against_oracle(inst2, warm, W, res)
+    _check_against_oracle(inst2, cold, W, res)
+    assert int(warm.iters.sum()) < int(cold.iters.sum()), (warm.iters, cold.iters)
+    P.close(); P2.close()
+
+
+def test_eps_abs_loosens_the_stopping_rule():
+    inst = gen.config1(N=400, k=10, A=4)
+    P, r = _solve_gpu(inst)
+    r2 = P.solve(eps_abs=1e-5, first_check=10)
+    assert (r2.status.cpu().numpy() == 0).all() and int(r2.iters.sum()) < int(r.iters.sum())
+    assert float((r2.w - r.w).abs().max()) <= 1e-3
+    P.close()
