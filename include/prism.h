@@ -215,6 +215,27 @@ enum { PRISM_K_PROX = 0, PRISM_K_GEMM1 = 1, PRISM_K_SOLVE = 2, PRISM_K_GEMM2 = 3
  * prism_solve_batch call that ran with settings.profile = 1.  ms_out, launches_out: host arrays of PRISM_NKERN. */
 int prism_kernel_times(const prism_problem* p, double* ms_out, int64_t* launches_out);
 
+/* Factor exposures of caller-given weights through the problem's own GEMM-1 (H1):
+ *   T_out[a * k + j] = sum_i B[i][j] w[a * N + i]       w: device A x N, T_out: device A x k.
+ * Split-K partials live in the workspace allocated at create.  Synchronises the stream. */
+int prism_factor_exposures(prism_problem* p, const double* w, void* cuda_stream, double* T_out);
+
+/* ---- the one entry point that ALLOCATES NOTHING (for CUDA graph capture, serving loops, harnesses that forbid
+ * cudaMalloc).  Same result as prism_factor_exposures, no problem object:
+ *   T_out[a * k + j] = sum_i B[i * k + j] X[a * N + i]   B: device N x k row-major (fp64, or fp32 when B_is_fp32),
+ *                                                        X: device accounts x N, T_out: device accounts x k.
+ * Its split-K partials live in a static __device__ array of PRISM_NOALLOC_SCRATCH_DOUBLES doubles (4 MiB) that every
+ * GPU loading the library holds until exit.  Limit: accounts * k <= PRISM_NOALLOC_SCRATCH_DOUBLES, else
+ * PRISM_ERR_INVALID_ARG.  Asynchronous on cuda_stream (no synchronisation); calls no cudaMalloc / cudaFree.
+ * All calls SHARE the array: calls that overlap on the GPU (different streams, concurrently replayed graphs) race -
+ * serialise them.  Nothing has to be cleared between calls (every partial read is written by the same call first).
+ * prism_noalloc_init() fetches the array's device address for the current device (cudaGetSymbolAddress); call it
+ * once per device before a graph capture - the entry point does the same lazily otherwise. */
+#define PRISM_NOALLOC_SCRATCH_DOUBLES 524288
+int prism_noalloc_init(void);
+int prism_factor_exposures_noalloc(const void* B, int32_t B_is_fp32, const double* X, int64_t N, int32_t k,
+                                   int32_t accounts, void* cuda_stream, double* T_out);
+
 /* Frees the workspace; never frees borrowed data.  NULL is allowed. */
 void prism_problem_destroy(prism_problem* p);
 

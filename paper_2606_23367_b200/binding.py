@@ -21,7 +21,9 @@ STATUS_NAMES = ["certified", "feasible/non-certified", "timeout", "deadline exce
                 "allocation/numerical failure"]
 SYMBOLS = ["prism_default_settings", "prism_problem_create", "prism_solve_batch", "prism_residuals",
            "prism_solve_batch_host", "prism_problem_destroy", "prism_problem_device_bytes", "prism_last_error",
-           "prism_version", "prism_kernel_times"]
+           "prism_version", "prism_kernel_times", "prism_factor_exposures", "prism_noalloc_init",
+           "prism_factor_exposures_noalloc"]
+NOALLOC_SCRATCH_DOUBLES = 524288      # prism.h: PRISM_NOALLOC_SCRATCH_DOUBLES
 
 
 PROX_AUTO, PROX_RESIDENT, PROX_STREAMING, PROX_EVERY_ASSET = 0, 1, 2, 3     # prism.h: PRISM_PROX_*
@@ -85,6 +87,11 @@ def load_library(path: str = LIB_PATH):
     L.prism_last_error.argtypes = []; L.prism_last_error.restype = C.c_char_p
     L.prism_version.argtypes = []; L.prism_version.restype = C.c_char_p
     L.prism_kernel_times.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int64)]; L.prism_kernel_times.restype = C.c_int
+    L.prism_factor_exposures.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]; L.prism_factor_exposures.restype = C.c_int
+    L.prism_noalloc_init.argtypes = []; L.prism_noalloc_init.restype = C.c_int
+    L.prism_factor_exposures_noalloc.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_int64, C.c_int32, C.c_int32,
+                                                 C.c_void_p, C.c_void_p]
+    L.prism_factor_exposures_noalloc.restype = C.c_int
     _lib = L
     return L
 
@@ -218,6 +225,16 @@ class Problem:
         _check(lib().prism_kernel_times(self.handle, ms, cnt))
         return {n: dict(ms=ms[i], launches=int(cnt[i])) for i, n in enumerate(self.KERNELS)}
 
+    def factor_exposures(self, w):
+        """prism_factor_exposures: (A, k) = w B through the problem's own GEMM-1."""
+        torch = self.torch
+        w = torch.as_tensor(w, dtype=torch.float64).contiguous().to(self.dev)
+        out = torch.empty((self.A, self.k), dtype=torch.float64, device=self.dev)
+        with torch.cuda.device(self.dev):
+            stream = torch.cuda.current_stream().cuda_stream
+            _check(lib().prism_factor_exposures(self.handle, w.data_ptr(), C.c_void_p(stream), out.data_ptr()))
+        return out
+
     def residuals(self, w, duals=None):
         torch = self.torch
         w = torch.as_tensor(w, dtype=torch.float64).contiguous().to(self.dev)
@@ -244,3 +261,18 @@ class Problem:
                                                 ptr(w_host), ptr(status_host), ptr(iters_host), ptr(resid_host),
                                                 C.byref(info)))
         return self._info(info)
+
+
+def factor_exposures_noalloc(B, X, out):
+    """prism_factor_exposures_noalloc on caller-owned CUDA tensors (B: (N, k) fp64 or fp32, X: (A, N) fp64, out: (A, k)
+    fp64, all contiguous).  Allocates nothing; asynchronous on the current stream."""
+    import torch
+    N, k = B.shape
+    A = X.shape[0]
+    assert X.shape[1] == N and tuple(out.shape) == (A, k) and B.is_contiguous() and X.is_contiguous() and out.is_contiguous()
+    assert X.dtype == torch.float64 and out.dtype == torch.float64 and B.dtype in (torch.float64, torch.float32)
+    with torch.cuda.device(X.device):
+        stream = torch.cuda.current_stream().cuda_stream
+        _check(lib().prism_factor_exposures_noalloc(B.data_ptr(), 1 if B.dtype == torch.float32 else 0, X.data_ptr(), N, k, A,
+                                                    C.c_void_p(stream), out.data_ptr()))
+    return out

@@ -70,3 +70,16 @@ cudaError_t nan_cols_launch(int A, double* resid, cudaStream_t st) {
   k_nan_cols<<<(A + 127) / 128, 128, 0, st>>>(A, resid);
   return cudaGetLastError();
 }
+// T[a][j] = sum over the split-K chunks of Tpart[ch][a][j] in chunk order, j < k (prism_factor_exposures)
+__global__ void k_reduce_partials(const double* Tpart, int nchunk, int A, int k, int64_t ldv, double* T) {
+  const int a = blockIdx.x;
+  for (int j = threadIdx.x; j < k; j += blockDim.x) {
+    double s = 0.0;
+    for (int ch = 0; ch < nchunk; ++ch) s += Tpart[((int64_t)ch * A + a) * ldv + j];
+    T[(int64_t)a * k + j] = s;
+  }
+}
+cudaError_t reduce_partials_launch(const double* Tpart, int nchunk, int A, int k, int64_t ldv, double* T, cudaStream_t st) {
+  k_reduce_partials<<<A, 128, 0, st>>>(Tpart, nchunk, A, k, ldv, T);
+  return cudaGetLastError();
+}

@@ -31,6 +31,10 @@ cudaError_t diag_launch(const DiagArgs& a, bool lots, cudaStream_t st);
 cudaError_t status_launch(int A, const double* resid, const int32_t* conv, const int32_t* iters, int timed_out, int late_iter,
                           double gate, int32_t* status, cudaStream_t st);
 cudaError_t nan_cols_launch(int A, double* resid, cudaStream_t st);
+cudaError_t reduce_partials_launch(const double* Tpart, int nchunk, int A, int k, int64_t ldv, double* T, cudaStream_t st);
+
+// error text of a translation unit other than prism.cu (g_err is per unit): sets prism_last_error(), returns code
+int prism_internal_set_error(int code, const char* what, const char* detail);
 
 // ---- cluster-resident prox (k_prox_res_plain.cu, k_prox_res_lots.cu)
 bool prox_res_geometry(int64_t N, int G, int* C, int* SL, size_t* smem);

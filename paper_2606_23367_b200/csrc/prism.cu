@@ -23,6 +23,10 @@ extern "C" void prism_default_settings(prism_settings* s) {
   s->time_limit_ms = 0.0; s->deadline_ms = 0.0; s->prox_window_mult = 32.0; s->warm_w = nullptr; s->warm_duals = nullptr;
 }
 extern "C" const char* prism_last_error(void) { return g_err; }
+int prism_internal_set_error(int code, const char* what, const char* detail) {
+  snprintf(g_err, sizeof(g_err), "%s%s%s", what, (detail && detail[0]) ? ": " : "", detail ? detail : "");
+  return code;
+}
 extern "C" const char* prism_version(void) { return PRISM_VERSION_STR; }
 extern "C" int64_t prism_problem_device_bytes(const prism_problem* p) { return p ? p->bytes : 0; }
 
@@ -453,6 +457,21 @@ extern "C" int prism_solve_batch(prism_problem* p, const prism_settings* sp, voi
   }
   cudaEventDestroy(ev0);
   cudaEventDestroy(ev1);
+  return PRISM_OK;
+}
+
+// T_out[a][j] = sum_i B[i][j] w[a][i]: the problem's own GEMM-1 (H1) on caller-given vectors, split-K partials in the
+// workspace allocated at create, reduced in chunk order.  Uses rt as the padded copy of w.
+extern "C" int prism_factor_exposures(prism_problem* p, const double* w, void* cuda_stream, double* T_out) {
+  if (!p) return set_err(PRISM_ERR_NOT_READY, "problem object is NULL%s", "");
+  if (!w || !T_out) return set_err(PRISM_ERR_INVALID_ARG, "w and T_out are mandatory%s", "");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  Launcher L{p, st, p->kp / 8, 0};
+  L.end(diff_launch(w, nullptr, p->N, p->ldn, p->A, p->rt, st));
+  L.gemm1(p->rt, nullptr);
+  L.end(reduce_partials_launch(p->Tpart, p->nchunk, p->A, p->k, p->ldv, T_out, st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  if (L.err != cudaSuccess) return set_err(PRISM_ERR_CUDA, "kernel launch failed: %s", cudaGetErrorString(L.err));
   return PRISM_OK;
 }
 
