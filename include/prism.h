@@ -236,6 +236,10 @@ int prism_noalloc_init(void);
 int prism_factor_exposures_noalloc(const void* B, int32_t B_is_fp32, const double* X, int64_t N, int32_t k,
                                    int32_t accounts, void* cuda_stream, double* T_out);
 
+/* fp64 yardstick of THIS device: register-resident loops without memory traffic, CUDA-event timed on
+ * cuda_stream, best of 5.  tflops_out (host, 2 doubles): [0] tensor pipe (DMMA mma.sync m8n8k4), [1] FMA pipe. */
+int prism_fp64_yardstick(prism_problem* p, void* cuda_stream, double* tflops_out);
+
 /* Frees the workspace; never frees borrowed data.  NULL is allowed. */
 void prism_problem_destroy(prism_problem* p);
 

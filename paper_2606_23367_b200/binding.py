@@ -22,7 +22,7 @@ STATUS_NAMES = ["certified", "feasible/non-certified", "timeout", "deadline exce
 SYMBOLS = ["prism_default_settings", "prism_problem_create", "prism_solve_batch", "prism_residuals",
            "prism_solve_batch_host", "prism_problem_destroy", "prism_problem_device_bytes", "prism_last_error",
            "prism_version", "prism_kernel_times", "prism_factor_exposures", "prism_noalloc_init",
-           "prism_factor_exposures_noalloc"]
+           "prism_factor_exposures_noalloc", "prism_fp64_yardstick"]
 NOALLOC_SCRATCH_DOUBLES = 524288      # prism.h: PRISM_NOALLOC_SCRATCH_DOUBLES
 
 
@@ -89,6 +89,7 @@ def load_library(path: str = LIB_PATH):
     L.prism_kernel_times.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int64)]; L.prism_kernel_times.restype = C.c_int
     L.prism_factor_exposures.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]; L.prism_factor_exposures.restype = C.c_int
     L.prism_noalloc_init.argtypes = []; L.prism_noalloc_init.restype = C.c_int
+    L.prism_fp64_yardstick.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_double)]; L.prism_fp64_yardstick.restype = C.c_int
     L.prism_factor_exposures_noalloc.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_int64, C.c_int32, C.c_int32,
                                                  C.c_void_p, C.c_void_p]
     L.prism_factor_exposures_noalloc.restype = C.c_int
@@ -224,6 +225,14 @@ class Problem:
         ms = (C.c_double * 8)(); cnt = (C.c_int64 * 8)()
         _check(lib().prism_kernel_times(self.handle, ms, cnt))
         return {n: dict(ms=ms[i], launches=int(cnt[i])) for i, n in enumerate(self.KERNELS)}
+
+    def fp64_yardstick(self) -> dict:
+        """prism_fp64_yardstick: measured fp64 TFLOP/s of this device (tensor pipe DMMA, FMA pipe)."""
+        out = (C.c_double * 2)()
+        with self.torch.cuda.device(self.dev):
+            stream = self.torch.cuda.current_stream().cuda_stream
+            _check(lib().prism_fp64_yardstick(self.handle, C.c_void_p(stream), out))
+        return dict(dmma_tflops=out[0], fma_tflops=out[1])
 
     def factor_exposures(self, w):
         """prism_factor_exposures: (A, k) = w B through the problem's own GEMM-1."""

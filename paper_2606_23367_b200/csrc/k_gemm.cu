@@ -53,3 +53,58 @@ cudaError_t gemm2_launch(int gemm_mode, int mt, int mode, const Gemm2Args& a, cu
   else gemm2_mode<G2_SIGMA>(gemm_mode, mt, a, st);
   return cudaGetLastError();
 }
+
+// ------------------------------------------------------------------------------------------------ fp64 yardstick
+// Register-resident loops with no memory traffic: what the fp64 tensor pipe (mma.sync m8n8k4 DMMA) and the fp64 FMA pipe
+// of THIS device sustain.  bench.py quotes the factor GEMMs against these ("measure a yardstick on the box").
+__global__ void __launch_bounds__(256) k_yard_dmma(int iters, double* sink) {
+  double acc[8][2];
+#pragma unroll
+  for (int m = 0; m < 8; ++m) { acc[m][0] = 0.0; acc[m][1] = 0.0; }
+  const double a = 1.0 + 1e-9 * threadIdx.x, b = 1.0 - 1e-9 * threadIdx.x;
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int m = 0; m < 8; ++m) dmma884(acc[m][0], acc[m][1], a, b);
+  }
+  double s = 0.0;
+#pragma unroll
+  for (int m = 0; m < 8; ++m) s += acc[m][0] + acc[m][1];
+  if (s == 123.456) sink[0] = s;          // keeps the loop alive
+}
+__global__ void __launch_bounds__(256) k_yard_fma(int iters, double* sink) {
+  double acc[8];
+#pragma unroll
+  for (int m = 0; m < 8; ++m) acc[m] = 1e-3 * m;
+  const double a = 1.0 + 1e-9 * threadIdx.x, b = 1e-9 * threadIdx.x;
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int m = 0; m < 8; ++m) acc[m] = fma(acc[m], a, b);
+  }
+  double s = 0.0;
+#pragma unroll
+  for (int m = 0; m < 8; ++m) s += acc[m];
+  if (s == 123.456) sink[0] = s;
+}
+// tflops[0] = DMMA, tflops[1] = FMA (2 flops per multiply-add); best of 5 launches each, CUDA events on `st`
+cudaError_t fp64_yardstick(cudaStream_t st, double* sink_dev, int sm_count, double* tflops) {
+  cudaEvent_t e0, e1;
+  TRY(cudaEventCreate(&e0)); TRY(cudaEventCreate(&e1));
+  const int iters = 4096, grid = sm_count * 8, nt = 256;
+  for (int which = 0; which < 2; ++which) {
+    float best = 1e30f;
+    for (int rep = 0; rep < 6; ++rep) {
+      cudaEventRecord(e0, st);
+      if (which == 0) k_yard_dmma<<<grid, nt, 0, st>>>(iters, sink_dev); else k_yard_fma<<<grid, nt, 0, st>>>(iters, sink_dev);
+      cudaEventRecord(e1, st);
+      TRY(cudaEventSynchronize(e1));
+      float ms = 0.f;
+      cudaEventElapsedTime(&ms, e0, e1);
+      if (rep > 0 && ms < best) best = ms;
+    }
+    // DMMA m8n8k4: 8*8*4 multiply-adds per warp instruction; FMA: one per thread
+    const double per_thread_block = which == 0 ? 8.0 * (8 * 8 * 4) * 2.0 * (nt / 32) : 8.0 * 2.0 * nt;
+    tflops[which] = per_thread_block * (double)iters * (double)grid / (best * 1e-3) / 1e12;
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  return cudaGetLastError();
+}

@@ -13,6 +13,8 @@ cudaError_t gemm_set_attrs(int mt);
 cudaError_t gemm1_launch(int gemm_mode, int mt, int nchunk, int kp, const Gemm1Args& a, cudaStream_t st);
 cudaError_t gemm2_launch(int gemm_mode, int mt, int mode /* G2_* */, const Gemm2Args& a, cudaStream_t st);
 
+cudaError_t fp64_yardstick(cudaStream_t st, double* sink_dev, int sm_count, double* tflops /* host [2]: DMMA, FMA */);
+
 // ---- small kernels (k_small.cu)
 cudaError_t small_set_attrs(int Kp);
 cudaError_t setup_shared_launch(const void* B, int is32, const double* d, int64_t N, int k, int kp, int64_t ldn, double* Bp,

@@ -175,7 +175,14 @@ extern "C" int prism_problem_create(int64_t N, int32_t k, int32_t accounts, cons
     const bool res_ok = prox_res_geometry(N, G, &C, &SL, &sm);
     const bool str_ok = stream_applicable(p);
     int form = cs->prox_form;
-    if (form == PRISM_PROX_AUTO) form = res_ok ? PRISM_PROX_RESIDENT : (str_ok ? PRISM_PROX_STREAMING : PRISM_PROX_EVERY_ASSET);
+    // AUTO, by measurement on one B200 (kernel table): where both fast forms apply the streaming pair wins once
+    // an account needs more than one CTA of the resident form (configs[2]: 65 ms against 78 ms per batch: its streaming
+    // pass runs at three CTAs per SM with no wave quantisation), the resident form wins on accounts that fit one CTA
+    // (configs[1]: 11.6 against 12.6 ms) and is the only fast form for tax lots, per-asset caps and N % 16 != 0.
+    if (form == PRISM_PROX_AUTO) {
+      if (res_ok && (C == 1 || !str_ok)) form = PRISM_PROX_RESIDENT;
+      else form = str_ok ? PRISM_PROX_STREAMING : (res_ok ? PRISM_PROX_RESIDENT : PRISM_PROX_EVERY_ASSET);
+    }
     if ((form == PRISM_PROX_RESIDENT && !res_ok) || (form == PRISM_PROX_STREAMING && !str_ok)) {
       delete p;
       return set_err(PRISM_ERR_INVALID_ARG, "prox_form %s%lld does not apply to this problem (see prism.h)", "", form);
@@ -472,6 +479,15 @@ extern "C" int prism_factor_exposures(prism_problem* p, const double* w, void* c
   L.end(reduce_partials_launch(p->Tpart, p->nchunk, p->A, p->k, p->ldv, T_out, st));
   CUDA_TRY(cudaStreamSynchronize(st));
   if (L.err != cudaSuccess) return set_err(PRISM_ERR_CUDA, "kernel launch failed: %s", cudaGetErrorString(L.err));
+  return PRISM_OK;
+}
+
+// Measured fp64 rates of this device (register-resident loops, no memory traffic): tflops_out[0] = tensor pipe (DMMA
+// mma.sync m8n8k4), tflops_out[1] = FMA pipe.  Uses the problem's counter block as the (never written) sink.
+extern "C" int prism_fp64_yardstick(prism_problem* p, void* cuda_stream, double* tflops_out) {
+  if (!p || !tflops_out) return set_err(PRISM_ERR_INVALID_ARG, "null argument%s", "");
+  const cudaError_t e = fp64_yardstick((cudaStream_t)cuda_stream, p->resid, p->sm_count, tflops_out);
+  if (e != cudaSuccess) return set_err(PRISM_ERR_CUDA, "yardstick failed: %s", cudaGetErrorString(e));
   return PRISM_OK;
 }
 
