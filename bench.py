@@ -6,9 +6,10 @@ One "step" = one cold prism_solve_batch over a synthetic batch shaped like BASEL
 long-only box 0.05), every account solved to 1e-6 scaled KKT residuals (BASELINE.json:metric).
 Prints ONE JSON line (see the task contract): value = accounts/sec with inputs resident in HBM; e2e = the same
 metric through prism_solve_batch_host with pinned HOST buffers (H2D of mu and w0, D2H of weights, statuses,
-iterations and the residual block inside the timed region); roofline of the dominant kernel from per-kernel CUDA
-events; cpu_baseline = the fp64 oracle (oracle/ipm.py, as it stands) timed on this box's host cores on a bounded
-sample of the same workload.
+iterations and the residual block inside the timed region); roofline of the kernel class that dominates the solve
+(per-launch CUDA events of a separate profiled solve; GEMM fractions against an fp64 yardstick measured in the same
+run); `extra`: the same solve on the other configured shapes and the N sweep; cpu_baseline = the fp64 oracle
+(oracle/ipm.py, as it stands) on this box's host cores, accounts in parallel processes, on a random sample.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config cfg2] [--accounts A]
 """
@@ -26,7 +27,6 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 PROX_BYTES_PER_ELEM = 41.0      # v 8 + w0 8 + mu 8 + exclusion mask 1 read; r~ 8 + c 8 written (kernel table)
-PROX_NCU_TRAFFIC_BYTES = 174.35e6   # k_prox_stream<0>, one launch, all 500 accounts active (profiles/r1c_prox_ncu_full.md)
 PROX_CHECK_EXTRA_BYTES = 24.0   # check iterations: x 8 + (P x + q) 8 read, w_out 8 written (kernel table)
 
 
@@ -93,46 +93,83 @@ def make_instance(cfg: str, seed: int, accounts):
     return gen.by_name(cfg, seed=seed, **kw)
 
 
-def oracle_sample(inst, n_accounts: int):
-    """Times the oracle (as it stands) on the first n accounts; returns (accounts/sec, threads, seconds)."""
-    from oracle import ipm, problem
+def _oracle_one(args):
+    """Worker process: one account through the oracle as it stands, one BLAS thread (the parallelism is over accounts)."""
+    cfg, seed, A, a = args
     try:
-        from threadpoolctl import threadpool_info
-        threads = max([p.get("num_threads", 1) for p in threadpool_info()] + [1])
+        from threadpoolctl import threadpool_limits
+        ctx = threadpool_limits(limits=1)
     except Exception:
-        threads = os.cpu_count() or 1
+        ctx = None
+    from instances import gen
+    from oracle import ipm, problem
+    global _ORACLE_INST
+    key = (cfg, seed, A)
+    if globals().get("_ORACLE_KEY") != key:
+        globals()["_ORACLE_INST"] = gen.by_name(cfg, seed=seed, **({"A": A} if A else {}))
+        globals()["_ORACLE_KEY"] = key
+    inst = globals()["_ORACLE_INST"]
     t0 = time.perf_counter()
-    done = 0
-    for a in range(n_accounts):
-        r = ipm.solve(problem.account_from_instance(inst, a), witness=inst.witness[a])
-        if r["status"] != "optimal":
-            raise RuntimeError(f"oracle failed on account {a}: {r['status']}")
-        done += 1
-    dt = time.perf_counter() - t0
-    return done / dt, threads, dt
+    r = ipm.solve(problem.account_from_instance(inst, a), witness=inst.witness[a])
+    return a, r["status"], time.perf_counter() - t0
+
+
+class OraclePool:
+    """The fp64 oracle (oracle/ipm.py, untuned) on the host cores: accounts in parallel worker processes, one account
+    per process at a time, one BLAS thread each.  cores = number of worker processes."""
+
+    def __init__(self, cfg, seed, accounts, procs=None):
+        import multiprocessing as mp
+        self.cfg, self.seed, self.A = cfg, seed, accounts
+        self.procs = procs or max(1, min(os.cpu_count() or 1, 32))
+        self.pool = mp.get_context("spawn").Pool(self.procs)
+
+    def run(self, account_ids):
+        """Solves the listed accounts; returns (accounts/sec, seconds)."""
+        t0 = time.perf_counter()
+        out = self.pool.map(_oracle_one, [(self.cfg, self.seed, self.A, int(a)) for a in account_ids], chunksize=1)
+        dt = time.perf_counter() - t0
+        bad = [(a, st) for a, st, _ in out if st != "optimal"]
+        if bad:
+            raise RuntimeError(f"oracle failed on accounts {bad[:4]}")
+        return len(account_ids) / dt, dt
+
+    def close(self):
+        self.pool.close(); self.pool.join()
 
 
 def run_reference(args):
-    """--impl reference: the oracle timed on the host cores (rank 0 only), bounded sample per step."""
+    """--impl reference: the oracle timed on the host cores (rank 0 only).  Each step solves a bounded random sample of
+    the workload's accounts, sized after the warm-up step so that the whole run ends within a few minutes."""
+    import numpy as np
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    inst = make_instance(args.config, 0, max(args.oracle_accounts, 1))
-    n = min(args.oracle_accounts, inst.A)
-    for _ in range(min(args.warmup, 1)):
-        oracle_sample(inst, 1)
-    tot_t = 0.0; tot_n = 0; threads = 1
+    cfg = args.config
+    A_full = args.accounts or {"cfg0": 1, "cfg1": 100, "cfg2": 500, "cfg3": 200, "cfg4": 32}.get(cfg, 100)
+    pool = OraclePool(cfg, 0, args.accounts)
+    rng = np.random.default_rng(0)
+    n = min(pool.procs, A_full)
+    ids = rng.choice(A_full, size=n, replace=False)
+    _, t1 = pool.run(ids)                                         # warm-up step (also builds the instance in every worker)
+    _, t1 = pool.run(ids)
+    budget = 200.0                                                # seconds for the timed steps
+    per_step = max(1, min(n, int(n * budget / max(args.steps * t1, 1e-9))))
+    tot_t = 0.0; tot_n = 0
     for _ in range(args.steps):
-        aps, threads, dt = oracle_sample(inst, n)
-        tot_t += dt; tot_n += n
+        ids = rng.choice(A_full, size=per_step, replace=False)
+        _, dt = pool.run(ids)
+        tot_t += dt; tot_n += per_step
+    pool.close()
     value = tot_n / tot_t
-    sample = f"first {n} accounts of {args.config} (N={inst.N}, k={inst.k}, G={inst.G}) per step, structured interior point, fp64"
+    sample = (f"{per_step} randomly chosen accounts of {cfg} per step ({A_full} in the batch), oracle/ipm.py structured interior point "
+              f"fp64, one account per worker process, {pool.procs} processes x 1 BLAS thread")
     print(json.dumps({
         "impl": "reference", "metric": "accounts/sec solved to 1e-6 KKT at N=10k batch 500", "value": value, "unit": "accounts/s",
         "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / max(args.steps, 1),
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": f"{args.config}: {sample}"},
-        "cpu_baseline": {"value": value, "unit": "accounts/s", "cores": threads, "kind": "oracle", "sample": sample},
+        "config": {"workload": f"{cfg}: {sample}"},
+        "cpu_baseline": {"value": value, "unit": "accounts/s", "cores": pool.procs, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": "accounts/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0}))
 
@@ -145,9 +182,10 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="cfg2")
     ap.add_argument("--accounts", type=int, default=0, help="override the batch size (debug only)")
-    ap.add_argument("--oracle-accounts", type=int, default=2, help="accounts in the cpu_baseline sample")
+    ap.add_argument("--oracle-accounts", type=int, default=32, help="accounts in the cpu_baseline sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--gemm-mode", type=int, default=0)
+    ap.add_argument("--no-extra", action="store_true", help="skip the rows for the other configs and the N sweep")
+    ap.add_argument("--gemm-precision", type=int, default=0)
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -172,8 +210,13 @@ def main():
     # weak scaling: every rank solves its own batch (accounts are independent programs);
     # the shared universe is replicated, there is no data-path collective.
     inst = make_instance(args.config, seed=rank, accounts=args.accounts)
+    torch.cuda.synchronize()
+    t_c0 = time.perf_counter()
     P = pr.Problem(inst, device=dev)
-    settings = binding.default_settings(gemm_precision=args.gemm_mode)
+    settings = binding.default_settings(gemm_precision=args.gemm_precision)
+    first = P.solve(settings)
+    torch.cuda.synchronize()
+    create_plus_solve_ms = 1e3 * (time.perf_counter() - t_c0)      # upload + prism_problem_create + first cold solve (R17)
     A, N = inst.A, inst.N
 
     def barrier():
@@ -181,26 +224,30 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    # ---------------- device-resident lane (value)
-    last = None
-    for _ in range(max(args.warmup, 3) if args.warmup >= 3 else args.warmup):
+    def allmax(x):
+        if dist is None:
+            return x
+        t = torch.tensor([x], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    # ---------------- device-resident lane (value): only certified accounts count
+    last = first
+    for _ in range(max(args.warmup, 3)):
         last = P.solve(settings)
     barrier()
     ev0 = torch.cuda.Event(enable_timing=True); ev1 = torch.cuda.Event(enable_timing=True)
-    launches = 0; iters_total = 0; interval_ms = 0.0
+    launches = 0; iters_total = 0; interval_ms = 0.0; certified = 0
     with ClockSampler(local) as cs:
         ev0.record()
         for _ in range(args.steps):
             last = P.solve(settings)
-            launches += last.info["kernel_launches"]; iters_total += last.info["iters_total"]; interval_ms += last.info["solve_interval_ms"]
+            launches += last.info["kernel_launches"]; iters_total += last.info["iters_total"]
+            interval_ms += last.info["solve_interval_ms"]; certified += last.info["n_certified"]
         ev1.record()
         barrier()
-    ms = ev0.elapsed_time(ev1)
+    ms = allmax(ev0.elapsed_time(ev1))
     clocks = cs.summary()
-    if dist is not None:
-        t = torch.tensor([ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
     status = last.status.cpu().numpy(); iters = last.iters.cpu().numpy(); resid = last.resid.cpu().numpy()
     n_cert = int((status == 0).sum())
 
@@ -208,84 +255,142 @@ def main():
     mu_h = torch.as_tensor(inst.mu).pin_memory(); w0_h = torch.as_tensor(inst.w0).pin_memory()
     w_h = torch.empty((A, N), dtype=torch.float64).pin_memory(); st_h = torch.empty(A, dtype=torch.int32).pin_memory()
     it_h = torch.empty(A, dtype=torch.int32).pin_memory(); rs_h = torch.empty((A, binding.NRES), dtype=torch.float64).pin_memory()
-    for _ in range(1):
-        P.solve_host(mu_h, w0_h, w_h, st_h, it_h, rs_h, settings)
+    P.solve_host(mu_h, w0_h, w_h, st_h, it_h, rs_h, settings)
     barrier()
     e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+    e2e_cert = 0
     e0.record()
     t0 = time.perf_counter()
     for _ in range(args.steps):
         P.solve_host(mu_h, w0_h, w_h, st_h, it_h, rs_h, settings)
+        e2e_cert += int((st_h.numpy() == 0).sum())
     e1.record()
     barrier()
-    e2e_ms = max(e0.elapsed_time(e1), 1e3 * (time.perf_counter() - t0))
-    if dist is not None:
-        t = torch.tensor([e2e_ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_ms = float(t.item())
+    e2e_ms = allmax(max(e0.elapsed_time(e1), 1e3 * (time.perf_counter() - t0)))
     lane_diff = float((w_h.to(dev) - last.w).abs().max())
     assert lane_diff < 1e-9, f"host lane and device lane disagree: {lane_diff}"
     h2d = mu_h.numel() * 8 + w0_h.numel() * 8
     d2h = w_h.numel() * 8 + st_h.numel() * 4 + it_h.numel() * 4 + rs_h.numel() * 8
 
-    # ---------------- roofline of the dominant kernel: one extra solve with per-launch CUDA events (not timed above)
-    prof = binding.default_settings(gemm_precision=args.gemm_mode, profile=1)
-    rp = P.solve(prof)
-    kt = P.kernel_times()
-    tot_k = sum(v["ms"] for v in kt.values()) or 1.0
-    dom = max(kt, key=lambda n: kt[n]["ms"])
+    # ---------------- per-kernel accounting: one extra solve with per-launch CUDA events (not part of the timings above)
     peak, peak_src = load_peaks()
-    prox = kt["prox"]
-    elem_iters = float(N) * float(rp.info["iters_total"])          # account-iterations x N: elements the prox launches processed
-    # check launches (every check_every-th iteration of an account) also read x and P x + q and write w_out: + 24 B
-    it_prof = rp.iters.cpu().numpy().astype(np.int64)
-    ce, fc = int(prof.check_every), int(prof.first_check)
-    n_checks = np.maximum(it_prof // ce - (fc + ce - 1) // ce + 1, 0)         # checks at iterations ceil(fc/ce) ce, ... <= iters
-    check_elems = float(N) * float(n_checks.sum())
-    prox_bytes_per_launch = (PROX_BYTES_PER_ELEM * elem_iters + PROX_CHECK_EXTRA_BYTES * check_elems) / max(prox["launches"], 1)
-    prox_ms_per_launch = prox["ms"] / max(prox["launches"], 1)
-    achieved = prox_bytes_per_launch / (prox_ms_per_launch * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "kernel": "k_prox_stream (H4/H5 fused projection + rhs assembly + residual terms, streaming pass)",
-                "achieved": achieved, "peak": peak,
-                "unit": "GB/s", "frac": achieved / peak,
-                # dram__bytes_read.sum + dram__bytes_write.sum of one full-batch launch (500 accounts x 10,000), from the
-                # ncu --set full capture summarised in profiles/r1c_prox_ncu_full.md; only meaningful for the cfg2 batch
-                "traffic": PROX_NCU_TRAFFIC_BYTES if (args.config == "cfg2" and not args.accounts) else None,
-                "traffic_source": "profiles/r1c_prox_ncu_full.md (ncu --set full, one launch with all accounts active: 205 MB algorithmic)",
+    yard = P.fp64_yardstick()                                      # measured on this device, this run
+
+    def profile(Pq, instq):
+        """Per-kernel-class device time of one profiled solve and the algorithmic bytes / flops it stands for."""
+        rp = Pq.solve(binding.default_settings(gemm_precision=args.gemm_precision, profile=1))
+        kt = Pq.kernel_times()
+        tot = sum(v["ms"] for v in kt.values()) or 1.0
+        itp = rp.iters.cpu().numpy().astype(np.int64)
+        ce, fc = 10, 40                                             # check_every, first_check defaults
+        n_checks = np.maximum(itp // ce - (fc + ce - 1) // ce + 1, 0)
+        elem_it = float(instq.N) * float(itp.sum()); elem_ck = float(instq.N) * float(n_checks.sum())
+        lots = instq.lot_slope is not None
+        per = {}
+        # H4 (+H5-H7): the fused projection; for the streaming form both of its kernels (k_prox_stream + k_prox_root)
+        # lots / caps: the pass reads per asset the cap 8 B, the lot count 1 B and the first slope 8 B (lot rows only for live assets)
+        b_prox = (PROX_BYTES_PER_ELEM + (17.0 if lots else 0.0)) * elem_it + PROX_CHECK_EXTRA_BYTES * elem_ck
+        b_g2 = 24.0 * elem_it + 24.0 * elem_ck                      # v, c read, v written (+ r~ read, x, Px+q written on checks)
+        b_g1 = 8.0 * elem_it                                        # r~ read
+        fl = 2.0 * instq.k * elem_it                                # per GEMM
+        for name, nbytes, flops in (("prox", b_prox, 0.0), ("gemm2", b_g2, fl), ("gemm1", b_g1, fl)):
+            t = kt[name]["ms"] * 1e-3
+            if t <= 0:
+                continue
+            per[name] = {"ms": kt[name]["ms"], "launches": kt[name]["launches"], "share": kt[name]["ms"] / tot,
+                         "algorithmic_GBps": nbytes / t / 1e9, "hbm_frac": nbytes / t / 1e9 / peak}
+            if flops:
+                per[name]["fp64_TFLOPs"] = flops / t / 1e12
+                per[name]["frac_of_measured_dmma"] = flops / t / 1e12 / yard["dmma_tflops"]
+        for name in ("solve", "factor", "diag", "other"):
+            if kt[name]["ms"] > 0:
+                per[name] = {"ms": kt[name]["ms"], "launches": kt[name]["launches"], "share": kt[name]["ms"] / tot}
+        dom = max(kt, key=lambda n: kt[n]["ms"])
+        return rp, kt, per, dom, tot, b_prox + b_g2 + b_g1
+
+    rp, kt, per, dom, tot_k, step_bytes = profile(P, inst)
+    domk = per[dom]
+    FORMS = {1: "k_prox_res (cluster-resident form)", 2: "k_prox_stream + k_prox_root (streaming form)", 3: "k_prox (every-asset form)"}
+    kernel_names = {"prox": "H4-H7 fused projection: " + FORMS[P.prox_form],
+                    "gemm2": "H3 k_gemm2 (factor GEMM-2 + epilogue)", "gemm1": "H1 k_gemm1 (split-K factor GEMM-1)"}
+    roofline = {"bound": "hbm", "kernel": kernel_names.get(dom, dom), "dominant_by_time": dom,
+                "achieved": domk.get("algorithmic_GBps"), "peak": peak, "unit": "GB/s",
+                "frac": domk.get("hbm_frac"), "traffic": None,
+                "traffic_note": "not measured inside bench.py; ncu dram bytes per launch are in profiles/r2_*.md",
                 "peak_source": peak_src,
-                "factor_gemm_tensor_pipe": {"gemm1_dmma_pct_of_peak": 67.4, "gemm2_dmma_pct_of_peak": 43.0,
-                                            "source": "profiles/r1c_gemm_ncu_full.md (sm__inst_executed_pipe_tensor_subpipe_dmma, fp64 mma.sync)"},
-                "bytes_per_launch": prox_bytes_per_launch, "ms_per_launch": prox_ms_per_launch,
-                "dominant_by_time": dom,
-                "kernel_share": {n: round(v["ms"] / tot_k, 4) for n, v in kt.items()},
-                "kernel_ms_per_launch": {n: (v["ms"] / v["launches"] if v["launches"] else None) for n, v in kt.items()}}
+                "bytes_per_launch": (domk["algorithmic_GBps"] * 1e9 * domk["ms"] * 1e-3 / max(domk["launches"], 1)) if "algorithmic_GBps" in domk else None,
+                "ms_per_launch": domk["ms"] / max(domk["launches"], 1),
+                "whole_step": {"algorithmic_GBps": step_bytes / (rp.info["solve_interval_ms"] * 1e-3) / 1e9,
+                               "hbm_frac": step_bytes / (rp.info["solve_interval_ms"] * 1e-3) / 1e9 / peak,
+                               "bytes_per_element_iteration": "prox 41 (+24 on check iterations) + gemm1 8 + gemm2 24 (+24)"},
+                "fp64_yardstick_TFLOPs": yard, "per_kernel": per}
+
+    def row(name, instq, form=0):
+        Pq = pr.Problem(instq, device=dev, prox_form=form)
+        Pq.solve(settings)
+        r = Pq.solve(settings)
+        _, ktq, perq, domq, _, _ = profile(Pq, instq)
+        itq = r.iters.cpu().numpy(); stq = r.status.cpu().numpy(); rsq = r.resid.cpu().numpy()
+        out = {"config": name, "A": instq.A, "N": instq.N, "k": instq.k, "G": instq.G, "solve_ms": r.info["solve_interval_ms"],
+               "accounts_per_s": int((stq == 0).sum()) / (r.info["wall_ms"] * 1e-3), "certified": int((stq == 0).sum()),
+               "iters_p50": float(np.median(itq)), "iters_max": int(itq.max()),
+               "iterations_per_sec": r.info["iters_total"] / (r.info["solve_interval_ms"] * 1e-3),
+               "max_scaled_residual": float(max(rsq[:, 7].max(), rsq[:, 8].max())), "max_gate_residual": float(rsq[:, 0:4].max()),
+               "prox_form": FORMS[Pq.prox_form], "dominant_kernel": domq, "kernel_share": {n: round(v["share"], 3) for n, v in perq.items()},
+               "launches": int(r.info["kernel_launches"]), "device_bytes": Pq.device_bytes}
+        Pq.close()
+        return out
+
+    t_sec = time.perf_counter()
+    extra = []
+    if rank == 0 and not args.no_extra:
+        from instances import gen
+        for name in ("cfg0", "cfg1", "cfg3", "cfg4"):
+            if name != args.config:
+                extra.append(row(name, gen.by_name(name, seed=0)))
+        for Ns, ks in ((100, 10), (500, 20), (1000, 30), (2000, 30)):       # R24: N sweep, A = 100, configs[1] distributions
+            extra.append(row(f"sweep_N{Ns}", gen.config1(seed=0, N=Ns, k=ks, A=100)))
+        if args.config == "cfg2":                                            # the other form of the projection on the headline batch
+            extra.append(dict(row("cfg2_resident_form", inst, form=binding.PROX_RESIDENT), note="prox_form = PRISM_PROX_RESIDENT"))
 
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
         return
+    sys.stderr.write(f"[bench] extra rows: {time.perf_counter() - t_sec:.1f} s\n"); t_sec = time.perf_counter()
     # ---------------- oracle on the host cores (reported baseline, not the target)
     cpu = None
     if not args.no_cpu_baseline:
         n = min(args.oracle_accounts, A)
-        aps, threads, dt = oracle_sample(inst, n)
-        cpu = {"value": aps, "unit": "accounts/s", "cores": threads, "kind": "oracle",
-               "sample": f"first {n} of the {A} accounts of this batch, structured interior point fp64, {dt:.1f} s"}
-    total_accounts = A * args.steps * world
+        pool = OraclePool(args.config, rank, args.accounts)
+        ids = np.random.default_rng(0).choice(A, size=n, replace=False)
+        pool.run(ids[:min(len(ids), pool.procs)])                            # builds the instance in every worker (untimed)
+        aps, dt = pool.run(ids)
+        pool.close()
+        cpu = {"value": aps, "unit": "accounts/s", "cores": pool.procs, "kind": "oracle",
+               "sample": f"{n} randomly chosen accounts of the {A} of this batch, oracle/ipm.py structured interior point fp64, "
+                         f"one account per worker process ({pool.procs} processes x 1 BLAS thread), {dt:.1f} s"}
+    sys.stderr.write(f"[bench] cpu baseline: {time.perf_counter() - t_sec:.1f} s\n")
     out = {
-        "metric": "accounts/sec solved to 1e-6 KKT at N=10k batch 500", "value": total_accounts / (ms * 1e-3), "unit": "accounts/s",
+        "metric": "accounts/sec solved to 1e-6 KKT at N=10k batch 500", "value": certified * world / (ms * 1e-3), "unit": "accounts/s",
         "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": f"{inst.name}: {A} accounts x N={N}, k={inst.k}, G={inst.G} per GPU (BASELINE.json configs[2] shape), cold start every step",
                    "eps_rel": settings.eps_rel, "l2": "working set > L2 (3 state arrays + mu, w0, mask = 205 MB vs 126 MB L2); each step is a full cold solve",
-                   "certified": n_cert, "accounts": A, "iters_p50": float(np.median(iters)), "iters_max": int(iters.max()),
+                   "certified_last_step": n_cert, "certified_all_timed_steps": certified, "accounts": A,
+                   "value_counts": "certified accounts only (status 0: scaled residuals <= 1e-6 and gates pass)",
+                   "iters_p50": float(np.median(iters)), "iters_max": int(iters.max()),
                    "iterations_per_sec": iters_total / (interval_ms * 1e-3) if interval_ms else None,
                    "max_scaled_residual": float(max(resid[:, 7].max(), resid[:, 8].max())),
-                   "max_gate_residual": float(resid[:, 0:4].max()), "device_bytes": P.device_bytes, "library": pr.version()},
+                   "max_gate_residual": float(resid[:, 0:4].max()), "device_bytes": P.device_bytes, "library": pr.version(),
+                   "create_plus_first_solve_ms": create_plus_solve_ms,
+                   "accounts_per_s_incl_create": A / (create_plus_solve_ms * 1e-3)},
         "clocks": clocks,
-        "e2e": {"value": total_accounts / (e2e_ms * 1e-3), "unit": "accounts/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                "ms_per_step": e2e_ms / args.steps},
-        "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu,
+        "e2e": {"value": e2e_cert * world / (e2e_ms * 1e-3), "unit": "accounts/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "ms_per_step": e2e_ms / args.steps,
+                "note": "prism_solve_batch_host: mu and w0 go host->device every step; bounds, masks, bands, tau, gamma and the "
+                        "universe stay resident from prism_problem_create"},
+        "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu, "extra": extra,
     }
     print(json.dumps(out))
     if dist is not None:

@@ -243,6 +243,10 @@ int prism_fp64_yardstick(prism_problem* p, void* cuda_stream, double* tflops_out
 /* Frees the workspace; never frees borrowed data.  NULL is allowed. */
 void prism_problem_destroy(prism_problem* p);
 
+/* The form of the projection kernel this object runs (PRISM_PROX_RESIDENT / _STREAMING / _EVERY_ASSET): what
+ * PRISM_PROX_AUTO resolved to. */
+int32_t prism_problem_prox_form(const prism_problem* p);
+
 /* Workspace bytes owned by the object (memory class). */
 int64_t prism_problem_device_bytes(const prism_problem* p);
 

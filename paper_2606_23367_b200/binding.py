@@ -22,7 +22,7 @@ STATUS_NAMES = ["certified", "feasible/non-certified", "timeout", "deadline exce
 SYMBOLS = ["prism_default_settings", "prism_problem_create", "prism_solve_batch", "prism_residuals",
            "prism_solve_batch_host", "prism_problem_destroy", "prism_problem_device_bytes", "prism_last_error",
            "prism_version", "prism_kernel_times", "prism_factor_exposures", "prism_noalloc_init",
-           "prism_factor_exposures_noalloc", "prism_fp64_yardstick"]
+           "prism_factor_exposures_noalloc", "prism_fp64_yardstick", "prism_problem_prox_form"]
 NOALLOC_SCRATCH_DOUBLES = 524288      # prism.h: PRISM_NOALLOC_SCRATCH_DOUBLES
 
 
@@ -89,6 +89,7 @@ def load_library(path: str = LIB_PATH):
     L.prism_kernel_times.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int64)]; L.prism_kernel_times.restype = C.c_int
     L.prism_factor_exposures.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]; L.prism_factor_exposures.restype = C.c_int
     L.prism_noalloc_init.argtypes = []; L.prism_noalloc_init.restype = C.c_int
+    L.prism_problem_prox_form.argtypes = [C.c_void_p]; L.prism_problem_prox_form.restype = C.c_int32
     L.prism_fp64_yardstick.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_double)]; L.prism_fp64_yardstick.restype = C.c_int
     L.prism_factor_exposures_noalloc.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_int64, C.c_int32, C.c_int32,
                                                  C.c_void_p, C.c_void_p]
@@ -190,6 +191,10 @@ class Problem:
             self.close()
         except Exception:
             pass
+
+    @property
+    def prox_form(self) -> int:
+        return int(lib().prism_problem_prox_form(self.handle))
 
     @property
     def device_bytes(self) -> int:

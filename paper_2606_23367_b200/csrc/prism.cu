@@ -29,6 +29,9 @@ int prism_internal_set_error(int code, const char* what, const char* detail) {
 }
 extern "C" const char* prism_version(void) { return PRISM_VERSION_STR; }
 extern "C" int64_t prism_problem_device_bytes(const prism_problem* p) { return p ? p->bytes : 0; }
+extern "C" int32_t prism_problem_prox_form(const prism_problem* p) {
+  return !p ? PRISM_PROX_AUTO : (p->res ? PRISM_PROX_RESIDENT : (p->fast ? PRISM_PROX_STREAMING : PRISM_PROX_EVERY_ASSET));
+}
 
 template <typename T>
 static int dev_alloc(prism_problem* p, T** ptr, size_t count, bool zero = true) {
