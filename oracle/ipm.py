@@ -321,7 +321,10 @@ def solve(acc: Account, mode: str = "auto", witness=None, tol: float = None, max
             best = (merit, v.copy(), y, s.copy(), z.copy(), it)
         elif it > best[5] + 12:
             break
-        th = z / s
+        # theta = z / s of the reduced KKT system.  At the end of the path s -> 0 on active rows: the quotient is capped so that
+        # the per-asset blocks stay finite (an active row then acts as an equality with weight 1e150, far beyond fp64
+        # resolution of the rest of the system) - without the cap the blocks held inf and the refinement produced NaNs.
+        th = np.minimum(z / np.maximum(s, 1e-300), 1e150)
 
         def newton(r_c):
             rhs1 = -r_d - qp.GT_mul((z * r_g - r_c) / s)
@@ -345,23 +348,39 @@ def solve(acc: Account, mode: str = "auto", witness=None, tol: float = None, max
                 return 1.0
             return min(1.0, float(np.min(-x[neg] / dx[neg])))
 
+        # A step that is not finite means the linear algebra has given out (end of the path, slacks at the floor): the
+        # iteration stops there, cleanly, and the best iterate so far is judged by the acceptance rule below.
+        def finite(*xs):
+            return all(np.all(np.isfinite(x)) for x in xs)
+
         try:
-            dv_a, dy_a, ds_a, dz_a = newton(s * z)
+            with np.errstate(over="ignore", invalid="ignore", divide="ignore"):
+                dv_a, dy_a, ds_a, dz_a = newton(s * z)
         except np.linalg.LinAlgError:
+            break
+        if not finite(dv_a, dy_a, ds_a, dz_a):
             break
         al = min(max_step(s, ds_a), max_step(z, dz_a))
         mu_aff = float((s + al * ds_a) @ (z + al * dz_a)) / m
         sigma = max((mu_aff / mu_c) ** 3, 0.03 if mu_c * m < 1e-6 else 0.0)   # do not outrun the linear algebra near the end
         try:
-            dv, dy, ds, dz = newton(s * z + ds_a * dz_a - sigma * mu_c)
+            with np.errstate(over="ignore", invalid="ignore", divide="ignore"):
+                dv, dy, ds, dz = newton(s * z + ds_a * dz_a - sigma * mu_c)
         except np.linalg.LinAlgError:
+            break
+        if not finite(dv, dy, ds, dz):
             break
         al = min(1.0, 0.995 * min(max_step(s, ds) if np.any(ds < 0) else 1e30, max_step(z, dz) if np.any(dz < 0) else 1e30))
         v = v + al * dv; y = y + al * dy; s = s + al * ds; z = z + al * dz
+        # slacks and multipliers stay strictly positive by the step rule; floored far below fp64 resolution of the data so that
+        # quotients by them cannot overflow when an active row's slack keeps shrinking after the residuals have stalled
+        s = np.maximum(s, 1e-150); z = np.maximum(z, 1e-150)
     if status != "optimal" and best is not None:
-        # never silent: only an iterate with merit <= max(100 tol, 1e-9) is accepted, else the status says failed
+        # never silent ("else oracle reports failure"): the best iterate is accepted only if its merit
+        # is <= 5e-10, five orders below the parity tolerance on the weights (DESIGN.md section 2 says why not 1e-10); anything
+        # else is a failure.  Tests additionally certify every accepted answer with the independent checker (kkt_check).
         merit, v, y, s, z, it_best = best
-        status = "optimal" if merit <= max(100 * tol, 1e-9) else f"failed(merit={merit:.1e})"
+        status = "optimal" if merit <= 5e-10 else f"failed(merit={merit:.1e})"
     w = qp.recover(v)
     # multipliers, paper convention g_i(w) <= 0 with lambda_i >= 0
     parts = qp._split(z)

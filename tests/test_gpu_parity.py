@@ -21,8 +21,18 @@ def _solve_gpu(inst, prox_form=0, **kw):
 
 
 def _oracle(inst, accounts=None):
-    from oracle import ipm
-    return ipm.solve_instance(inst, accounts=accounts)
+    """Oracle weights of the listed accounts, each certified by the independent checker before it is used as the expected
+    value: feasibility <= 1e-9, stationarity and complementarity <= 1e-7 with the IPM's multipliers (activity delta 1e-7:
+    an interior-point answer sits within ~1e-8 of the kinks and bounds it is converging to)."""
+    from oracle import ipm, kkt_check, problem
+    W, res = ipm.solve_instance(inst, accounts=accounts)
+    ids = list(range(inst.A)) if accounts is None else list(accounts)
+    for j, a in enumerate(ids):
+        acc = problem.account_from_instance(inst, a)
+        assert max(kkt_check.feasibility(acc, W[j]).values()) <= 1e-9
+        k = kkt_check.kkt(acc, W[j], res[j]["mult"], delta=1e-7)
+        assert k["r_stat"] <= 1e-7 * max(1.0, 20 * np.max(np.abs(acc.mu))) and k["r_comp"] <= 1e-7 and k["min_multiplier"] >= -1e-12, (a, k)
+    return W, res
 
 
 def _check_against_oracle(inst, r, W, res, accounts=None):
