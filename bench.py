@@ -186,6 +186,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extra", action="store_true", help="skip the rows for the other configs and the N sweep")
     ap.add_argument("--gemm-precision", type=int, default=0)
+    ap.add_argument("--prox-form", type=int, default=0, help="PRISM_PROX_* (0 = AUTO) for the headline problem object")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -212,7 +213,7 @@ def main():
     inst = make_instance(args.config, seed=rank, accounts=args.accounts)
     torch.cuda.synchronize()
     t_c0 = time.perf_counter()
-    P = pr.Problem(inst, device=dev)
+    P = pr.Problem(inst, device=dev, prox_form=args.prox_form)
     settings = binding.default_settings(gemm_precision=args.gemm_precision)
     first = P.solve(settings)
     torch.cuda.synchronize()
