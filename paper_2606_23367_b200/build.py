@@ -16,6 +16,7 @@ OBJ = os.path.join(HERE, "_obj")
 LIB = os.path.join(HERE, "libprism.so")
 HEADER = os.path.join(os.path.dirname(HERE), "include", "prism.h")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC,-pthread"]
+FLAGS += os.environ.get("PRISM_NVCC_FLAGS", "").split()       # builder's switch, e.g. -DPRISM_STATS (pass counts of the root find)
 
 
 def sources():

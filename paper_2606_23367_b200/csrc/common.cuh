@@ -67,6 +67,7 @@ struct prism_problem {
   int32_t *lcnt, *lflag;
   unsigned long long* cbin;
   double* chkp;
+  int32_t* act;           // H6 compaction: the accounts not done, ascending (rebuilt after a check that finished accounts)
   int32_t* counters;      // [0] number of done accounts
   int32_t* h_counters;    // pinned host mirror
   int64_t bytes;

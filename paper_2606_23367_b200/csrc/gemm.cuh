@@ -31,12 +31,8 @@ __global__ void __launch_bounds__(256) k_gemm1(Gemm1Args p) {
   double* As = smem;                                   // [STAGES][KP][G1_LD]
   double* Bs = smem + (size_t)G1_STAGES * KP * G1_LD;  // [STAGES][TA][G1_LD]
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int a0 = blockIdx.y * G1_TA;
-  if (p.done) {                                        // convergence mask: skip tiles whose accounts all finished
-    int alive = 0;
-    for (int n = 0; n < G1_TA && a0 + n < p.A; ++n) alive |= !p.done[a0 + n];
-    if (!alive) return;
-  }
+  const int a0 = blockIdx.y * G1_TA;                   // first slot of the tile (H6: slots of the active-account list)
+  if (a0 >= p.nact) return;
   const int64_t i_begin = (int64_t)blockIdx.x * p.chunk;
   const int64_t i_end = min(i_begin + p.chunk, p.Npad);
   const int nst = (int)((i_end - i_begin) / G1_KS);
@@ -50,7 +46,8 @@ __global__ void __launch_bounds__(256) k_gemm1(Gemm1Args p) {
     }
     for (int c = tid; c < G1_TA * (G1_KS / 2); c += 256) {
       const int r = c / (G1_KS / 2), cc = (c % (G1_KS / 2)) * 2;
-      const int a = min(a0 + r, p.A - 1);
+      const int slot = min(a0 + r, p.nact - 1);
+      const int a = p.act ? p.act[slot] : slot;
       cp_async16(bs + r * G1_LD + cc, p.X + (int64_t)a * p.ldw + i0 + cc);
     }
   };
@@ -84,8 +81,11 @@ __global__ void __launch_bounds__(256) k_gemm1(Gemm1Args p) {
   for (int m = 0; m < MT; ++m) {
 #pragma unroll
     for (int h = 0; h < 2; ++h) {
-      const int a = a0 + warp * 8 + fc * 2 + h;
-      if (a < p.A) p.Tpart[((int64_t)blockIdx.x * p.A + a) * p.ldv + m * 8 + fr] = acc[m][h];
+      const int slot = a0 + warp * 8 + fc * 2 + h;
+      if (slot < p.nact) {
+        const int a = p.act ? p.act[slot] : slot;
+        p.Tpart[((int64_t)blockIdx.x * p.A + a) * p.ldv + m * 8 + fr] = acc[m][h];
+      }
     }
   }
 }
@@ -93,8 +93,9 @@ __global__ void __launch_bounds__(256) k_gemm1(Gemm1Args p) {
 // reference: one thread per (a, j), plain FMA, same chunking
 __global__ void k_gemm1_ref(Gemm1Args p, int kp) {
   const int64_t t = (int64_t)blockIdx.y * blockDim.x + threadIdx.x;
-  if (t >= (int64_t)p.A * kp) return;
-  const int a = (int)(t / kp), j = (int)(t % kp);
+  if (t >= (int64_t)p.nact * kp) return;
+  const int slot = (int)(t / kp), j = (int)(t % kp);
+  const int a = p.act ? p.act[slot] : slot;
   const int64_t i_begin = (int64_t)blockIdx.x * p.chunk, i_end = min(i_begin + p.chunk, p.Npad);
   double s = 0.0;
   for (int64_t i = i_begin; i < i_end; ++i) s = fma(p.Bt[(int64_t)j * p.ldn + i], p.X[(int64_t)a * p.ldw + i], s);
@@ -134,16 +135,13 @@ __global__ void __launch_bounds__(256, 3) k_gemm2(Gemm2Args p) {
   double* Vs = smem;                       // [TM][LD]
   double* Bs = smem + (size_t)G2_TM * LD;  // [TN][LD]
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int a0 = blockIdx.y * G2_TM;
+  const int a0 = blockIdx.y * G2_TM;                    // first slot of the tile (H6: slots of the active-account list)
   const int64_t i0 = (int64_t)blockIdx.x * G2_TN;
-  if (p.done) {
-    int alive = 0;
-    for (int n = 0; n < G2_TM && a0 + n < p.A; ++n) alive |= !p.done[a0 + n];
-    if (!alive) return;
-  }
+  if (a0 >= p.nact) return;
   for (int c = tid; c < G2_TM * (KP / 2); c += 256) {
     const int r = c / (KP / 2), cc = (c % (KP / 2)) * 2;
-    const int a = min(a0 + r, p.A - 1);
+    const int slot = min(a0 + r, p.nact - 1);
+    const int a = p.act ? p.act[slot] : slot;
     cp_async16(Vs + r * LD + cc, p.V + (int64_t)a * p.ldv + cc);
   }
   for (int c = tid; c < G2_TN * (KP / 2); c += 256) {
@@ -153,8 +151,9 @@ __global__ void __launch_bounds__(256, 3) k_gemm2(Gemm2Args p) {
   }
   cp_async_commit();
   const int fr = lane >> 2, fc = lane & 3;
-  const int a = a0 + warp * 8 + fr;
-  const bool arow = a < p.A && !(p.done && p.done[a]);
+  const int slot = a0 + warp * 8 + fr;
+  const bool arow = slot < p.nact;
+  const int a = arow ? (p.act ? p.act[slot] : slot) : 0;
   const bool fastep = MODE != G2_SIGMA && !p.G;          // pair-wise epilogue (the rows are padded to 32: always in range)
   double gsc = 0.0, gam = 0.0;
   if (arow && MODE != G2_SIGMA) { gam = p.gamma[a]; gsc = 1.0 / (gam * (1.0 + p.c[a])); }
@@ -230,8 +229,8 @@ __global__ void __launch_bounds__(256, 3) k_gemm2(Gemm2Args p) {
 template <int MODE>
 __global__ void k_gemm2_ref(Gemm2Args p) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  const int a = blockIdx.y;
-  if (i >= p.N || (p.done && p.done[a])) return;
+  if (i >= p.N || (int)blockIdx.y >= p.nact) return;
+  const int a = p.act ? p.act[blockIdx.y] : (int)blockIdx.y;
   double bv = 0.0;
   for (int j = 0; j < p.kp; ++j) bv = fma(p.Bp[i * p.kp + j], p.V[(int64_t)a * p.ldv + j], bv);
   g2_epilogue<MODE>(p, a, i, bv);

@@ -12,7 +12,8 @@ struct Gemm1Args {
   const double* X; int64_t ldw;
   double* Tpart; int64_t ldv;
   int32_t A; int64_t chunk; int64_t Npad;
-  const int32_t* done;
+  // H6 compaction: tile rows are SLOTS of the active-account list; act[slot] = account (NULL: identity, nact = A)
+  const int32_t* act; int32_t nact;
 };
 
 
@@ -31,6 +32,6 @@ struct Gemm2Args {
   const double *q, *mu;       // q (ldw) or mu (ld N)
   const double* X;            // SIGMA: the vector Sigma is applied to (ldw)
   double relax;
-  const int32_t* done;
+  const int32_t* act; int32_t nact;   // as in Gemm1Args
 };
 

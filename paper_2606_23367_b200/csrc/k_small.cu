@@ -33,7 +33,32 @@ cudaError_t factor_launch(const double* gram, const double* f, const double* gam
   return cudaGetLastError();
 }
 cudaError_t solve_launch(const SolveArgs& a, cudaStream_t st) {
-  k_solve<<<a.A, 256, 0, st>>>(a);
+  k_solve<<<a.nact, 256, 0, st>>>(a);
+  return cudaGetLastError();
+}
+// H6 compaction: act[0 .. n) = the accounts that are not done, ascending (one CTA, ballot scan: a fixed order).
+__global__ void __launch_bounds__(1024) k_compact(int A, const int32_t* done, int32_t* act) {
+  __shared__ int wsum[32];
+  __shared__ int base_s;
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  if (tid == 0) base_s = 0;
+  __syncthreads();
+  for (int a0 = 0; a0 < A; a0 += 1024) {
+    const int a = a0 + tid;
+    const bool live = a < A && !done[a];
+    const unsigned m = __ballot_sync(0xffffffffu, live);
+    if (lane == 0) wsum[wid] = __popc(m);
+    __syncthreads();
+    int off = base_s;
+    for (int w = 0; w < wid; ++w) off += wsum[w];
+    if (live) act[off + __popc(m & ((1u << lane) - 1u))] = a;
+    __syncthreads();
+    if (tid == 0) { int t = 0; for (int w = 0; w < 32; ++w) t += wsum[w]; base_s += t; }
+    __syncthreads();
+  }
+}
+cudaError_t compact_launch(int A, const int32_t* done, int32_t* act, cudaStream_t st) {
+  k_compact<<<1, 1024, 0, st>>>(A, done, act);
   return cudaGetLastError();
 }
 cudaError_t scale_fs_launch(const double* Tpart, int nchunk, int A, int k, int kp, int64_t ldv, const double* f,

@@ -25,6 +25,7 @@ cudaError_t warm_start_launch(const WarmArgs& a, cudaStream_t st);
 cudaError_t factor_launch(const double* gram, const double* f, const double* gamma, const AccountParams& ap, int A, int k,
                           int kp, double* Sinv, cudaStream_t st);
 cudaError_t solve_launch(const SolveArgs& a, cudaStream_t st);
+cudaError_t compact_launch(int A, const int32_t* done, int32_t* act, cudaStream_t st);   // H6: list of the accounts not done
 cudaError_t scale_fs_launch(const double* Tpart, int nchunk, int A, int k, int kp, int64_t ldv, const double* f,
                             const double* gamma, double* V, cudaStream_t st);
 cudaError_t diff_launch(const double* w, const double* wb, int64_t N, int64_t ldw, int A, double* X, cudaStream_t st);

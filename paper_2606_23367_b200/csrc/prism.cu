@@ -50,7 +50,7 @@ extern "C" void prism_problem_destroy(prism_problem* p) {
   void* ptrs[] = {p->Bp, p->Bt, p->invd, p->gram, p->q, p->v, p->rt, p->cc, p->xs, p->pxq, p->Tpart, p->V, p->Sinv,
                   p->gw0, p->lamG, p->resid, p->duals, p->status, p->ap.c, p->ap.alpha, p->ap.beta,
                   p->ap.mode, p->ap.bsum, p->ap.done, p->ap.conv, p->ap.iters, p->ap.refactor,
-                  p->ap.nadapt, p->ap.win, p->ap.wins, p->ap.slack, p->counters, p->w_stage, p->i_stage, p->lraw, p->lcomp, p->lcnt, p->cbin, p->chkp, p->lflag};
+                  p->ap.nadapt, p->ap.win, p->ap.wins, p->ap.slack, p->counters, p->act, p->w_stage, p->i_stage, p->lraw, p->lcomp, p->lcnt, p->cbin, p->chkp, p->lflag};
   for (void* q : ptrs) if (q) cudaFree(q);
   if (p->h_counters) cudaFreeHost(p->h_counters);
   delete p;
@@ -90,10 +90,11 @@ struct Launcher {
     }
     evs.clear();
   }
-  void gemm1(const double* X, const int32_t* done) {
+  // act / nact: the compacted list of active accounts (H6); NULL / A = every account
+  void gemm1(const double* X, const int32_t* act, int nact) {
     Gemm1Args a;
     a.Bt = p->Bt; a.ldn = p->ldn; a.X = X; a.ldw = p->ldn; a.Tpart = p->Tpart; a.ldv = p->ldv; a.A = p->A;
-    a.chunk = p->chunk; a.Npad = p->ldn; a.done = done;
+    a.chunk = p->chunk; a.Npad = p->ldn; a.act = act; a.nact = nact;
     begin(PRISM_K_GEMM1);
     end(gemm1_launch(gemm_mode, mt, p->nchunk, p->kp, a, st));
   }
@@ -107,12 +108,12 @@ struct Launcher {
     a.Bp = p->Bp; a.kp = p->kp; a.V = p->V; a.ldv = p->ldv; a.N = p->N; a.ldw = p->ldn; a.A = p->A; a.G = 0;     // no consensus rows in the x-update: U = Bp
     a.group_id = nullptr; a.invd = p->invd; a.d = p->d.d; a.gamma = p->d.gamma; a.c = p->ap.c;
     a.v = p->v; a.cc = p->cc; a.rt = p->rt; a.xs = p->xs; a.pxq = p->pxq; a.q = p->q; a.mu = p->d.mu;
-    a.relax = 1.0; a.done = nullptr;
+    a.relax = 1.0; a.act = nullptr; a.nact = p->A;
     return a;
   }
   // pxq <- gamma Sigma X   (H8: Sigma W = B (F (B'W)) + D o W, fp64)
   void sigma_apply(const double* X) {
-    gemm1(X, nullptr);
+    gemm1(X, nullptr, p->A);
     begin(PRISM_K_OTHER);
     end(scale_fs_launch(p->Tpart, p->nchunk, p->A, p->k, p->kp, p->ldv, p->d.f, p->d.gamma, p->V, st));
     Gemm2Args a = g2base();
@@ -235,6 +236,7 @@ extern "C" int prism_problem_create(int64_t N, int32_t k, int32_t accounts, cons
   ALLOC_TRY(dev_alloc(p, &p->ap.wins, (size_t)A));
   ALLOC_TRY(dev_alloc(p, &p->ap.slack, (size_t)A));
   ALLOC_TRY(dev_alloc(p, &p->counters, (size_t)4));
+  ALLOC_TRY(dev_alloc(p, &p->act, (size_t)A));
   ALLOC_TRY(dev_alloc(p, &p->w_stage, (size_t)A * N));      // staging of the host-buffer lane (prism_solve_batch_host)
   ALLOC_TRY(dev_alloc(p, &p->i_stage, (size_t)A));
   cudaError_t ke = cudaSuccess;
@@ -389,9 +391,13 @@ extern "C" int prism_solve_batch(prism_problem* p, const prism_settings* sp, voi
   SolveArgs sa;
   memset(&sa, 0, sizeof(sa));
   sa.A = A; sa.kp = p->kp; sa.nchunk = p->nchunk; sa.ldv = p->ldv; sa.Tpart = p->Tpart; sa.Sinv = p->Sinv;
-  sa.V = p->V; sa.ap = p->ap;
+  sa.V = p->V; sa.ap = p->ap; sa.act = nullptr; sa.nact = A;
   Gemm2Args g2 = L.g2base();
-  g2.relax = s.alpha; g2.done = p->ap.done;
+  g2.relax = s.alpha;
+  // H6: the GEMMs and the small solve run over the compacted list of accounts still active (identity until the first
+  // account finishes); the list is rebuilt after every check that finished accounts
+  const int32_t* act = nullptr;
+  int nact = A;
 
   int it = 1, timed_out = 0, late_iter = -1, ndone = 0;
   for (; it <= s.max_iter; ++it) {
@@ -408,11 +414,18 @@ extern "C" int prism_solve_batch(prism_problem* p, const prism_settings* sp, voi
       const double el = elapsed_ms();
       // accounts that converge at this very check are late if the deadline has already passed
       if (s.deadline_ms > 0 && late_iter < 0 && el > s.deadline_ms) late_iter = it - 2;
+      const int ndone_prev = ndone;
       ndone = p->h_counters[0];
       if (ndone >= A) break;
+      if (ndone != ndone_prev) {
+        L.begin(PRISM_K_OTHER);
+        L.end(compact_launch(A, p->ap.done, p->act, st));
+        act = p->act; nact = A - ndone;
+        sa.act = act; sa.nact = nact; g2.act = act; g2.nact = nact;
+      }
       if (s.time_limit_ms > 0 && el > s.time_limit_ms) { timed_out = 1; break; }
     }
-    L.gemm1(p->rt, p->ap.done);
+    L.gemm1(p->rt, act, nact);
     L.begin(PRISM_K_SOLVE);
     L.end(solve_launch(sa, st));
     const bool next_check = (it % s.check_every == 0) && (it >= s.first_check);
@@ -478,7 +491,7 @@ extern "C" int prism_factor_exposures(prism_problem* p, const double* w, void* c
   cudaStream_t st = (cudaStream_t)cuda_stream;
   Launcher L{p, st, p->kp / 8, 0};
   L.end(diff_launch(w, nullptr, p->N, p->ldn, p->A, p->rt, st));
-  L.gemm1(p->rt, nullptr);
+  L.gemm1(p->rt, nullptr, p->A);
   L.end(reduce_partials_launch(p->Tpart, p->nchunk, p->A, p->k, p->ldv, T_out, st));
   CUDA_TRY(cudaStreamSynchronize(st));
   if (L.err != cudaSuccess) return set_err(PRISM_ERR_CUDA, "kernel launch failed: %s", cudaGetErrorString(L.err));

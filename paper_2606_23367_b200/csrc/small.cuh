@@ -137,7 +137,7 @@ __global__ void k_factor(const double* gram, const double* f, const double* gamm
 __global__ void __launch_bounds__(256) k_solve(SolveArgs p) {
   __shared__ double T[PRISM_MAX_KPRIME];
   __shared__ double Tq[4][PRISM_MAX_KPRIME];
-  const int a = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int a = p.act ? p.act[blockIdx.x] : (int)blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   if (p.ap.done[a]) return;
   const int Kp = p.kp;
   {

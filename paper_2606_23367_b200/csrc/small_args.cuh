@@ -16,6 +16,7 @@ struct SolveArgs {
   const double *Tpart, *Sinv;
   double *V;
   AccountParams ap;
+  const int32_t* act; int32_t nact;   // H6: grid = nact, block s solves account act[s] (NULL: identity)
 };
 
 // warm start (prism_settings.warm_w / warm_duals): carried state from previous weights and multipliers
