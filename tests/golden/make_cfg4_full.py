@@ -1,0 +1,45 @@
+"""Writes tests/golden/cfg4_full_a{a}.npz: oracle weights of accounts of configs[4] at FULL width (32 x 384,800, seed 0).
+
+Calls only instances/ (seeded generator) and oracle/ (structured interior point, as it stands): no value comes from the
+CUDA path.  The oracle needs many minutes per account at this width, which is why the values are stored instead of
+being recomputed inside the GPU test (tests/test_gpu_parity.py::test_full_size_cfg4_elementwise).
+Stored per account: the full weight vector as float64 (zlib-compressed npz), the oracle's objective, its KKT
+certificate (kkt_check with the oracle's multipliers) and the SHA-256 of the account's mu / w0 rows (generator drift).
+
+    python tests/golden/make_cfg4_full.py [account ...]        (default: 0 17)
+"""
+import hashlib
+import os
+import sys
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
+sys.path.insert(0, ROOT)
+from instances import gen            # noqa: E402
+from oracle import ipm, kkt_check, problem   # noqa: E402
+
+
+def main():
+    accounts = [int(x) for x in sys.argv[1:]] or [0, 17]
+    inst = gen.by_name("cfg4", seed=0)
+    for a in accounts:
+        acc = problem.account_from_instance(inst, a)
+        t0 = time.perf_counter()
+        r = ipm.solve(acc, witness=inst.witness[a])
+        dt = time.perf_counter() - t0
+        assert r["status"] == "optimal", r["status"]
+        w = r["w"]
+        feas = kkt_check.feasibility(acc, w)
+        out = os.path.join(os.path.dirname(os.path.abspath(__file__)), f"cfg4_full_a{a}.npz")
+        np.savez_compressed(out, w=w, objective=problem.objective(acc, w), iterations=r["iters"],
+                            seconds=dt, feas=np.array([feas[k] for k in sorted(feas)]),
+                            sha_mu=hashlib.sha256(np.ascontiguousarray(inst.mu[a]).tobytes()).hexdigest(),
+                            sha_w0=hashlib.sha256(np.ascontiguousarray(inst.w0[a]).tobytes()).hexdigest())
+        print(f"account {a}: {dt:.0f} s, objective {problem.objective(acc, w):.12e}, max feasibility residual "
+              f"{max(feas.values()):.2e} -> {out}", flush=True)
+
+
+if __name__ == "__main__":
+    main()

@@ -112,25 +112,51 @@ def test_product_path_does_not_touch_the_oracle_or_any_cpu_fallback():
             binding._lib = None
 
 
-def test_sharding_plan_world_size_2_gloo(tmp_path):
-    """Multi-GPU path: accounts shard with no data-path collective; the only communication is
-    the barrier and the max-reduction of the timing, exercised here with gloo on CPU, world size 2."""
+def test_shard_plan_covers_every_account_once():
+    """paper_2606_23367_b200.shard.account_range: contiguous, balanced, disjoint, complete."""
+    from paper_2606_23367_b200 import shard
+    for A in (0, 1, 2, 5, 32, 100, 500, 501):
+        for world in (1, 2, 3, 4, 8):
+            blocks = shard.plan(A, world)
+            assert blocks[0][0] == 0 and blocks[-1][1] == A
+            assert all(blocks[r][1] == blocks[r + 1][0] for r in range(world - 1))
+            sizes = [b - a for a, b in blocks]
+            assert max(sizes) - min(sizes) <= 1 and sum(sizes) == A
+    with pytest.raises(ValueError):
+        shard.account_range(4, 2, 2)
+    from instances import gen
+    inst = gen.config2(N=64, k=4, A=5, G=3)
+    sub = shard.slice_instance(inst, 1, 4)
+    assert sub.A == 3 and sub.mu.shape == (3, 64) and sub.B is inst.B and sub.band_lo.shape == (3, 3)
+    assert (sub.w0 == inst.w0[1:4]).all() and (sub.tau == inst.tau[1:4]).all()
+
+
+def test_sharded_solve_world_size_2_gloo(tmp_path):
+    """Multi-GPU path through the PRODUCT code paper_2606_23367_b200.shard on gloo, world size 2:
+    every rank takes its block of one batch, a stand-in block solver returns per-account rows computed from the
+    block's own data, and the gathered result must equal the same rows computed on the whole batch, in account order.
+    The only communication is the gather (and the barrier / max-reduction bench.py uses for its timings)."""
     import subprocess, sys, textwrap
     code = textwrap.dedent("""
-        import os, sys, torch, torch.distributed as dist
+        import os, sys, numpy as np, torch, torch.distributed as dist
         sys.path.insert(0, %r)
         from instances import gen
+        from paper_2606_23367_b200 import shard
         dist.init_process_group('gloo')
         r, w = dist.get_rank(), dist.get_world_size()
-        inst = gen.config1(seed=r, N=64, k=4, A=3)          # every rank draws its own batch (weak scaling)
-        t = torch.tensor([float(10 + r)], dtype=torch.float64)
+        inst = gen.config1(seed=0, N=64, k=4, A=5)             # one batch, the same on every rank (strong scaling)
+        def rows(sub):                                         # stand-in for Problem(sub).solve(): one row per account
+            return {'sig': torch.tensor(np.stack([sub.mu.sum(1), sub.w0.max(1), sub.tau], 1)),
+                    'n': torch.tensor(np.full((sub.A, 1), sub.A, dtype=np.int64))}
+        out = shard.solve_sharded(inst, rows)
+        want = rows(inst)['sig']
+        assert out['sig'].shape == (5, 3) and torch.equal(out['sig'], want), (out['sig'], want)
+        a, b = shard.account_range(inst.A, w, r)
+        assert (out['n'][a:b] == b - a).all() and int(out['n'].sum()) == 3 * 3 + 2 * 2
+        t = torch.tensor([float(10 + r)], dtype=torch.float64)  # bench.py: barrier + max over ranks of the timing
         dist.barrier()
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        s = torch.tensor([float(inst.mu.sum())], dtype=torch.float64)
-        g = [torch.zeros(1, dtype=torch.float64) for _ in range(w)]
-        dist.all_gather(g, s)
         assert t.item() == 10 + w - 1
-        assert g[0].item() != g[1].item()                    # different seeds -> different batches
         dist.destroy_process_group()
         print('rank' + str(r) + 'done', flush=True)
     """ % ROOT)
