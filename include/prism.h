@@ -196,6 +196,18 @@ int prism_solve_batch(prism_problem* p, const prism_settings* s, void* cuda_stre
 int prism_residuals(prism_problem* p, const double* w, const double* duals, void* cuda_stream,
                     double* resid_out);
 
+/* ONE application of the fused projection (H4) to caller-given points, outside any iteration - the prox of every
+ * nonsmooth / polyhedral term of Eq. (1) in the metric the splitting uses:
+ *   z_a = argmin_z  sum_i rho_ai / 2 (z_i - v_ai)^2 + kappa_a |z_i - w0_ai| + c_buy,a (z_i - w0_ai)_+ + psi_ai((w0_ai - z_i)_+)
+ *         s.t.  1'z = 1,  lo <= z <= hi (exclusions z_i = 0),  band_lo <= E z <= band_hi,  ||z - w0||_1 <= tau_a
+ *   rho_ai = rho_scale * gamma_a * d_i.
+ * Solved exactly (the piecewise-linear equations for the multipliers to 2e-15) by the same kernel the iteration
+ * launches, from a cold start.  v: device A x N; z_out: device A x N; duals_out: device A x PRISM_NDUAL(G) multipliers
+ * of the projection (layout above), or NULL.  Overwrites the solver's iterate (the next prism_solve_batch starts
+ * cold anyway).  Synchronises the stream. */
+int prism_project(prism_problem* p, const double* v, double rho_scale, void* cuda_stream, double* z_out,
+                  double* duals_out);
+
 /* Same solve as prism_solve_batch but with HOST buffers for the per-account data that changes between
  * rebalances (mu, w0) and for the outputs: copies mu and w0 host->device into the problem's borrowed arrays,
  * solves, copies weights / status / iterations / residual block back.  NULL host pointers skip that copy.

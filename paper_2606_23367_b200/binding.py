@@ -22,7 +22,7 @@ STATUS_NAMES = ["certified", "feasible/non-certified", "timeout", "deadline exce
 SYMBOLS = ["prism_default_settings", "prism_problem_create", "prism_solve_batch", "prism_residuals",
            "prism_solve_batch_host", "prism_problem_destroy", "prism_problem_device_bytes", "prism_last_error",
            "prism_version", "prism_kernel_times", "prism_factor_exposures", "prism_noalloc_init",
-           "prism_factor_exposures_noalloc", "prism_fp64_yardstick", "prism_problem_prox_form"]
+           "prism_factor_exposures_noalloc", "prism_fp64_yardstick", "prism_problem_prox_form", "prism_project"]
 NOALLOC_SCRATCH_DOUBLES = 524288      # prism.h: PRISM_NOALLOC_SCRATCH_DOUBLES
 
 
@@ -88,6 +88,7 @@ def load_library(path: str = LIB_PATH):
     L.prism_version.argtypes = []; L.prism_version.restype = C.c_char_p
     L.prism_kernel_times.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int64)]; L.prism_kernel_times.restype = C.c_int
     L.prism_factor_exposures.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]; L.prism_factor_exposures.restype = C.c_int
+    L.prism_project.argtypes = [C.c_void_p, C.c_void_p, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p]; L.prism_project.restype = C.c_int
     L.prism_noalloc_init.argtypes = []; L.prism_noalloc_init.restype = C.c_int
     L.prism_problem_prox_form.argtypes = [C.c_void_p]; L.prism_problem_prox_form.restype = C.c_int32
     L.prism_fp64_yardstick.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_double)]; L.prism_fp64_yardstick.restype = C.c_int
@@ -248,6 +249,18 @@ class Problem:
             stream = torch.cuda.current_stream().cuda_stream
             _check(lib().prism_factor_exposures(self.handle, w.data_ptr(), C.c_void_p(stream), out.data_ptr()))
         return out
+
+    def project(self, v, rho_scale: float = 100.0):
+        """prism_project: one exact application of the fused projection to the points v (A, N); returns (z, duals)."""
+        torch = self.torch
+        v = torch.as_tensor(v, dtype=torch.float64).contiguous().to(self.dev)
+        z = torch.empty((self.A, self.N), dtype=torch.float64, device=self.dev)
+        duals = torch.empty((self.A, 2 + 2 * self.G), dtype=torch.float64, device=self.dev)
+        with torch.cuda.device(self.dev):
+            stream = torch.cuda.current_stream().cuda_stream
+            _check(lib().prism_project(self.handle, v.data_ptr(), C.c_double(rho_scale), C.c_void_p(stream), z.data_ptr(),
+                                       duals.data_ptr()))
+        return z, duals
 
     def residuals(self, w, duals=None):
         torch = self.torch

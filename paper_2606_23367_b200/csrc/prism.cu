@@ -483,6 +483,34 @@ extern "C" int prism_solve_batch(prism_problem* p, const prism_settings* sp, voi
   return PRISM_OK;
 }
 
+// One exact application of the projection kernel to caller-given points (prism.h): cold account state with
+// rho = rho_scale gamma d, v copied into the padded iterate, one PROX_FINAL launch (exact thresholds, z -> z_out).
+extern "C" int prism_project(prism_problem* p, const double* v, double rho_scale, void* cuda_stream, double* z_out,
+                             double* duals_out) {
+  if (!p) return set_err(PRISM_ERR_NOT_READY, "problem object is NULL%s", "");
+  if (!v || !z_out || !(rho_scale > 0)) return set_err(PRISM_ERR_INVALID_ARG, "v, z_out and rho_scale > 0 are mandatory%s", "");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const int A = p->A, G = p->G;
+  Launcher L{p, st, p->kp / 8, 0};
+  CUDA_TRY(cudaMemsetAsync(p->counters, 0, 4 * sizeof(int32_t), st));
+  InitArgs ia;
+  memset(&ia, 0, sizeof(ia));
+  ia.N = p->N; ia.ldw = p->ldn; ia.A = A; ia.G = G; ia.w0 = p->d.w0; ia.gamma = p->d.gamma;
+  ia.group_id = p->d.group_id; ia.v = p->v; ia.gw0 = p->gw0; ia.lamG = p->lamG; ia.ap = p->ap; ia.rho_scale = rho_scale;
+  L.end(init_accounts_launch(ia, st));
+  L.end(diff_launch(v, nullptr, p->N, p->ldn, A, p->v, st));
+  prism_settings s;
+  prism_default_settings(&s);
+  ProxArgs pa = make_prox_args(p, s, z_out);
+  pa.band_start = -1;                       // no band ramp: the full projection
+  launch_prox(L, pa, PROX_FINAL, 0);
+  if (duals_out) CUDA_TRY(cudaMemcpyAsync(duals_out, p->duals, (size_t)A * PRISM_NDUAL(G) * sizeof(double), cudaMemcpyDeviceToDevice, st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  CUDA_TRY(cudaGetLastError());
+  if (L.err != cudaSuccess) return set_err(PRISM_ERR_CUDA, "kernel launch failed: %s", cudaGetErrorString(L.err));
+  return PRISM_OK;
+}
+
 // T_out[a][j] = sum_i B[i][j] w[a][i]: the problem's own GEMM-1 (H1) on caller-given vectors, split-K partials in the
 // workspace allocated at create, reduced in chunk order.  Uses rt as the padded copy of w.
 extern "C" int prism_factor_exposures(prism_problem* p, const double* w, void* cuda_stream, double* T_out) {

@@ -563,7 +563,9 @@ struct RootState {
   int amode;             // 0: turnover cap inactive (alpha == beta), 1: active
   int n_eval;            // trial evaluations (passes over the source) spent
   int nobands;           // in: 1 = solve with every band multiplier fixed at 0 (band ramp of the first iterations)
-  int capped;            // out: 1 = the evaluation budget ran out (PROX_EVAL_CAP): the thresholds are the last iterate, NOT a
+  int max_rounds;        // in: Gauss-Seidel rounds over the bands the nested solve may take before it reports capped = 2
+  int capped;            // out: 2 = the Gauss-Seidel rounds ran out before every band held (the caller polishes with the joint
+                         // Newton iteration and calls again); 1 = the evaluation budget ran out (PROX_EVAL_CAP): the thresholds are the last iterate, NOT a
                          // solution.  The caller may use them for a plain iteration (an inexact prox) but must not
                          // certify convergence with them.
 };
@@ -735,9 +737,10 @@ __device__ __noinline__ void prox_rootfind(const ProxArgs& p, const Src& src, in
     }
   }
 
-  for (int round = 0; round < 2 * G + 2 && n_eval <= PROX_EVAL_CAP; ++round) {
+  bool gs_done = false;      // every band holds (or there are none)
+  for (int round = 0; round < rs.max_rounds && n_eval <= PROX_EVAL_CAP; ++round) {
     solve_ab(-1);
-    if (G == 0) break;
+    if (G == 0) { gs_done = true; break; }
     // all group sums at the current solution (deterministic binned pass)
     prox_group_sums<LOTS>(src, lamS, G, alpha, beta - Delta, sh.gw0, sh.gbin, sh.gsum);
     if (tid == 0) {
@@ -755,7 +758,7 @@ __device__ __noinline__ void prox_rootfind(const ProxArgs& p, const Src& src, in
     }
     __syncthreads();
     const int sel = sh.selS[0], sgn = sh.selS[1];
-    if (sel < 0) break;
+    if (sel < 0) { gs_done = true; break; }
     // scalar problem in m = sgn * lambda_sel >= 0:  h(m) = sgn * (S_sel - bound) is non-increasing, want h = 0 or m = 0
     if (!have_br) brackets();
     const double Lmax = 2.0 * (fmax(a_max, b_max) - fmin(a_min, b_min)) + 1.0;
@@ -786,6 +789,7 @@ __device__ __noinline__ void prox_rootfind(const ProxArgs& p, const Src& src, in
   __syncthreads();
   rs.alpha = alpha; rs.beta = beta; rs.amode = amode; rs.n_eval += n_eval;
   if (n_eval > PROX_EVAL_CAP) rs.capped = 1;
+  else if (!gs_done) rs.capped = 2;
 }
 
 __device__ __forceinline__ double next_window(const ProxArgs& p, double alpha, double beta, double mv) {
@@ -812,6 +816,7 @@ __device__ __forceinline__ void prox_body(const ProxArgs& p, int mode, Src& src,
 
   RootState rs;
   rs.alpha = p.ap.alpha[a]; rs.beta = p.ap.beta[a]; rs.amode = p.ap.mode[a]; rs.n_eval = 0; rs.nobands = 0; rs.capped = 0;
+  rs.max_rounds = 1 << 30;       // this form has no joint Newton iteration to polish with: rounds until every band holds
   if (!(rs.amode == 1 && isfinite(tau))) { rs.amode = 0; rs.beta = rs.alpha; }
   const double alpha_w = rs.alpha, beta_w = rs.beta;       // warm start (previous iteration's thresholds)
   const int amode_w = rs.amode;

@@ -353,3 +353,60 @@ def test_eps_abs_loosens_the_stopping_rule():
     assert (r2.status.cpu().numpy() == 0).all() and int(r2.iters.sum()) < int(r.iters.sum())
     assert float((r2.w - r.w).abs().max()) <= 1e-3
     P.close()
+
+
+# ---------------------------------------------------------------------------------- the projection kernel on its own
+PROX_CASES = {
+    # name: (instance, forms of the kernel that apply: 1 cluster-resident, 2 streaming pair, 3 every-asset)
+    "plain": (lambda: gen.config1(seed=3, N=640, k=8, A=3), (1, 2, 3)),
+    "bands": (lambda: gen.config2(seed=2, N=640, k=8, A=3, G=5, band_half=0.005), (1, 2, 3)),
+    "lots_caps": (lambda: gen.config3(seed=1, N=600, k=8, A=3), (1, 3)),
+    "odd_N": (lambda: gen.config1(seed=4, N=333, k=6, A=2), (1, 3)),
+    "penalty": (lambda: gen.section9(seed=2, N=480, k=8, A=2), (1, 2, 3)),
+}
+
+
+@pytest.mark.parametrize("name", sorted(PROX_CASES))
+@pytest.mark.parametrize("sd", [0.01, 0.0005])
+def test_projection_kernel_alone_against_its_definition(name, sd):
+    """ONE application of the fused projection (prism_project, the same kernel the iteration
+    launches) on random points v against the prox computed from its definition by the oracle (oracle/prox_ref.py:
+    the prox problem as an Eq. (1) instance with diagonal risk through the IPM; pinned on CPU against nested 1-D
+    searches).  Two bars: (1) element-wise against the IPM's answer at the accuracy an interior-point answer has on
+    these nearly degenerate problems (its own stationarity residual is ~1e-8, so ~1e-6 on the weights); (2) the sharp one:
+    the independent checker certifies the kernel's (z, multipliers) as a KKT point of the prox problem to 1e-12 - with the
+    strong convexity min_i rho_i of the prox objective that pins z to the exact prox far below (1) - and the kernel's
+    objective value is not above the oracle's.  A projection that is slightly inexact but still lets the iteration
+    converge fails (2)."""
+    import paper_2606_23367_b200 as pr
+    from oracle import kkt_check, prox_ref, problem
+    build, forms = PROX_CASES[name]
+    inst = build()
+    rng = np.random.default_rng(11)
+    v = inst.w0 + rng.normal(0.0, sd, inst.w0.shape)
+    rho_scale = 100.0
+    G = inst.G
+    accs, Z = [], []
+    for a in range(inst.A):
+        acc = problem.account_from_instance(inst, a)
+        rho = rho_scale * acc.gamma * acc.d
+        r = prox_ref.prox_qp(acc, v[a], rho, witness=inst.witness[a])
+        assert r["status"] == "optimal"
+        accs.append(prox_ref.prox_problem(acc, v[a], rho)); Z.append(r["w"])
+    for form in forms:
+        P = pr.Problem(inst, prox_form=form)
+        assert P.prox_form == form
+        z, duals = P.project(v, rho_scale)
+        z = z.cpu().numpy(); du = duals.cpu().numpy()
+        for a in range(inst.A):
+            pa = accs[a]
+            err = np.max(np.abs(z[a] - Z[a]))
+            assert err <= 3e-6, f"{name} form {form} account {a}: |z - prox(v)| = {err:.2e}"
+            feas = kkt_check.feasibility(pa, z[a])
+            assert max(feas.values()) <= 1e-8, (name, form, a, feas)
+            mult = dict(nu=du[a, 0], theta=du[a, 1], lam_hi=du[a, 2:2 + G], lam_lo=du[a, 2 + G:2 + 2 * G])
+            k = kkt_check.kkt(pa, z[a], mult, delta=1e-9)
+            scale = max(1.0, float(np.max(np.abs(pa.mu))))
+            assert k["r_stat"] <= 1e-12 * scale and k["r_comp"] <= 1e-12 and k["min_multiplier"] >= 0.0, (name, form, a, k)
+            assert problem.objective(pa, z[a]) <= problem.objective(pa, Z[a]) + 1e-12
+        P.close()

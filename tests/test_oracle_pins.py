@@ -203,3 +203,35 @@ def test_objective_factor_form_equals_dense_form():
     acc = _acc(inst)
     w = inst.witness[0]
     assert abs(problem.objective(acc, w) - problem.objective(acc, w, dense=True)) < 1e-14
+
+
+# ---------------------------------------------------------------------------------- prox reference (oracle/prox_ref.py)
+@pytest.mark.parametrize("seed,tau,kappa", [(0, 0.25, 0.0), (1, 0.05, 0.0), (2, np.inf, 0.002), (3, 0.12, 0.001)])
+def test_prox_reference_qp_equals_nested_one_dimensional_searches(seed, tau, kappa):
+    """prox_qp (the prox as an Eq. (1) instance with diagonal risk, through the IPM) against prox_nested (the
+    definition through one-dimensional golden-section / bisection searches only) on random points v."""
+    from oracle import prox_ref
+    inst = gen.make_instance("prox", seed, 14, 3, 1, hi_fixed=0.2, tau_fixed=tau if np.isfinite(tau) else None,
+                             excl_frac=0.15, kappa_fixed=kappa)
+    acc = _acc(inst)                                   # (the generator floors tau so that the exclusions can be sold)
+    rng = np.random.default_rng(100 + seed)
+    rho = 100.0 * acc.gamma * acc.d
+    v = acc.w0 + rng.normal(0.0, 0.08, acc.N)
+    r = prox_ref.prox_qp(acc, v, rho, witness=inst.witness[0])
+    assert r["status"] == "optimal"
+    z_nested = prox_ref.prox_nested(acc, v, rho)
+    assert abs(z_nested.sum() - 1.0) < 1e-7
+    assert np.max(np.abs(r["w"] - z_nested)) < 2e-7
+    # and the answer carries a KKT certificate for the prox problem itself
+    _certify(prox_ref.prox_problem(acc, v, rho), r)
+
+
+def test_prox_reference_box_and_budget_only_is_the_capped_simplex_projection():
+    """rho = 1, no cap, no penalty: the prox of the indicator of {1'z = 1, 0 <= z <= u} is the Euclidean projection."""
+    from oracle import prox_ref
+    inst = gen.make_instance("proxproj", 7, 40, 3, 1, hi_fixed=0.06, gamma_fixed=1.0)
+    acc = _acc(inst)
+    acc.tau = np.inf
+    v = np.random.default_rng(7).normal(0.02, 0.05, acc.N)
+    r = prox_ref.prox_qp(acc, v, np.ones(acc.N), witness=inst.witness[0])
+    assert np.max(np.abs(r["w"] - closed_form.capped_simplex_projection(v, 0.06))) < 1e-8
