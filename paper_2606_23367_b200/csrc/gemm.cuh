@@ -90,7 +90,9 @@ __global__ void __launch_bounds__(256) k_gemm1(Gemm1Args p) {
   }
 }
 
-// reference: one thread per (a, j), plain FMA, same chunking
+// reference: one thread per (a, j), plain FMA, same chunking.  F32: the precision experiment of DESIGN.md (would a
+// TF32x3 / fp32 tensor path hold the tolerance?): both operands rounded to fp32, products and sums in fp32.
+template <bool F32>
 __global__ void k_gemm1_ref(Gemm1Args p, int kp) {
   const int64_t t = (int64_t)blockIdx.y * blockDim.x + threadIdx.x;
   if (t >= (int64_t)p.nact * kp) return;
@@ -98,7 +100,13 @@ __global__ void k_gemm1_ref(Gemm1Args p, int kp) {
   const int a = p.act ? p.act[slot] : slot;
   const int64_t i_begin = (int64_t)blockIdx.x * p.chunk, i_end = min(i_begin + p.chunk, p.Npad);
   double s = 0.0;
-  for (int64_t i = i_begin; i < i_end; ++i) s = fma(p.Bt[(int64_t)j * p.ldn + i], p.X[(int64_t)a * p.ldw + i], s);
+  if (F32) {
+    float sf = 0.f;
+    for (int64_t i = i_begin; i < i_end; ++i) sf = fmaf((float)p.Bt[(int64_t)j * p.ldn + i], (float)p.X[(int64_t)a * p.ldw + i], sf);
+    s = (double)sf;
+  } else {
+    for (int64_t i = i_begin; i < i_end; ++i) s = fma(p.Bt[(int64_t)j * p.ldn + i], p.X[(int64_t)a * p.ldw + i], s);
+  }
   p.Tpart[((int64_t)blockIdx.x * p.A + a) * p.ldv + j] = s;
 }
 
@@ -226,12 +234,18 @@ __global__ void __launch_bounds__(256, 3) k_gemm2(Gemm2Args p) {
   }
 }
 
-template <int MODE>
+template <int MODE, bool F32>
 __global__ void k_gemm2_ref(Gemm2Args p) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= p.N || (int)blockIdx.y >= p.nact) return;
   const int a = p.act ? p.act[blockIdx.y] : (int)blockIdx.y;
   double bv = 0.0;
-  for (int j = 0; j < p.kp; ++j) bv = fma(p.Bp[i * p.kp + j], p.V[(int64_t)a * p.ldv + j], bv);
+  if (F32) {
+    float bf = 0.f;
+    for (int j = 0; j < p.kp; ++j) bf = fmaf((float)p.Bp[i * p.kp + j], (float)p.V[(int64_t)a * p.ldv + j], bf);
+    bv = (double)bf;
+  } else {
+    for (int j = 0; j < p.kp; ++j) bv = fma(p.Bp[i * p.kp + j], p.V[(int64_t)a * p.ldv + j], bv);
+  }
   g2_epilogue<MODE>(p, a, i, bv);
 }

@@ -27,9 +27,9 @@ cudaError_t gemm_set_attrs(int mt) {
 }
 
 cudaError_t gemm1_launch(int gemm_mode, int mt, int nchunk, int kp, const Gemm1Args& a, cudaStream_t st) {
-  if (gemm_mode == 1) {
+  if (gemm_mode >= 1) {
     dim3 grid(nchunk, (unsigned)(((int64_t)a.nact * kp + 127) / 128));
-    k_gemm1_ref<<<grid, 128, 0, st>>>(a, kp);
+    if (gemm_mode == 2) k_gemm1_ref<true><<<grid, 128, 0, st>>>(a, kp); else k_gemm1_ref<false><<<grid, 128, 0, st>>>(a, kp);
   } else {
     dim3 grid(nchunk, (a.nact + G1_TA - 1) / G1_TA);
     MT_SWITCH(mt, k_gemm1<MT><<<grid, 256, g1_smem(MT), st>>>(a));
@@ -39,9 +39,9 @@ cudaError_t gemm1_launch(int gemm_mode, int mt, int nchunk, int kp, const Gemm1A
 
 template <int MODE>
 static void gemm2_mode(int gemm_mode, int mt, const Gemm2Args& a, cudaStream_t st) {
-  if (gemm_mode == 1) {
+  if (gemm_mode >= 1) {
     dim3 grid((unsigned)((a.N + 127) / 128), a.nact);
-    k_gemm2_ref<MODE><<<grid, 128, 0, st>>>(a);
+    if (gemm_mode == 2) k_gemm2_ref<MODE, true><<<grid, 128, 0, st>>>(a); else k_gemm2_ref<MODE, false><<<grid, 128, 0, st>>>(a);
   } else {
     dim3 grid((unsigned)((a.N + G2_TN - 1) / G2_TN), (a.nact + G2_TM - 1) / G2_TM);
     MT_SWITCH(mt, k_gemm2<MT, MODE><<<grid, 256, g2_smem(MT), st>>>(a));

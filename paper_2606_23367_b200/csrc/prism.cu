@@ -349,7 +349,7 @@ extern "C" int prism_solve_batch(prism_problem* p, const prism_settings* sp, voi
   prism_settings s;
   if (sp) s = *sp; else prism_default_settings(&s);
   if (!(s.eps_rel > 0) || !(s.eps_abs >= 0) || s.max_iter < 1 || s.check_every < 1 || !(s.alpha > 0 && s.alpha < 2) || !(s.rho_scale > 0) ||
-      (s.gemm_precision != PRISM_GEMM_FP64_TENSOR && s.gemm_precision != PRISM_GEMM_FP64_FMA))
+      (s.gemm_precision < PRISM_GEMM_FP64_TENSOR || s.gemm_precision > PRISM_GEMM_FP32_EXPERIMENT))
     return set_err(PRISM_ERR_INVALID_ARG, "invalid settings%s", "");
   if (s.warm_duals && !s.warm_w) return set_err(PRISM_ERR_INVALID_ARG, "warm_duals needs warm_w%s", "");
   cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -442,6 +442,7 @@ extern "C" int prism_solve_batch(prism_problem* p, const prism_settings* sp, voi
     launch_prox(L, pa, PROX_FINAL, it > s.max_iter ? s.max_iter : it - 1);
   }
   // H8 / H9: external diagnostics of the returned weights with the solver's multipliers, then statuses
+  if (L.gemm_mode == PRISM_GEMM_FP32_EXPERIMENT) L.gemm_mode = PRISM_GEMM_FP64_FMA;   // diagnostics are always fp64
   run_diag(p, L, w_out, p->duals, p->resid);
   L.begin(PRISM_K_OTHER);
   L.end(status_launch(A, p->resid, p->ap.conv, p->ap.iters, timed_out, late_iter, 1e-6, p->status, st));

