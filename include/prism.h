@@ -130,6 +130,8 @@ typedef struct prism_data {
 
 enum { PRISM_GEMM_FP64_TENSOR = 0,   /* fp64 on the tensor pipe (DMMA mma.sync.m8n8k4)                              */
        PRISM_GEMM_FP64_FMA = 1,      /* fp64 FMA kernels of the same contract (validation twin)                     */
+       PRISM_GEMM_TF32X3 = 3,        /* TF32 tensor path with the 3xTF32 split (fp32-level accuracy, fp32 accumulators):
+                                        both GEMMs become HBM-bound instead of fp64-pipe-bound                    */
        PRISM_GEMM_FP32_EXPERIMENT = 2 /* the FMA twins with both operands rounded to fp32 and fp32 accumulation: NOT a
                                         production path - the measurement behind the precision choice: the
                                         Sigma-apply of the external diagnostics stays fp64                         */ };

@@ -39,6 +39,7 @@ struct prism_problem {
   // shared precomputed (owned)
   double* Bp;       // N x kp, asset-major, zero padded            (GEMM-2 operand)
   double* Bt;       // kp x ldn, factor-major                      (GEMM-1 operand)
+  float *Bp_hi, *Bp_lo, *Bt_hi, *Bt_lo;   // the universe split for the 3xTF32 GEMMs (gemm_tf32.cuh)
   int64_t ldn;      // N padded to 32
   double* invd;     // N
   double* gram;     // Kp x Kp : Bp' D^-1 Bp

@@ -35,3 +35,9 @@ struct Gemm2Args {
   const int32_t* act; int32_t nact;   // as in Gemm1Args
 };
 
+
+// the universe split for the 3xTF32 kernels (gemm_tf32.cuh): tf32-rounded values in fp32 storage, built at create
+struct TfSplit {
+  const float *Bt_hi, *Bt_lo;   // kp x ldn, factor-major
+  const float *Bp_hi, *Bp_lo;   // N x kp, asset-major
+};

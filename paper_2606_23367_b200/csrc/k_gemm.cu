@@ -1,5 +1,6 @@
 // k_gemm.cu - translation unit of the factor GEMMs (H1, H3): kernels in gemm.cuh, launch wrappers of kernels.h.
 #include "gemm.cuh"
+#include "gemm_tf32.cuh"
 #include "kernels.h"
 
 #define MT_SWITCH(mt, ...)                                            \
@@ -22,14 +23,27 @@ cudaError_t gemm_set_attrs(int mt) {
     TRY(cudaFuncSetAttribute(k_gemm2<MT, G2_ADMM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g2_smem(MT)));
     TRY(cudaFuncSetAttribute(k_gemm2<MT, G2_ADMM_CHECK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g2_smem(MT)));
     TRY(cudaFuncSetAttribute(k_gemm2<MT, G2_SIGMA>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g2_smem(MT)));
+    TRY(cudaFuncSetAttribute(k_gemm1_tf32<MT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)t1_smem(8 * MT)));
+    TRY(cudaFuncSetAttribute(k_gemm2_tf32<MT, G2_ADMM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)t2_smem(8 * MT)));
+    TRY(cudaFuncSetAttribute(k_gemm2_tf32<MT, G2_ADMM_CHECK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)t2_smem(8 * MT)));
   });
   return cudaSuccess;
 }
+cudaError_t split_universe_launch(const double* Bp, const double* Bt, int64_t N, int kp, int64_t ldn, float* Bp_hi, float* Bp_lo,
+                                  float* Bt_hi, float* Bt_lo, cudaStream_t st) {
+  const int64_t n = (int64_t)kp * ldn;          // ldn >= N
+  k_split_universe<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(Bp, Bt, N, kp, ldn, Bp_hi, Bp_lo, Bt_hi, Bt_lo);
+  return cudaGetLastError();
+}
 
-cudaError_t gemm1_launch(int gemm_mode, int mt, int nchunk, int kp, const Gemm1Args& a, cudaStream_t st) {
-  if (gemm_mode >= 1) {
+cudaError_t gemm1_launch(int gemm_mode, int mt, int nchunk, int kp, const Gemm1Args& a, const TfSplit& tf, cudaStream_t st) {
+  if (gemm_mode == PRISM_GEMM_TF32X3) {
+    TfUniverse u{tf.Bt_hi, tf.Bt_lo, tf.Bp_hi, tf.Bp_lo};
+    dim3 grid(nchunk, (a.nact + T1_TA - 1) / T1_TA);
+    MT_SWITCH(mt, k_gemm1_tf32<MT><<<grid, 128, t1_smem(8 * MT), st>>>(a, u));
+  } else if (gemm_mode >= 1) {
     dim3 grid(nchunk, (unsigned)(((int64_t)a.nact * kp + 127) / 128));
-    if (gemm_mode == 2) k_gemm1_ref<true><<<grid, 128, 0, st>>>(a, kp); else k_gemm1_ref<false><<<grid, 128, 0, st>>>(a, kp);
+    if (gemm_mode == PRISM_GEMM_FP32_EXPERIMENT) k_gemm1_ref<true><<<grid, 128, 0, st>>>(a, kp); else k_gemm1_ref<false><<<grid, 128, 0, st>>>(a, kp);
   } else {
     dim3 grid(nchunk, (a.nact + G1_TA - 1) / G1_TA);
     MT_SWITCH(mt, k_gemm1<MT><<<grid, 256, g1_smem(MT), st>>>(a));
@@ -38,19 +52,24 @@ cudaError_t gemm1_launch(int gemm_mode, int mt, int nchunk, int kp, const Gemm1A
 }
 
 template <int MODE>
-static void gemm2_mode(int gemm_mode, int mt, const Gemm2Args& a, cudaStream_t st) {
-  if (gemm_mode >= 1) {
+static void gemm2_mode(int gemm_mode, int mt, const Gemm2Args& a, const TfSplit& tf, cudaStream_t st) {
+  if (gemm_mode == PRISM_GEMM_TF32X3 && MODE != G2_SIGMA) {
+    constexpr int M2 = MODE == G2_SIGMA ? G2_ADMM : MODE;
+    TfUniverse u{tf.Bt_hi, tf.Bt_lo, tf.Bp_hi, tf.Bp_lo};
+    dim3 grid((unsigned)((a.N + T2_TN - 1) / T2_TN), (a.nact + T2_TM - 1) / T2_TM);
+    MT_SWITCH(mt, k_gemm2_tf32<MT, M2><<<grid, 128, t2_smem(8 * MT), st>>>(a, u));
+  } else if (gemm_mode == 1 || gemm_mode == 2) {
     dim3 grid((unsigned)((a.N + 127) / 128), a.nact);
-    if (gemm_mode == 2) k_gemm2_ref<MODE, true><<<grid, 128, 0, st>>>(a); else k_gemm2_ref<MODE, false><<<grid, 128, 0, st>>>(a);
+    if (gemm_mode == PRISM_GEMM_FP32_EXPERIMENT) k_gemm2_ref<MODE, true><<<grid, 128, 0, st>>>(a); else k_gemm2_ref<MODE, false><<<grid, 128, 0, st>>>(a);
   } else {
     dim3 grid((unsigned)((a.N + G2_TN - 1) / G2_TN), (a.nact + G2_TM - 1) / G2_TM);
     MT_SWITCH(mt, k_gemm2<MT, MODE><<<grid, 256, g2_smem(MT), st>>>(a));
   }
 }
-cudaError_t gemm2_launch(int gemm_mode, int mt, int mode, const Gemm2Args& a, cudaStream_t st) {
-  if (mode == G2_ADMM) gemm2_mode<G2_ADMM>(gemm_mode, mt, a, st);
-  else if (mode == G2_ADMM_CHECK) gemm2_mode<G2_ADMM_CHECK>(gemm_mode, mt, a, st);
-  else gemm2_mode<G2_SIGMA>(gemm_mode, mt, a, st);
+cudaError_t gemm2_launch(int gemm_mode, int mt, int mode, const Gemm2Args& a, const TfSplit& tf, cudaStream_t st) {
+  if (mode == G2_ADMM) gemm2_mode<G2_ADMM>(gemm_mode, mt, a, tf, st);
+  else if (mode == G2_ADMM_CHECK) gemm2_mode<G2_ADMM_CHECK>(gemm_mode, mt, a, tf, st);
+  else gemm2_mode<G2_SIGMA>(gemm_mode, mt, a, tf, st);
   return cudaGetLastError();
 }
 

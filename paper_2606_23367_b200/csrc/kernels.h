@@ -10,8 +10,10 @@
 
 // ---- factor GEMMs (k_gemm.cu): fp64 DMMA (gemm_mode 0) or plain FMA (gemm_mode 1)
 cudaError_t gemm_set_attrs(int mt);
-cudaError_t gemm1_launch(int gemm_mode, int mt, int nchunk, int kp, const Gemm1Args& a, cudaStream_t st);
-cudaError_t gemm2_launch(int gemm_mode, int mt, int mode /* G2_* */, const Gemm2Args& a, cudaStream_t st);
+cudaError_t gemm1_launch(int gemm_mode, int mt, int nchunk, int kp, const Gemm1Args& a, const TfSplit& tf, cudaStream_t st);
+cudaError_t gemm2_launch(int gemm_mode, int mt, int mode /* G2_* */, const Gemm2Args& a, const TfSplit& tf, cudaStream_t st);
+cudaError_t split_universe_launch(const double* Bp, const double* Bt, int64_t N, int kp, int64_t ldn, float* Bp_hi, float* Bp_lo,
+                                  float* Bt_hi, float* Bt_lo, cudaStream_t st);
 
 cudaError_t fp64_yardstick(cudaStream_t st, double* sink_dev, int sm_count, double* tflops /* host [2]: DMMA, FMA */);
 

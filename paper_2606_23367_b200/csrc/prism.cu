@@ -47,7 +47,7 @@ static int dev_alloc(prism_problem* p, T** ptr, size_t count, bool zero = true) 
 
 extern "C" void prism_problem_destroy(prism_problem* p) {
   if (!p) return;
-  void* ptrs[] = {p->Bp, p->Bt, p->invd, p->gram, p->q, p->v, p->rt, p->cc, p->xs, p->pxq, p->Tpart, p->V, p->Sinv,
+  void* ptrs[] = {p->Bp, p->Bt, p->Bp_hi, p->Bp_lo, p->Bt_hi, p->Bt_lo, p->invd, p->gram, p->q, p->v, p->rt, p->cc, p->xs, p->pxq, p->Tpart, p->V, p->Sinv,
                   p->gw0, p->lamG, p->resid, p->duals, p->status, p->ap.c, p->ap.alpha, p->ap.beta,
                   p->ap.mode, p->ap.bsum, p->ap.done, p->ap.conv, p->ap.iters, p->ap.refactor,
                   p->ap.nadapt, p->ap.win, p->ap.wins, p->ap.slack, p->counters, p->act, p->w_stage, p->i_stage, p->lraw, p->lcomp, p->lcnt, p->cbin, p->chkp, p->lflag};
@@ -96,11 +96,12 @@ struct Launcher {
     a.Bt = p->Bt; a.ldn = p->ldn; a.X = X; a.ldw = p->ldn; a.Tpart = p->Tpart; a.ldv = p->ldv; a.A = p->A;
     a.chunk = p->chunk; a.Npad = p->ldn; a.act = act; a.nact = nact;
     begin(PRISM_K_GEMM1);
-    end(gemm1_launch(gemm_mode, mt, p->nchunk, p->kp, a, st));
+    end(gemm1_launch(gemm_mode, mt, p->nchunk, p->kp, a, tf(), st));
   }
+  TfSplit tf() const { return TfSplit{p->Bt_hi, p->Bt_lo, p->Bp_hi, p->Bp_lo}; }
   void gemm2(int mode, const Gemm2Args& a) {
     begin(PRISM_K_GEMM2);
-    end(gemm2_launch(gemm_mode, mt, mode, a, st));
+    end(gemm2_launch(gemm_mode, mt, mode, a, tf(), st));
   }
   Gemm2Args g2base() const {
     Gemm2Args a;
@@ -207,6 +208,10 @@ extern "C" int prism_problem_create(int64_t N, int32_t k, int32_t accounts, cons
   const size_t AN = (size_t)A * p->ldn;
   ALLOC_TRY(dev_alloc(p, &p->Bp, (size_t)N * p->kp));
   ALLOC_TRY(dev_alloc(p, &p->Bt, (size_t)p->kp * p->ldn));
+  ALLOC_TRY(dev_alloc(p, &p->Bp_hi, (size_t)N * p->kp));
+  ALLOC_TRY(dev_alloc(p, &p->Bp_lo, (size_t)N * p->kp));
+  ALLOC_TRY(dev_alloc(p, &p->Bt_hi, (size_t)p->kp * p->ldn));
+  ALLOC_TRY(dev_alloc(p, &p->Bt_lo, (size_t)p->kp * p->ldn));
   ALLOC_TRY(dev_alloc(p, &p->invd, (size_t)p->ldn));       // padded with zeros (pair-wise GEMM-2 epilogue)
   ALLOC_TRY(dev_alloc(p, &p->gram, (size_t)p->Kp * p->Kp));
   ALLOC_TRY(dev_alloc(p, &p->v, AN));
@@ -272,6 +277,7 @@ extern "C" int prism_problem_create(int64_t N, int32_t k, int32_t accounts, cons
   Launcher L{p, st, mt, 0};
   L.end(setup_shared_launch(data->B, data->B_is_fp32, data->d, N, k, p->kp, p->ldn, p->Bp, p->Bt, p->invd, st));
   L.end(gram_launch(p->Bt, p->ldn, p->invd, N, p->kp, p->gram, st));
+  L.end(split_universe_launch(p->Bp, p->Bt, N, p->kp, p->ldn, p->Bp_hi, p->Bp_lo, p->Bt_hi, p->Bt_lo, st));
   if (p->d.w_b) L.build_q();            // q = -mu - gamma Sigma w_b
   cudaError_t e = cudaStreamSynchronize(st);
   if (e == cudaSuccess) e = L.err;
@@ -349,7 +355,7 @@ extern "C" int prism_solve_batch(prism_problem* p, const prism_settings* sp, voi
   prism_settings s;
   if (sp) s = *sp; else prism_default_settings(&s);
   if (!(s.eps_rel > 0) || !(s.eps_abs >= 0) || s.max_iter < 1 || s.check_every < 1 || !(s.alpha > 0 && s.alpha < 2) || !(s.rho_scale > 0) ||
-      (s.gemm_precision < PRISM_GEMM_FP64_TENSOR || s.gemm_precision > PRISM_GEMM_FP32_EXPERIMENT))
+      (s.gemm_precision < PRISM_GEMM_FP64_TENSOR || s.gemm_precision > PRISM_GEMM_TF32X3))
     return set_err(PRISM_ERR_INVALID_ARG, "invalid settings%s", "");
   if (s.warm_duals && !s.warm_w) return set_err(PRISM_ERR_INVALID_ARG, "warm_duals needs warm_w%s", "");
   cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -442,7 +448,9 @@ extern "C" int prism_solve_batch(prism_problem* p, const prism_settings* sp, voi
     launch_prox(L, pa, PROX_FINAL, it > s.max_iter ? s.max_iter : it - 1);
   }
   // H8 / H9: external diagnostics of the returned weights with the solver's multipliers, then statuses
-  if (L.gemm_mode == PRISM_GEMM_FP32_EXPERIMENT) L.gemm_mode = PRISM_GEMM_FP64_FMA;   // diagnostics are always fp64
+  // the external diagnostics are always fp64
+  if (L.gemm_mode == PRISM_GEMM_FP32_EXPERIMENT) L.gemm_mode = PRISM_GEMM_FP64_FMA;
+  if (L.gemm_mode == PRISM_GEMM_TF32X3) L.gemm_mode = PRISM_GEMM_FP64_TENSOR;
   run_diag(p, L, w_out, p->duals, p->resid);
   L.begin(PRISM_K_OTHER);
   L.end(status_launch(A, p->resid, p->ap.conv, p->ap.iters, timed_out, late_iter, 1e-6, p->status, st));

@@ -114,6 +114,23 @@ def test_dmma_and_fma_gemms_agree():
     P.close()
 
 
+@pytest.mark.parametrize("name", ["cfg1_ragged", "cfg1_multi_tile", "cfg2_stream", "cfg3_small", "cfg4_small", "benchmark_shift"])
+def test_tf32x3_gemms_against_fp64_and_oracle(name):
+    """The 3xTF32 tensor-path GEMMs (PRISM_GEMM_TF32X3: fp32-level operand accuracy, fp32 accumulators, fp64 epilogue)
+    against the fp64 DMMA GEMMs on the same problem - same statuses, weights within 1e-6 (two orders below the parity
+    tolerance) - and against the oracle at the full parity bar.  Ragged N, > 64 accounts (two account tiles of each
+    kernel), k = 50 and k = 100 (7 and 13 factor tiles), lots, fp32 loadings, benchmark shift."""
+    inst = CASES[name]()
+    P, r0 = _solve_gpu(inst, gemm_precision=0)
+    r3 = P.solve(gemm_precision=3)
+    assert (r3.status == 0).all() and (r0.status == 0).all()
+    assert float((r0.w - r3.w).abs().max()) <= 1e-6
+    assert int((r0.iters - r3.iters).abs().max()) <= 20
+    W, res = _oracle(inst)
+    _check_against_oracle(inst, r3, W, res)
+    P.close()
+
+
 def test_batch_equals_single_accounts_and_identical_accounts():
     inst = gen.config1(N=400, k=10, A=4)
     P, r = _solve_gpu(inst)
