@@ -185,7 +185,7 @@ def main():
     ap.add_argument("--oracle-accounts", type=int, default=32, help="accounts in the cpu_baseline sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extra", action="store_true", help="skip the rows for the other configs and the N sweep")
-    ap.add_argument("--gemm-precision", type=int, default=0)
+    ap.add_argument("--gemm-precision", type=int, default=3, help="PRISM_GEMM_*: 3 = 3xTF32 tensor path (library default), 0 = fp64 DMMA")
     ap.add_argument("--prox-form", type=int, default=0, help="PRISM_PROX_* (0 = AUTO) for the headline problem object")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -301,8 +301,11 @@ def main():
             per[name] = {"ms": kt[name]["ms"], "launches": kt[name]["launches"], "share": kt[name]["ms"] / tot,
                          "algorithmic_GBps": nbytes / t / 1e9, "hbm_frac": nbytes / t / 1e9 / peak}
             if flops:
-                per[name]["fp64_TFLOPs"] = flops / t / 1e12
-                per[name]["frac_of_measured_dmma"] = flops / t / 1e12 / yard["dmma_tflops"]
+                per[name]["TFLOPs"] = flops / t / 1e12          # contraction flops 2 N k per account-iteration
+                if args.gemm_precision in (0, 1):
+                    per[name]["frac_of_measured_dmma"] = flops / t / 1e12 / yard["dmma_tflops"]
+                else:
+                    per[name]["tensor_path"] = "3xTF32 mma.sync m16n8k8 (3 MMAs per product, fp32 accumulate): HBM-bound, see hbm_frac"
         for name in ("solve", "factor", "diag", "other"):
             if kt[name]["ms"] > 0:
                 per[name] = {"ms": kt[name]["ms"], "launches": kt[name]["launches"], "share": kt[name]["ms"] / tot}
@@ -312,8 +315,9 @@ def main():
     rp, kt, per, dom, tot_k, step_bytes = profile(P, inst)
     domk = per[dom]
     FORMS = {1: "k_prox_res (cluster-resident form)", 2: "k_prox_stream + k_prox_root (streaming form)", 3: "k_prox (every-asset form)"}
+    gk = "_tf32" if args.gemm_precision == 3 else ""
     kernel_names = {"prox": "H4-H7 fused projection: " + FORMS[P.prox_form],
-                    "gemm2": "H3 k_gemm2 (factor GEMM-2 + epilogue)", "gemm1": "H1 k_gemm1 (split-K factor GEMM-1)"}
+                    "gemm2": f"H3 k_gemm2{gk} (factor GEMM-2 + epilogue)", "gemm1": f"H1 k_gemm1{gk} (split-K factor GEMM-1)"}
     roofline = {"bound": "hbm", "kernel": kernel_names.get(dom, dom), "dominant_by_time": dom,
                 "achieved": domk.get("algorithmic_GBps"), "peak": peak, "unit": "GB/s",
                 "frac": domk.get("hbm_frac"), "traffic": None,
@@ -324,7 +328,8 @@ def main():
                 "whole_step": {"algorithmic_GBps": step_bytes / (rp.info["solve_interval_ms"] * 1e-3) / 1e9,
                                "hbm_frac": step_bytes / (rp.info["solve_interval_ms"] * 1e-3) / 1e9 / peak,
                                "bytes_per_element_iteration": "prox 41 (+24 on check iterations) + gemm1 8 + gemm2 24 (+24)"},
-                "fp64_yardstick_TFLOPs": yard, "per_kernel": per}
+                "fp64_yardstick_TFLOPs": yard, "gemm_precision": {0: "fp64 DMMA", 1: "fp64 FMA", 2: "fp32 experiment", 3: "3xTF32"}[args.gemm_precision],
+                "per_kernel": per}
 
     def row(name, instq, form=0):
         Pq = pr.Problem(instq, device=dev, prox_form=form)

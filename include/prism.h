@@ -146,7 +146,8 @@ typedef struct prism_settings {
   int32_t adapt_rho;        /* 1 => per-account rho adaptation at check iterations (default 1)                   */
   double alpha;             /* over-relaxation in (0, 2) (default 1.6)                                           */
   double rho_scale;         /* initial c: rho_i = c gamma_a d_i (default 100)                                    */
-  int32_t gemm_precision;   /* PRISM_GEMM_* (default fp64 tensor); DESIGN.md records why no TF32 path is built   */
+  int32_t gemm_precision;   /* PRISM_GEMM_* (default PRISM_GEMM_TF32X3, chosen against the tolerance by measurement:
+                               DESIGN.md section 5); the external diagnostics are fp64 whatever this says        */
   int32_t profile;          /* 1 => bracket every kernel launch with CUDA events (read with prism_kernel_times);
                                adds event overhead, so never combine with a throughput measurement           */
   double time_limit_ms;     /* 0 => none; accounts unfinished at the limit get PRISM_STATUS_TIMEOUT              */

@@ -40,4 +40,5 @@ struct Gemm2Args {
 struct TfSplit {
   const float *Bt_hi, *Bt_lo;   // kp x ldn, factor-major
   const float *Bp_hi, *Bp_lo;   // N x kp, asset-major
+  int sm_count;
 };

@@ -122,32 +122,43 @@ __global__ void __launch_bounds__(128) k_gemm1_tf32(Gemm1Args p, TfUniverse u) {
 }
 
 // GEMM-2 + fused epilogue (modes G2_ADMM, G2_ADMM_CHECK; the Sigma-apply of the diagnostics stays on the fp64 kernels).
-// Tile: 64 accounts x 64 assets, K = kp; warp w owns accounts 16 w .. 16 w + 15 and walks the assets in two column groups
-// of 32 whose epilogue operands (v, c pairs) are requested before the group's MMA loop.
+// A CTA owns 64 accounts and walks `tpc` consecutive 64-asset tiles: V = S^-1 T of its accounts is split ONCE into shared
+// memory, the universe tiles are double-buffered with cp.async (the next tile loads during the MMA loop and the
+// epilogue of the current one), and the epilogue operands (v, c pairs) are requested before the tile's MMA loop.
+// 8 warps: warp w owns accounts 16 (w & 3) .. + 15 and the assets 32 (w >> 2) .. + 31 of the tile.
 #define T2_TM 64
 #define T2_TN 64
-__host__ __device__ inline size_t t2_smem(int kp) { return (size_t)2 * (T2_TM + T2_TN) * (kp + 4) * sizeof(float); }
+__host__ __device__ inline size_t t2_smem(int kp) { return (size_t)(2 * T2_TM + 4 * T2_TN) * (kp + 4) * sizeof(float); }
 
 template <int NT, int MODE>
-__global__ void __launch_bounds__(128, 3) k_gemm2_tf32(Gemm2Args p, TfUniverse u) {
+__global__ void __launch_bounds__(256, 2) k_gemm2_tf32(Gemm2Args p, TfUniverse u, int tpc) {
   extern __shared__ __align__(16) unsigned char t2_raw[];
   constexpr int KP = 8 * NT, LD = KP + 4;
   float* Vh = (float*)t2_raw;                 // [T2_TM][LD]
   float* Vl = Vh + (size_t)T2_TM * LD;
-  float* Bh = Vl + (size_t)T2_TM * LD;        // [T2_TN][LD]
-  float* Bl = Bh + (size_t)T2_TN * LD;
+  float* Bbuf = Vl + (size_t)T2_TM * LD;      // 2 x { hi [T2_TN][LD], lo [T2_TN][LD] }
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3;
+  const int wr = warp & 3, wc = warp >> 2;
   const int a0 = blockIdx.y * T2_TM;
-  const int64_t i0 = (int64_t)blockIdx.x * T2_TN;
   if (a0 >= p.nact) return;
-  for (int c = tid; c < T2_TN * (KP / 4); c += 128) {
-    const int r = c / (KP / 4), cc = (c % (KP / 4)) * 4;
-    const int64_t i = min(i0 + r, p.N - 1);
-    cp_async16(Bh + r * LD + cc, u.Bp_hi + i * KP + cc);
-    cp_async16(Bl + r * LD + cc, u.Bp_lo + i * KP + cc);
-  }
+  const int64_t ntile = (p.N + T2_TN - 1) / T2_TN;
+  const int64_t tile0 = (int64_t)blockIdx.x * tpc;
+  const int nt = (int)min((int64_t)tpc, ntile - tile0);
+  if (nt <= 0) return;
+  auto load_B = [&](int buf, int64_t tile) {
+    float* bh = Bbuf + (size_t)buf * 2 * T2_TN * LD;
+    float* bl = bh + (size_t)T2_TN * LD;
+    const int64_t i0 = tile * T2_TN;
+    for (int c = tid; c < T2_TN * (KP / 4); c += 256) {
+      const int r = c / (KP / 4), cc = (c % (KP / 4)) * 4;
+      const int64_t i = min(i0 + r, p.N - 1);
+      cp_async16(bh + r * LD + cc, u.Bp_hi + i * KP + cc);
+      cp_async16(bl + r * LD + cc, u.Bp_lo + i * KP + cc);
+    }
+  };
+  load_B(0, tile0);
   cp_async_commit();
-  for (int c = tid; c < T2_TM * (KP / 2); c += 128) {      // V is fp64 in memory: split on the way to shared memory
+  for (int c = tid; c < T2_TM * (KP / 2); c += 256) {      // V is fp64 in memory: split on the way to shared memory
     const int r = c / (KP / 2), cc = (c % (KP / 2)) * 2;
     const int slot = min(a0 + r, p.nact - 1);
     const int a = p.act ? p.act[slot] : slot;
@@ -162,20 +173,22 @@ __global__ void __launch_bounds__(128, 3) k_gemm2_tf32(Gemm2Args p, TfUniverse u
   double gsc[2], gam[2];
 #pragma unroll
   for (int h = 0; h < 2; ++h) {
-    const int slot = a0 + warp * 16 + g + 8 * h;
+    const int slot = a0 + wr * 16 + g + 8 * h;
     arow[h] = slot < p.nact;
     acct[h] = arow[h] ? (p.act ? p.act[slot] : slot) : 0;
     gam[h] = arow[h] ? p.gamma[acct[h]] : 1.0;
     gsc[h] = arow[h] ? 1.0 / (gam[h] * (1.0 + p.c[acct[h]])) : 0.0;
   }
-  cp_async_wait<0>();
-  __syncthreads();
-  const float* vh = Vh + (size_t)(warp * 16 + g) * LD + t;
-  const float* vl = Vl + (size_t)(warp * 16 + g) * LD + t;
+  const float* vh = Vh + (size_t)(wr * 16 + g) * LD + t;
+  const float* vl = Vl + (size_t)(wr * 16 + g) * LD + t;
 #pragma unroll 1
-  for (int cg = 0; cg < T2_TN / 32; ++cg) {
+  for (int tt = 0; tt < nt; ++tt) {
+    cp_async_wait<0>();
+    __syncthreads();                                       // tile tt (and, the first time, V) has landed; tile tt - 1 is done with
+    if (tt + 1 < nt) load_B((tt + 1) & 1, tile0 + tt + 1);
+    cp_async_commit();
     // D[account row g (+8)][asset = ib + 8 n + {0, 1}], n = 0..3
-    const int64_t ib = i0 + cg * 32 + 2 * t;
+    const int64_t ib = (tile0 + tt) * T2_TN + wc * 32 + 2 * t;
     double2 v2[2][4], c2[2][4];
 #pragma unroll
     for (int h = 0; h < 2; ++h) {
@@ -192,8 +205,8 @@ __global__ void __launch_bounds__(128, 3) k_gemm2_tf32(Gemm2Args p, TfUniverse u
     float acc[4][4];
 #pragma unroll
     for (int n = 0; n < 4; ++n) { acc[n][0] = acc[n][1] = acc[n][2] = acc[n][3] = 0.f; }
-    const float* bh = Bh + (size_t)(cg * 32 + g) * LD + t;
-    const float* bl = Bl + (size_t)(cg * 32 + g) * LD + t;
+    const float* bh = Bbuf + (size_t)(tt & 1) * 2 * T2_TN * LD + (size_t)(wc * 32 + g) * LD + t;
+    const float* bl = bh + (size_t)T2_TN * LD;
 #pragma unroll
     for (int k0 = 0; k0 < KP; k0 += 8) {
       uint32_t ah[4], al[4];
@@ -244,6 +257,7 @@ __global__ void __launch_bounds__(128, 3) k_gemm2_tf32(Gemm2Args p, TfUniverse u
       }
     }
   }
+  cp_async_wait<0>();
 }
 
 // universe split at create: Bt_hi/lo (kp x ldn) and Bp_hi/lo (N x kp) from the padded fp64 copies

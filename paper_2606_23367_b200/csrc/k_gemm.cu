@@ -56,8 +56,13 @@ static void gemm2_mode(int gemm_mode, int mt, const Gemm2Args& a, const TfSplit&
   if (gemm_mode == PRISM_GEMM_TF32X3 && MODE != G2_SIGMA) {
     constexpr int M2 = MODE == G2_SIGMA ? G2_ADMM : MODE;
     TfUniverse u{tf.Bt_hi, tf.Bt_lo, tf.Bp_hi, tf.Bp_lo};
-    dim3 grid((unsigned)((a.N + T2_TN - 1) / T2_TN), (a.nact + T2_TM - 1) / T2_TM);
-    MT_SWITCH(mt, k_gemm2_tf32<MT, M2><<<grid, 128, t2_smem(8 * MT), st>>>(a, u));
+    // tiles per CTA: about two waves of CTAs at two CTAs per SM (the split of V is amortised over the CTA's tiles)
+    const int64_t ntile = (a.N + T2_TN - 1) / T2_TN, ta = (a.nact + T2_TM - 1) / T2_TM;
+    int tpc = (int)((ntile * ta + (int64_t)4 * tf.sm_count - 1) / ((int64_t)4 * tf.sm_count));
+    if (tpc < 1) tpc = 1;
+    if (tpc > 16) tpc = 16;
+    dim3 grid((unsigned)((ntile + tpc - 1) / tpc), (unsigned)ta);
+    MT_SWITCH(mt, k_gemm2_tf32<MT, M2><<<grid, 256, t2_smem(8 * MT), st>>>(a, u, tpc));
   } else if (gemm_mode == 1 || gemm_mode == 2) {
     dim3 grid((unsigned)((a.N + 127) / 128), a.nact);
     if (gemm_mode == PRISM_GEMM_FP32_EXPERIMENT) k_gemm2_ref<MODE, true><<<grid, 128, 0, st>>>(a); else k_gemm2_ref<MODE, false><<<grid, 128, 0, st>>>(a);

@@ -7,7 +7,7 @@
 
 #include "kernels.h"
 
-#define PRISM_VERSION_STR "prism-b200 r2 (sm_100a, fp64 DMMA factor GEMMs, cluster-resident fused projection with DSMEM reductions)"
+#define PRISM_VERSION_STR "prism-b200 r2 (sm_100a; factor GEMMs: 3xTF32 tensor path or fp64 DMMA; fused projection: cluster-resident / streaming pair)"
 
 static const int kMT[] = {2, 4, 7, 8, 13, 16};
 static int pick_mt(int k) {
@@ -19,7 +19,7 @@ extern "C" void prism_default_settings(prism_settings* s) {
   if (!s) return;
   memset(s, 0, sizeof(*s));
   s->eps_rel = 1e-6; s->eps_abs = 0.0; s->max_iter = 4000; s->check_every = 10; s->first_check = 40; s->adapt_rho = 1;
-  s->alpha = 1.6; s->rho_scale = 100.0; s->gemm_precision = PRISM_GEMM_FP64_TENSOR; s->profile = 0;
+  s->alpha = 1.6; s->rho_scale = 100.0; s->gemm_precision = PRISM_GEMM_TF32X3; s->profile = 0;
   s->time_limit_ms = 0.0; s->deadline_ms = 0.0; s->prox_window_mult = 32.0; s->warm_w = nullptr; s->warm_duals = nullptr;
 }
 extern "C" const char* prism_last_error(void) { return g_err; }
@@ -98,7 +98,7 @@ struct Launcher {
     begin(PRISM_K_GEMM1);
     end(gemm1_launch(gemm_mode, mt, p->nchunk, p->kp, a, tf(), st));
   }
-  TfSplit tf() const { return TfSplit{p->Bt_hi, p->Bt_lo, p->Bp_hi, p->Bp_lo}; }
+  TfSplit tf() const { return TfSplit{p->Bt_hi, p->Bt_lo, p->Bp_hi, p->Bp_lo, p->sm_count}; }
   void gemm2(int mode, const Gemm2Args& a) {
     begin(PRISM_K_GEMM2);
     end(gemm2_launch(gemm_mode, mt, mode, a, tf(), st));

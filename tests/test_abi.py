@@ -37,7 +37,7 @@ def test_default_settings_and_version(lib):
     from paper_2606_23367_b200 import binding
     s = binding.default_settings()
     assert s.eps_rel == 1e-6 and s.max_iter == 4000 and s.check_every == 10 and s.alpha == 1.6 and s.rho_scale == 100.0
-    assert s.adapt_rho == 1 and s.gemm_precision == 0 and s.profile == 0 and s.eps_abs == 0.0 and s.first_check == 40
+    assert s.adapt_rho == 1 and s.gemm_precision == 3 and s.profile == 0 and s.eps_abs == 0.0 and s.first_check == 40
     assert not s.warm_w and not s.warm_duals
     assert "sm_100a" in binding.version()
 
