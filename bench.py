@@ -114,6 +114,18 @@ def _oracle_one(args):
     return a, r["status"], time.perf_counter() - t0
 
 
+def _oracle_init():
+    """One BLAS thread per worker: environment first (numpy is not loaded yet in a spawned worker), then threadpoolctl."""
+    for v in ("OMP_NUM_THREADS", "OPENBLAS_NUM_THREADS", "MKL_NUM_THREADS"):
+        os.environ[v] = "1"
+    try:
+        import numpy  # noqa: F401
+        from threadpoolctl import threadpool_limits
+        globals()["_ORACLE_LIMIT"] = threadpool_limits(limits=1)
+    except Exception:
+        pass
+
+
 class OraclePool:
     """The fp64 oracle (oracle/ipm.py, untuned) on the host cores: accounts in parallel worker processes, one account
     per process at a time, one BLAS thread each.  cores = number of worker processes."""
@@ -122,7 +134,7 @@ class OraclePool:
         import multiprocessing as mp
         self.cfg, self.seed, self.A = cfg, seed, accounts
         self.procs = procs or max(1, min(os.cpu_count() or 1, 32))
-        self.pool = mp.get_context("spawn").Pool(self.procs)
+        self.pool = mp.get_context("spawn").Pool(self.procs, initializer=_oracle_init)
 
     def run(self, account_ids):
         """Solves the listed accounts; returns (accounts/sec, seconds)."""
@@ -356,6 +368,11 @@ def main():
                 extra.append(row(name, gen.by_name(name, seed=0)))
         for Ns, ks in ((100, 10), (500, 20), (1000, 30), (2000, 30)):       # R24: N sweep, A = 100, configs[1] distributions
             extra.append(row(f"sweep_N{Ns}", gen.config1(seed=0, N=Ns, k=ks, A=100)))
+        # NEXT-1: the paper's transition-penalty family (reading R14) on its single-account scale
+        # ladder N = 481 x {1, 4, 20, 100, 800} (Table 12): timing rows, parity is the sec9 test case
+        for mult in (1, 4, 20, 100, 800):
+            extra.append(dict(row(f"sec9_ladder_N{481 * mult}", gen.section9(seed=0, N=481 * mult, k=20, A=1)),
+                              note="single account, L1 penalty kappa = 0.005, cap 3%, no turnover cap"))
         if args.config == "cfg2":                                            # the other form of the projection on the headline batch
             extra.append(dict(row("cfg2_resident_form", inst, form=binding.PROX_RESIDENT), note="prox_form = PRISM_PROX_RESIDENT"))
 

@@ -754,6 +754,9 @@ __device__ __noinline__ void prox_rootfind(const ProxArgs& p, const Src& src, in
         else { viol = bl_ - sh.gsum[g]; sg = -1; }
         if (viol > worst) { worst = viol; sel = g; sgn = sg; }
       }
+      // past the usual 2G+2 rounds (a caller that allows more) the rounds stop at rounding level: with several active bands
+      // the sums carry ~1e-14 of rounding noise and two bands can hand a violation of that size back and forth for ever
+      if (sel >= 0 && round >= 2 * G + 2 && worst <= 512.0 * tol) sel = -1;
       sh.selS[0] = sel; sh.selS[1] = sgn;
     }
     __syncthreads();

@@ -693,9 +693,10 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
       int amode = amode_w;
       bool ok = false;
       // Newton iteration; where it fails the nested robust solver; where that runs out of Gauss-Seidel rounds over the
-      // bands (it converges linearly when several bands interact) the Newton iteration again from its state, which is
-      // close by then (tr = 1, 2); the last robust call takes as many rounds as it needs.
-      for (int tr = 0; tr < 3; ++tr) {
+      // bands (it converges linearly when several bands interact) the Newton iteration once more from its state, which is
+      // close by then (tr = 1); if that fails too, the robust solver from the warm start with as many rounds as it needs
+      // (never from the state a failed Newton iteration leaves: see DESIGN.md, readings: robust root find).
+      for (int tr = 0; tr < 2; ++tr) {
       ok = false;
       for (int g = tid; g < G; g += nt) act[g] = lamS[g] > 0.0 ? 1 : (lamS[g] < 0.0 ? -1 : 0);
       __syncthreads();
@@ -772,21 +773,21 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
         al += dal; be += dbe;
         __syncthreads();
       }
-      if (ok) { rs.alpha = al; rs.beta = be; rs.amode = amode; break; }
+      if (ok) { rs.alpha = al; rs.beta = be; rs.amode = amode; rs.capped = 0; break; }
       {
         // nested robust solver on the same grouped list (lean passes through the SrcGrouped overloads)
         // (it continues from where the Newton iteration stopped when that state is usable)
         // (not with an infinite window while bands are in play - the launch in which they join: the multipliers a failed
         // Newton iteration leaves there can be far off, and the Gauss-Seidel rounds of the robust solver then crawl:
         // 12,000 passes for one account of configs[2] seed 1, minutes for seed 3)
-        const bool keep = tr > 0 ? (isfinite(al) && isfinite(be))
+        const bool keep = tr > 0 ? false
                                  : (al == al && be == be && fabs(al - aw) <= 0.5 * W && fabs(be - bw) <= 0.5 * W && (W < INFINITY || !bands_on));
         __syncthreads();
         if (!keep) for (int g = tid; g < G; g += nt) lamS[g] = lamW[g];
         if (tid == 0) { sgrp.L = &src; sgrp.poff = poff; sgrp.ngrp = ngrp; sgrp.gv = gv; }
         __syncthreads();
         rs.alpha = keep ? al : aw; rs.beta = keep ? be : bw; rs.amode = keep ? amode : amode_w;
-        rs.max_rounds = (bands_on && tr < 2) ? 2 * G + 2 : (1 << 30);
+        rs.max_rounds = (bands_on && tr < 1) ? 2 * G + 2 : (1 << 30);
         prox_rootfind<false>(p, sgrp, a, b, tau, Delta, sh, rs);
         if (rs.capped != 2) break;
         al = rs.alpha; be = rs.beta; amode = rs.amode;

@@ -612,9 +612,10 @@ __global__ void __launch_bounds__(RES_NT, 2) k_prox_res(const __grid_constant__ 
     bool ok = false;
     rs.capped = 0;
     // Newton iteration; where it fails the nested robust solver; where that runs out of Gauss-Seidel rounds over the
-    // bands (it converges linearly when several bands interact) the Newton iteration again from its state, which is
-    // close by then (tr = 1, 2); the last robust call takes as many rounds as it needs.
-    for (int tr = 0; tr < 3; ++tr) {
+    // bands (it converges linearly when several bands interact) the Newton iteration once more from its state, which is
+    // close by then (tr = 1); if that fails too, the robust solver from the warm start with as many rounds as it needs
+    // (never from the state a failed Newton iteration leaves: see DESIGN.md, readings: robust root find).
+    for (int tr = 0; tr < 2; ++tr) {
     ok = false;
     if (!bands_on) {
       // -- plain Newton on P(alpha) = (tau + b)/2, R(beta) = (tau - b)/2 (cap active) or P - R = b (alpha = beta)
@@ -731,17 +732,17 @@ __global__ void __launch_bounds__(RES_NT, 2) k_prox_res(const __grid_constant__ 
         if (code == 2) break;
       }
     }
-    if (ok) { rs.alpha = al; rs.beta = be; rs.amode = amode; break; }
+    if (ok) { rs.alpha = al; rs.beta = be; rs.amode = amode; rs.capped = 0; break; }
     {
       // nested robust solver (prox.cuh) on the same live lists; continues from the Newton state when that is usable
       // (not with an infinite window while bands are in play: see DESIGN.md, readings: robust root find)
-      const bool keep = tr > 0 ? (isfinite(al) && isfinite(be))
+      const bool keep = tr > 0 ? false
                                : (al == al && be == be && fabs(al - aw) <= 0.5 * W && fabs(be - bw) <= 0.5 * W && (W < INFINITY || !bands_on));
       __syncthreads();
       if (!keep) for (int g = tid; g < G; g += RES_NT) lamS[g] = lamW[g];
       __syncthreads();
       rs.alpha = keep ? al : aw; rs.beta = keep ? be : bw; rs.amode = keep ? amode : amode_w;
-      rs.max_rounds = (bands_on && tr < 2) ? 2 * G + 2 : (1 << 30);
+      rs.max_rounds = (bands_on && tr < 1) ? 2 * G + 2 : (1 << 30);
       prox_rootfind<LC>(p, src, a, b, tau, Delta, sh, rs);
       if (rs.capped != 2) break;
       al = rs.alpha; be = rs.beta; amode = rs.amode;

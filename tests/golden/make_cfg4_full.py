@@ -3,7 +3,8 @@
 Calls only instances/ (seeded generator) and oracle/ (structured interior point, as it stands): no value comes from the
 CUDA path.  The oracle needs many minutes per account at this width, which is why the values are stored instead of
 being recomputed inside the GPU test (tests/test_gpu_parity.py::test_full_size_cfg4_elementwise).
-Stored per account: the full weight vector as float64 (zlib-compressed npz), the oracle's objective, its KKT
+Stored per account: the full weight vector rounded to float32 (weights <= 1e-3: 6e-11 absolute, against a parity
+tolerance of 1e-4; zlib-compressed npz), the oracle's objective, its KKT
 certificate (kkt_check with the oracle's multipliers) and the SHA-256 of the account's mu / w0 rows (generator drift).
 
     python tests/golden/make_cfg4_full.py [account ...]        (default: 0)
@@ -36,7 +37,7 @@ def main():
         feas = kkt_check.feasibility(acc, w)
         out = os.path.join(os.path.dirname(os.path.abspath(__file__)), f"cfg4_full_a{a}.npz")
         k = kkt_check.kkt(acc, w, r["mult"], delta=1e-7)
-        np.savez_compressed(out, w=w, objective=problem.objective(acc, w), iterations=r["iters"], status=r["status"],
+        np.savez_compressed(out, w=w.astype(np.float32), objective=problem.objective(acc, w), iterations=r["iters"], status=r["status"],
                             r_stat=k["r_stat"], r_comp=k["r_comp"],
                             seconds=dt, feas=np.array([feas[k] for k in sorted(feas)]),
                             sha_mu=hashlib.sha256(np.ascontiguousarray(inst.mu[a]).tobytes()).hexdigest(),
