@@ -144,6 +144,9 @@ typedef struct prism_settings {
   int32_t first_check;      /* no residual check before this many iterations (default 40): the first checks of a
                                cold start never pass and a check launch costs more than a plain one          */
   int32_t adapt_rho;        /* 1 => per-account rho adaptation at check iterations (default 1)                   */
+  int32_t adapt_start;      /* first iteration at which an account's rho may be adapted (default 200: typical
+                               accounts finish before, and adapting them earlier slows them down)               */
+  int32_t adapt_every;      /* minimum iterations between two adaptations of one account (default 100)           */
   double alpha;             /* over-relaxation in (0, 2) (default 1.6)                                           */
   double rho_scale;         /* initial c: rho_i = c gamma_a d_i (default 100)                                    */
   int32_t gemm_precision;   /* PRISM_GEMM_* (default PRISM_GEMM_TF32X3, chosen against the tolerance by measurement:

@@ -45,7 +45,8 @@ class Data(C.Structure):
 
 class Settings(C.Structure):
     _fields_ = [("eps_rel", C.c_double), ("eps_abs", C.c_double), ("max_iter", C.c_int32), ("check_every", C.c_int32),
-                ("first_check", C.c_int32), ("adapt_rho", C.c_int32), ("alpha", C.c_double), ("rho_scale", C.c_double),
+                ("first_check", C.c_int32), ("adapt_rho", C.c_int32), ("adapt_start", C.c_int32), ("adapt_every", C.c_int32),
+                ("alpha", C.c_double), ("rho_scale", C.c_double),
                 ("gemm_precision", C.c_int32), ("profile", C.c_int32), ("time_limit_ms", C.c_double),
                 ("deadline_ms", C.c_double), ("prox_window_mult", C.c_double), ("warm_w", C.c_void_p),
                 ("warm_duals", C.c_void_p)]

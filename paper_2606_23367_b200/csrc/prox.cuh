@@ -53,6 +53,7 @@ struct ProxArgs {
   // settings
   double eps, eps_abs;      // converged when r <= eps_abs + eps * scale for both residuals
   int32_t adapt, iter;
+  int32_t adapt_start, adapt_every;   // first iteration at which an account's rho may be adapted; minimum iterations between two
   double win_mult;         // next window = win_mult x (movement of the thresholds in this launch)
   double win_ratio;        // streaming pass: its (wide) window = win_ratio x the solve's (tight) window
   int32_t band_start;      // streaming form: group bands join the projection after this iteration (their multipliers are 0 before)
@@ -72,8 +73,6 @@ struct ProxArgs {
 };
 
 enum { PROX_CHECK = 1, PROX_FINAL = 2 };
-#define PRISM_ADAPT_START 200   // first iteration at which an account's rho may be adapted
-#define PRISM_ADAPT_EVERY 100   // minimum iterations between two adaptations of one account
 
 // Per-element constants of one launch, in "threshold space":  T = rho u - (kappa + c_buy),  Delta = 2 kappa + c_buy:
 //   buy_i(a)  = bl + clamp((T - a) / rho - bl, 0, wB)            a  = alpha + lambda_g
@@ -855,7 +854,7 @@ __device__ __forceinline__ void prox_body(const ProxArgs& p, int mode, Src& src,
     if (conv || bad) {
       finished = 1;
       if (tid == 0) p.ap.conv[a] = bad ? -1 : 1;
-    } else if (p.adapt && p.iter >= PRISM_ADAPT_START && p.iter - p.ap.nadapt[a] >= PRISM_ADAPT_EVERY) {
+    } else if (p.adapt && p.iter >= p.adapt_start && p.iter - p.ap.nadapt[a] >= p.adapt_every) {
       // H7: only accounts that are unusually slow are re-scaled (typical accounts finish before PRISM_ADAPT_START);
       // rho <- rho sqrt(r_p / r_d), clipped, applied when the two scaled residuals are out of balance
       const double ratio = sqrt(rp / fmax(rd, 1e-300));

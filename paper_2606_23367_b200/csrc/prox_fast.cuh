@@ -886,7 +886,7 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
       const bool conv = val[2] <= p.eps_abs + p.eps * fmax(val[0], val[1]) && val[3] <= p.eps_abs + p.eps * fmax(val[4], fmax(val[5], val[6])) &&
                         !rs.capped;                                          // never certify on an unfinished root find
       if (!(rp < INFINITY) || !(rd < INFINITY)) fallback = true;             // NaN / Inf: the generic path classifies it
-      else if (!conv && p.adapt && p.iter >= PRISM_ADAPT_START && p.iter - p.ap.nadapt[a] >= PRISM_ADAPT_EVERY) {
+      else if (!conv && p.adapt && p.iter >= p.adapt_start && p.iter - p.ap.nadapt[a] >= p.adapt_every) {
         const double ratio = sqrt(rp / fmax(rd, 1e-300));
         if (ratio > 3.0 || ratio < 1.0 / 3.0) fallback = true;               // rho changes: every asset is rewritten
         else if (tid == 0) p.ap.nadapt[a] = p.iter;

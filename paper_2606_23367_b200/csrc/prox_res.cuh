@@ -820,7 +820,7 @@ __global__ void __launch_bounds__(RES_NT, 2) k_prox_res(const __grid_constant__ 
     if (conv || bad) {
       finished = 1;
       if (tid == 0 && rank == 0) p.ap.conv[a] = bad ? -1 : 1;
-    } else if (p.adapt && p.iter >= PRISM_ADAPT_START && p.iter - nadapt_prev >= PRISM_ADAPT_EVERY) {
+    } else if (p.adapt && p.iter >= p.adapt_start && p.iter - nadapt_prev >= p.adapt_every) {
       const double ratio = sqrt(rp / fmax(rd, 1e-300));
       if (ratio > 3.0 || ratio < 1.0 / 3.0) {
         c_new = c * fmin(fmax(ratio, 0.2), 5.0);
