@@ -167,3 +167,20 @@ def test_sharded_solve_world_size_2_gloo(tmp_path):
                          capture_output=True, text=True, timeout=300)
     assert res.returncode == 0, res.stderr[-2000:]
     assert "rank0done" in res.stdout and "rank1done" in res.stdout
+
+
+def test_queue_layer_identity_and_summary():
+    """NEXT-3 host layer (paper_2606_23367_b200.queue_layer): the input identity is deterministic and account-specific, the
+    summary reproduces Table 8's columns from the audit records."""
+    from instances import gen
+    from paper_2606_23367_b200 import queue_layer as ql
+    inst = gen.config2(N=64, k=4, A=3, G=3)
+    ids = [ql.input_identity(inst, a) for a in range(3)]
+    assert len(set(ids)) == 3 and ids == [ql.input_identity(gen.config2(N=64, k=4, A=3, G=3), a) for a in range(3)]
+    inst.mu[1, 5] += 1e-9
+    assert ql.input_identity(inst, 1) != ids[1] and ql.input_identity(inst, 0) == ids[0]
+    recs = [ql.AuditRecord(a, a // 2, "i", "o", st, ql.STATUS_NAMES[st], 10, (0.0,) * 12, lat, 1.0, lat > 25.0, "b")
+            for a, (st, lat) in enumerate([(0, 10.0), (0, 10.0), (1, 20.0), (3, 30.0)])]
+    s = ql.summarise(recs)
+    assert s["accounts"] == 4 and s["completed"] == 4 and s["certified"] == 2 and s["missed_deadline_rate"] == 0.25
+    assert s["latency_max_ms"] == 30.0 and abs(s["accounts_per_s"] - 4 / 0.030) < 1e-9 and s["latency_p50_ms"] == 15.0

@@ -73,7 +73,7 @@ def _check_against_oracle(inst, r, W, res, accounts=None):
         mult = dict(nu=du[a, 0], theta=du[a, 1], lam_hi=du[a, 2:2 + G], lam_lo=du[a, 2 + G:2 + 2 * G])
         k = kkt_check.kkt(acc, w[a], mult, delta=1e-9)
         scale = max(np.max(np.abs(acc.mu)), 1e-12)
-        assert k["r_stat"] <= 1e-5 * scale * 10 and k["r_comp"] <= 1e-9 and k["min_multiplier"] >= -1e-15, k
+        assert k["r_stat"] <= 2e-5 * scale and k["r_comp"] <= 1e-9 and k["min_multiplier"] >= -1e-15, k   # observed: <= 7e-6 * scale
         assert abs(rs[a, 4] - k["r_stat"]) <= 1e-10 and abs(rs[a, 5] - k["r_comp"]) <= 1e-12
 
 
@@ -260,7 +260,7 @@ def test_full_size_sampled_accounts(cfg, n_sample, n_min):
     st = r.status.cpu().numpy(); rs = r.resid.cpu().numpy()
     assert (st == 0).all(), np.bincount(st)
     assert rs[:, 0:4].max() <= TOL_GATE and rs[:, 7].max() <= TOL_RES and rs[:, 8].max() <= TOL_RES
-    assert rs[:, 4].max() <= 1e-5 and rs[:, 5].max() <= 1e-9
+    assert rs[:, 4].max() <= 2e-6 and rs[:, 5].max() <= 1e-9   # r_stat observed <= 6.5e-7 on seeds 0-4
     rng = np.random.default_rng(0)
     sample = sorted(rng.choice(inst.A, size=n_sample, replace=False).tolist())
     kept, W, res = _oracle(inst, accounts=sample, pool=(cfg, 0))
@@ -281,7 +281,7 @@ def test_full_size_cfg4_properties():
     st = r.status.cpu().numpy(); rs = r.resid.cpu().numpy(); w = r.w.cpu().numpy(); du = r.duals.cpu().numpy()
     assert (st == 0).all(), np.bincount(st)
     assert rs[:, 0:4].max() <= TOL_GATE and rs[:, 7].max() <= TOL_RES and rs[:, 8].max() <= TOL_RES
-    assert rs[:, 4].max() <= 1e-5 and rs[:, 5].max() <= 1e-9
+    assert rs[:, 4].max() <= 2e-6 and rs[:, 5].max() <= 1e-9   # r_stat observed <= 6.5e-7 on seeds 0-4
     for a in (0, 17, 31):
         acc = problem.account_from_instance(inst, a)
         feas = kkt_check.feasibility(acc, w[a])
@@ -291,7 +291,7 @@ def test_full_size_cfg4_properties():
         assert abs(rs[a, 6] - fg) <= 1e-12 * max(1.0, abs(fg))
         k = kkt_check.kkt(acc, w[a], dict(nu=du[a, 0], theta=du[a, 1], lam_hi=du[a, 2:2], lam_lo=du[a, 2:2]), delta=1e-9)
         scale = max(np.max(np.abs(acc.mu)), 1e-12)
-        assert k["r_stat"] <= 1e-4 * scale and k["r_comp"] <= 1e-9 and k["min_multiplier"] >= -1e-15, k
+        assert k["r_stat"] <= 1e-5 * scale and k["r_comp"] <= 1e-9 and k["min_multiplier"] >= -1e-15, k   # observed: 1.2e-7
         assert abs(rs[a, 4] - k["r_stat"]) <= 1e-10
     P.close()
 
@@ -479,3 +479,25 @@ def test_projection_kernel_alone_against_its_definition(name, sd):
             assert k["r_stat"] <= 1e-12 * scale and k["r_comp"] <= 1e-12 and k["min_multiplier"] >= 0.0, (name, form, a, k)
             assert problem.objective(pa, z[a]) <= problem.objective(pa, Z[a]) + 1e-12
         P.close()
+
+
+def test_queue_layer_batches_deadline_and_audit_records():
+    """NEXT-3: a queue of 7 accounts in batches of 3 through paper_2606_23367_b200.queue_layer - the same
+    weights as one batch, one audit record per account (input / output identity, status, build id), and the deadline
+    semantics of Table 8: with an impossible deadline every account is a missed deadline."""
+    import hashlib
+    import paper_2606_23367_b200 as pr
+    from paper_2606_23367_b200 import queue_layer as ql
+    inst = gen.config1(seed=5, N=320, k=8, A=7)
+    P, r = _solve_gpu(inst)
+    W, recs = ql.run_queue(inst, batch_size=3)
+    assert len(recs) == 7 and [x.batch for x in recs] == [0, 0, 0, 1, 1, 1, 2] and all(x.status == 0 for x in recs)
+    assert np.max(np.abs(W - r.w.cpu().numpy())) <= 1e-12                       # batch composition does not change an account's answer
+    assert all(x.output_sha256 == hashlib.sha256(np.ascontiguousarray(W[x.account]).tobytes()).hexdigest() for x in recs)
+    assert len({x.input_sha256 for x in recs}) == 7 and all(x.build_id == pr.version() for x in recs)
+    s = ql.summarise(recs)
+    assert s["completed"] == 7 and s["certified"] == 7 and s["missed_deadline_rate"] == 0.0 and s["latency_p99_ms"] <= s["queue_ms"]
+    _, late = ql.run_queue(inst, batch_size=3, deadline_ms=1e-3)
+    assert all(x.missed_deadline for x in late) and ql.summarise(late)["missed_deadline_rate"] == 1.0
+    assert all(x.status in (0, 3) for x in late)                                  # finished, after the deadline: LATE (or done at once)
+    P.close()
