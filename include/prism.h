@@ -93,7 +93,8 @@ enum {
   PRISM_R_DUAL = 8,     /* scaled dual residual of the splitting at exit   (solver only, else NaN)              */
   PRISM_R_TURNOVER_VALUE = 9, /* ||w-w0||_1                                                                      */
   PRISM_R_RHO = 10,     /* final rho scale c_a (solver only, else NaN)                                           */
-  PRISM_R_RESERVED = 11,
+  PRISM_R_RESERVED = 11,/* 0, or why the constraint-set precheck returned the account at iteration 0 with w = w0 and status
+                           NO_FEASIBLE: 1 box / budget, 2 turnover cap below the forced trades, 3 group bands        */
   PRISM_NRES = 12
 };
 
@@ -157,6 +158,13 @@ typedef struct prism_settings {
   double deadline_ms;       /* 0 => none; accounts finishing after it get PRISM_STATUS_LATE                      */
   double prox_window_mult;  /* projection: next live-list window = this x the last movement of the thresholds
                                (default 32)                                                                   */
+  int32_t sample_until;     /* streaming form of the projection: plain (non-check) launches of iterations < sample_until,
+                               while the group bands are still out of the projection (the first 21 iterations of a cold
+                               start), find the thresholds on a SAMPLE of the live assets (every stride-th, scaled) and
+                               apply them to all - an inexact prox.  The splitting's only carried state is v, so this
+                               perturbs the path of the iteration, not its fixed point; check / final launches are always
+                               exact.  0 => never (default: see prism_default_settings)                          */
+  int32_t reserved0;
   /* warm start - the repeated-run lane (cold rows "pass no previous solution"): previous weights and
      multipliers of the same accounts, e.g. the w_out / duals_out of an earlier call.  Both NULL => cold start.       */
   const double* warm_w;     /* device, A x N, or NULL                                                            */

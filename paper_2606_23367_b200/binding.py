@@ -48,7 +48,8 @@ class Settings(C.Structure):
                 ("first_check", C.c_int32), ("adapt_rho", C.c_int32), ("adapt_start", C.c_int32), ("adapt_every", C.c_int32),
                 ("alpha", C.c_double), ("rho_scale", C.c_double),
                 ("gemm_precision", C.c_int32), ("profile", C.c_int32), ("time_limit_ms", C.c_double),
-                ("deadline_ms", C.c_double), ("prox_window_mult", C.c_double), ("warm_w", C.c_void_p),
+                ("deadline_ms", C.c_double), ("prox_window_mult", C.c_double), ("sample_until", C.c_int32),
+                ("reserved0", C.c_int32), ("warm_w", C.c_void_p),
                 ("warm_duals", C.c_void_p)]
 
 

@@ -23,6 +23,10 @@ cudaError_t init_accounts_launch(const InitArgs& a, cudaStream_t st) {
   k_init_accounts<<<a.A, 256, 0, st>>>(a);
   return cudaGetLastError();
 }
+cudaError_t precheck_launch(const PrecheckArgs& a, cudaStream_t st) {
+  k_precheck<<<a.A, 256, 0, st>>>(a);
+  return cudaGetLastError();
+}
 cudaError_t warm_start_launch(const WarmArgs& a, cudaStream_t st) {
   k_warm_start<<<dim3((unsigned)((a.N + 255) / 256), a.A), 256, 0, st>>>(a);
   return cudaGetLastError();

@@ -23,6 +23,7 @@ cudaError_t setup_shared_launch(const void* B, int is32, const double* d, int64_
                                 double* Bt, double* invd, cudaStream_t st);
 cudaError_t gram_launch(const double* Bt, int64_t ldn, const double* invd, int64_t N, int kp, double* gram, cudaStream_t st);
 cudaError_t init_accounts_launch(const InitArgs& a, cudaStream_t st);
+cudaError_t precheck_launch(const PrecheckArgs& a, cudaStream_t st);     // NEXT-4: accounts whose constraint set is empty by inspection
 cudaError_t warm_start_launch(const WarmArgs& a, cudaStream_t st);
 cudaError_t factor_launch(const double* gram, const double* f, const double* gamma, const AccountParams& ap, int A, int k,
                           int kp, double* Sinv, cudaStream_t st);

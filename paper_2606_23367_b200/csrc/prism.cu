@@ -18,7 +18,7 @@ static int pick_mt(int k) {
 extern "C" void prism_default_settings(prism_settings* s) {
   if (!s) return;
   memset(s, 0, sizeof(*s));
-  s->eps_rel = 1e-6; s->eps_abs = 0.0; s->max_iter = 4000; s->check_every = 10; s->first_check = 40; s->adapt_rho = 1; s->adapt_start = 200; s->adapt_every = 100;
+  s->eps_rel = 1e-6; s->eps_abs = 0.0; s->max_iter = 4000; s->check_every = 10; s->first_check = 40; s->adapt_rho = 1; s->adapt_start = 200; s->adapt_every = 100; s->sample_until = 0; s->reserved0 = 0;
   s->alpha = 1.6; s->rho_scale = 100.0; s->gemm_precision = PRISM_GEMM_TF32X3; s->profile = 0;
   s->time_limit_ms = 0.0; s->deadline_ms = 0.0; s->prox_window_mult = 32.0; s->warm_w = nullptr; s->warm_duals = nullptr;
 }
@@ -300,6 +300,7 @@ static ProxArgs make_prox_args(prism_problem* p, const prism_settings& s, double
   a.ap = p->ap; a.w_out = w_out; a.duals = p->duals; a.resid = p->resid; a.counters = p->counters;
   a.eps = s.eps_rel; a.eps_abs = s.eps_abs;
   a.adapt = s.adapt_rho; a.iter = 0; a.ldw = p->ldn;
+  a.sample_until = s.warm_w ? 0 : s.sample_until;       // a warm start has its bands in from the first launch
   a.adapt_start = s.adapt_start; a.adapt_every = s.adapt_every < 1 ? 1 : s.adapt_every;
   a.lraw = p->lraw; a.lcomp = p->lcomp; a.lcnt = p->lcnt; a.cbin = p->cbin; a.chkp = p->chkp; a.lflag = p->lflag;
   a.S = p->S; a.capw = p->capw; a.slice_len = p->slice_len; a.ldc = p->ldc;
@@ -378,6 +379,16 @@ extern "C" int prism_solve_batch(prism_problem* p, const prism_settings* sp, voi
   ia.group_id = p->d.group_id; ia.v = p->v; ia.gw0 = p->gw0; ia.lamG = p->lamG; ia.ap = p->ap; ia.rho_scale = s.rho_scale;
   L.begin(PRISM_K_OTHER);
   L.end(init_accounts_launch(ia, st));
+  {
+    PrecheckArgs pc;
+    memset(&pc, 0, sizeof(pc));
+    pc.N = p->N; pc.A = A; pc.G = G; pc.max_lots = p->max_lots; pc.w0 = p->d.w0; pc.lo = p->d.lo; pc.hi = p->d.hi; pc.hi_full = p->d.hi_full;
+    pc.tau = p->d.tau; pc.band_lo = p->d.band_lo; pc.band_hi = p->d.band_hi; pc.lot_width = p->d.lot_width; pc.excl = p->d.excl;
+    pc.lot_count = p->d.lot_count; pc.group_id = p->d.group_id; pc.w_out = w_out; pc.resid = p->resid; pc.duals = p->duals; pc.ap = p->ap;
+    pc.counters = p->counters;
+    L.begin(PRISM_K_OTHER);
+    L.end(precheck_launch(pc, st));
+  }
   if (s.warm_w) {
     // warm start from previous weights w and multipliers: at a fixed point of the splitting x = z = w and the dual is
     // y = -(P w + q) = mu - gamma Sigma (w - w_b), so the carried state is v = w + y / rho; thresholds from the duals

@@ -53,6 +53,7 @@ struct ProxArgs {
   // settings
   double eps, eps_abs;      // converged when r <= eps_abs + eps * scale for both residuals
   int32_t adapt, iter;
+  int32_t sample_until;    // streaming form: plain launches of iterations < sample_until (bands still out) use the sampled root find
   int32_t adapt_start, adapt_every;   // first iteration at which an account's rho may be adapted; minimum iterations between two
   double win_mult;         // next window = win_mult x (movement of the thresholds in this launch)
   double win_ratio;        // streaming pass: its (wide) window = win_ratio x the solve's (tight) window

@@ -262,6 +262,7 @@ struct SrcLiveG {
   const unsigned long long* cbin;   // shared memory: fixed-point totals of the assets that are not in the list
   int Gb;
   double cPt, cRt;
+  double scale;                     // 1, or the stride of a SAMPLED list (every stride-th live asset stands for stride of them)
   template <int NV, int OP>
   __device__ __forceinline__ void reduce(double (&val)[NV], double* scratch) const { block_reduce<NV, OP>(val, scratch); }
   __device__ __forceinline__ double cP() const { return cPt; }
@@ -388,7 +389,7 @@ __device__ __forceinline__ void root_pass(const SrcLiveG& src, const int* poff, 
       root_entry(src, ea, eb, a0, b0, sp, sr, slp, slr);
     }
     sp = warp_sum(sp); sr = warp_sum(sr); slp = warp_sum(slp); slr = warp_sum(slr);
-    if (lane == 0) { gv[4 * q] = sp; gv[4 * q + 1] = sr; gv[4 * q + 2] = slp; gv[4 * q + 3] = slr; }
+    if (lane == 0) { const double sc = src.scale; gv[4 * q] = sp * sc; gv[4 * q + 1] = sr * sc; gv[4 * q + 2] = slp * sc; gv[4 * q + 3] = slr * sc; }
   }
   __syncthreads();
 }
@@ -468,7 +469,7 @@ __device__ __noinline__ void prox_eval_multi(const SrcGrouped& s, const double* 
   block_reduce<PROX_KSEC, 0>(sp, scratch);
   block_reduce<PROX_KSEC, 0>(sr, scratch);
 #pragma unroll
-  for (int k = 0; k < PROX_KSEC; ++k) { outP[k] = sp[k] + L.cPt; outR[k] = sr[k] + L.cRt; }
+  for (int k = 0; k < PROX_KSEC; ++k) { outP[k] = sp[k] * L.scale + L.cPt; outR[k] = sr[k] * L.scale + L.cRt; }
 }
 
 template <bool CHECK>
@@ -569,6 +570,12 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
     const LiveEnt* lr = p.lraw + (int64_t)a * nsub * p.capw;
     const int32_t* lcw = p.lcnt + (int64_t)p.A * nsub + (int64_t)a * nsub;   // lengths of the backs
     int nlist = nsub, nraw = 0, j_beg = 0, j_end = 0;
+    // Sampled root find (prism_settings.sample_until): plain launches of the first iterations, while the bands are still
+    // out of the projection, solve for the thresholds on every stride-th live asset (each standing for stride of them,
+    // stride such that the sample fits the shared-memory list) and apply them to all: an inexact prox where exactness buys
+    // nothing - every asset is still live then and an exact solve walks the 9,800-entry lists 7-24 times.
+    const bool sampm = !exact && !bands_on && p.iter < p.sample_until;
+    int stride = 1;
     auto scan_lists = [&](int level) {
       nlist = level ? 2 * nsub : nsub;
       __syncthreads();
@@ -587,8 +594,10 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
       }
       __syncthreads();
       nraw = offs[nlist];
-      const int segw = (((nraw + nw - 1) / nw) + 31) & ~31;
-      j_beg = min(nraw, wid * segw); j_end = min(nraw, (wid + 1) * segw);
+      stride = (sampm && nraw > ROOT_SCAP) ? (nraw + ROOT_SCAP - 1) / ROOT_SCAP : 1;
+      const int nsmp = (nraw + stride - 1) / stride;       // the sort and the solve see samples j = 0 .. nsmp - 1 (entry j * stride)
+      const int segw = (((nsmp + nw - 1) / nw) + 31) & ~31;
+      j_beg = min(nsmp, wid * segw); j_end = min(nsmp, (wid + 1) * segw);
     };
     auto locate = [&](int j) -> const LiveEnt* {         // entry j of the sequence
       int lo = 0, hi = nlist;
@@ -609,7 +618,7 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
           for (int u = 0; u < 4; ++u) {
             const int j = j0 + 32 * u + lane;
             g4[u] = 0x100 + lane;
-            if (j < j_end) g4[u] = (int)((__ldg(&locate(j)->meta) >> PROX_META_IDX_BITS) & 0xffu);
+            if (j < j_end) g4[u] = (int)((__ldg(&locate(j * stride)->meta) >> PROX_META_IDX_BITS) & 0xffu);
           }
 #pragma unroll
           for (int u = 0; u < 4; ++u) {
@@ -637,6 +646,7 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
         for (int g = 0; g < Gb; ++g) { sp += ubin[g]; sr += ubin[Gb + g]; }
         src.lo_a = src_lo; src.hi_a = src_hi; src.ent = n <= ROOT_SCAP ? ents : p.lcomp + (int64_t)a * p.ldc; src.nsl = 1; src.stride = 0; src.cnt[0] = n;
         src.cbin = ubin; src.Gb = Gb; src.cPt = (double)sp * PRISM_FIX_INV; src.cRt = (double)sr * PRISM_FIX_INV;
+        src.scale = (double)stride;
       }
       __syncthreads();
       LiveEnt* dst = const_cast<LiveEnt*>(src.ent);
@@ -646,7 +656,7 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
         for (int u = 0; u < 4; ++u) {
           const int j = j0 + 32 * u + lane;
           ea[u] = make_double2(0, 0); eb[u] = make_double2(0, 0);
-          if (j < j_end) { const LiveEnt* e = locate(j); ea[u] = __ldg((const double2*)e); eb[u] = __ldg((const double2*)e + 1); }
+          if (j < j_end) { const LiveEnt* e = locate(j * stride); ea[u] = __ldg((const double2*)e); eb[u] = __ldg((const double2*)e + 1); }
         }
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
@@ -796,7 +806,7 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
       double mv_l = 0.0;
       for (int g = 0; g < G; ++g) mv_l = fmax(mv_l, fabs(lamS[g] - lamW[g]));
       mv = fmax(fmax(fabs(rs.alpha - aw), fabs(rs.beta - bw)), mv_l);
-      if (mv <= 0.5 * fmin(Wf, W)) break;
+      if (stride > 1 || mv <= 0.5 * fmin(Wf, W)) break;     // (a sampled solve is inexact by design: no second level, no every-asset path)
       if (!(Wf < INFINITY)) { fallback = true; break; }   // left the streaming window (or NaN): the dead assets were misjudged
       Wf = INFINITY;
       __syncthreads();

@@ -71,6 +71,78 @@ __global__ void k_init_accounts(InitArgs p) {
   }
 }
 
+// NEXT-4, the cheap half: an account whose CONSTRAINT SET is empty by inspection is returned at once
+// instead of burning max_iter iterations.  Necessary conditions, each exact for the constraints it looks at (checked with
+// a slack of 1e-9): (1) box and budget: sum lo' <= 1 <= sum hi (lo' = the sell floor: with lots w0 - held lots);
+// (2) turnover: forced buys Pf (w0 < lo) and forced sells Rf (w0 > hi, exclusions) plus the trade that then closes the
+// budget, Pf + Rf + |b - (Pf - Rf)|, must fit tau; (3) bands: every band must meet its group's reachable range
+// [sum lo', sum hi], and the bands cut to those ranges must leave room for the budget.  A failed condition is a proof
+// that no w satisfies the account's constraints (this is NOT the paper's status 4 claim about an optimisation run,
+// PAPER.md:491; it is a statement about the data); the account is marked done with conv = 2, w_out = w0, zero
+// multipliers, and the reason in column PRISM_R_RESERVED (1 box / budget, 2 turnover, 3 bands).  Its status then follows
+// from the gates of w0 like any other return (NO_FEASIBLE).  Bands and turnover JOINTLY are not checked (that is an LP).
+__global__ void __launch_bounds__(256) k_precheck(PrecheckArgs p) {
+  __shared__ double scratch[6 * 32];
+  __shared__ double gs[2 * 8 * PRISM_MAX_GROUPS];
+  __shared__ int bad_s;
+  const int a = blockIdx.x, tid = threadIdx.x, G = p.G;
+  const int64_t row = (int64_t)a * p.N;
+  for (int g = tid; g < 2 * 8 * G; g += blockDim.x) gs[g] = 0.0;
+  __syncthreads();
+  const double lo_a = p.lo[a], hi_a = p.hi[a];
+  double s_w0 = 0, s_lo = 0, s_hi = 0, Pf = 0, Rf = 0;
+  for (int64_t i0 = 0; i0 < p.N; i0 += blockDim.x) {
+    const int64_t i = i0 + tid;
+    const bool valid = i < p.N;
+    double lo = 0.0, hi = 0.0;
+    if (valid) {
+      const double w = p.w0[row + i];
+      lo = lo_a; hi = p.hi_full ? p.hi_full[row + i] : hi_a;
+      if (p.excl && p.excl[row + i]) { lo = 0.0; hi = 0.0; }
+      if (p.lot_count && p.lot_count[row + i] > 0) {           // sells limited to the lots held (reading R10)
+        double Q = 0.0;
+        for (int l = 0; l < p.lot_count[row + i]; ++l) Q += p.lot_width[(row + i) * PRISM_MAX_LOTS + l];
+        lo = fmax(lo, w - Q);
+      }
+      s_w0 += w; s_lo += lo; s_hi += hi;
+      Pf += fmax(lo - w, 0.0); Rf += fmax(w - hi, 0.0);
+    }
+    if (G) {
+      const int g = valid ? p.group_id[i] : 0;
+      warp_group_add(gs, G, g, lo, valid);
+      warp_group_add(gs + 8 * G, G, g, hi, valid);
+    }
+  }
+  double val[5] = {s_w0, s_lo, s_hi, Pf, Rf};
+  block_reduce<5, 0>(val, scratch);
+  if (tid == 0) {
+    const double eps = 1e-9, b = 1.0 - val[0];
+    const double tau = p.tau ? p.tau[a] : INFINITY;
+    int bad = 0;
+    if (val[1] > 1.0 + eps || val[2] < 1.0 - eps) bad = 1;
+    else if (val[3] + val[4] + fabs(b - (val[3] - val[4])) > tau + eps) bad = 2;
+    else if (G) {
+      double slo = 0.0, shi = 0.0;
+      for (int g = 0; g < G; ++g) {
+        const double smin = group_total(gs, G, g), smax = group_total(gs + 8 * G, G, g);
+        const double bl = p.band_lo[(int64_t)a * G + g], bh = p.band_hi[(int64_t)a * G + g];
+        if (bl > smax + eps || bh < smin - eps) bad = 3;
+        slo += fmax(bl, smin); shi += fmin(bh, smax);
+      }
+      if (slo > 1.0 + eps || shi < 1.0 - eps) bad = 3;
+    }
+    bad_s = bad;
+    if (bad) {
+      p.ap.done[a] = 1; p.ap.conv[a] = 2; p.ap.iters[a] = 0;
+      atomicAdd(&p.counters[0], 1);
+      p.resid[(int64_t)a * PRISM_NRES + PRISM_R_RESERVED] = (double)bad;
+      for (int q = 0; q < PRISM_NDUAL(G); ++q) p.duals[(int64_t)a * PRISM_NDUAL(G) + q] = 0.0;
+    }
+  }
+  __syncthreads();
+  if (bad_s) for (int64_t i = tid; i < p.N; i += blockDim.x) p.w_out[row + i] = p.w0[row + i];
+}
+
 // Warm start: at a fixed point of the splitting x = z = w and y = -(P w + q) = mu - gamma Sigma (w - w_b), so the
 // carried state is v = w + y / rho with rho_i = c gamma d_i; thresholds alpha = nu + theta, beta = nu - theta and the
 // band multipliers lambda_g = lam_hi - lam_lo come from the given duals (prism.h: PRISM_NDUAL layout).

@@ -28,3 +28,13 @@ struct WarmArgs {
   double *v, *lamG;
   AccountParams ap;
 };
+
+// constraint-set precheck (k_precheck): necessary conditions for the feasible set of one account to be non-empty
+struct PrecheckArgs {
+  int64_t N; int32_t A, G, max_lots;
+  const double *w0, *lo, *hi, *hi_full, *tau, *band_lo, *band_hi, *lot_width;
+  const uint8_t *excl, *lot_count, *group_id;
+  double *w_out, *resid, *duals;
+  AccountParams ap;
+  int32_t* counters;
+};

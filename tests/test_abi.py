@@ -55,7 +55,7 @@ def test_header_constants_match_binding():
     assert int(flags["PRISM_BENCHMARK_SHIFT"]) == gen.F_BENCHMARK_SHIFT and int(flags["PRISM_EXCLUSION"]) == gen.F_EXCLUSION
     assert len(binding.STATUS_NAMES) == 6                                               # Table 14
     # struct sizes (natural alignment) as the C compiler lays them out
-    assert C.sizeof(binding.Settings) == 104 and C.sizeof(binding.ConstraintSet) == 16
+    assert C.sizeof(binding.Settings) == 112 and C.sizeof(binding.ConstraintSet) == 16
     assert C.sizeof(binding.Data) == 22 * 8
 
 

@@ -13,6 +13,11 @@ pytestmark = pytest.mark.gpu
 TOL_W, TOL_GAP, TOL_RES, TOL_GATE = 1e-4, 1e-6, 1e-6, 1e-6
 
 
+def torch_w0(inst, r):
+    import torch
+    return torch.as_tensor(inst.w0, device=r.w.device)
+
+
 def _solve_gpu(inst, prox_form=0, **kw):
     import paper_2606_23367_b200 as pr
     P = pr.Problem(inst, prox_form=prox_form)
@@ -233,7 +238,18 @@ def test_status_vocabulary():
     inf.tau[0] = 1e-6                                        # infeasible with exclusions held: no accepted feasible return
     Pi, ri = _solve_gpu(inf, max_iter=200)
     assert ri.status.cpu().numpy()[0] == 4 and ri.status.cpu().numpy()[1] == 0
+    # NEXT-4, cheap half: the constraint-set precheck proves the account's set empty (forced sells of the exclusions exceed
+    # tau) and returns it at iteration 0 with w = w0 and the reason code, instead of burning the iteration cap
+    assert int(ri.iters[0]) == 0 and float(ri.resid[0, 11]) == 2.0 and float((ri.w[0] - torch_w0(inf, ri)[0]).abs().max()) == 0.0
+    assert int(ri.iters[1]) > 0 and float(ri.resid[1, 11]) == 0.0
     Pi.close()
+    inf2 = gen.config2(N=320, k=8, A=3, G=4)
+    inf2.band_lo[2, 1] = 0.9; inf2.band_hi[2, 1] = 0.95     # with the other groups' lower bands (~0.2 each) the bands cannot meet the budget
+    inf2.hi[1] = 1.0 / 640.0                                 # caps too small for the budget: sum hi < 1
+    Pj, rj = _solve_gpu(inf2)
+    sj = rj.status.cpu().numpy()
+    assert sj.tolist() == [0, 4, 4] and rj.resid[:, 11].cpu().numpy().tolist() == [0.0, 1.0, 3.0] and rj.iters.cpu().numpy()[1:].tolist() == [0, 0]
+    Pj.close()
 
 
 def test_edge_cases():
