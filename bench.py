@@ -373,6 +373,14 @@ def main():
         for mult in (1, 4, 20, 100, 800):
             extra.append(dict(row(f"sec9_ladder_N{481 * mult}", gen.section9(seed=0, N=481 * mult, k=20, A=1)),
                               note="single account, L1 penalty kappa = 0.005, cap 3%, no turnover cap"))
+        if args.config == "cfg2":                                            # the paper's queue framing (Table 8) on the headline batch
+            from paper_2606_23367_b200 import queue_layer
+            for bs in (500, 125):
+                queue_layer.run_queue(inst, batch_size=bs, device=dev)          # warm-up (first-touch of the allocations)
+                _, recs = queue_layer.run_queue(inst, batch_size=bs, deadline_ms=1.5e6, device=dev)
+                extra.append(dict(queue_layer.summarise(recs), config=f"queue_cfg2_batches_of_{bs}",
+                                  note="NEXT-3 queue layer: consecutive batches incl. prism_problem_create per batch, 1,500 s window; "
+                                       "latency = queue start -> result available; paper: 109.5 s total, p50 212 ms per account on its hardware"))
         if args.config == "cfg2":                                            # the other form of the projection on the headline batch
             extra.append(dict(row("cfg2_resident_form", inst, form=binding.PROX_RESIDENT), note="prox_form = PRISM_PROX_RESIDENT"))
 

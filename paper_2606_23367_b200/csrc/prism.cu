@@ -18,7 +18,7 @@ static int pick_mt(int k) {
 extern "C" void prism_default_settings(prism_settings* s) {
   if (!s) return;
   memset(s, 0, sizeof(*s));
-  s->eps_rel = 1e-6; s->eps_abs = 0.0; s->max_iter = 4000; s->check_every = 10; s->first_check = 40; s->adapt_rho = 1; s->adapt_start = 200; s->adapt_every = 100; s->sample_until = 0; s->reserved0 = 0;
+  s->eps_rel = 1e-6; s->eps_abs = 0.0; s->max_iter = 4000; s->check_every = 10; s->first_check = 40; s->adapt_rho = 1; s->adapt_start = 200; s->adapt_every = 100; s->sample_until = 6; s->reserved0 = 0;
   s->alpha = 1.6; s->rho_scale = 100.0; s->gemm_precision = PRISM_GEMM_TF32X3; s->profile = 0;
   s->time_limit_ms = 0.0; s->deadline_ms = 0.0; s->prox_window_mult = 32.0; s->warm_w = nullptr; s->warm_duals = nullptr;
 }

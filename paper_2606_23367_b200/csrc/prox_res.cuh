@@ -147,6 +147,8 @@ struct SrcRes {
   double *wpart, *inbox, *ginbox, *gbin;
   double *cPg_, *cRg_;                     // per group: constant buys / sells of the dead assets (whole cluster)
   double cPt, cRt;
+  int sstride;                             // 1, or the stride of a SAMPLED root find (prism_settings.sample_until): the passes
+  double sscale;                           // visit every sstride-th live entry of a warp's list and scale this CTA's sums
 
   __device__ __forceinline__ double cP() const { return cPt; }
   __device__ __forceinline__ double cR() const { return cRt; }
@@ -177,6 +179,15 @@ struct SrcRes {
     const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const uint16_t* L = live + wid * capw;
     const int n = lcnt[wid];
+    if (sstride > 1) {                       // sampled pass
+      for (int j = lane * sstride; j < n; j += 32 * sstride) {
+        const int i = L[j];
+        ElemConst e; int g, nl; const double *sl, *wd;
+        make(i, ir_of(wid, j, i), e, g, nl, sl, wd);
+        f(i_beg + i, e, g, nl, sl, wd);
+      }
+      return;
+    }
     int j = lane;
     for (; j + 96 < n; j += 128) {
       int i4[4]; double r4[4];
@@ -219,7 +230,7 @@ struct SrcRes {
         double x = wpart[q];
 #pragma unroll
         for (int w = 1; w < RES_NW; ++w) x = red_op<OP>(x, wpart[w * RES_NV + q]);
-        val[q] = x;
+        val[q] = OP == 0 ? x * sscale : x;
       }
       __syncthreads();
       return;
@@ -232,7 +243,7 @@ struct SrcRes {
       double x = wpart[q];
 #pragma unroll
       for (int w = 1; w < RES_NW; ++w) x = red_op<OP>(x, wpart[w * RES_NV + q]);
-      res_store_peer(box + rank * RES_NV + q, (uint32_t)r, x);
+      res_store_peer(box + rank * RES_NV + q, (uint32_t)r, OP == 0 ? x * sscale : x);
     }
     res_cluster_barrier();
 #pragma unroll
@@ -472,7 +483,7 @@ __global__ void __launch_bounds__(RES_NT, 2) k_prox_res(const __grid_constant__ 
     src.seq = (uint32_t*)(res_raw + lay.seq); src.irc = irc;
     src.wpart = (double*)(res_raw + lay.wpart); src.inbox = (double*)(res_raw + lay.inbox);
     src.ginbox = (double*)(res_raw + lay.ginbox); src.gbin = (double*)(res_raw + lay.gbin);
-    src.cPg_ = cPg; src.cRg_ = cRg; src.cPt = 0.0; src.cRt = 0.0;
+    src.cPg_ = cPg; src.cRg_ = cRg; src.cPt = 0.0; src.cRt = 0.0; src.sstride = 1; src.sscale = 1.0;
     sh.scratch = nst; sh.gbin = src.gbin; sh.lamS = lamS; sh.gsum = gsum; sh.selS = selS;
     sh.band_lo = band_lo; sh.band_hi = band_hi; sh.gw0 = gw0;
     res_mbar_init((uint64_t*)(res_raw + lay.mbar), 1);
@@ -600,6 +611,20 @@ __global__ void __launch_bounds__(RES_NT, 2) k_prox_res(const __grid_constant__ 
   }
 
   // ---- B. root find
+  // Sampled root find (prism_settings.sample_until): plain launches of the first iterations, while no band is in the
+  // projection, find the thresholds on every stride-th live entry of each warp's list (at most 64 per warp, scaled) and
+  // apply them to all live assets: an inexact prox where exactness buys nothing yet.
+  const bool sampm = !exact && !bands_on && p.iter < p.sample_until;
+  if (sampm) {
+    __syncthreads();
+    if (tid == 0) {
+      int mx = 0;
+      for (int w = 0; w < RES_NW; ++w) mx = max(mx, lcnt[w]);
+      const int st = (mx + 63) / 64;
+      src.sstride = st < 1 ? 1 : st; src.sscale = (double)src.sstride;
+    }
+    __syncthreads();
+  }
   const double tol = 2e-15 * fmax(1.0, fabs(b) + (isfinite(tau) ? tau : 0.0));
   const double Pt = 0.5 * (tau + b), Rt = 0.5 * (tau - b);
   RootState rs;
@@ -751,7 +776,7 @@ __global__ void __launch_bounds__(RES_NT, 2) k_prox_res(const __grid_constant__ 
     double mv_l = 0.0;
     if (bands_on) for (int g = 0; g < G; ++g) mv_l = fmax(mv_l, fabs(lamS[g] - lamW[g]));
     mv = fmax(fmax(fabs(rs.alpha - aw), fabs(rs.beta - bw)), mv_l);
-    if (!(W < INFINITY) || mv <= 0.5 * W) break;
+    if (sampm || !(W < INFINITY) || mv <= 0.5 * W) break;   // (a sampled solve is inexact by design: no reclassification)
     // the solution left the window the live lists were built for: every asset live, solve again from the warm start
     __syncthreads();
     for (int g = tid; g < G; g += RES_NT) lamS[g] = lamW[g];
