@@ -107,13 +107,22 @@ __device__ __forceinline__ double sell_amt(const ElemConst& e, double bd, const 
                                            int nl, double& mv) {   // bd = beta + lambda_g - Delta
   mv = 0.0;
   if (LOTS && nl > 0) {
+    // the asset's whole lot row (4 slopes, 4 widths: two 32-byte rows, 16-byte aligned by the ABI) in ONE round of loads -
+    // a loop that fetches lot l only after lot l - 1 has been accounted for is a chain of up to eight global-load latencies
+    // per live asset per pass (14% of the lots kernel's stall samples, profiles/r2_kernels_ncu_full.md)
+    const double2 s01 = *(const double2*)slope, s23 = *(const double2*)(slope + 2);
+    const double2 w01 = *(const double2*)width, w23 = *(const double2*)(width + 2);
+    const double sl4[PRISM_MAX_LOTS] = {s01.x, s01.y, s23.x, s23.y}, wd4[PRISM_MAX_LOTS] = {w01.x, w01.y, w23.x, w23.y};
     double raw = 0.0, Q = 0.0, inside = 0.0;
-    for (int l = 0; l < nl; ++l) {
-      const double r = (bd - slope[l] - e.T) * e.ir - Q;
-      const double ql = width[l];
-      if (r > 0.0 && r < ql) inside = 1.0;
-      raw += fmin(fmax(r, 0.0), ql);
-      Q += ql;
+#pragma unroll
+    for (int l = 0; l < PRISM_MAX_LOTS; ++l) {
+      if (l < nl) {
+        const double r = (bd - sl4[l] - e.T) * e.ir - Q;
+        const double ql = wd4[l];
+        if (r > 0.0 && r < ql) inside = 1.0;
+        raw += fmin(fmax(r, 0.0), ql);
+        Q += ql;
+      }
     }
     const double sh = fmin(e.sl + e.wS, Q);
     if (inside > 0.0 && raw > e.sl && raw < sh) mv = e.ir;

@@ -46,13 +46,20 @@ class AuditRecord:
     build_id: str
 
 
-def input_identity(inst, a: int) -> str:
-    """SHA-256 over the account's own data in a fixed field order (shared universe: its own hash is part of the stream)."""
+def universe_identity(inst) -> str:
+    """SHA-256 of the shared universe (B, f, d, group ids), hashed once per queue."""
     h = hashlib.sha256()
     for name in ("B", "f", "d", "group_id"):
         v = getattr(inst, name)
         if v is not None:
             h.update(name.encode()); h.update(np.ascontiguousarray(v).tobytes())
+    return h.hexdigest()
+
+
+def input_identity(inst, a: int, universe: str = None) -> str:
+    """SHA-256 over the universe's digest and the account's own data in a fixed field order."""
+    h = hashlib.sha256()
+    h.update((universe or universe_identity(inst)).encode())
     for name in shard.PER_ACCOUNT:
         if name in ("witness", "tau_drawn"):
             continue
@@ -68,6 +75,8 @@ def run_queue(inst, batch_size: int, deadline_ms: float = 0.0, time_limit_ms: fl
     if batch_size < 1:
         raise ValueError("batch_size must be >= 1")
     build = binding.version()
+    uni = universe_identity(inst)
+    ids = [input_identity(inst, a, uni) for a in range(inst.A)]       # (identity of the inputs: before the clock starts)
     W = np.empty((inst.A, inst.N))
     records = []
     t0 = time.perf_counter()
@@ -85,7 +94,7 @@ def run_queue(inst, batch_size: int, deadline_ms: float = 0.0, time_limit_ms: fl
         for j in range(stop - start):
             a = start + j
             missed = deadline_ms > 0 and (latency > deadline_ms or int(st[j]) in (2, 3))
-            records.append(AuditRecord(a, b, input_identity(inst, a), hashlib.sha256(np.ascontiguousarray(w[j]).tobytes()).hexdigest(),
+            records.append(AuditRecord(a, b, ids[a], hashlib.sha256(np.ascontiguousarray(w[j]).tobytes()).hexdigest(),
                                        int(st[j]), STATUS_NAMES.get(int(st[j]), "?"), int(it[j]), tuple(float(x) for x in rs[j]),
                                        latency, float(r.info["solve_interval_ms"]), bool(missed), build))
     return W, records
