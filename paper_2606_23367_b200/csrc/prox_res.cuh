@@ -71,9 +71,22 @@ __device__ __forceinline__ void res_bulk_g2s(void* dst, const void* src, uint32_
 
 // lanes holding the same group are summed in ascending lane order, the lowest lane adds the sums to this warp's bins
 // bins[NQ * g + q] (deterministic; call from warp-uniform control flow)
+// single: the problem has one (pseudo-)group (G = 0): the warp's terms are summed by a fixed butterfly instead - five
+// steps, not one per contributing lane (the serial form was 12% of this kernel's stall samples on configs[1])
 template <int NQ>
-__device__ __forceinline__ void res_group_add(double* bins, int g, const double (&x)[NQ], bool valid) {
+__device__ __forceinline__ void res_group_add(double* bins, int g, const double (&x)[NQ], bool valid, bool single = false) {
   const int lane = threadIdx.x & 31;
+  if (single) {
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) {
+      double y = valid ? x[q] : 0.0;
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) y += __shfl_xor_sync(0xffffffffu, y, o);
+      if (lane == 0) bins[q] += y;
+    }
+    __syncwarp();
+    return;
+  }
   const int key = valid ? g : (0x40000000 + lane);
   const unsigned m = __match_any_sync(0xffffffffu, key);
   unsigned rem = m;
@@ -376,7 +389,7 @@ __device__ __noinline__ void res_reclassify_all(SrcRes<LC>& s) {
       if (pos < RES_IRC) s.irc[wid * RES_IRC + pos] = ir;
     }
     n += __popc(m);
-    if (__any_sync(0xffffffffu, x[0] != 0.0 || x[1] != 0.0)) res_group_add<2>(bins, g, x, valid && !lv);
+    if (__any_sync(0xffffffffu, x[0] != 0.0 || x[1] != 0.0)) res_group_add<2>(bins, g, x, valid && !lv, s.G == 0);
   }
   if (lane == 0) s.lcnt[wid] = n;
   res_publish_constants(s);
@@ -603,7 +616,7 @@ __global__ void __launch_bounds__(RES_NT, 2) k_prox_res(const __grid_constant__ 
           n += __popc(m);
         }
         const bool cst = valid && !lv && (bcst != 0.0 || scst != 0.0);
-        if (__any_sync(0xffffffffu, cst)) { const double x2[2] = {bcst, scst}; res_group_add<2>(bins, g, x2, cst); }
+        if (__any_sync(0xffffffffu, cst)) { const double x2[2] = {bcst, scst}; res_group_add<2>(bins, g, x2, cst, G == 0); }
       }
     }
     if (lane == 0) lcnt[wid] = n;

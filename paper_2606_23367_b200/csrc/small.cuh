@@ -212,6 +212,25 @@ __global__ void __launch_bounds__(256) k_solve(SolveArgs p) {
   const int a = p.act ? p.act[blockIdx.x] : (int)blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   if (p.ap.done[a]) return;
   const int Kp = p.kp;
+  // The rows of the inverse this thread will need do not depend on T: for Kp <= 64 (8 rows x 2 entries per lane) they
+  // are requested now, so that their latency overlaps the reduction of the partials instead of following it (the
+  // matvec's loads were 60% of this kernel's stall samples).
+  const double* Si = p.Sinv + (int64_t)a * Kp * Kp;
+  const bool pre = Kp <= 64;
+  double sv[8][2];
+  if (pre) {
+#pragma unroll
+    for (int h = 0; h < 2; ++h)
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int r = warp + 32 * h + 8 * u;
+#pragma unroll
+        for (int k = 0; k < 2; ++k) {
+          const int c = lane + 32 * k;
+          sv[4 * h + u][k] = (r < Kp && c < Kp) ? Si[(int64_t)r * Kp + c] : 0.0;
+        }
+      }
+  }
   {
     const int part = tid >> 6, nper = (p.nchunk + 3) >> 2;
     const int c0 = part * nper, c1 = min(p.nchunk, c0 + nper);
@@ -225,7 +244,22 @@ __global__ void __launch_bounds__(256) k_solve(SolveArgs p) {
   __syncthreads();
   for (int j = tid; j < Kp; j += 256) T[j] = ((Tq[0][j] + Tq[1][j]) + Tq[2][j]) + Tq[3][j];
   __syncthreads();
-  const double* Si = p.Sinv + (int64_t)a * Kp * Kp;
+  if (pre) {
+    const double t0 = lane < Kp ? T[lane] : 0.0, t1 = lane + 32 < Kp ? T[lane + 32] : 0.0;
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      double acc[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) acc[u] = fma(sv[4 * h + u][1], t1, sv[4 * h + u][0] * t0);
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const double v = warp_sum(acc[u]);
+        const int r = warp + 32 * h + 8 * u;
+        if (lane == 0 && r < Kp) p.V[(int64_t)a * p.ldv + r] = v;
+      }
+    }
+    return;
+  }
   for (int r0 = warp; r0 < Kp; r0 += 32) {               // rows r0, r0 + 8, r0 + 16, r0 + 24 of this warp together
     double acc[4] = {0.0, 0.0, 0.0, 0.0};
 #pragma unroll
