@@ -189,7 +189,9 @@ __global__ void __launch_bounds__(256, 2) k_gemm2_tf32(Gemm2Args p, TfUniverse u
     cp_async_commit();
     // D[account row g (+8)][asset = ib + 8 n + {0, 1}], n = 0..3
     const int64_t ib = (tile0 + tt) * T2_TN + wc * 32 + 2 * t;
-    double2 v2[2][4], c2[2][4];
+    double2 v2[2][4], c2[2][4], iv4[4];
+#pragma unroll
+    for (int n = 0; n < 4; ++n) iv4[n] = ib + n * 8 < p.ldw ? *(const double2*)(p.invd + ib + n * 8) : make_double2(0.0, 0.0);   // (padded with zeros to ldw)
 #pragma unroll
     for (int h = 0; h < 2; ++h) {
       const int64_t rowp = (int64_t)acct[h] * p.ldw;
@@ -233,7 +235,7 @@ __global__ void __launch_bounds__(256, 2) k_gemm2_tf32(Gemm2Args p, TfUniverse u
         const int64_t i = ib + n * 8;
         if (i >= p.ldw) continue;
         const double b0 = (double)acc[n][2 * h], b1 = (double)acc[n][2 * h + 1];
-        const double2 iv = *(const double2*)(p.invd + i);                  // (invd is padded with zeros to ldw)
+        const double2 iv = iv4[n];
         const double s0 = b0 * iv.x * gsc[h], s1 = b1 * iv.y * gsc[h];
         double2 vn;
         vn.x = v2[h][n].x + p.relax * (c2[h][n].x - s0);
