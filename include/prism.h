@@ -163,7 +163,8 @@ typedef struct prism_settings {
                                start), find the thresholds on a SAMPLE of the live assets (every stride-th, scaled) and
                                apply them to all - an inexact prox.  The splitting's only carried state is v, so this
                                perturbs the path of the iteration, not its fixed point; check / final launches are always
-                               exact.  0 => never.  Default 6: measured on configs[2] / [3], DESIGN.md section 2                            */
+                               exact.  0 => never; -1 (default) => 6, or 12 for universes of 65,536 instruments and more (measured on
+                               configs[2] / [3] / [4])                                          */
   int32_t reserved0;
   /* warm start - the repeated-run lane (cold rows "pass no previous solution"): previous weights and
      multipliers of the same accounts, e.g. the w_out / duals_out of an earlier call.  Both NULL => cold start.       */

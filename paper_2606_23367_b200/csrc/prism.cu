@@ -18,7 +18,7 @@ static int pick_mt(int k) {
 extern "C" void prism_default_settings(prism_settings* s) {
   if (!s) return;
   memset(s, 0, sizeof(*s));
-  s->eps_rel = 1e-6; s->eps_abs = 0.0; s->max_iter = 4000; s->check_every = 10; s->first_check = 40; s->adapt_rho = 1; s->adapt_start = 200; s->adapt_every = 100; s->sample_until = 6; s->reserved0 = 0;
+  s->eps_rel = 1e-6; s->eps_abs = 0.0; s->max_iter = 4000; s->check_every = 10; s->first_check = 40; s->adapt_rho = 1; s->adapt_start = 200; s->adapt_every = 100; s->sample_until = -1; s->reserved0 = 0;
   s->alpha = 1.6; s->rho_scale = 100.0; s->gemm_precision = PRISM_GEMM_TF32X3; s->profile = 0;
   s->time_limit_ms = 0.0; s->deadline_ms = 0.0; s->prox_window_mult = 32.0; s->warm_w = nullptr; s->warm_duals = nullptr;
 }
@@ -300,7 +300,10 @@ static ProxArgs make_prox_args(prism_problem* p, const prism_settings& s, double
   a.ap = p->ap; a.w_out = w_out; a.duals = p->duals; a.resid = p->resid; a.counters = p->counters;
   a.eps = s.eps_rel; a.eps_abs = s.eps_abs;
   a.adapt = s.adapt_rho; a.iter = 0; a.ldw = p->ldn;
-  a.sample_until = s.warm_w ? 0 : s.sample_until;       // a warm start has its bands in from the first launch
+  // -1 = by measurement: 6 launches; 12 for universes beyond the cluster-resident form's reach, where
+  // a pass over a full list costs the root kernel's one CTA per account milliseconds (configs[4]: 22 ms per launch)
+  const int sample_auto = (p->fast && p->N >= 65536) ? 12 : 6;
+  a.sample_until = s.warm_w ? 0 : (s.sample_until < 0 ? sample_auto : s.sample_until);   // a warm start has its bands in from the first launch
   a.adapt_start = s.adapt_start; a.adapt_every = s.adapt_every < 1 ? 1 : s.adapt_every;
   a.lraw = p->lraw; a.lcomp = p->lcomp; a.lcnt = p->lcnt; a.cbin = p->cbin; a.chkp = p->chkp; a.lflag = p->lflag;
   a.S = p->S; a.capw = p->capw; a.slice_len = p->slice_len; a.ldc = p->ldc;
