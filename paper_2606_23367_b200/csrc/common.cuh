@@ -22,7 +22,9 @@ struct AccountParams {            // per-account scalars, struct of arrays on th
   int32_t* done;    // convergence mask (H6)
   int32_t* conv;    // 1 if own tolerance met
   int32_t* iters;
-  int32_t* refactor;// capacitance must be rebuilt (rho changed)
+  int32_t* refactor;// 1: capacitance must be rebuilt (rho changed); 2: streaming form - a new rho scale is pending in c_new:
+                    // k_prox_rescale rewrites the account's iterate for it, k_factor then adopts it
+  double* c_new;    // pending rho scale (refactor == 2)
   int32_t* nadapt;  // iteration of the account's last rho adaptation
   double* win;      // live-list window of the prox for the next launch (threshold units)
   double* wins;     // window of the streaming pass (prox_fast.cuh), >= win

@@ -27,3 +27,8 @@ cudaError_t prox_stream_launch(bool check, int S, int A, int G, const ProxArgs& 
   if (check) k_prox_root<true><<<A, ROOT_NT, smr, st>>>(a, mode & ~PROX_CHECK); else k_prox_root<false><<<A, ROOT_NT, smr, st>>>(a, mode);
   return cudaGetLastError();
 }
+cudaError_t prox_rescale_launch(int A, const ProxArgs& a, cudaStream_t st) {
+  const unsigned nb = (unsigned)((a.N + RESCALE_PER_CTA - 1) / RESCALE_PER_CTA);
+  k_prox_rescale<<<dim3(nb, (unsigned)A), 256, 0, st>>>(a);
+  return cudaGetLastError();
+}

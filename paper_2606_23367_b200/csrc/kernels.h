@@ -51,6 +51,7 @@ cudaError_t prox_res_launch(bool lots, bool check, int C, int A, size_t smem, co
 size_t prox_stream_smem(int G);
 cudaError_t prox_stream_set_attrs(int G, int nsub);
 cudaError_t prox_stream_launch(bool check, int S, int A, int G, const ProxArgs& a, int mode, cudaStream_t st);
+cudaError_t prox_rescale_launch(int A, const ProxArgs& a, cudaStream_t st);
 int prox_stream_chunk();          // FAST_CH
 int prox_stream_warps();          // FAST_NW
 int prox_stream_idx_bits();       // PROX_META_IDX_BITS

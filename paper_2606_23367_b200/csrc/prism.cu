@@ -50,7 +50,7 @@ extern "C" void prism_problem_destroy(prism_problem* p) {
   void* ptrs[] = {p->Bp, p->Bt, p->Bp_hi, p->Bp_lo, p->Bt_hi, p->Bt_lo, p->invd, p->gram, p->q, p->v, p->rt, p->cc, p->xs, p->pxq, p->Tpart, p->V, p->Sinv,
                   p->gw0, p->lamG, p->resid, p->duals, p->status, p->ap.c, p->ap.alpha, p->ap.beta,
                   p->ap.mode, p->ap.bsum, p->ap.done, p->ap.conv, p->ap.iters, p->ap.refactor,
-                  p->ap.nadapt, p->ap.win, p->ap.wins, p->ap.slack, p->counters, p->act, p->w_stage, p->i_stage, p->lraw, p->lcomp, p->lcnt, p->cbin, p->chkp, p->lflag};
+                  p->ap.nadapt, p->ap.win, p->ap.wins, p->ap.slack, p->ap.c_new, p->counters, p->act, p->w_stage, p->i_stage, p->lraw, p->lcomp, p->lcnt, p->cbin, p->chkp, p->lflag};
   for (void* q : ptrs) if (q) cudaFree(q);
   if (p->h_counters) cudaFreeHost(p->h_counters);
   delete p;
@@ -240,6 +240,7 @@ extern "C" int prism_problem_create(int64_t N, int32_t k, int32_t accounts, cons
   ALLOC_TRY(dev_alloc(p, &p->ap.win, (size_t)A));
   ALLOC_TRY(dev_alloc(p, &p->ap.wins, (size_t)A));
   ALLOC_TRY(dev_alloc(p, &p->ap.slack, (size_t)A));
+  ALLOC_TRY(dev_alloc(p, &p->ap.c_new, (size_t)A));
   ALLOC_TRY(dev_alloc(p, &p->counters, (size_t)4));
   ALLOC_TRY(dev_alloc(p, &p->act, (size_t)A));
   ALLOC_TRY(dev_alloc(p, &p->w_stage, (size_t)A * N));      // staging of the host-buffer lane (prism_solve_batch_host)
@@ -322,7 +323,12 @@ static void launch_prox(Launcher& L, ProxArgs& a, int mode, int iter) {
   const bool chk = (mode & (PROX_CHECK | PROX_FINAL)) != 0;       // the final extraction also needs w_out
   L.begin(PRISM_K_PROX);
   if (p->res) L.end(prox_res_launch(p->d.lot_count != nullptr, chk, p->res_C, p->A, p->res_smem, a, mode & ~PROX_CHECK, L.st));
-  else if (p->fast) L.end(prox_stream_launch(chk, p->S, p->A, p->G, a, mode, L.st), 2);
+  else if (p->fast) {
+    L.end(prox_stream_launch(chk, p->S, p->A, p->G, a, mode, L.st), 2);
+    // a check may have decided a rho change for some accounts: their iterate is rewritten for the new rho by a streaming
+    // pass of its own (exits at once for every other account)
+    if ((mode & PROX_CHECK) && a.adapt) L.end(prox_rescale_launch(p->A, a, L.st));
+  }
   else {
     const int grid = p->A < p->sm_count ? p->A : p->sm_count;
     const size_t sm = (size_t)p->N * 20 + 16;

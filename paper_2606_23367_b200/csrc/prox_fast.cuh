@@ -902,9 +902,15 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
                         !rs.capped;                                          // never certify on an unfinished root find
       if (!(rp < INFINITY) || !(rd < INFINITY)) fallback = true;             // NaN / Inf: the generic path classifies it
       else if (!conv && p.adapt && p.iter >= p.adapt_start && p.iter - p.ap.nadapt[a] >= p.adapt_every) {
+        // H7: rho <- rho sqrt(r_p / r_d), clipped, when the two scaled residuals are out of balance.  The thresholds found
+        // above stay valid (they belong to the old rho); every asset's v, r~ and c are rewritten for the new rho by
+        // k_prox_rescale right after this kernel (one streaming pass instead of the every-asset path: 10-40 ms per event
+        // on configs[4]), and k_factor adopts c_new.
         const double ratio = sqrt(rp / fmax(rd, 1e-300));
-        if (ratio > 3.0 || ratio < 1.0 / 3.0) fallback = true;               // rho changes: every asset is rewritten
-        else if (tid == 0) p.ap.nadapt[a] = p.iter;
+        if (tid == 0) {
+          if (ratio > 3.0 || ratio < 1.0 / 3.0) { p.ap.c_new[a] = c * fmin(fmax(ratio, 0.2), 5.0); p.ap.refactor[a] = 2; }
+          p.ap.nadapt[a] = p.iter;
+        }
       }
       if (!fallback) {
         finished = conv ? 1 : 0;
@@ -951,4 +957,48 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
   ProxShared shg = sh;
   prox_body<false>(p, mode | (CHECK ? PROX_CHECK : 0), gsrc, a, gam, c, kappa, lam_b, shg, false);
   if (tid == 0) p.ap.wins[a] = p.win_ratio * p.ap.win[a];
+}
+
+// ------------------------------------------------------------------------------------------------ rho change
+// Accounts for which the check decided a new rho scale (refactor == 2, c_new): with the thresholds of this launch (exact
+// for every asset, live or not: z_i is a closed form of T_i and the thresholds) the carried state is re-expressed,
+// v' = z + y / rho_new with y = rho_old (v - z), and r~ = M_new^-1 (rho_new z - y - q), c = r~ - z are rewritten.
+// grid = (ceil(N / RESCALE_PER_CTA), accounts); exits at once for every other account.
+#define RESCALE_PER_CTA 4096
+__global__ void __launch_bounds__(256) k_prox_rescale(const __grid_constant__ ProxArgs p) {
+  __shared__ double lamS[PRISM_MAX_GROUPS];
+  const int a = blockIdx.y;
+  if (p.ap.done[a] || p.ap.refactor[a] != 2) return;
+  const int tid = threadIdx.x, G = p.G;
+  for (int g = tid; g < G; g += blockDim.x) lamS[g] = p.lamG[(int64_t)a * G + g];
+  __syncthreads();
+  const int64_t N = p.N, row = (int64_t)a * N, rowp = (int64_t)a * p.ldw;
+  const double gam = p.gamma[a], c = p.ap.c[a], cn = p.ap.c_new[a], cg = c * gam, icg = 1.0 / cg, cgn = cn * gam, icgn = 1.0 / cgn;
+  const double igc = 1.0 / (gam * (1.0 + cn));
+  const double kappa = p.kappa ? p.kappa[a] : 0.0, lam_b = kappa + (p.c_buy ? p.c_buy[a] : 0.0), Delta = lam_b + kappa;
+  const double tau = p.tau ? p.tau[a] : INFINITY;
+  const double alpha = p.ap.alpha[a];
+  const double beta = (p.ap.mode[a] == 1 && isfinite(tau)) ? p.ap.beta[a] : alpha;
+  const double lo_a = p.lo[a], hi_a = p.hi[a], bdf = beta - Delta;
+  const int64_t i0 = (int64_t)blockIdx.x * RESCALE_PER_CTA, i1 = min(N, i0 + RESCALE_PER_CTA);
+  for (int64_t i = i0 + tid; i < i1; i += blockDim.x) {
+    const double iv = p.invd[i], di = p.d[i];
+    ElemConst e;
+    e.w0 = p.w0[row + i];
+    const double v = p.v[rowp + i];
+    e.T = (v - e.w0) * (cg * di) - lam_b;
+    e.ir = iv * icg;
+    const bool ex = p.excl && p.excl[row + i];
+    elem_ranges(e, ex ? 0.0 : lo_a, ex ? 0.0 : hi_a);
+    const double lg = G ? lamS[p.group_id[i]] : 0.0;
+    double mvb, mvs;
+    const double tr = buy_amt(e, alpha + lg, mvb) - sell_amt<false>(e, bdf + lg, nullptr, nullptr, 0, mvs);
+    const double z = e.w0 + tr;
+    const double y = e.T + lam_b - tr * (cg * di);         // rho_old (v - z)
+    const double qi = p.q ? p.q[rowp + i] : -p.mu[row + i];
+    p.v[rowp + i] = z + y * iv * icgn;
+    const double rt = (cgn * di * z - y - qi) * iv * igc;  // M_i = gamma d_i (1 + c_new)
+    p.rt[rowp + i] = rt;
+    p.cc[rowp + i] = rt - z;
+  }
 }

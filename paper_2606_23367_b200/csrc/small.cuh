@@ -174,7 +174,8 @@ __global__ void k_factor(const double* gram, const double* f, const double* gamm
   const int a = blockIdx.x, tid = threadIdx.x, nt = blockDim.x;
   if (!ap.refactor[a] || ap.done[a]) return;
   const int Kp = kp + G;
-  const double gam = gamma[a], c = ap.c[a];
+  const bool pending = ap.refactor[a] == 2;            // streaming form: the new rho scale waits in c_new (k_prox_rescale ran)
+  const double gam = gamma[a], c = pending ? ap.c_new[a] : ap.c[a];
   const double sc = 1.0 / (gam * (1.0 + c));
   for (int e = tid; e < Kp * Kp; e += nt) {
     const int r = e / Kp, cc = e % Kp;
@@ -199,7 +200,7 @@ __global__ void k_factor(const double* gram, const double* f, const double* gamm
     __syncthreads();
   }
   for (int e = tid; e < Kp * Kp; e += nt) Sinv[(int64_t)a * Kp * Kp + e] = S[e];
-  if (tid == 0) ap.refactor[a] = 0;
+  if (tid == 0) { if (pending) ap.c[a] = c; ap.refactor[a] = 0; }
 }
 
 // ---------------------------------------------------------------------------------- H2: V = S^-1 T
