@@ -44,6 +44,13 @@
 extern "C" {
 #endif
 
+/* the library is built with hidden default visibility: exactly the functions declared here are exported */
+#if defined(__GNUC__)
+#define PRISM_API __attribute__((visibility("default")))
+#else
+#define PRISM_API
+#endif
+
 #define PRISM_MAX_LOTS 4
 #define PRISM_MAX_GROUPS 64
 #define PRISM_MAX_FACTORS 128
@@ -185,14 +192,14 @@ typedef struct prism_solve_info {
 typedef struct prism_problem prism_problem;
 
 /* Fills *s with the defaults listed above. */
-void prism_default_settings(prism_settings* s);
+PRISM_API void prism_default_settings(prism_settings* s);
 
 /* Validates shapes and flags, adopts the borrowed device pointers in `data`, allocates ALL workspace once and
  * precomputes what does not depend on the iterate (padded copies of B, the shared Gram matrix U' D^-1 U, q when a
  * benchmark shift is present).  N >= 1, 1 <= k <= PRISM_MAX_FACTORS, accounts >= 1.  Runs on `cuda_stream`
  * (a cudaStream_t, NULL = default stream) and synchronises it.  On failure *out = NULL; PRISM_ERR_ALLOC means
  * the problem object was not allocated (status 5 for every account). */
-int prism_problem_create(int64_t N, int32_t k, int32_t accounts, const prism_constraint_set* cs,
+PRISM_API int prism_problem_create(int64_t N, int32_t k, int32_t accounts, const prism_constraint_set* cs,
                          const prism_data* data, void* cuda_stream, prism_problem** out);
 
 /* Runs the batched solver on `cuda_stream` and synchronises it before returning.  Cold start (default):
@@ -204,14 +211,14 @@ int prism_problem_create(int64_t N, int32_t k, int32_t accounts, const prism_con
  *   duals_out  device, A x PRISM_NDUAL(G) doubles, or NULL
  *   info       host, or NULL
  * Re-entrant per problem object; not thread-safe on one object. */
-int prism_solve_batch(prism_problem* p, const prism_settings* s, void* cuda_stream, double* w_out,
+PRISM_API int prism_solve_batch(prism_problem* p, const prism_settings* s, void* cuda_stream, double* w_out,
                       int32_t* status_out, int32_t* iters_out, double* resid_out, double* duals_out,
                       prism_solve_info* info);
 
 /* External-diagnostic semantics: depends only on the problem data and the given w (and
  * multipliers, if any), never on solver state, so it applies to any solver's weights.  Fills columns 0..6 and 9
  * of the residual block (4, 5 are NaN when duals == NULL; 7, 8, 10 are NaN).  Synchronises the stream. */
-int prism_residuals(prism_problem* p, const double* w, const double* duals, void* cuda_stream,
+PRISM_API int prism_residuals(prism_problem* p, const double* w, const double* duals, void* cuda_stream,
                     double* resid_out);
 
 /* ONE application of the fused projection (H4) to caller-given points, outside any iteration - the prox of every
@@ -223,7 +230,7 @@ int prism_residuals(prism_problem* p, const double* w, const double* duals, void
  * launches, from a cold start.  v: device A x N; z_out: device A x N; duals_out: device A x PRISM_NDUAL(G) multipliers
  * of the projection (layout above), or NULL.  Overwrites the solver's iterate (the next prism_solve_batch starts
  * cold anyway).  Synchronises the stream. */
-int prism_project(prism_problem* p, const double* v, double rho_scale, void* cuda_stream, double* z_out,
+PRISM_API int prism_project(prism_problem* p, const double* v, double rho_scale, void* cuda_stream, double* z_out,
                   double* duals_out);
 
 /* Same solve as prism_solve_batch but with HOST buffers for the per-account data that changes between
@@ -231,7 +238,7 @@ int prism_project(prism_problem* p, const double* v, double rho_scale, void* cud
  * solves, copies weights / status / iterations / residual block back.  NULL host pointers skip that copy.
  * The other per-account data (bounds, masks, bands, tau, gamma) stays resident from prism_problem_create.
  * This is the end-to-end lane of bench.py ("e2e"). */
-int prism_solve_batch_host(prism_problem* p, const prism_settings* s, void* cuda_stream, const double* mu_host,
+PRISM_API int prism_solve_batch_host(prism_problem* p, const prism_settings* s, void* cuda_stream, const double* mu_host,
                            const double* w0_host, double* w_host, int32_t* status_host, int32_t* iters_host,
                            double* resid_host, prism_solve_info* info);
 
@@ -243,12 +250,12 @@ enum { PRISM_K_PROX = 0, PRISM_K_GEMM1 = 1, PRISM_K_SOLVE = 2, PRISM_K_GEMM2 = 3
 
 /* Device time (ms, CUDA events on the solve stream) and launch count per kernel class of the last
  * prism_solve_batch call that ran with settings.profile = 1.  ms_out, launches_out: host arrays of PRISM_NKERN. */
-int prism_kernel_times(const prism_problem* p, double* ms_out, int64_t* launches_out);
+PRISM_API int prism_kernel_times(const prism_problem* p, double* ms_out, int64_t* launches_out);
 
 /* Factor exposures of caller-given weights through the problem's own GEMM-1 (H1):
  *   T_out[a * k + j] = sum_i B[i][j] w[a * N + i]       w: device A x N, T_out: device A x k.
  * Split-K partials live in the workspace allocated at create.  Synchronises the stream. */
-int prism_factor_exposures(prism_problem* p, const double* w, void* cuda_stream, double* T_out);
+PRISM_API int prism_factor_exposures(prism_problem* p, const double* w, void* cuda_stream, double* T_out);
 
 /* ---- the one entry point that ALLOCATES NOTHING (for CUDA graph capture, serving loops, harnesses that forbid
  * cudaMalloc).  Same result as prism_factor_exposures, no problem object:
@@ -262,29 +269,29 @@ int prism_factor_exposures(prism_problem* p, const double* w, void* cuda_stream,
  * prism_noalloc_init() fetches the array's device address for the current device (cudaGetSymbolAddress); call it
  * once per device before a graph capture - the entry point does the same lazily otherwise. */
 #define PRISM_NOALLOC_SCRATCH_DOUBLES 524288
-int prism_noalloc_init(void);
-int prism_factor_exposures_noalloc(const void* B, int32_t B_is_fp32, const double* X, int64_t N, int32_t k,
+PRISM_API int prism_noalloc_init(void);
+PRISM_API int prism_factor_exposures_noalloc(const void* B, int32_t B_is_fp32, const double* X, int64_t N, int32_t k,
                                    int32_t accounts, void* cuda_stream, double* T_out);
 
 /* fp64 yardstick of THIS device: register-resident loops without memory traffic, CUDA-event timed on
  * cuda_stream, best of 5.  tflops_out (host, 2 doubles): [0] tensor pipe (DMMA mma.sync m8n8k4), [1] FMA pipe. */
-int prism_fp64_yardstick(prism_problem* p, void* cuda_stream, double* tflops_out);
+PRISM_API int prism_fp64_yardstick(prism_problem* p, void* cuda_stream, double* tflops_out);
 
 /* Frees the workspace; never frees borrowed data.  NULL is allowed. */
-void prism_problem_destroy(prism_problem* p);
+PRISM_API void prism_problem_destroy(prism_problem* p);
 
 /* The form of the projection kernel this object runs (PRISM_PROX_RESIDENT / _STREAMING / _EVERY_ASSET): what
  * PRISM_PROX_AUTO resolved to. */
-int32_t prism_problem_prox_form(const prism_problem* p);
+PRISM_API int32_t prism_problem_prox_form(const prism_problem* p);
 
 /* Workspace bytes owned by the object (memory class). */
-int64_t prism_problem_device_bytes(const prism_problem* p);
+PRISM_API int64_t prism_problem_device_bytes(const prism_problem* p);
 
 /* Thread-local message for the last non-zero return of this thread. */
-const char* prism_last_error(void);
+PRISM_API const char* prism_last_error(void);
 
 /* Build id (the paper records an "evidence build" id). */
-const char* prism_version(void);
+PRISM_API const char* prism_version(void);
 
 #ifdef __cplusplus
 }

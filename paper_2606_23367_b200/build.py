@@ -15,7 +15,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "_obj")
 LIB = os.path.join(HERE, "libprism.so")
 HEADER = os.path.join(os.path.dirname(HERE), "include", "prism.h")
-FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC,-pthread"]
+FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC,-pthread,-fvisibility=hidden"]
 FLAGS += os.environ.get("PRISM_NVCC_FLAGS", "").split()       # builder's switch, e.g. -DPRISM_STATS (pass counts of the root find)
 
 

@@ -184,3 +184,15 @@ def test_queue_layer_identity_and_summary():
     s = ql.summarise(recs)
     assert s["accounts"] == 4 and s["completed"] == 4 and s["certified"] == 2 and s["missed_deadline_rate"] == 0.25
     assert s["latency_max_ms"] == 30.0 and abs(s["accounts_per_s"] - 4 / 0.030) < 1e-9 and s["latency_p50_ms"] == 15.0
+
+
+def test_library_exports_exactly_the_declared_symbols(lib):
+    """nm -D: the dynamic symbol table of libprism.so holds the functions include/prism.h declares and nothing else
+    (the library is built with hidden default visibility)."""
+    import subprocess
+    from paper_2606_23367_b200 import binding
+    out = subprocess.run(["nm", "-D", "--defined-only", binding.LIB_PATH], capture_output=True, text=True, check=True).stdout
+    exported = {l.split()[2] for l in out.splitlines() if len(l.split()) == 3 and l.split()[1] == "T"}
+    declared = set(re.findall(r"\b(prism_[a-z0-9_]+)\s*\(", _header()))
+    declared -= {"prism_problem", "prism_settings", "prism_data", "prism_constraint_set", "prism_solve_info"}
+    assert exported == declared, (sorted(exported - declared), sorted(declared - exported))
