@@ -64,6 +64,12 @@ template <bool CHECK>
 __global__ void __launch_bounds__(FAST_NW * 32, 3) k_prox_stream(const __grid_constant__ ProxArgs p) {
   extern __shared__ __align__(16) unsigned char stream_raw[];
   __shared__ double cst[12];
+  // fixed-point bins of this CTA (dead bins, then speculative bins), used when the problem has no groups (one bin per side
+  // and account): the constant trades are added up in shared memory and reach the account's global bins with ONE atomic
+  // per bin and CTA.  (Per-asset global atomics on one address per
+  // account serialise in L2: on configs[4], where a quarter of the 384,800 assets is sold out or at its cap, they held
+  // the whole kernel at 1.2 TB/s - the bulk copies queued behind them.)  Integer sums: the order does not matter.
+  __shared__ unsigned long long sbin[4 * PRISM_MAX_GROUPS];
   const int a = blockIdx.y, sl = blockIdx.x;
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   const int G = p.G, Gb = G > 0 ? G : 1;
@@ -124,6 +130,7 @@ __global__ void __launch_bounds__(FAST_NW * 32, 3) k_prox_stream(const __grid_co
     for (int c = 0; c < FAST_NST - 1 && c < nchunk; ++c) issue(c);
   }
   if (wid == 1 && lane < 12) cst[lane] = cv;
+  for (int t = tid; t < 4 * Gb; t += FAST_NW * 32) sbin[t] = 0ull;
   if (tid >= 64 && tid - 64 < G) lamS[tid - 64] = lam_mine;
   for (int g = tid + FAST_NW * 32 - 64; g < G; g += FAST_NW * 32) lamS[g] = p.lamG[(int64_t)a * G + g];   // (G > 192 only)
   __syncthreads();
@@ -212,7 +219,7 @@ __global__ void __launch_bounds__(FAST_NW * 32, 3) k_prox_stream(const __grid_co
       if (valid && !live) {
         rtp[h * 256] = rt;
         ccp[h * 256] = rt - z;
-        unsigned long long* bin = spec ? cbin + fbin_off : cbin;
+        unsigned long long* bin = G == 0 ? (spec ? sbin + 2 * Gb : sbin) : (spec ? cbin + fbin_off : cbin);   // (with groups the bins are spread: direct)
         if (bc > 0.0) atomicAdd(&bin[g], (unsigned long long)__double2ull_rn(bc * PRISM_FIX_SCALE));
         if (sc > 0.0) atomicAdd(&bin[Gb + g], (unsigned long long)__double2ull_rn(sc * PRISM_FIX_SCALE));
         if (CHECK) {
@@ -244,6 +251,13 @@ __global__ void __launch_bounds__(FAST_NW * 32, 3) k_prox_stream(const __grid_co
     if (lane == 0) mbar_arrive(&bar_empty[st]);
   }
   if (lane == 0) { p.lcnt[sub] = n; p.lcnt[p.A * p.S * FAST_NW + sub] = nw_; }
+  if (G == 0) {
+    __syncthreads();
+    for (int t = tid; t < 4 * Gb; t += FAST_NW * 32) {
+      const unsigned long long x = sbin[t];
+      if (x) atomicAdd(t < 2 * Gb ? &cbin[t] : &cbin[fbin_off + (t - 2 * Gb)], x);
+    }
+  }
   if (CHECK) {
     double val[7] = {nx, nz, nrp, nrd, nPx, ny, nq};
     block_reduce<7, 1>(val, scratch);
