@@ -37,7 +37,8 @@ cudaError_t factor_launch(const double* gram, const double* f, const double* gam
   return cudaGetLastError();
 }
 cudaError_t solve_launch(const SolveArgs& a, cudaStream_t st) {
-  k_solve<<<a.nact, 256, 0, st>>>(a);
+  if (a.nchunk > 64 && a.kp > 64) k_solve<1024><<<a.nact, 1024, 0, st>>>(a);
+  else k_solve<256><<<a.nact, 256, 0, st>>>(a);
   return cudaGetLastError();
 }
 // H6 compaction: act[0 .. n) = the accounts that are not done, ascending (one CTA, ballot scan: a fixed order).

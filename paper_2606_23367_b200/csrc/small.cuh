@@ -207,9 +207,13 @@ __global__ void k_factor(const double* gram, const double* f, const double* gamm
 // 256 threads.  (1) T = sum of the split-K partials: four threads per entry, each over a quarter of the chunks with all
 // its loads in flight, combined in a fixed order (deterministic).  (2) V = S^-1 T: one warp per row group, a row of
 // the (symmetric) inverse read coalesced by the lanes, warp-shuffle reduction: one round of global-load latency.
-__global__ void __launch_bounds__(256) k_solve(SolveArgs p) {
+// Many split-K chunks and a wide capacitance (configs[4]: 296 chunks, Kp = 104, 32 accounts = 32 CTAs): the launch uses
+// 1024 threads, i.e. 16 parts of the chunk range instead of 4 and 32 warps on the rows.
+#define SOLVE_MAX_PARTS 16
+template <int NT>                // threads per CTA: 256, or 1024 for many chunks and a wide capacitance
+__global__ void __launch_bounds__(NT) k_solve(SolveArgs p) {
   __shared__ double T[PRISM_MAX_KPRIME];
-  __shared__ double Tq[4][PRISM_MAX_KPRIME];
+  __shared__ double Tq[SOLVE_MAX_PARTS][PRISM_MAX_KPRIME];
   const int a = p.act ? p.act[blockIdx.x] : (int)blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   if (p.ap.done[a]) return;
   const int Kp = p.kp;
@@ -217,7 +221,8 @@ __global__ void __launch_bounds__(256) k_solve(SolveArgs p) {
   // are requested now, so that their latency overlaps the reduction of the partials instead of following it (the
   // matvec's loads were 60% of this kernel's stall samples).
   const double* Si = p.Sinv + (int64_t)a * Kp * Kp;
-  const bool pre = Kp <= 64;
+  const int nparts = blockDim.x >> 6, nwarp = blockDim.x >> 5;
+  const bool pre = Kp <= 64 && blockDim.x == 256;
   double sv[8][2];
   if (pre) {
 #pragma unroll
@@ -233,7 +238,7 @@ __global__ void __launch_bounds__(256) k_solve(SolveArgs p) {
       }
   }
   {
-    const int part = tid >> 6, nper = (p.nchunk + 3) >> 2;
+    const int part = tid >> 6, nper = (p.nchunk + nparts - 1) / nparts;
     const int c0 = part * nper, c1 = min(p.nchunk, c0 + nper);
     for (int j = tid & 63; j < Kp; j += 64) {
       double s = 0.0;
@@ -243,7 +248,11 @@ __global__ void __launch_bounds__(256) k_solve(SolveArgs p) {
     }
   }
   __syncthreads();
-  for (int j = tid; j < Kp; j += 256) T[j] = ((Tq[0][j] + Tq[1][j]) + Tq[2][j]) + Tq[3][j];
+  for (int j = tid; j < Kp; j += blockDim.x) {
+    double t = Tq[0][j];
+    for (int q = 1; q < nparts; ++q) t += Tq[q][j];     // fixed order (4 parts: ((0 + 1) + 2) + 3 as before)
+    T[j] = t;
+  }
   __syncthreads();
   if (pre) {
     const double t0 = lane < Kp ? T[lane] : 0.0, t1 = lane + 32 < Kp ? T[lane + 32] : 0.0;
@@ -261,18 +270,18 @@ __global__ void __launch_bounds__(256) k_solve(SolveArgs p) {
     }
     return;
   }
-  for (int r0 = warp; r0 < Kp; r0 += 32) {               // rows r0, r0 + 8, r0 + 16, r0 + 24 of this warp together
+  for (int r0 = warp; r0 < Kp; r0 += 4 * nwarp) {        // rows r0, r0 + nwarp, r0 + 2 nwarp, r0 + 3 nwarp of this warp together
     double acc[4] = {0.0, 0.0, 0.0, 0.0};
 #pragma unroll
     for (int u = 0; u < 4; ++u) {
-      const int r = r0 + 8 * u;
+      const int r = r0 + nwarp * u;
       if (r < Kp)
         for (int c = lane; c < Kp; c += 32) acc[u] = fma(Si[(int64_t)r * Kp + c], T[c], acc[u]);
     }
 #pragma unroll
     for (int u = 0; u < 4; ++u) {
       const double v = warp_sum(acc[u]);
-      const int r = r0 + 8 * u;
+      const int r = r0 + nwarp * u;
       if (lane == 0 && r < Kp) p.V[(int64_t)a * p.ldv + r] = v;
     }
   }
