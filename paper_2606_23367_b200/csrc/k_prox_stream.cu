@@ -12,8 +12,10 @@ int prox_stream_idx_bits() { return PROX_META_IDX_BITS; }
 size_t prox_stream_entry_bytes() { return sizeof(LiveEnt); }
 
 cudaError_t prox_stream_set_attrs(int G, int nsub) {
-  TRY(cudaFuncSetAttribute(k_prox_stream<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)stream_smem_bytes(G)));
-  TRY(cudaFuncSetAttribute(k_prox_stream<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)stream_smem_bytes(G)));
+  TRY(cudaFuncSetAttribute(k_prox_stream<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)stream_smem_bytes(G)));
+  TRY(cudaFuncSetAttribute(k_prox_stream<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)stream_smem_bytes(G)));
+  TRY(cudaFuncSetAttribute(k_prox_stream<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)stream_smem_bytes(G)));
+  TRY(cudaFuncSetAttribute(k_prox_stream<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)stream_smem_bytes(G)));
   const size_t smr = root_smem_bytes(G, nsub);
   TRY(cudaFuncSetAttribute(k_prox_root<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smr));
   TRY(cudaFuncSetAttribute(k_prox_root<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smr));
@@ -22,7 +24,8 @@ cudaError_t prox_stream_set_attrs(int G, int nsub) {
 cudaError_t prox_stream_launch(bool check, int S, int A, int G, const ProxArgs& a, int mode, cudaStream_t st) {
   const dim3 grid((unsigned)S, (unsigned)A);
   const size_t sm = stream_smem_bytes(G), smr = root_smem_bytes(G, 2 * S * FAST_NW);
-  if (check) k_prox_stream<true><<<grid, FAST_NW * 32, sm, st>>>(a); else k_prox_stream<false><<<grid, FAST_NW * 32, sm, st>>>(a);
+  if (G == 0) { if (check) k_prox_stream<true, true><<<grid, FAST_NW * 32, sm, st>>>(a); else k_prox_stream<false, true><<<grid, FAST_NW * 32, sm, st>>>(a); }
+  else { if (check) k_prox_stream<true, false><<<grid, FAST_NW * 32, sm, st>>>(a); else k_prox_stream<false, false><<<grid, FAST_NW * 32, sm, st>>>(a); }
   TRY(cudaGetLastError());
   if (check) k_prox_root<true><<<A, ROOT_NT, smr, st>>>(a, mode & ~PROX_CHECK); else k_prox_root<false><<<A, ROOT_NT, smr, st>>>(a, mode);
   return cudaGetLastError();

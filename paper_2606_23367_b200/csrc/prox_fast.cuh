@@ -60,7 +60,7 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
 
 // ------------------------------------------------------------------------------------------------ streaming kernel
 // grid = (slices, accounts), block = 256.  Needs N % 16 == 0 (every row of every streamed array 16-byte aligned).
-template <bool CHECK>
+template <bool CHECK, bool SB>    // SB: no groups - per-CTA fixed-point bins in shared memory (see sbin)
 __global__ void __launch_bounds__(FAST_NW * 32, 3) k_prox_stream(const __grid_constant__ ProxArgs p) {
   extern __shared__ __align__(16) unsigned char stream_raw[];
   __shared__ double cst[12];
@@ -69,7 +69,7 @@ __global__ void __launch_bounds__(FAST_NW * 32, 3) k_prox_stream(const __grid_co
   // per bin and CTA.  (Per-asset global atomics on one address per
   // account serialise in L2: on configs[4], where a quarter of the 384,800 assets is sold out or at its cap, they held
   // the whole kernel at 1.2 TB/s - the bulk copies queued behind them.)  Integer sums: the order does not matter.
-  __shared__ unsigned long long sbin[4 * PRISM_MAX_GROUPS];
+  __shared__ unsigned long long sbin[SB ? 4 : 1];
   const int a = blockIdx.y, sl = blockIdx.x;
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   const int G = p.G, Gb = G > 0 ? G : 1;
@@ -130,7 +130,7 @@ __global__ void __launch_bounds__(FAST_NW * 32, 3) k_prox_stream(const __grid_co
     for (int c = 0; c < FAST_NST - 1 && c < nchunk; ++c) issue(c);
   }
   if (wid == 1 && lane < 12) cst[lane] = cv;
-  for (int t = tid; t < 4 * Gb; t += FAST_NW * 32) sbin[t] = 0ull;
+  if (SB && tid < 4) sbin[tid] = 0ull;
   if (tid >= 64 && tid - 64 < G) lamS[tid - 64] = lam_mine;
   for (int g = tid + FAST_NW * 32 - 64; g < G; g += FAST_NW * 32) lamS[g] = p.lamG[(int64_t)a * G + g];   // (G > 192 only)
   __syncthreads();
@@ -219,7 +219,7 @@ __global__ void __launch_bounds__(FAST_NW * 32, 3) k_prox_stream(const __grid_co
       if (valid && !live) {
         rtp[h * 256] = rt;
         ccp[h * 256] = rt - z;
-        unsigned long long* bin = G == 0 ? (spec ? sbin + 2 * Gb : sbin) : (spec ? cbin + fbin_off : cbin);   // (with groups the bins are spread: direct)
+        unsigned long long* bin = SB ? (spec ? sbin + 2 : sbin) : (spec ? cbin + fbin_off : cbin);   // (with groups the bins are spread: direct)
         if (bc > 0.0) atomicAdd(&bin[g], (unsigned long long)__double2ull_rn(bc * PRISM_FIX_SCALE));
         if (sc > 0.0) atomicAdd(&bin[Gb + g], (unsigned long long)__double2ull_rn(sc * PRISM_FIX_SCALE));
         if (CHECK) {
@@ -251,11 +251,11 @@ __global__ void __launch_bounds__(FAST_NW * 32, 3) k_prox_stream(const __grid_co
     if (lane == 0) mbar_arrive(&bar_empty[st]);
   }
   if (lane == 0) { p.lcnt[sub] = n; p.lcnt[p.A * p.S * FAST_NW + sub] = nw_; }
-  if (G == 0) {
+  if (SB) {
     __syncthreads();
-    for (int t = tid; t < 4 * Gb; t += FAST_NW * 32) {
-      const unsigned long long x = sbin[t];
-      if (x) atomicAdd(t < 2 * Gb ? &cbin[t] : &cbin[fbin_off + (t - 2 * Gb)], x);
+    if (tid < 4) {
+      const unsigned long long x = sbin[tid];
+      if (x) atomicAdd(tid < 2 ? &cbin[tid] : &cbin[fbin_off + (tid - 2)], x);
     }
   }
   if (CHECK) {
