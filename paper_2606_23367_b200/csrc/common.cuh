@@ -42,6 +42,7 @@ struct prism_problem {
   double* Bp;       // N x kp, asset-major, zero padded            (GEMM-2 operand)
   double* Bt;       // kp x ldn, factor-major                      (GEMM-1 operand)
   float *Bp_hi, *Bp_lo, *Bt_hi, *Bt_lo;   // the universe split for the 3xTF32 GEMMs (gemm_tf32.cuh)
+  float *Bp32, *Bt32;                     // the universe rounded to fp32 (N x kp, kp x ldn) for the few-account GEMMs (gemm_skinny.cuh)
   int64_t ldn;      // N padded to 32
   double* invd;     // N
   double* gram;     // Kp x Kp : Bp' D^-1 Bp

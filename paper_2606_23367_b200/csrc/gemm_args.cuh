@@ -40,5 +40,6 @@ struct Gemm2Args {
 struct TfSplit {
   const float *Bt_hi, *Bt_lo;   // kp x ldn, factor-major
   const float *Bp_hi, *Bp_lo;   // N x kp, asset-major
+  const float *Bp32, *Bt32;     // the unsplit fp32 copies (gemm_skinny.cuh)
   int sm_count;
 };

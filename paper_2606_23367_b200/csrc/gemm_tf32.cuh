@@ -264,16 +264,18 @@ __global__ void __launch_bounds__(256, 2) k_gemm2_tf32(Gemm2Args p, TfUniverse u
 
 // universe split at create: Bt_hi/lo (kp x ldn) and Bp_hi/lo (N x kp) from the padded fp64 copies
 __global__ void k_split_universe(const double* Bp, const double* Bt, int64_t N, int kp, int64_t ldn, float* Bp_hi, float* Bp_lo,
-                                 float* Bt_hi, float* Bt_lo) {
+                                 float* Bt_hi, float* Bt_lo, float* Bp32, float* Bt32) {
   const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (e < N * kp) {
     uint32_t h, l;
     tf32_split((float)Bp[e], h, l);
     Bp_hi[e] = __uint_as_float(h); Bp_lo[e] = __uint_as_float(l);
+    Bp32[e] = (float)Bp[e];
   }
   if (e < (int64_t)kp * ldn) {
     uint32_t h, l;
     tf32_split((float)Bt[e], h, l);
     Bt_hi[e] = __uint_as_float(h); Bt_lo[e] = __uint_as_float(l);
+    Bt32[e] = (float)Bt[e];
   }
 }

@@ -1,6 +1,7 @@
 // k_gemm.cu - translation unit of the factor GEMMs (H1, H3): kernels in gemm.cuh, launch wrappers of kernels.h.
 #include "gemm.cuh"
 #include "gemm_tf32.cuh"
+#include "gemm_skinny.cuh"
 #include "kernels.h"
 
 #define MT_SWITCH(mt, ...)                                            \
@@ -30,14 +31,17 @@ cudaError_t gemm_set_attrs(int mt) {
   return cudaSuccess;
 }
 cudaError_t split_universe_launch(const double* Bp, const double* Bt, int64_t N, int kp, int64_t ldn, float* Bp_hi, float* Bp_lo,
-                                  float* Bt_hi, float* Bt_lo, cudaStream_t st) {
+                                  float* Bt_hi, float* Bt_lo, float* Bp32, float* Bt32, cudaStream_t st) {
   const int64_t n = (int64_t)kp * ldn;          // ldn >= N
-  k_split_universe<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(Bp, Bt, N, kp, ldn, Bp_hi, Bp_lo, Bt_hi, Bt_lo);
+  k_split_universe<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(Bp, Bt, N, kp, ldn, Bp_hi, Bp_lo, Bt_hi, Bt_lo, Bp32, Bt32);
   return cudaGetLastError();
 }
 
 cudaError_t gemm1_launch(int gemm_mode, int mt, int nchunk, int kp, const Gemm1Args& a, const TfSplit& tf, cudaStream_t st) {
-  if (gemm_mode == PRISM_GEMM_TF32X3) {
+  if (gemm_mode == PRISM_GEMM_TF32X3 && a.nact <= SKINNY_MAX_ACCOUNTS) {
+    if (a.nact <= 16) { MT_SWITCH(mt, k_gemm1_skinny<MT, 1><<<nchunk, 128, 0, st>>>(a, tf.Bt32)); }
+    else { MT_SWITCH(mt, k_gemm1_skinny<MT, 2><<<nchunk, 128, 0, st>>>(a, tf.Bt32)); }
+  } else if (gemm_mode == PRISM_GEMM_TF32X3) {
     TfUniverse u{tf.Bt_hi, tf.Bt_lo, tf.Bp_hi, tf.Bp_lo};
     dim3 grid(nchunk, (a.nact + T1_TA - 1) / T1_TA);
     MT_SWITCH(mt, k_gemm1_tf32<MT><<<grid, 128, t1_smem(8 * MT), st>>>(a, u));
@@ -53,7 +57,16 @@ cudaError_t gemm1_launch(int gemm_mode, int mt, int nchunk, int kp, const Gemm1A
 
 template <int MODE>
 static void gemm2_mode(int gemm_mode, int mt, const Gemm2Args& a, const TfSplit& tf, cudaStream_t st) {
-  if (gemm_mode == PRISM_GEMM_TF32X3 && MODE != G2_SIGMA) {
+  if (gemm_mode == PRISM_GEMM_TF32X3 && MODE != G2_SIGMA && a.nact <= SKINNY_MAX_ACCOUNTS) {
+    // few active accounts: every warp streams its own universe rows (gemm_skinny.cuh); about three CTAs per SM, >= 2 tiles per warp
+    constexpr int M2 = MODE == G2_SIGMA ? G2_ADMM : MODE;
+    const int64_t ntile = (a.N + 7) / 8;
+    int64_t tpw = (ntile + (int64_t)12 * tf.sm_count - 1) / ((int64_t)12 * tf.sm_count);
+    if (tpw < 2) tpw = 2;
+    const unsigned grid = (unsigned)((ntile + 4 * tpw - 1) / (4 * tpw));
+    if (a.nact <= 16) { MT_SWITCH(mt, k_gemm2_skinny<MT, 1, M2><<<grid, 128, sk2_smem(8 * MT, 1), st>>>(a, tf.Bp32, (int)tpw)); }
+    else { MT_SWITCH(mt, k_gemm2_skinny<MT, 2, M2><<<grid, 128, sk2_smem(8 * MT, 2), st>>>(a, tf.Bp32, (int)tpw)); }
+  } else if (gemm_mode == PRISM_GEMM_TF32X3 && MODE != G2_SIGMA) {
     constexpr int M2 = MODE == G2_SIGMA ? G2_ADMM : MODE;
     TfUniverse u{tf.Bt_hi, tf.Bt_lo, tf.Bp_hi, tf.Bp_lo};
     // tiles per CTA: about two waves of CTAs at two CTAs per SM (the split of V is amortised over the CTA's tiles)

@@ -13,7 +13,7 @@ cudaError_t gemm_set_attrs(int mt);
 cudaError_t gemm1_launch(int gemm_mode, int mt, int nchunk, int kp, const Gemm1Args& a, const TfSplit& tf, cudaStream_t st);
 cudaError_t gemm2_launch(int gemm_mode, int mt, int mode /* G2_* */, const Gemm2Args& a, const TfSplit& tf, cudaStream_t st);
 cudaError_t split_universe_launch(const double* Bp, const double* Bt, int64_t N, int kp, int64_t ldn, float* Bp_hi, float* Bp_lo,
-                                  float* Bt_hi, float* Bt_lo, cudaStream_t st);
+                                  float* Bt_hi, float* Bt_lo, float* Bp32, float* Bt32, cudaStream_t st);
 
 cudaError_t fp64_yardstick(cudaStream_t st, double* sink_dev, int sm_count, double* tflops /* host [2]: DMMA, FMA */);
 

@@ -47,7 +47,7 @@ static int dev_alloc(prism_problem* p, T** ptr, size_t count, bool zero = true) 
 
 extern "C" void prism_problem_destroy(prism_problem* p) {
   if (!p) return;
-  void* ptrs[] = {p->Bp, p->Bt, p->Bp_hi, p->Bp_lo, p->Bt_hi, p->Bt_lo, p->invd, p->gram, p->q, p->v, p->rt, p->cc, p->xs, p->pxq, p->Tpart, p->V, p->Sinv,
+  void* ptrs[] = {p->Bp, p->Bt, p->Bp_hi, p->Bp_lo, p->Bt_hi, p->Bt_lo, p->Bp32, p->Bt32, p->invd, p->gram, p->q, p->v, p->rt, p->cc, p->xs, p->pxq, p->Tpart, p->V, p->Sinv,
                   p->gw0, p->lamG, p->resid, p->duals, p->status, p->ap.c, p->ap.alpha, p->ap.beta,
                   p->ap.mode, p->ap.bsum, p->ap.done, p->ap.conv, p->ap.iters, p->ap.refactor,
                   p->ap.nadapt, p->ap.win, p->ap.wins, p->ap.slack, p->ap.c_new, p->counters, p->act, p->w_stage, p->i_stage, p->lraw, p->lcomp, p->lcnt, p->cbin, p->chkp, p->lflag};
@@ -98,7 +98,7 @@ struct Launcher {
     begin(PRISM_K_GEMM1);
     end(gemm1_launch(gemm_mode, mt, p->nchunk, p->kp, a, tf(), st));
   }
-  TfSplit tf() const { return TfSplit{p->Bt_hi, p->Bt_lo, p->Bp_hi, p->Bp_lo, p->sm_count}; }
+  TfSplit tf() const { return TfSplit{p->Bt_hi, p->Bt_lo, p->Bp_hi, p->Bp_lo, p->Bp32, p->Bt32, p->sm_count}; }
   void gemm2(int mode, const Gemm2Args& a) {
     begin(PRISM_K_GEMM2);
     end(gemm2_launch(gemm_mode, mt, mode, a, tf(), st));
@@ -210,6 +210,8 @@ extern "C" int prism_problem_create(int64_t N, int32_t k, int32_t accounts, cons
   ALLOC_TRY(dev_alloc(p, &p->Bt, (size_t)p->kp * p->ldn));
   ALLOC_TRY(dev_alloc(p, &p->Bp_hi, (size_t)N * p->kp));
   ALLOC_TRY(dev_alloc(p, &p->Bp_lo, (size_t)N * p->kp));
+  ALLOC_TRY(dev_alloc(p, &p->Bp32, (size_t)N * p->kp));
+  ALLOC_TRY(dev_alloc(p, &p->Bt32, (size_t)p->kp * p->ldn));
   ALLOC_TRY(dev_alloc(p, &p->Bt_hi, (size_t)p->kp * p->ldn));
   ALLOC_TRY(dev_alloc(p, &p->Bt_lo, (size_t)p->kp * p->ldn));
   ALLOC_TRY(dev_alloc(p, &p->invd, (size_t)p->ldn));       // padded with zeros (pair-wise GEMM-2 epilogue)
@@ -278,7 +280,7 @@ extern "C" int prism_problem_create(int64_t N, int32_t k, int32_t accounts, cons
   Launcher L{p, st, mt, 0};
   L.end(setup_shared_launch(data->B, data->B_is_fp32, data->d, N, k, p->kp, p->ldn, p->Bp, p->Bt, p->invd, st));
   L.end(gram_launch(p->Bt, p->ldn, p->invd, N, p->kp, p->gram, st));
-  L.end(split_universe_launch(p->Bp, p->Bt, N, p->kp, p->ldn, p->Bp_hi, p->Bp_lo, p->Bt_hi, p->Bt_lo, st));
+  L.end(split_universe_launch(p->Bp, p->Bt, N, p->kp, p->ldn, p->Bp_hi, p->Bp_lo, p->Bt_hi, p->Bt_lo, p->Bp32, p->Bt32, st));
   if (p->d.w_b) L.build_q();            // q = -mu - gamma Sigma w_b
   cudaError_t e = cudaStreamSynchronize(st);
   if (e == cudaSuccess) e = L.err;
