@@ -19,10 +19,23 @@
 // row stride (floats) of the V hi / lo copies: >= 16 ceil(kp / 16), = 16 mod 32 (128-bit fragment loads of rows g and g + 1
 // of a quarter-warp then fall into different halves of the banks)
 __host__ __device__ constexpr int sk_ld(int kp) { return ((kp + 15) / 16 * 16) % 32 == 16 ? (kp + 15) / 16 * 16 : (kp + 15) / 16 * 16 + 16; }
-__host__ __device__ inline size_t sk2_smem(int kp, int mtiles) { return (size_t)2 * 16 * mtiles * sk_ld(kp) * sizeof(float); }
+// shared memory of GEMM-2: V hi / lo, then the two-stage ring of epilogue operands (v and c pairs, 16 bytes per lane and row)
+__host__ __device__ inline size_t sk2_smem(int kp, int mtiles) {
+  return (size_t)2 * 16 * mtiles * sk_ld(kp) * sizeof(float) + (size_t)2 * 2 * 2 * mtiles * 128 * 16;
+}
+__device__ __forceinline__ void sk_cp16(void* smem, const void* gmem) {
+  const uint32_t s = (uint32_t)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void sk_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int NLEFT>
+__device__ __forceinline__ void sk_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(NLEFT) : "memory"); }
 
 // GEMM-2 + fused epilogue (G2_ADMM, G2_ADMM_CHECK), contract of k_gemm2_tf32.  128 threads; warp w of the grid walks the
-// 8-asset tiles [tile_begin(w), tile_end(w)); the universe rows of the NEXT tile are requested before the MMAs of the current one.
+// 8-asset tiles [tile_begin(w), tile_end(w)); the universe rows of the NEXT tile are requested (into registers) before the
+// MMAs of the current one, and so are its epilogue operands v, c - by cp.async into a per-lane ring in shared memory,
+// because the register file is what bounds the bytes in flight here (each lane copies exactly the 16 bytes it reads later:
+// no barrier, only cp.async.wait_group).
 template <int NT, int MTILES, int MODE>
 __global__ void __launch_bounds__(128) k_gemm2_skinny(Gemm2Args p, const float* __restrict__ Bp32, int tiles_per_warp) {
   extern __shared__ __align__(16) unsigned char sk_raw[];
@@ -30,6 +43,7 @@ __global__ void __launch_bounds__(128) k_gemm2_skinny(Gemm2Args p, const float* 
   constexpr bool TAIL8 = (KP % 16) != 0;                  // the last block holds 8 indices only
   float* Vh = (float*)sk_raw;                              // [ROWS][LD]
   float* Vl = Vh + (size_t)ROWS * LD;
+  double2* ring = (double2*)(Vl + (size_t)ROWS * LD);      // [stage 2][v, c][m][h][128 lanes]
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3;
   for (int c = tid; c < ROWS * (LD / 2); c += 128) {       // V = S^-1 T (fp64) -> hi / lo, zero beyond kp
     const int r = c / (LD / 2), cc = (c % (LD / 2)) * 2;
@@ -70,29 +84,35 @@ __global__ void __launch_bounds__(128) k_gemm2_skinny(Gemm2Args p, const float* 
       b[K16 - 1] = make_float4(q.x, q.y, 0.f, 0.f);
     }
   };
+  auto ring_at = [&](int stage, int arr, int m, int h) { return ring + (size_t)(((stage * 2 + arr) * MTILES + m) * 2 + h) * 128 + tid; };
+  auto request_vc = [&](int stage, int64_t tile) {
+    const int64_t ib = tile * 8 + 2 * t;
+    if (ib >= p.ldw) return;
+#pragma unroll
+    for (int m = 0; m < MTILES; ++m)
+#pragma unroll
+      for (int h = 0; h < 2; ++h)
+        if (arow[m][h]) {
+          const int64_t rowp = (int64_t)acct[m][h] * p.ldw;
+          sk_cp16(ring_at(stage, 0, m, h), p.v + rowp + ib);
+          sk_cp16(ring_at(stage, 1, m, h), p.cc + rowp + ib);
+        }
+  };
   float4 bcur[K16], bnext[K16];
   load_B(bcur, tb);
+  request_vc(0, tb);
+  sk_commit();
   const float* vh = Vh + (size_t)g * LD + 4 * t;
   const float* vl = Vl + (size_t)g * LD + 4 * t;
 #pragma unroll 1
   for (int64_t tile = tb; tile < te; ++tile) {
-    if (tile + 1 < te) load_B(bnext, tile + 1);
+    const int stage = (int)(tile - tb) & 1;
+    if (tile + 1 < te) { load_B(bnext, tile + 1); request_vc(stage ^ 1, tile + 1); }
+    sk_commit();
     // D[slot 16 m + g (+8)][asset ib, ib + 1]
     const int64_t ib = tile * 8 + 2 * t;
     const bool iin = ib < p.ldw;
-    double2 v2[MTILES][2], c2[MTILES][2];
     const double2 iv = iin ? *(const double2*)(p.invd + ib) : make_double2(0.0, 0.0);   // (padded with zeros to ldw)
-#pragma unroll
-    for (int m = 0; m < MTILES; ++m)
-#pragma unroll
-      for (int h = 0; h < 2; ++h) {
-        v2[m][h] = make_double2(0.0, 0.0); c2[m][h] = make_double2(0.0, 0.0);
-        if (arow[m][h] && iin) {
-          const int64_t rowp = (int64_t)acct[m][h] * p.ldw;
-          v2[m][h] = *(const double2*)(p.v + rowp + ib);
-          c2[m][h] = *(const double2*)(p.cc + rowp + ib);
-        }
-      }
     float acc[MTILES][4];
 #pragma unroll
     for (int m = 0; m < MTILES; ++m) { acc[m][0] = acc[m][1] = acc[m][2] = acc[m][3] = 0.f; }
@@ -134,18 +154,20 @@ __global__ void __launch_bounds__(128) k_gemm2_skinny(Gemm2Args p, const float* 
         mma_tf32(acc[m], ah, bh[0], bh[1]);
       }
     }
+    sk_wait<1>();                                           // this tile's v, c have landed (the next tile's group may be in flight)
 #pragma unroll
     for (int m = 0; m < MTILES; ++m)
 #pragma unroll
       for (int h = 0; h < 2; ++h) {
         if (!arow[m][h] || !iin) continue;
         const int a = acct[m][h];
+        const double2 v2 = *ring_at(stage, 0, m, h), c2 = *ring_at(stage, 1, m, h);
         const int64_t rowp = (int64_t)a * p.ldw, i = ib;
         const double b0 = (double)acc[m][2 * h], b1 = (double)acc[m][2 * h + 1];
         const double s0 = b0 * iv.x * gsc[m][h], s1 = b1 * iv.y * gsc[m][h];
         double2 vn;
-        vn.x = v2[m][h].x + p.relax * (c2[m][h].x - s0);
-        vn.y = v2[m][h].y + p.relax * (c2[m][h].y - s1);
+        vn.x = v2.x + p.relax * (c2.x - s0);
+        vn.y = v2.y + p.relax * (c2.y - s1);
         const bool in0 = i < p.N, in1 = i + 1 < p.N;
         if (in1) *(double2*)(p.v + rowp + i) = vn; else if (in0) p.v[rowp + i] = vn.x;
         if (MODE == G2_ADMM_CHECK) {

@@ -27,6 +27,10 @@ cudaError_t gemm_set_attrs(int mt) {
     TRY(cudaFuncSetAttribute(k_gemm1_tf32<MT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)t1_smem(8 * MT)));
     TRY(cudaFuncSetAttribute(k_gemm2_tf32<MT, G2_ADMM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)t2_smem(8 * MT)));
     TRY(cudaFuncSetAttribute(k_gemm2_tf32<MT, G2_ADMM_CHECK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)t2_smem(8 * MT)));
+    TRY(cudaFuncSetAttribute(k_gemm2_skinny<MT, 1, G2_ADMM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sk2_smem(8 * MT, 1)));
+    TRY(cudaFuncSetAttribute(k_gemm2_skinny<MT, 1, G2_ADMM_CHECK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sk2_smem(8 * MT, 1)));
+    TRY(cudaFuncSetAttribute(k_gemm2_skinny<MT, 2, G2_ADMM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sk2_smem(8 * MT, 2)));
+    TRY(cudaFuncSetAttribute(k_gemm2_skinny<MT, 2, G2_ADMM_CHECK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sk2_smem(8 * MT, 2)));
   });
   return cudaSuccess;
 }

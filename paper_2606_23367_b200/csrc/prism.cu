@@ -195,9 +195,10 @@ extern "C" int prism_problem_create(int64_t N, int32_t k, int32_t accounts, cons
     p->res = form == PRISM_PROX_RESIDENT; p->fast = form == PRISM_PROX_STREAMING;
     if (p->res) { p->res_C = C; p->res_SL = SL; p->res_smem = sm; }
   }
-  // split-K chunking of GEMM-1: about two waves of CTAs
+  // split-K chunking of GEMM-1: about two waves of CTAs; three CTAs per SM in one wave for the few-account kernel
+  // (gemm_skinny.cuh: 128 threads, no shared memory - its bytes in flight grow with the resident warps)
   const int tilesA = (A + G1_TA - 1) / G1_TA;
-  int64_t want = (2 * p->sm_count + tilesA - 1) / tilesA;
+  int64_t want = ((A <= 32 ? 3 : 2) * p->sm_count + tilesA - 1) / tilesA;
   const int64_t nst = p->ldn / G1_KS;
   if (want > nst) want = nst;
   if (want < 1) want = 1;
