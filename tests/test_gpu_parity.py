@@ -138,6 +138,24 @@ def test_tf32x3_gemms_against_fp64_and_oracle(name):
     P.close()
 
 
+@pytest.mark.parametrize("A", [16, 17, 32, 33])
+@pytest.mark.parametrize("k", [30, 50])
+def test_few_account_gemms_at_their_boundaries(A, k):
+    """gemm_skinny.cuh takes over from the tiled 3xTF32 kernels at nact <= 32 (one account tile at <= 16, two above):
+    batches on both sides of each boundary - and, as accounts converge and H6 compaction shrinks the active list, every
+    batch crosses the lower ones during its solve - against the fp64 DMMA GEMMs.  k = 30 / 50: contraction length 32
+    (whole 16-index blocks) and 56 (an 8-index tail block); N = 700 is not a multiple of the 8-asset tile."""
+    inst = gen.config1(seed=5, N=700, k=k, A=A)
+    P, r0 = _solve_gpu(inst, gemm_precision=0)
+    r3 = P.solve(gemm_precision=3)
+    assert (r3.status == 0).all() and (r0.status == 0).all()
+    assert float((r0.w - r3.w).abs().max()) <= 1e-6
+    assert int((r0.iters - r3.iters).abs().max()) <= 20
+    r3b = P.solve(gemm_precision=3)
+    assert (r3.w == r3b.w).all() and (r3.iters == r3b.iters).all()
+    P.close()
+
+
 def test_batch_equals_single_accounts_and_identical_accounts():
     inst = gen.config1(N=400, k=10, A=4)
     P, r = _solve_gpu(inst)
