@@ -375,12 +375,32 @@ def main():
                               note="single account, L1 penalty kappa = 0.005, cap 3%, no turnover cap"))
         if args.config == "cfg2":                                            # the paper's queue framing (Table 8) on the headline batch
             from paper_2606_23367_b200 import queue_layer
-            for bs in (500, 125):
-                queue_layer.run_queue(inst, batch_size=bs, device=dev)          # warm-up (first-touch of the allocations)
-                _, recs = queue_layer.run_queue(inst, batch_size=bs, deadline_ms=1.5e6, device=dev)
-                extra.append(dict(queue_layer.summarise(recs), config=f"queue_cfg2_batches_of_{bs}",
+            for bs, lanes in ((500, 1), (125, 1), (125, 4)):
+                queue_layer.run_queue(inst, batch_size=bs, lanes=lanes, device=dev)          # warm-up (first-touch of the allocations)
+                _, recs = queue_layer.run_queue(inst, batch_size=bs, lanes=lanes, deadline_ms=1.5e6, device=dev)
+                extra.append(dict(queue_layer.summarise(recs), config=f"queue_cfg2_batches_of_{bs}" + (f"_lanes_{lanes}" if lanes > 1 else ""),
                                   note="NEXT-3 queue layer: consecutive batches incl. prism_problem_create per batch, 1,500 s window; "
                                        "latency = queue start -> result available; paper: 109.5 s total, p50 212 ms per account on its hardware"))
+            # a deeper queue: four times the batch (the same accounts, replicated) as four batches of 500 in four lanes -
+            # one solve is a chain of short launches that leaves most of the GPU idle, independent batches fill it
+            inst4 = inst.subset(list(range(inst.A)) * 4)
+            queue_layer.run_queue(inst4, batch_size=inst.A, lanes=4, device=dev)
+            _, recs = queue_layer.run_queue(inst4, batch_size=inst.A, lanes=4, deadline_ms=1.5e6, device=dev)
+            extra.append(dict(queue_layer.summarise(recs), config=f"queue_4x_cfg2_batches_of_{inst.A}_lanes_4",
+                              note="2,000 accounts (the headline batch four times) as four concurrent batches, one host thread and CUDA stream each, "
+                                   "incl. prism_problem_create and the read-back of every batch"))
+            del inst4
+            # the same without the host-side work: four resident problem objects of the headline batch solved at once
+            Ps = [binding.Problem(inst, device=dev, prox_form=args.prox_form) for _ in range(4)]
+            queue_layer.solve_concurrently(Ps, gemm_precision=args.gemm_precision)
+            rs4, ms4 = min((queue_layer.solve_concurrently(Ps, gemm_precision=args.gemm_precision) for _ in range(3)), key=lambda x: x[1])
+            extra.append(dict(config="cfg2_four_resident_batches_at_once", A=4 * inst.A, N=inst.N, ms_per_solve=ms4,
+                              accounts_per_s=sum(int((r.status == 0).sum()) for r in rs4) / (ms4 * 1e-3),
+                              certified=sum(int((r.status == 0).sum()) for r in rs4),
+                              note="four problem objects of the headline batch, one host thread and CUDA stream each, wall clock between device "
+                                   "synchronisations; the headline value above is ONE batch at a time"))
+            for P4 in Ps:
+                P4.close()
         if args.config == "cfg2":                                            # the other form of the projection on the headline batch
             extra.append(dict(row("cfg2_resident_form", inst, form=binding.PROX_RESIDENT), note="prox_form = PRISM_PROX_RESIDENT"))
 

@@ -531,6 +531,14 @@ def test_queue_layer_batches_deadline_and_audit_records():
     assert len({x.input_sha256 for x in recs}) == 7 and all(x.build_id == pr.version() for x in recs)
     s = ql.summarise(recs)
     assert s["completed"] == 7 and s["certified"] == 7 and s["missed_deadline_rate"] == 0.0 and s["latency_p99_ms"] <= s["queue_ms"]
+    W3, recs3 = ql.run_queue(inst, batch_size=3, lanes=3)                          # three batches at once, one stream each
+    assert (W3 == W).all() and [(x.account, x.batch, x.output_sha256, x.status, x.iterations) for x in recs3] == \
+        [(x.account, x.batch, x.output_sha256, x.status, x.iterations) for x in recs]
+    Ps = [pr.Problem(inst.subset([0, 1, 2])), pr.Problem(inst.subset([3, 4, 5])), pr.Problem(inst.subset([6]))]
+    rs, ms = ql.solve_concurrently(Ps)                                           # resident problem objects, all at once
+    assert ms > 0 and (np.concatenate([x.w.cpu().numpy() for x in rs]) == W).all()
+    for Pc in Ps:
+        Pc.close()
     _, late = ql.run_queue(inst, batch_size=3, deadline_ms=1e-3)
     assert all(x.missed_deadline for x in late) and ql.summarise(late)["missed_deadline_rate"] == 1.0
     assert all(x.status in (0, 3) for x in late)                                  # finished, after the deadline: LATE (or done at once)
