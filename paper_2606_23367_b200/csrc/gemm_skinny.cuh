@@ -45,6 +45,7 @@ __global__ void __launch_bounds__(128) k_gemm2_skinny(Gemm2Args p, const float* 
   float* Vl = Vh + (size_t)ROWS * LD;
   double2* ring = (double2*)(Vl + (size_t)ROWS * LD);      // [stage 2][v, c][m][h][128 lanes]
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3;
+  if (p.nact <= 0) return;
   for (int c = tid; c < ROWS * (LD / 2); c += 128) {       // V = S^-1 T (fp64) -> hi / lo, zero beyond kp
     const int r = c / (LD / 2), cc = (c % (LD / 2)) * 2;
     uint32_t h0 = 0, l0 = 0, h1 = 0, l1 = 0;
@@ -198,7 +199,7 @@ template <int NT, int MTILES>
 __global__ void __launch_bounds__(128) k_gemm1_skinny(Gemm1Args p, const float* __restrict__ Bt32) {
   constexpr int NW = (NT + 3) / 4;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3;
-  if (warp >= NT) return;
+  if (warp >= NT || p.nact <= 0) return;
   const int64_t i_begin = (int64_t)blockIdx.x * p.chunk;
   const int64_t i_end = min(i_begin + p.chunk, p.Npad);
   const int nblk = (int)((i_end - i_begin) / 16);
