@@ -401,6 +401,21 @@ def main():
                                    "synchronisations; the headline value above is ONE batch at a time"))
             for P4 in Ps:
                 P4.close()
+        if args.config == "cfg2":                                            # configs[3] as four sub-batches of 50 accounts at once
+            from paper_2606_23367_b200 import queue_layer, shard
+            inst3 = gen.config3(seed=0)
+            q = [shard.slice_instance(inst3, a0, a1) for a0, a1 in zip(range(0, inst3.A, 50), range(50, inst3.A + 50, 50))]
+            Ps = [binding.Problem(x, device=dev) for x in q]
+            queue_layer.solve_concurrently(Ps, gemm_precision=args.gemm_precision)
+            rs3, ms3 = min((queue_layer.solve_concurrently(Ps, gemm_precision=args.gemm_precision) for _ in range(3)), key=lambda x: x[1])
+            extra.append(dict(config="cfg3_four_sub_batches_at_once", A=inst3.A, N=inst3.N, ms_per_solve=ms3,
+                              accounts_per_s=sum(int((r.status == 0).sum()) for r in rs3) / (ms3 * 1e-3),
+                              certified=sum(int((r.status == 0).sum()) for r in rs3),
+                              note="configs[3] cut into four resident problem objects of 50 accounts, solved at once on four streams (wall clock); "
+                                   "the cfg3 row above is the same batch as ONE problem object"))
+            for P3 in Ps:
+                P3.close()
+            del inst3, q
         if args.config == "cfg2":                                            # the other form of the projection on the headline batch
             extra.append(dict(row("cfg2_resident_form", inst, form=binding.PROX_RESIDENT), note="prox_form = PRISM_PROX_RESIDENT"))
 
