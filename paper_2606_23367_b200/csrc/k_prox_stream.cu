@@ -17,8 +17,10 @@ cudaError_t prox_stream_set_attrs(int G, int nsub) {
   TRY(cudaFuncSetAttribute(k_prox_stream<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)stream_smem_bytes(G)));
   TRY(cudaFuncSetAttribute(k_prox_stream<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)stream_smem_bytes(G)));
   const size_t smr = root_smem_bytes(G, nsub);
-  TRY(cudaFuncSetAttribute(k_prox_root<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smr));
-  TRY(cudaFuncSetAttribute(k_prox_root<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smr));
+  TRY(cudaFuncSetAttribute(k_prox_root<true, ROOT_NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smr));
+  TRY(cudaFuncSetAttribute(k_prox_root<false, ROOT_NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smr));
+  TRY(cudaFuncSetAttribute(k_prox_root<true, ROOT_NT_WIDE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smr));
+  TRY(cudaFuncSetAttribute(k_prox_root<false, ROOT_NT_WIDE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smr));
   return cudaSuccess;
 }
 cudaError_t prox_stream_launch(bool check, int S, int A, int G, const ProxArgs& a, int mode, cudaStream_t st) {
@@ -27,7 +29,12 @@ cudaError_t prox_stream_launch(bool check, int S, int A, int G, const ProxArgs& 
   if (G == 0) { if (check) k_prox_stream<true, true><<<grid, FAST_NW * 32, sm, st>>>(a); else k_prox_stream<false, true><<<grid, FAST_NW * 32, sm, st>>>(a); }
   else { if (check) k_prox_stream<true, false><<<grid, FAST_NW * 32, sm, st>>>(a); else k_prox_stream<false, false><<<grid, FAST_NW * 32, sm, st>>>(a); }
   TRY(cudaGetLastError());
-  if (check) k_prox_root<true><<<A, ROOT_NT, smr, st>>>(a, mode & ~PROX_CHECK); else k_prox_root<false><<<A, ROOT_NT, smr, st>>>(a, mode);
+  // one CTA per account: 128 threads, or 512 when the universe is wide and the accounts are fewer than the SMs
+  if (a.N >= ROOT_WIDE_MIN_N && A <= ROOT_WIDE_MAX_A) {
+    if (check) k_prox_root<true, ROOT_NT_WIDE><<<A, ROOT_NT_WIDE, smr, st>>>(a, mode & ~PROX_CHECK); else k_prox_root<false, ROOT_NT_WIDE><<<A, ROOT_NT_WIDE, smr, st>>>(a, mode);
+  } else {
+    if (check) k_prox_root<true, ROOT_NT><<<A, ROOT_NT, smr, st>>>(a, mode & ~PROX_CHECK); else k_prox_root<false, ROOT_NT><<<A, ROOT_NT, smr, st>>>(a, mode);
+  }
   return cudaGetLastError();
 }
 cudaError_t prox_rescale_launch(int A, const ProxArgs& a, cudaStream_t st) {

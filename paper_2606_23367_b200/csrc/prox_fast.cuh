@@ -28,6 +28,10 @@ struct __align__(16) LiveEnt { double T, w0, ir; uint32_t meta, pad; };   // one
 #define FAST_NST 3           // stages of the bulk-copy pipeline
 #define FAST_STAGE_BYTES (5 * FAST_CH * 8 + 2 * FAST_CH)
 #define ROOT_NT 128          // threads of a root CTA
+#define ROOT_NT_WIDE 512     // ... for wide universes with few accounts (one CTA per account: 384,800-entry universes on 32 of 148 SMs)
+#define ROOT_MAXW (ROOT_NT_WIDE / 32)   // warps the per-warp arrays of the root kernel are sized for
+#define ROOT_WIDE_MIN_N 32768
+#define ROOT_WIDE_MAX_A 148
 #define ROOT_SCAP 512         // a sorted list up to this length is kept in shared memory (no global-load latency per pass)
 
 __host__ __device__ inline size_t stream_smem_bytes(int G) {
@@ -340,7 +344,7 @@ struct SrcLiveG {
 
 __host__ __device__ inline size_t root_smem_bytes(int G, int nsub) {
   const int Gb = G > 0 ? G : 1;
-  return (size_t)(16 * 32 + 4 * Gb + 6 * Gb + 6 * Gb + 8 + 4 * (Gb + 4)) * 8 + (size_t)(nsub + 1 + 4 * Gb + 3 * Gb + 16 + ROOT_NSL) * 4 + 32 + (size_t)ROOT_SCAP * 32;
+  return (size_t)(16 * 32 + ROOT_MAXW * Gb + 6 * Gb + 6 * Gb + 8 + 4 * (Gb + ROOT_MAXW)) * 8 + (size_t)(nsub + 1 + ROOT_MAXW * Gb + 3 * Gb + 16 + ROOT_MAXW + ROOT_NSL) * 4 + 32 + (size_t)ROOT_SCAP * 32;
 }
 
 // Sum over the block of terms that only the first `nfront` threads hold (the others pass zeros): with nfront <= 32
@@ -486,8 +490,8 @@ __device__ __noinline__ void prox_eval_multi(const SrcGrouped& s, const double* 
   for (int k = 0; k < PROX_KSEC; ++k) { outP[k] = sp[k] * L.scale + L.cPt; outR[k] = sr[k] * L.scale + L.cRt; }
 }
 
-template <bool CHECK>
-__global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant__ ProxArgs p, int mode) {
+template <bool CHECK, int NT>
+__global__ void __launch_bounds__(NT, NT <= 128 ? 4 : 1) k_prox_root(const __grid_constant__ ProxArgs p, int mode) {
   extern __shared__ __align__(16) unsigned char root_raw[];
   __shared__ SrcLiveG src;                 // CTA-uniform objects live in shared memory, not on the threads' stacks
   __shared__ SrcGrouped sgrp;
@@ -503,7 +507,7 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
   const int ngrp = G > 0 ? G : nw;                       // without groups: nw slices of the list, for load balance
   double* d0 = (double*)root_raw;
   double* scratch = d0; d0 += 16 * 32;
-  double* gbin = d0; d0 += 4 * Gb;                       // nw = 4 warps
+  double* gbin = d0; d0 += ROOT_MAXW * Gb;               // nw x Gb
   double* lamS = d0; d0 += Gb;
   double* gsum = d0; d0 += Gb;
   double* band_lo = d0; double* band_hi = d0 + Gb; double* gw0 = d0 + 2 * Gb; double* lamW = d0 + 3 * Gb; d0 += 4 * Gb;
@@ -511,12 +515,12 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
   unsigned long long* fbin = (unsigned long long*)d0; d0 += 2 * Gb;    // + list entries outside the tight window
   unsigned long long* ubin = (unsigned long long*)d0; d0 += 2 * Gb;    // their sum: what the solve uses
   double* chk = d0; d0 += 8;
-  double* gv = d0; d0 += 4 * (Gb + 4);                   // per (pseudo-)group sums of one pass
+  double* gv = d0; d0 += 4 * (Gb + ROOT_MAXW);           // per (pseudo-)group sums of one pass (ngrp <= max(G, nw))
   int* offs = (int*)d0;                                  // 2 nsub + 1: start of raw list k in the sequence of lists in use
   int* wcnt = offs + 2 * nsub + 1;                       // nw x Gb: entries of group g in warp w's part (then running offsets)
-  int* goff = wcnt + 4 * Gb;                             // Gb + 1 group offsets of the grouped list
+  int* goff = wcnt + ROOT_MAXW * Gb;                     // Gb + 1 group offsets of the grouped list
   int* poff = goff + Gb + 1;                             // ngrp + 1 (pseudo-)group offsets used by the passes
-  int* act = poff + Gb + 5;                              // Gb: band state -1 lower active, 0 inactive, +1 upper active
+  int* act = poff + Gb + ROOT_MAXW + 1;                  // Gb: band state -1 lower active, 0 inactive, +1 upper active
   int* selS = act + Gb;
   LiveEnt* ents = (LiveEnt*)(((uintptr_t)(selS + 4) + 15) & ~(uintptr_t)15);   // ROOT_SCAP entries
 
@@ -548,7 +552,7 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
     fbin[g] = *src_bin;
     *src_bin = 0ull;
   }
-  for (int e = tid; e < 4 * Gb; e += nt) wcnt[e] = 0;
+  for (int e = tid; e < nw * Gb; e += nt) wcnt[e] = 0;
   for (int k = tid; k < nsub; k += nt) offs[k + 1] = p.lcnt[(int64_t)a * nsub + k];
   __syncthreads();
   bool fallback = generic != 0;
@@ -624,7 +628,7 @@ __global__ void __launch_bounds__(ROOT_NT, 4) k_prox_root(const __grid_constant_
     // ---- group sort (counting sort, stable in sequence order => deterministic): entries -> lcomp (or shared memory) by
     // group.  use_f: the speculative trades of the backs (fbin) count as constants (level 0 of a two-level list).
     auto sort_lists = [&](bool use_f) {
-      for (int e = tid; e < 4 * Gb; e += nt) wcnt[e] = 0;
+      for (int e = tid; e < nw * Gb; e += nt) wcnt[e] = 0;
       __syncthreads();
       if (!G) { if (lane == 0) wcnt[wid] = j_end - j_beg; }
       else {

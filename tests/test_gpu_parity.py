@@ -303,6 +303,39 @@ def test_full_size_sampled_accounts(cfg, n_sample, n_min):
     P.close()
 
 
+@pytest.mark.parametrize("family", ["no_groups", "bands"])
+def test_wide_root_find_properties_and_other_form(family):
+    """Universes of >= 32,768 instruments with fewer accounts than SMs run the per-account root find with 512 threads
+    (16 warps, k_prox_root<CHECK, 512>) instead of 128.  At this size the oracle's interior point hovers around its own
+    acceptance bar (merit 5e-10 ... 2e-9 depending on the host), so element-wise oracle parity of this code path is the
+    stored full-width configs[4] case below; here, at 3 x 32,768 without groups and with 8 group bands: the properties
+    that hold at any size (statuses, gates, and the INDEPENDENT checker's KKT certificate of the returned weights with
+    the returned multipliers) and agreement with the every-asset form of the projection, which
+    shares neither the lists nor the root-find kernel."""
+    from oracle import kkt_check, problem
+    from paper_2606_23367_b200 import binding
+    inst = gen.config4(N=32768, k=20, A=3, hi=0.001) if family == "no_groups" else gen.config2(N=32768, k=20, A=3, G=8, band_half=0.01)
+    P, r = _solve_gpu(inst)
+    assert P.prox_form == binding.PROX_STREAMING
+    st = r.status.cpu().numpy(); rs = r.resid.cpu().numpy(); w = r.w.cpu().numpy(); du = r.duals.cpu().numpy()
+    assert (st == 0).all(), np.bincount(st)
+    assert rs[:, 0:4].max() <= TOL_GATE and rs[:, 7].max() <= TOL_RES and rs[:, 8].max() <= TOL_RES
+    G = inst.G
+    for a in range(inst.A):
+        acc = problem.account_from_instance(inst, a)
+        feas = kkt_check.feasibility(acc, w[a])
+        assert max(feas.values()) <= TOL_GATE, feas
+        k = kkt_check.kkt(acc, w[a], dict(nu=du[a, 0], theta=du[a, 1], lam_hi=du[a, 2:2 + G], lam_lo=du[a, 2 + G:2 + 2 * G]), delta=1e-9)
+        scale = max(np.max(np.abs(acc.mu)), 1e-12)
+        assert k["r_stat"] <= 2e-5 * scale and k["r_comp"] <= 1e-9 and k["min_multiplier"] >= -1e-15, k
+        assert abs(rs[a, 4] - k["r_stat"]) <= 1e-10
+    P.close()
+    P3, r3 = _solve_gpu(inst, prox_form=binding.PROX_EVERY_ASSET)
+    assert (r3.status == 0).all()
+    assert float((r3.w - r.w).abs().max()) <= 1e-5            # two answers, each at 1e-6 scaled residuals (observed 3.4e-6 with bands)
+    P3.close()
+
+
 def test_full_size_cfg4_properties():
     """configs[4] at full width (32 x 384,800, k = 100, fp32 loadings).  The oracle cannot finish one such account in
     minutes (structured interior point: > 15 min), so every account is certified through properties that hold at
