@@ -28,10 +28,16 @@ struct __align__(16) LiveEnt { double T, w0, ir; uint32_t meta, pad; };   // one
 #define FAST_NST 3           // stages of the bulk-copy pipeline
 #define FAST_STAGE_BYTES (5 * FAST_CH * 8 + 2 * FAST_CH)
 #define ROOT_NT 128          // threads of a root CTA
-#define ROOT_NT_WIDE 512     // ... for wide universes with few accounts (one CTA per account: 384,800-entry universes on 32 of 148 SMs)
+#ifndef ROOT_NT_WIDE
+#define ROOT_NT_WIDE 512     // ... when the accounts are fewer than the SMs (one CTA per account: the idle SMs cannot help, width can)
+#endif
 #define ROOT_MAXW (ROOT_NT_WIDE / 32)   // warps the per-warp arrays of the root kernel are sized for
-#define ROOT_WIDE_MIN_N 32768
+#ifndef ROOT_WIDE_MIN_N
+#define ROOT_WIDE_MIN_N 4096
+#endif
+#ifndef ROOT_WIDE_MAX_A
 #define ROOT_WIDE_MAX_A 148
+#endif
 #define ROOT_SCAP 512         // a sorted list up to this length is kept in shared memory (no global-load latency per pass)
 
 __host__ __device__ inline size_t stream_smem_bytes(int G) {

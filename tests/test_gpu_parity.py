@@ -96,6 +96,8 @@ CASES = {
     # account 1 needs the robust root find with interacting bands in the cluster-resident kernel (regression: round 2)
     "cfg3_small": lambda: gen.config3(N=600, k=12, A=4),
     "cfg4_small": lambda: gen.config4(N=4000, k=100, A=3, hi=0.001),          # fp32 loadings, k = 100 (13 factor tiles)
+    "cfg2_wide_root": lambda: gen.config2(N=4096, k=20, A=4, G=6, band_half=0.01),   # N >= 4,096, fewer accounts than SMs: 512-thread root find
+    "cfg4_wide_root": lambda: gen.config4(N=4096, k=40, A=3, hi=0.002),               # the same without groups (warp slices of the list)
     "sec9": lambda: gen.section9(N=481, k=20, A=2),                           # PAPER.md:378 transition objective (R14)
     "benchmark_shift": lambda: gen.make_instance("wb", 7, 400, 8, 3, hi_fixed=0.05, tau_range=(0.2, 0.5), benchmark_in_risk=True),
 }
@@ -305,10 +307,11 @@ def test_full_size_sampled_accounts(cfg, n_sample, n_min):
 
 @pytest.mark.parametrize("family", ["no_groups", "bands"])
 def test_wide_root_find_properties_and_other_form(family):
-    """Universes of >= 32,768 instruments with fewer accounts than SMs run the per-account root find with 512 threads
-    (16 warps, k_prox_root<CHECK, 512>) instead of 128.  At this size the oracle's interior point hovers around its own
-    acceptance bar (merit 5e-10 ... 2e-9 depending on the host), so element-wise oracle parity of this code path is the
-    stored full-width configs[4] case below; here, at 3 x 32,768 without groups and with 8 group bands: the properties
+    """Universes of >= 4,096 instruments with fewer accounts than SMs run the per-account root find with 512 threads
+    (16 warps, k_prox_root<CHECK, 512>) instead of 128; element-wise oracle parity of that code path: the cases
+    cfg2_wide_root / cfg4_wide_root above and the stored full-width configs[4] case below.  At 32,768 instruments the
+    oracle's interior point hovers around its own acceptance bar (merit 5e-10 ... 2e-9 depending on the host), so
+    here, at 3 x 32,768 without groups and with 8 group bands: the properties
     that hold at any size (statuses, gates, and the INDEPENDENT checker's KKT certificate of the returned weights with
     the returned multipliers) and agreement with the every-asset form of the projection, which
     shares neither the lists nor the root-find kernel."""
