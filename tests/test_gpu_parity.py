@@ -425,11 +425,12 @@ def test_solver_settings_do_not_change_the_answer(case, kw):
     P.close()
 
 
-def test_wide_box_and_no_cap():
+@pytest.mark.parametrize("N", [640, 4096])       # 4,096: the generic path inside the 512-thread root kernel
+def test_wide_box_and_no_cap(N):
     """Bounds far from the budget scale (lo = -10, hi = +10: the streaming form's fixed-point range does not hold them,
     ADVICE r1) on an N % 16 == 0 instance, against the oracle; the default form and the streaming request."""
     from paper_2606_23367_b200 import binding
-    inst = gen.make_instance("wide", 11, 640, 8, 3, hi_fixed=10.0, tau_range=(0.2, 0.6))
+    inst = gen.make_instance("wide", 11, N, 8, 3, hi_fixed=10.0, tau_range=(0.2, 0.6))
     inst.lo[:] = -10.0
     W, res = _oracle(inst)
     for form in (binding.PROX_AUTO, binding.PROX_STREAMING, binding.PROX_EVERY_ASSET):
