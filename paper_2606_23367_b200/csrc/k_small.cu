@@ -37,6 +37,18 @@ cudaError_t factor_launch(const double* gram, const double* f, const double* gam
   return cudaGetLastError();
 }
 cudaError_t solve_launch(const SolveArgs& a, cudaStream_t st) {
+  if (a.nchunk >= 128 && a.nact * SOLVE_CL <= 148) {       // few accounts, many chunks: a cluster of CTAs per account
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)(a.nact * SOLVE_CL), 1, 1);
+    cfg.blockDim = dim3(1024, 1, 1);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = SOLVE_CL; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, k_solve_cluster, a);
+  }
   if (a.nchunk > 64 && a.kp > 64) k_solve<1024><<<a.nact, 1024, 0, st>>>(a);
   else k_solve<256><<<a.nact, 256, 0, st>>>(a);
   return cudaGetLastError();

@@ -1,6 +1,7 @@
 // small.cuh - setup (H0), capacitance factorisation (H0/H7), per-account small solve + band block (H2),
 // external diagnostics (H8/H9: PAPER.md:142-146) and status assignment (Table 14).
 #pragma once
+#include <cooperative_groups.h>
 #include "common.cuh"
 #include "small_args.cuh"
 
@@ -284,6 +285,61 @@ __global__ void __launch_bounds__(NT) k_solve(SolveArgs p) {
       const int r = r0 + nwarp * u;
       if (lane == 0 && r < Kp) p.V[(int64_t)a * p.ldv + r] = v;
     }
+  }
+}
+
+// k_solve for FEW accounts and MANY split-K chunks (configs[4]: 32 accounts, 430 chunks of 104 doubles each - 11 MB of
+// partials that 32 CTAs pull at 0.5 TB/s, L2 hit rate 11%: 28 us per launch).  A cluster of SOLVE_CL CTAs per account:
+// CTA r reduces the r-th quarter of the chunks (16 parts of 64 threads, as above), the cluster exchanges the SOLVE_CL partial
+// vectors through distributed shared memory (summed in rank order by every CTA: fixed order, same bits in all), and CTA r
+// computes the r-th quarter of the rows of V = S^-1 T.
+#define SOLVE_CL 4
+__global__ void __launch_bounds__(1024) k_solve_cluster(SolveArgs p) {
+  namespace cg = cooperative_groups;
+  __shared__ double T[PRISM_MAX_KPRIME];
+  __shared__ double Tc[PRISM_MAX_KPRIME];                  // this CTA's partial (read by the cluster)
+  __shared__ double Tq[SOLVE_MAX_PARTS][PRISM_MAX_KPRIME];
+  cg::cluster_group cluster = cg::this_cluster();
+  const int rank = (int)cluster.block_rank();
+  const int slot = blockIdx.x / SOLVE_CL;
+  const int a = p.act ? p.act[slot] : slot, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const bool done = p.ap.done[a] != 0;                      // (cluster-uniform: the barriers below are reached by all or by none)
+  if (done) return;
+  const int Kp = p.kp;
+  const double* Si = p.Sinv + (int64_t)a * Kp * Kp;
+  const int nparts = blockDim.x >> 6, nwarp = blockDim.x >> 5;
+  {
+    const int nper_c = (p.nchunk + SOLVE_CL - 1) / SOLVE_CL;
+    const int cb = rank * nper_c, ce = min(p.nchunk, cb + nper_c);
+    const int part = tid >> 6, nper = (max(ce - cb, 0) + nparts - 1) / nparts;
+    const int c0 = cb + part * nper, c1 = min(ce, c0 + nper);
+    for (int j = tid & 63; j < Kp; j += 64) {
+      double s = 0.0;
+#pragma unroll 4
+      for (int ch = c0; ch < c1; ++ch) s += p.Tpart[((int64_t)ch * p.A + a) * p.ldv + j];
+      Tq[part][j] = s;
+    }
+  }
+  __syncthreads();
+  for (int j = tid; j < Kp; j += blockDim.x) {
+    double t = Tq[0][j];
+    for (int q = 1; q < nparts; ++q) t += Tq[q][j];
+    Tc[j] = t;
+  }
+  cluster.sync();
+  for (int j = tid; j < Kp; j += blockDim.x) {
+    double t = 0.0;
+#pragma unroll
+    for (int r = 0; r < SOLVE_CL; ++r) t += cluster.map_shared_rank(Tc, r)[j];
+    T[j] = t;
+  }
+  cluster.sync();                                           // nobody leaves while its partial is still being read
+  const int rows_c = (Kp + SOLVE_CL - 1) / SOLVE_CL, rb = rank * rows_c, re = min(Kp, rb + rows_c);
+  for (int r = rb + warp; r < re; r += nwarp) {
+    double acc = 0.0;
+    for (int c = lane; c < Kp; c += 32) acc = fma(Si[(int64_t)r * Kp + c], T[c], acc);
+    const double v = warp_sum(acc);
+    if (lane == 0) p.V[(int64_t)a * p.ldv + r] = v;
   }
 }
 
