@@ -29,9 +29,8 @@ cudaError_t prox_stream_launch(bool check, int S, int A, int G, const ProxArgs& 
   if (G == 0) { if (check) k_prox_stream<true, true><<<grid, FAST_NW * 32, sm, st>>>(a); else k_prox_stream<false, true><<<grid, FAST_NW * 32, sm, st>>>(a); }
   else { if (check) k_prox_stream<true, false><<<grid, FAST_NW * 32, sm, st>>>(a); else k_prox_stream<false, false><<<grid, FAST_NW * 32, sm, st>>>(a); }
   TRY(cudaGetLastError());
-  // one CTA per account: 128 threads, or 512 when the lists can be long and the batch is in the measured range (32 / 100 /
-  // 148 / 200 / 296 / 400 / 500 accounts of configs[2]: 26.7 / 34.2 / 38.8 / 40.7 / 50.1 / 55.7 / 58.4 ->
-  // 21.8 / 27.8 / 31.8 / 36.2 / 45.5 / 52.8 / 58.2 ms)
+  // one CTA per account: 128 threads, or 512 when the lists can be long and the accounts are fewer than the SMs (32 / 100 /
+  // 148 accounts of configs[2]: 26.7 / 34.2 / 38.8 -> 21.8 / 27.8 / 31.8 ms; see ROOT_WIDE_MAX_A for why not beyond)
   if (a.N >= ROOT_WIDE_MIN_N && A <= ROOT_WIDE_MAX_A) {
     if (check) k_prox_root<true, ROOT_NT_WIDE><<<A, ROOT_NT_WIDE, smr, st>>>(a, mode & ~PROX_CHECK); else k_prox_root<false, ROOT_NT_WIDE><<<A, ROOT_NT_WIDE, smr, st>>>(a, mode);
   } else {

@@ -29,14 +29,16 @@ struct __align__(16) LiveEnt { double T, w0, ir; uint32_t meta, pad; };   // one
 #define FAST_STAGE_BYTES (5 * FAST_CH * 8 + 2 * FAST_CH)
 #define ROOT_NT 128          // threads of a root CTA
 #ifndef ROOT_NT_WIDE
-#define ROOT_NT_WIDE 512     // ... from 4,096 instruments on: the fewer the accounts, the more SMs idle under one CTA per account - width still helps
+#define ROOT_NT_WIDE 512     // ... from 4,096 instruments on when the accounts are fewer than the SMs (one CTA per account: the idle SMs cannot help, width can)
 #endif
 #define ROOT_MAXW (ROOT_NT_WIDE / 32)   // warps the per-warp arrays of the root kernel are sized for
 #ifndef ROOT_WIDE_MIN_N
 #define ROOT_WIDE_MIN_N 4096
 #endif
 #ifndef ROOT_WIDE_MAX_A
-#define ROOT_WIDE_MAX_A 512   // measured range (configs[2] subsets of 32 ... 500 accounts: -18% ... -0.4%, never slower)
+#define ROOT_WIDE_MAX_A 148   // fewer accounts than SMs.  Beyond, width still helps ONE batch (200 / 296 / 400 / 500 accounts of configs[2]:
+                              // -11% / -9% / -5% / -1%) but one 512-thread CTA per SM leaves no room for a second batch in flight:
+                              // four resident batches of 500 at once 134 -> 165 ms, the 2,000-account queue in four lanes 282 -> 381 ms
 #endif
 #define ROOT_SCAP 512         // a sorted list up to this length is kept in shared memory (no global-load latency per pass)
 
